@@ -1,0 +1,443 @@
+/*
+ * cap_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded CPU restatement of the five stages of CAP's
+ * per-token routing-trace pipeline (arXiv 2607.05116, "Communication-Aware
+ * Placement and Pruning for Efficient Mixture-of-Experts Inference"), written
+ * from the paper (P:Lnnn = /root/reference/PAPER.md line nnn) and from the
+ * readings listed in DESIGN.md section 3 (R1..R21).  It shares no code, header,
+ * table or helper with the CUDA path under paper_2607_05116_b200/csrc/ and
+ * neither imports the other.  Only tests/, __graft_entry__.smoke() and the
+ * cpu_baseline / --impl reference legs of bench.py may call it.
+ *
+ * Build: gcc -O2 -std=c11 -ffp-contract=off -fPIC -shared (see oracle/build.py).
+ * -ffp-contract=off matters: every fp32 step below is one IEEE operation, the
+ * only fused operations are the explicit fmaf() calls in expS.
+ *
+ * Pins (tests/test_oracle_pins.py): every function here is pinned by something
+ * other than itself -- closed forms, brute force, library routines, the
+ * paper's Table III "Default" value.  No function is "parity unpinned"; the one
+ * reading that cannot be pinned against the paper (which load definition the
+ * paper's Table IV uses, R6) is handled by exporting both quantities.
+ *
+ * All arrays are HOST pointers, row-major, layouts as in include/cap.h.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define CAPO_OK 0
+#define CAPO_EINVAL (-1)
+
+/* ------------------------------------------------------------------------- *
+ * expS / sigS: the reproducible fp32 exponential of DESIGN.md R-S1.3.
+ * Only IEEE-exact fp32 operations (mul, add, fma, round-to-nearest-even,
+ * divide), so that any conforming implementation returns identical bits.
+ * Accuracy (pinned against libm exp in double in the tests): < 1 ulp.
+ * ------------------------------------------------------------------------- */
+static float capo_expS(float x)
+{
+    float t = x;
+    if (t < -87.0f) t = -87.0f;
+    if (t > 87.0f) t = 87.0f;
+    float n = nearbyintf(t * 0x1.715476p+0f);      /* round-half-even of t*log2(e) */
+    float r = fmaf(n, -0x1.62ep-1f, t);            /* Cody-Waite, ln2 high part    */
+    r = fmaf(n, -0x1.0bfbe8p-15f, r);              /* ln2 low part                 */
+    float p = 0x1.a01a02p-13f;                     /* 1/5040 */
+    p = fmaf(p, r, 0x1.6c16c2p-10f);               /* 1/720  */
+    p = fmaf(p, r, 0x1.111112p-7f);                /* 1/120  */
+    p = fmaf(p, r, 0x1.555556p-5f);                /* 1/24   */
+    p = fmaf(p, r, 0x1.555556p-3f);                /* 1/6    */
+    p = fmaf(p, r, 0x1p-1f);                       /* 1/2    */
+    p = fmaf(p, r, 1.0f);
+    p = fmaf(p, r, 1.0f);
+    /* exact scaling by 2^n, n in [-126,126] after the clamp */
+    union { uint32_t u; float f; } s;
+    s.u = (uint32_t)((int32_t)n + 127) << 23;
+    return p * s.f;
+}
+
+static float capo_sigS(float x)
+{
+    return 1.0f / (1.0f + capo_expS(-x));
+}
+
+float capo_exp_s(float x) { return capo_expS(x); }
+float capo_sig_s(float x) { return capo_sigS(x); }
+
+/* ------------------------------------------------------------------------- *
+ * S1  gate top-k.  P:L35-40 (sec. II-A, Eq. 1): "a gating network selects the
+ * top-k experts for each token ... Gate_i(x) denotes the normalized routing
+ * weight of the i-th selected expert".  Scoring function, tie rule, group-
+ * limited routing: BASELINE.json north_star/configs, R1,R2,R14,R21.
+ *
+ * logits [L][T][E] fp32, bias [L][E] fp32 or NULL (sigmoid only)
+ * idx    [L][T][k] int32 (slot 0 = best selection score), w [L][T][k] fp32
+ * ------------------------------------------------------------------------- */
+int capo_gate_topk(const float *logits, const float *bias, int32_t L, int64_t T,
+                   int32_t E, int32_t k, int32_t scoring, int32_t renormalize,
+                   int32_t n_group, int32_t topk_group, int32_t group_score,
+                   float scale, int32_t *idx, float *w)
+{
+    if (L < 0 || T < 0 || E < 1 || E > 1024 || k < 1 || k > 16 || k > E) return CAPO_EINVAL;
+    if (scoring != 0 && scoring != 1) return CAPO_EINVAL;
+    if (scoring == 0 && bias != NULL) return CAPO_EINVAL;
+    if (n_group < 1 || E % n_group != 0) return CAPO_EINVAL;
+    if (n_group > 1) {
+        if (topk_group < 1 || topk_group > n_group) return CAPO_EINVAL;
+        if ((int64_t)k > (int64_t)topk_group * (E / n_group)) return CAPO_EINVAL;
+        if (group_score != 0 && group_score != 1) return CAPO_EINVAL;
+        if (group_score == 1 && E / n_group < 2) return CAPO_EINVAL;
+    }
+    float *c = (float *)malloc(sizeof(float) * (size_t)E);   /* selection score */
+    float *s = (float *)malloc(sizeof(float) * (size_t)E);   /* unbiased sigmoid */
+    uint8_t *elig = (uint8_t *)malloc((size_t)E);
+    float *gs = (float *)malloc(sizeof(float) * (size_t)n_group);
+    uint8_t *gsel = (uint8_t *)malloc((size_t)n_group);
+    const int32_t gsz = E / n_group;
+
+    for (int32_t l = 0; l < L; ++l) {
+        const float *b = bias ? bias + (size_t)l * E : NULL;
+        for (int64_t t = 0; t < T; ++t) {
+            const float *x = logits + ((size_t)l * (size_t)T + (size_t)t) * (size_t)E;
+            int32_t *oi = idx + ((size_t)l * (size_t)T + (size_t)t) * (size_t)k;
+            float *ow = w + ((size_t)l * (size_t)T + (size_t)t) * (size_t)k;
+            /* step 1: selection score c_e */
+            for (int32_t e = 0; e < E; ++e) {
+                if (scoring == 0) {
+                    c[e] = x[e];             /* softmax is monotone: raw logit */
+                } else {
+                    s[e] = capo_sigS(x[e]);
+                    c[e] = b ? s[e] + b[e] : s[e];
+                }
+                elig[e] = 1;
+            }
+            /* step 3: group-limited pre-selection */
+            if (n_group > 1) {
+                for (int32_t g = 0; g < n_group; ++g) {
+                    const float *cg = c + (size_t)g * gsz;
+                    if (group_score == 0) {
+                        float m = cg[0];
+                        for (int32_t j = 1; j < gsz; ++j) if (cg[j] > m) m = cg[j];
+                        gs[g] = m;
+                    } else {
+                        /* fp32 sum of the two largest c_e of the group */
+                        int32_t i1 = 0;
+                        for (int32_t j = 1; j < gsz; ++j) if (cg[j] > cg[i1]) i1 = j;
+                        int32_t i2 = -1;
+                        for (int32_t j = 0; j < gsz; ++j) {
+                            if (j == i1) continue;
+                            if (i2 < 0 || cg[j] > cg[i2]) i2 = j;
+                        }
+                        gs[g] = cg[i1] + cg[i2];
+                    }
+                    gsel[g] = 0;
+                }
+                for (int32_t r = 0; r < topk_group; ++r) {
+                    int32_t best = -1;
+                    for (int32_t g = 0; g < n_group; ++g) {
+                        if (gsel[g]) continue;
+                        if (best < 0 || gs[g] > gs[best]) best = g;   /* ties -> lower g */
+                    }
+                    gsel[best] = 1;
+                }
+                for (int32_t e = 0; e < E; ++e) elig[e] = gsel[e / gsz];
+            }
+            /* step 4: k passes of linear arg-max, ties -> lower expert index */
+            for (int32_t r = 0; r < k; ++r) {
+                int32_t best = -1;
+                for (int32_t e = 0; e < E; ++e) {
+                    if (!elig[e]) continue;
+                    if (best < 0 || c[e] > c[best]) best = e;
+                }
+                oi[r] = best;
+                elig[best] = 0;
+            }
+            /* step 5: weights */
+            if (scoring == 0) {
+                if (renormalize) {
+                    float raw[16];
+                    for (int32_t r = 0; r < k; ++r) raw[r] = capo_expS(x[oi[r]] - x[oi[0]]);
+                    float Z = raw[0];
+                    for (int32_t r = 1; r < k; ++r) Z = Z + raw[r];
+                    for (int32_t r = 0; r < k; ++r) {
+                        float v = raw[r] / Z;
+                        ow[r] = (scale == 1.0f) ? v : v * scale;
+                    }
+                } else {
+                    /* full softmax probability of the selected experts
+                       (tolerance-only mode, DESIGN.md R-S1.5) */
+                    float m = x[0];
+                    for (int32_t e = 1; e < E; ++e) if (x[e] > m) m = x[e];
+                    double Zall = 0.0;
+                    for (int32_t e = 0; e < E; ++e) Zall += (double)capo_expS(x[e] - m);
+                    for (int32_t r = 0; r < k; ++r) {
+                        float v = (float)((double)capo_expS(x[oi[r]] - m) / Zall);
+                        ow[r] = (scale == 1.0f) ? v : v * scale;
+                    }
+                }
+            } else {
+                if (renormalize) {
+                    float Z = s[oi[0]];
+                    for (int32_t r = 1; r < k; ++r) Z = Z + s[oi[r]];
+                    for (int32_t r = 0; r < k; ++r) {
+                        float v = s[oi[r]] / Z;
+                        ow[r] = (scale == 1.0f) ? v : v * scale;
+                    }
+                } else {
+                    for (int32_t r = 0; r < k; ++r)
+                        ow[r] = (scale == 1.0f) ? s[oi[r]] : s[oi[r]] * scale;
+                }
+            }
+        }
+    }
+    free(c); free(s); free(elig); free(gs); free(gsel);
+    return CAPO_OK;
+}
+
+/* ------------------------------------------------------------------------- *
+ * S2  activation counts and co-activation.  P:L104 (sec. IV-A: "we collect
+ * pairwise expert co-activation frequencies from inference-time routing
+ * traces"), P:L148 ("the number of times they are selected together"),
+ * P:L224 (placement runs on the pruned routing data -> optional kept mask).
+ * counts[i] = #(token,slot) kept with expert i; C[i][j] = #tokens that keep
+ * both i and j (i != j); C[i][i] = counts[i].  Plain triple loop over (t,a,b).
+ * ------------------------------------------------------------------------- */
+int capo_coactivation(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T,
+                      int32_t k, int32_t E, int64_t *counts, int32_t *coact)
+{
+    if (L < 0 || T < 0 || E < 1 || k < 1 || k > 16) return CAPO_EINVAL;
+    memset(counts, 0, sizeof(int64_t) * (size_t)L * (size_t)E);
+    memset(coact, 0, sizeof(int32_t) * (size_t)L * (size_t)E * (size_t)E);
+    for (int32_t l = 0; l < L; ++l) {
+        int64_t *cnt = counts + (size_t)l * E;
+        int32_t *C = coact + (size_t)l * E * E;
+        for (int64_t t = 0; t < T; ++t) {
+            size_t base = ((size_t)l * (size_t)T + (size_t)t) * (size_t)k;
+            for (int32_t a = 0; a < k; ++a) {
+                if (kept && !kept[base + a]) continue;
+                int32_t i = idx[base + a];
+                cnt[i] += 1;
+                C[(size_t)i * E + i] += 1;
+                for (int32_t b = 0; b < k; ++b) {
+                    if (b == a) continue;
+                    if (kept && !kept[base + b]) continue;
+                    int32_t j = idx[base + b];
+                    C[(size_t)i * E + j] += 1;
+                }
+            }
+        }
+    }
+    return CAPO_OK;
+}
+
+/* ------------------------------------------------------------------------- *
+ * S3  evaluation of P candidate placements.
+ *  - P:L58 (sec. II-C): "each token is sent once to each device that hosts
+ *    activated experts" -> per token the SET of devices, not the experts.
+ *  - P:L152-158 (Eq. 2-3): cost 0 same device, 1 same node, c across nodes.
+ *  - P:L186-188 (Eq. 4): imbalance = max_g L_g / mean_g L_g.
+ *  - P:L196 (Fig. 6 x-axis): "average number of devices each token is routed
+ *    to"; Table III fixes that this counts ALL devices (R4).
+ *  - Table II: "Node per Token".
+ * expert_dev [L][P][E], dev_node [D], token_src [L][T] or NULL (= t*D/T).
+ * Scalar outputs [L][P]; load_pairs/recv_tokens [L][P][D]; tok_* [L][P][T].
+ * Any output pointer may be NULL.
+ * ------------------------------------------------------------------------- */
+int capo_eval_placements(const int32_t *idx, const uint8_t *kept, const int32_t *token_src,
+                         int32_t L, int64_t T, int32_t k, int32_t E,
+                         const int32_t *expert_dev, int32_t P,
+                         int32_t D, int32_t N, const int32_t *dev_node,
+                         int32_t cost_local, int32_t cost_intra, int32_t cost_inter,
+                         int64_t bytes_per_token,
+                         int64_t *dev_visits, int64_t *remote_dev, int64_t *remote_intra,
+                         int64_t *remote_inter, int64_t *node_visits, int64_t *remote_node,
+                         int64_t *cost, int64_t *bytes,
+                         int64_t *load_pairs, int64_t *recv_tokens,
+                         double *imbalance, double *imbalance_recv,
+                         uint8_t *tok_remote_dev, uint8_t *tok_remote_node)
+{
+    if (L < 0 || T < 0 || E < 1 || k < 1 || k > 16 || P < 0 || D < 1 || D > 64 || N < 1 || N > 64)
+        return CAPO_EINVAL;
+    for (int32_t d = 0; d < D; ++d)
+        if (dev_node[d] < 0 || dev_node[d] >= N) return CAPO_EINVAL;
+    for (int32_t l = 0; l < L; ++l) {
+        for (int32_t p = 0; p < P; ++p) {
+            const int32_t *pi = expert_dev + ((size_t)l * P + p) * (size_t)E;
+            for (int32_t e = 0; e < E; ++e)
+                if (pi[e] < 0 || pi[e] >= D) return CAPO_EINVAL;
+            int64_t a_dev = 0, a_rdev = 0, a_intra = 0, a_inter = 0, a_node = 0, a_rnode = 0, a_local = 0;
+            int64_t lp[64], rt[64];
+            for (int32_t d = 0; d < D; ++d) { lp[d] = 0; rt[d] = 0; }
+            for (int64_t t = 0; t < T; ++t) {
+                size_t base = ((size_t)l * (size_t)T + (size_t)t) * (size_t)k;
+                int32_t src = token_src ? token_src[(size_t)l * (size_t)T + (size_t)t]
+                                        : (int32_t)(((int64_t)t * D) / T);
+                int32_t srcn = dev_node[src];
+                uint8_t indev[64], innode[64];
+                memset(indev, 0, sizeof indev);
+                memset(innode, 0, sizeof innode);
+                for (int32_t sl = 0; sl < k; ++sl) {
+                    if (kept && !kept[base + sl]) continue;
+                    int32_t d = pi[idx[base + sl]];
+                    lp[d] += 1;                       /* every kept pair is load */
+                    indev[d] = 1;
+                    innode[dev_node[d]] = 1;
+                }
+                int32_t rd = 0, rn = 0;
+                for (int32_t d = 0; d < D; ++d) {
+                    if (!indev[d]) continue;
+                    a_dev += 1;
+                    rt[d] += 1;
+                    if (d == src) { a_local += 1; continue; }
+                    rd += 1;
+                    if (dev_node[d] == srcn) a_intra += 1; else a_inter += 1;
+                }
+                for (int32_t n = 0; n < N; ++n) {
+                    if (!innode[n]) continue;
+                    a_node += 1;
+                    if (n != srcn) rn += 1;
+                }
+                a_rdev += rd;
+                a_rnode += rn;
+                if (tok_remote_dev) tok_remote_dev[((size_t)l * P + p) * (size_t)T + (size_t)t] = (uint8_t)rd;
+                if (tok_remote_node) tok_remote_node[((size_t)l * P + p) * (size_t)T + (size_t)t] = (uint8_t)rn;
+            }
+            size_t o = (size_t)l * P + p;
+            if (dev_visits) dev_visits[o] = a_dev;
+            if (remote_dev) remote_dev[o] = a_rdev;
+            if (remote_intra) remote_intra[o] = a_intra;
+            if (remote_inter) remote_inter[o] = a_inter;
+            if (node_visits) node_visits[o] = a_node;
+            if (remote_node) remote_node[o] = a_rnode;
+            if (cost) cost[o] = (int64_t)cost_local * a_local + (int64_t)cost_intra * a_intra
+                                + (int64_t)cost_inter * a_inter;
+            if (bytes) bytes[o] = a_rdev * bytes_per_token;
+            int64_t mx = 0, sm = 0, mxr = 0, smr = 0;
+            for (int32_t d = 0; d < D; ++d) {
+                if (load_pairs) load_pairs[o * D + d] = lp[d];
+                if (recv_tokens) recv_tokens[o * D + d] = rt[d];
+                if (lp[d] > mx) mx = lp[d];
+                sm += lp[d];
+                if (rt[d] > mxr) mxr = rt[d];
+                smr += rt[d];
+            }
+            /* Eq. 4: max / mean = max*D / sum; integer product exact, one divide */
+            if (imbalance) imbalance[o] = sm ? (double)(mx * D) / (double)sm : 0.0;
+            if (imbalance_recv) imbalance_recv[o] = smr ? (double)(mxr * D) / (double)smr : 0.0;
+        }
+    }
+    return CAPO_OK;
+}
+
+/* ------------------------------------------------------------------------- *
+ * S4  communication-aware pruning, P:L208-218 (sec. VI, Eq. 6 and the greedy
+ * solver: "compute the ratio a_d/c_d for each device and retain devices in
+ * descending order of this ratio until the target accuracy 1-p is
+ * satisfied").  Heuristic: followed step by step, fp32, no reassociation.
+ * Readings R7..R10: c_local = 0 -> ratio +inf (own device first),
+ * keep while cum < 1-p, ties -> lower device id, p <= 0 is the identity.
+ * expert_dev [L][E].  kept [L][T][k] out.  near_margin [L] out (nullable):
+ * tokens whose deciding margin is below 1e-6 (R-S4.7).
+ * ------------------------------------------------------------------------- */
+int capo_prune(const int32_t *idx, const float *w, const int32_t *token_src,
+               int32_t L, int64_t T, int32_t k, int32_t E,
+               const int32_t *expert_dev, int32_t D, int32_t N, const int32_t *dev_node,
+               int32_t cost_local, int32_t cost_intra, int32_t cost_inter,
+               float p, uint8_t *kept, int64_t *near_margin)
+{
+    if (L < 0 || T < 0 || E < 1 || k < 1 || k > 16 || D < 1 || D > 64 || N < 1 || N > 64)
+        return CAPO_EINVAL;
+    if (!(p < 1.0f) || p != p) return CAPO_EINVAL;
+    if (cost_local < 0 || cost_intra < 0 || cost_inter < 0) return CAPO_EINVAL;
+    for (int32_t l = 0; l < L; ++l) {
+        const int32_t *pi = expert_dev + (size_t)l * E;
+        int64_t nm = 0;
+        for (int64_t t = 0; t < T; ++t) {
+            size_t base = ((size_t)l * (size_t)T + (size_t)t) * (size_t)k;
+            if (p <= 0.0f) {                                  /* step 1: identity */
+                for (int32_t s = 0; s < k; ++s) kept[base + s] = 1;
+                continue;
+            }
+            int32_t src = token_src ? token_src[(size_t)l * (size_t)T + (size_t)t]
+                                    : (int32_t)(((int64_t)t * D) / T);
+            /* step 2: a_d in slot order */
+            float a[64];
+            uint8_t present[64], keepd[64];
+            for (int32_t d = 0; d < D; ++d) { a[d] = 0.0f; present[d] = 0; keepd[d] = 0; }
+            for (int32_t s = 0; s < k; ++s) {
+                int32_t d = pi[idx[base + s]];
+                a[d] = a[d] + w[base + s];
+                present[d] = 1;
+            }
+            /* step 3: cost and ratio; step 4: order by ratio desc, ties lower d */
+            int32_t order[64], m = 0;
+            float ratio[64];
+            for (int32_t d = 0; d < D; ++d) {
+                if (!present[d]) continue;
+                int32_t c = (d == src) ? cost_local
+                          : (dev_node[d] == dev_node[src]) ? cost_intra : cost_inter;
+                ratio[d] = (c == 0) ? INFINITY : a[d] / (float)c;
+                order[m++] = d;
+            }
+            for (int32_t i = 1; i < m; ++i) {               /* stable insertion sort */
+                int32_t d = order[i], j = i - 1;
+                while (j >= 0 && ratio[order[j]] < ratio[d]) { order[j + 1] = order[j]; --j; }
+                order[j + 1] = d;
+            }
+            /* step 5: keep while cum < target */
+            float target = 1.0f - p;
+            float cum = 0.0f;
+            int near = 0;
+            int32_t nk = 0;
+            for (int32_t i = 0; i < m; ++i) {
+                if (fabsf(cum - target) < 1e-6f) near = 1;
+                if (cum >= target) break;
+                keepd[order[i]] = 1;
+                cum = cum + a[order[i]];
+                nk = i + 1;
+            }
+            /* step 7: the ratio margin that decided kept-vs-dropped */
+            if (nk < m) {
+                float r1 = ratio[order[nk - 1]], r2 = ratio[order[nk]];
+                if (isfinite(r1) && isfinite(r2) && (r1 - r2) < 1e-6f) near = 1;
+            }
+            nm += near;
+            /* step 6 */
+            for (int32_t s = 0; s < k; ++s) kept[base + s] = keepd[pi[idx[base + s]]];
+        }
+        if (near_margin) near_margin[l] = nm;
+    }
+    return CAPO_OK;
+}
+
+/* ------------------------------------------------------------------------- *
+ * S5  dispatch layout, P:L58 (device-centric routing) + BASELINE.json (5):
+ * stable counting sort of kept (token,slot) pairs i = t*k+s by destination
+ * device pi(idx[i]).  Written as the definition: for each device in order,
+ * scan the pairs in ascending i.
+ * expert_dev [E].  sorted_pairs [>= n_kept], pair_pos [T*k] (nullable),
+ * offsets [D+1].
+ * ------------------------------------------------------------------------- */
+int capo_dispatch_layout(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k,
+                         int32_t E, const int32_t *expert_dev, int32_t D,
+                         int32_t *sorted_pairs, int32_t *pair_pos, int64_t *offsets)
+{
+    if (T < 0 || E < 1 || k < 1 || k > 16 || D < 1 || D > 64) return CAPO_EINVAL;
+    if (T * k >= ((int64_t)1 << 31)) return CAPO_EINVAL;
+    int64_t n = T * k, pos = 0;
+    if (pair_pos) for (int64_t i = 0; i < n; ++i) pair_pos[i] = -1;
+    for (int32_t d = 0; d < D; ++d) {
+        offsets[d] = pos;
+        for (int64_t i = 0; i < n; ++i) {
+            if (kept && !kept[i]) continue;
+            if (expert_dev[idx[i]] != d) continue;
+            sorted_pairs[pos] = (int32_t)i;
+            if (pair_pos) pair_pos[i] = (int32_t)pos;
+            ++pos;
+        }
+    }
+    offsets[D] = pos;
+    return CAPO_OK;
+}

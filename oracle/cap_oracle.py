@@ -1,0 +1,166 @@
+"""ctypes front-end to the CPU oracle (oracle/cap_oracle.c).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this module.  It takes
+and returns numpy arrays on the host and never touches the CUDA path.
+"""
+import ctypes as C
+from types import SimpleNamespace
+
+import numpy as np
+
+from . import build as _build
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        _lib.capo_exp_s.restype = C.c_float
+        _lib.capo_exp_s.argtypes = [C.c_float]
+        _lib.capo_sig_s.restype = C.c_float
+        _lib.capo_sig_s.argtypes = [C.c_float]
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _c(a, dt):
+    if a is None:
+        return None
+    a = np.ascontiguousarray(a, dtype=dt)
+    return a
+
+
+def exp_s(x):
+    return float(lib().capo_exp_s(C.c_float(float(x))))
+
+
+def sig_s(x):
+    return float(lib().capo_sig_s(C.c_float(float(x))))
+
+
+def gate_topk(logits, bias=None, *, k, scoring=0, renormalize=1, n_group=1, topk_group=1,
+              group_score=0, scale=1.0):
+    """S1. logits [L,T,E] fp32 -> (idx [L,T,k] int32, w [L,T,k] fp32)."""
+    logits = _c(logits, np.float32)
+    L, T, E = logits.shape
+    bias = _c(bias, np.float32)
+    idx = np.empty((L, T, k), np.int32)
+    w = np.empty((L, T, k), np.float32)
+    rc = lib().capo_gate_topk(_p(logits), _p(bias), C.c_int32(L), C.c_int64(T), C.c_int32(E),
+                              C.c_int32(k), C.c_int32(scoring), C.c_int32(renormalize),
+                              C.c_int32(n_group), C.c_int32(topk_group), C.c_int32(group_score),
+                              C.c_float(scale), _p(idx), _p(w))
+    if rc != 0:
+        raise ValueError(f"capo_gate_topk -> {rc}")
+    return idx, w
+
+
+def coactivation(idx, kept=None, *, E):
+    """S2. idx [L,T,k] -> (counts [L,E] int64, coact [L,E,E] int32)."""
+    idx = _c(idx, np.int32)
+    L, T, k = idx.shape
+    kept = _c(kept, np.uint8)
+    counts = np.empty((L, E), np.int64)
+    coact = np.empty((L, E, E), np.int32)
+    rc = lib().capo_coactivation(_p(idx), _p(kept), C.c_int32(L), C.c_int64(T), C.c_int32(k),
+                                 C.c_int32(E), _p(counts), _p(coact))
+    if rc != 0:
+        raise ValueError(f"capo_coactivation -> {rc}")
+    return counts, coact
+
+
+def eval_placements(idx, expert_dev, dev_node, *, kept=None, token_src=None, E=None,
+                    cost_local=0, cost_intra=1, cost_inter=1, bytes_per_token=0,
+                    per_token=False):
+    """S3. idx [L,T,k]; expert_dev [L,P,E]; dev_node [D] -> namespace of arrays."""
+    idx = _c(idx, np.int32)
+    L, T, k = idx.shape
+    expert_dev = _c(expert_dev, np.int32)
+    _, P, E2 = expert_dev.shape
+    E = E2 if E is None else E
+    dev_node = _c(dev_node, np.int32)
+    D = dev_node.shape[0]
+    N = int(dev_node.max()) + 1 if D else 1
+    kept = _c(kept, np.uint8)
+    token_src = _c(token_src, np.int32)
+    o = SimpleNamespace()
+    for name in ("dev_visits", "remote_dev", "remote_intra", "remote_inter", "node_visits",
+                 "remote_node", "cost", "bytes"):
+        setattr(o, name, np.empty((L, P), np.int64))
+    o.load_pairs = np.empty((L, P, D), np.int64)
+    o.recv_tokens = np.empty((L, P, D), np.int64)
+    o.imbalance = np.empty((L, P), np.float64)
+    o.imbalance_recv = np.empty((L, P), np.float64)
+    o.tok_remote_dev = np.empty((L, P, T), np.uint8) if per_token else None
+    o.tok_remote_node = np.empty((L, P, T), np.uint8) if per_token else None
+    rc = lib().capo_eval_placements(
+        _p(idx), _p(kept), _p(token_src), C.c_int32(L), C.c_int64(T), C.c_int32(k), C.c_int32(E),
+        _p(expert_dev), C.c_int32(P), C.c_int32(D), C.c_int32(N), _p(dev_node),
+        C.c_int32(cost_local), C.c_int32(cost_intra), C.c_int32(cost_inter),
+        C.c_int64(bytes_per_token),
+        _p(o.dev_visits), _p(o.remote_dev), _p(o.remote_intra), _p(o.remote_inter),
+        _p(o.node_visits), _p(o.remote_node), _p(o.cost), _p(o.bytes),
+        _p(o.load_pairs), _p(o.recv_tokens), _p(o.imbalance), _p(o.imbalance_recv),
+        _p(o.tok_remote_dev), _p(o.tok_remote_node))
+    if rc != 0:
+        raise ValueError(f"capo_eval_placements -> {rc}")
+    return o
+
+
+def prune(idx, w, expert_dev, dev_node, p, *, token_src=None, cost_local=0, cost_intra=1,
+          cost_inter=1):
+    """S4. idx,w [L,T,k]; expert_dev [L,E] -> (kept [L,T,k] uint8, near_margin [L] int64)."""
+    idx = _c(idx, np.int32)
+    w = _c(w, np.float32)
+    L, T, k = idx.shape
+    expert_dev = _c(expert_dev, np.int32)
+    E = expert_dev.shape[-1]
+    dev_node = _c(dev_node, np.int32)
+    D = dev_node.shape[0]
+    N = int(dev_node.max()) + 1
+    token_src = _c(token_src, np.int32)
+    kept = np.empty((L, T, k), np.uint8)
+    near = np.zeros((L,), np.int64)
+    rc = lib().capo_prune(_p(idx), _p(w), _p(token_src), C.c_int32(L), C.c_int64(T), C.c_int32(k),
+                          C.c_int32(E), _p(expert_dev), C.c_int32(D), C.c_int32(N), _p(dev_node),
+                          C.c_int32(cost_local), C.c_int32(cost_intra), C.c_int32(cost_inter),
+                          C.c_float(p), _p(kept), _p(near))
+    if rc != 0:
+        raise ValueError(f"capo_prune -> {rc}")
+    return kept, near
+
+
+def dispatch_layout(idx, expert_dev, D, *, kept=None, want_pos=True):
+    """S5. idx [T,k]; expert_dev [E] -> (sorted_pairs [n_kept], offsets [D+1], pair_pos [T*k])."""
+    idx = _c(idx, np.int32)
+    T, k = idx.shape
+    expert_dev = _c(expert_dev, np.int32)
+    E = expert_dev.shape[0]
+    kept = _c(kept, np.uint8)
+    sorted_pairs = np.empty((T * k,), np.int32)
+    pair_pos = np.empty((T * k,), np.int32) if want_pos else None
+    offsets = np.empty((D + 1,), np.int64)
+    rc = lib().capo_dispatch_layout(_p(idx), _p(kept), C.c_int64(T), C.c_int32(k), C.c_int32(E),
+                                    _p(expert_dev), C.c_int32(D), _p(sorted_pairs), _p(pair_pos),
+                                    _p(offsets))
+    if rc != 0:
+        raise ValueError(f"capo_dispatch_layout -> {rc}")
+    return sorted_pairs[: int(offsets[D])], offsets, pair_pos
+
+
+def trace_fused(logits, bias, gate, expert_dev, dev_node, *, token_src=None, cost_local=0,
+                cost_intra=1, cost_inter=1, bytes_per_token=0, per_token=False):
+    """S1 -> S2 -> S3 composed (what cap_trace_fused computes in one pass)."""
+    idx, w = gate_topk(logits, bias, **gate)
+    E = logits.shape[-1]
+    counts, coact = coactivation(idx, E=E)
+    ev = eval_placements(idx, expert_dev, dev_node, token_src=token_src, cost_local=cost_local,
+                         cost_intra=cost_intra, cost_inter=cost_inter,
+                         bytes_per_token=bytes_per_token, per_token=per_token)
+    return idx, w, counts, coact, ev
