@@ -1,0 +1,185 @@
+/*
+ * cap.h -- C ABI of the B200 (sm_100a) routing-trace hot path of CAP
+ * (arXiv 2607.05116, "Communication-Aware Placement and Pruning for Efficient
+ * Mixture-of-Experts Inference").  P:Lnnn = PAPER.md line nnn; Rn = reading n
+ * in DESIGN.md section 3.
+ *
+ * Conventions (all entry points)
+ *  - Every array pointer is a DEVICE pointer owned by the caller unless the
+ *    comment says "host".  The structs (cap_gate_cfg, cap_topology,
+ *    cap_eval_out) are read on the HOST at call time; the pointers inside them
+ *    are device pointers.
+ *  - The library never allocates, frees or synchronises device memory.  Work is enqueued on
+ *    `stream` (a cudaStream_t passed as void*, NULL = default stream) and the
+ *    call returns immediately.  Scratch comes from the caller's workspace `ws`
+ *    of `ws_bytes` >= cap_workspace_bytes(...); it must stay untouched until the
+ *    enqueued work has finished.  Calls with distinct workspaces are re-entrant.
+ *  - Layouts are dense row-major with the dimensions written in brackets.
+ *  - Return value: CAP_OK, or CAP_EINVAL (bad size / NULL / unsupported
+ *    combination, detected on the host before anything is launched),
+ *    CAP_EWORKSPACE (workspace too small), CAP_ECUDA (a launch failed;
+ *    cap_last_cuda_error() returns the cudaError_t).
+ *  - Values inside device arrays are not validated by the compute calls:
+ *    expert_dev >= D, token_src >= D or non-finite logits give undefined but
+ *    memory-safe results.  cap_validate_placements checks maps (synchronous).
+ *  - T = 0 is valid: aggregate outputs are zeroed.
+ *  - Limits: 1 <= E <= 1024, 1 <= k <= 16, k <= E, 1 <= D <= 64, 1 <= N <= 64,
+ *    T*k < 2^31, L*T*k < 2^40.
+ */
+#ifndef CAP_H_
+#define CAP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CAP_OK 0
+#define CAP_EINVAL (-1)
+#define CAP_EWORKSPACE (-2)
+#define CAP_ECUDA (-3)
+
+/* which_call values for cap_workspace_bytes */
+#define CAP_CALL_GATE_TOPK 0
+#define CAP_CALL_COACTIVATION 1
+#define CAP_CALL_EVAL_PLACEMENTS 2
+#define CAP_CALL_PRUNE 3
+#define CAP_CALL_DISPATCH_LAYOUT 4
+#define CAP_CALL_TRACE_FUSED 5
+
+/* Gate configuration (Eq. 1; scoring / group-limited routing / tie rule from
+ * BASELINE.json, readings R1, R2, R14, R21). */
+typedef struct {
+    int32_t E;            /* experts */
+    int32_t k;            /* experts selected per token */
+    int32_t scoring;      /* 0 softmax (selection on the raw logit), 1 sigmoid (+bias) */
+    int32_t renormalize;  /* 1: weights renormalised over the selected k */
+    int32_t n_group;      /* 1 = no group-limited routing; else E % n_group == 0, n_group <= 32 */
+    int32_t topk_group;   /* groups kept when n_group > 1 */
+    int32_t group_score;  /* 0: max of the group; 1: fp32 sum of its two largest scores */
+    float scale;          /* routed scaling factor applied to the weights (1.0 = none) */
+} cap_gate_cfg;
+
+/* Topology of a candidate placement (Eq. 3: d = 0 same device, 1 same node, c across nodes). */
+typedef struct {
+    int32_t D;               /* devices */
+    int32_t N;               /* nodes */
+    const int32_t *dev_node; /* [D] device ptr: node of each device, values in [0,N) */
+    int32_t cost_local;      /* cost of staying on the token's own device (0, R7) */
+    int32_t cost_intra;      /* cost of another device on the same node (1) */
+    int32_t cost_inter;      /* cost of a device on another node (c) */
+    int64_t bytes_per_token; /* bytes one token copy moves in one direction (R12) */
+} cap_topology;
+
+/* Outputs of the placement evaluation.  Any member may be NULL (not wanted). */
+typedef struct {
+    int64_t *dev_visits;    /* [L][P] sum over tokens of |Dev(t)|: "Device per Token" x T (Fig. 6, Table III) */
+    int64_t *remote_dev;    /* [L][P] sum of |Dev(t) \ {src(t)}|: token copies sent by dispatch */
+    int64_t *remote_intra;  /* [L][P] ... of which on the source's node */
+    int64_t *remote_inter;  /* [L][P] ... of which on another node */
+    int64_t *node_visits;   /* [L][P] sum of distinct nodes: "Node per Token" x T (Table II) */
+    int64_t *remote_node;   /* [L][P] sum of distinct nodes other than the source's */
+    int64_t *cost;          /* [L][P] cost_local*local + cost_intra*remote_intra + cost_inter*remote_inter */
+    int64_t *bytes;         /* [L][P] remote_dev * bytes_per_token */
+    int64_t *load_pairs;    /* [L][P][D] kept (token,expert) pairs computed on each device (L_g of Eq. 4, R6) */
+    int64_t *recv_tokens;   /* [L][P][D] distinct tokens present on each device (local included) */
+    double *imbalance;      /* [L][P] max_d load_pairs * D / sum_d load_pairs (Eq. 4), 0 if the sum is 0 */
+    double *imbalance_recv; /* [L][P] same on recv_tokens */
+    uint8_t *tok_remote_dev;  /* [L][P][T] |Dev(t) \ {src(t)}| per token */
+    uint8_t *tok_remote_node; /* [L][P][T] distinct remote nodes per token */
+} cap_eval_out;
+
+/* S1 -- top-k gating (Eq. 1).
+ * logits [L][T][E] fp32 (finite); bias [L][E] fp32 or NULL (sigmoid scoring only: selection
+ * score = sigmoid(logit) + bias, weights from the unbiased sigmoid).
+ * topk_idx [L][T][k] int32, slot 0 = largest selection score, ties -> lower expert index;
+ * topk_w [L][T][k] fp32 routing weights (within 1e-6 of the definition).
+ * EINVAL: bias with softmax, k > topk_group*E/n_group, n_group > 32, limits above. */
+int cap_gate_topk(const float *logits, const float *bias, int32_t L, int64_t T,
+                  const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w,
+                  void *ws, size_t ws_bytes, void *stream);
+
+/* S2 -- activation counts and E x E co-activation (pruned trace P:L224).
+ * topk_idx [L][T][k]; kept [L][T][k] uint8 or NULL (all kept).
+ * counts [L][E] int64: kept (token,slot) pairs per expert.
+ * coact [L][E][E] int32, full symmetric: tokens keeping both i and j; diagonal = counts. */
+int cap_coactivation(const int32_t *topk_idx, const uint8_t *kept, int32_t L, int64_t T,
+                     int32_t k, int32_t E, int64_t *counts, int32_t *coact,
+                     void *ws, size_t ws_bytes, void *stream);
+
+/* S3 -- score P candidate placements in one pass over the trace (Eq. 3, Eq. 4,
+ * Fig. 6 axes, Tables II-IV).
+ * token_src [L][T] int32 source device of each token, or NULL = floor(t*D/T) (R5).
+ * expert_dev [L][P][E] int32 expert -> device maps, values in [0,D).
+ * counts: optional [L][E] int64 from cap_coactivation on the SAME (topk_idx, kept); when
+ * given, load_pairs is gathered from it instead of being recounted. */
+int cap_eval_placements(const int32_t *topk_idx, const uint8_t *kept, const int32_t *token_src,
+                        int32_t L, int64_t T, int32_t k, int32_t E,
+                        const int32_t *expert_dev, int32_t P, const cap_topology *topo,
+                        const int64_t *counts, const cap_eval_out *out,
+                        void *ws, size_t ws_bytes, void *stream);
+
+/* S4 -- communication-aware pruning under one placement (Eq. 6 + greedy).
+ * Per token: a_d = sum of its weights on device d (slot order, fp32); c_d = cost_local /
+ * cost_intra / cost_inter relative to token_src; devices kept by descending a_d/c_d (c_d = 0
+ * first; ties -> lower device id) while the kept sum is < 1-p.  p <= 0 keeps everything.
+ * expert_dev [L][E].  kept [L][T][k] uint8 out.  after: optional S3 outputs (P = 1) of the
+ * kept trace ("new volume and load").  near_margin [L] int64 or NULL: tokens whose deciding
+ * comparison had a margin below 1e-6 (R-S4.7).  EINVAL unless p < 1. */
+int cap_prune(const int32_t *topk_idx, const float *topk_w, const int32_t *token_src,
+              int32_t L, int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
+              const cap_topology *topo, float p, uint8_t *kept, const cap_eval_out *after,
+              int64_t *near_margin, void *ws, size_t ws_bytes, void *stream);
+
+/* S5 -- dispatch layout (P:L58 device-centric routing; BASELINE.json stage 5): stable
+ * counting sort of the kept pairs i = t*k + s by destination device expert_dev[topk_idx[i]].
+ * topk_idx [T][k]; kept [T][k] or NULL; expert_dev [E].
+ * sorted_pairs [T*k] int32 (first offsets[D] entries valid): pair ids grouped by device,
+ * ascending inside a device.  pair_pos [T*k] int32 or NULL: inverse (-1 if pruned).
+ * offsets [D+1] int64: offsets[d] = kept pairs with device < d. */
+int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T, int32_t k,
+                        int32_t E, const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs,
+                        int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes,
+                        void *stream);
+
+/* S1 + S2 + S3 in one call over the logits (the measured pass).  Arguments as in the three
+ * calls above; counts/coact/out members may be NULL to skip an output. */
+int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T,
+                    const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w,
+                    int64_t *counts, int32_t *coact, const int32_t *token_src,
+                    const int32_t *expert_dev, int32_t P, const cap_topology *topo,
+                    const cap_eval_out *out, void *ws, size_t ws_bytes, void *stream);
+
+/* Bytes of workspace the given call needs for these sizes (0 on invalid sizes). */
+size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int32_t k,
+                           int32_t D, int32_t P);
+
+/* Synchronous check that every expert_dev[l][p][e] lies in [0,D).  Returns CAP_OK, or
+ * CAP_EINVAL if a value is out of range, or CAP_ECUDA.  Blocks on `stream`. */
+int cap_validate_placements(const int32_t *expert_dev, int32_t L, int32_t P, int32_t E,
+                            int32_t D, void *stream);
+
+/* cudaError_t of the last failed launch on the calling thread (0 if none). */
+int cap_last_cuda_error(void);
+
+/* Number of kernels the library has launched since it was loaded (all threads). */
+int64_t cap_launch_count(void);
+
+/* Profiling aid (not part of the data path; not thread-safe).  cap_kernel_timer_arm(tag, slot)
+ * makes the next launch of the kernel tagged `tag` ("gate_topk", "coact", "eval", "eval_finalize",
+ * "masked_counts", "prune", "dispatch_hist", "dispatch_scan", "dispatch_scatter", "trace_fused")
+ * record a CUDA event pair, owned by the library, around itself on its stream; up to 32 arms
+ * may be pending, slot in [0,4096).  cap_kernel_timer_ms(slot) returns the elapsed device time
+ * in milliseconds once that work has completed (the caller synchronises), or -1. */
+int cap_kernel_timer_arm(const char *tag, int slot);
+float cap_kernel_timer_ms(int slot);
+
+/* Library version string (static storage). */
+const char *cap_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAP_H_ */

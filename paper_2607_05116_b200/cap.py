@@ -1,0 +1,360 @@
+"""Thin ctypes binding of libcap_b200.so (include/cap.h).  Argument marshalling only: every
+step of the path runs in the library's CUDA kernels.  torch is used for device memory and
+streams.  There is no CPU fallback: a missing library or a missing GPU raises.
+"""
+import ctypes as C
+import os
+from types import SimpleNamespace
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcap_b200.so")
+
+CALL_GATE_TOPK, CALL_COACTIVATION, CALL_EVAL_PLACEMENTS, CALL_PRUNE, CALL_DISPATCH_LAYOUT, CALL_TRACE_FUSED = range(6)
+OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
+
+EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
+           "cap_dispatch_layout", "cap_trace_fused", "cap_workspace_bytes",
+           "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
+           "cap_kernel_timer_arm", "cap_kernel_timer_ms")
+
+KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval", "eval_finalize", "prune",
+               "dispatch_hist", "dispatch_scan", "dispatch_scatter")
+
+
+class GateCfg(C.Structure):
+    _fields_ = [("E", C.c_int32), ("k", C.c_int32), ("scoring", C.c_int32),
+                ("renormalize", C.c_int32), ("n_group", C.c_int32), ("topk_group", C.c_int32),
+                ("group_score", C.c_int32), ("scale", C.c_float)]
+
+
+class Topology(C.Structure):
+    _fields_ = [("D", C.c_int32), ("N", C.c_int32), ("dev_node", C.c_void_p),
+                ("cost_local", C.c_int32), ("cost_intra", C.c_int32), ("cost_inter", C.c_int32),
+                ("bytes_per_token", C.c_int64)]
+
+
+_EVAL_I64 = ("dev_visits", "remote_dev", "remote_intra", "remote_inter", "node_visits",
+             "remote_node", "cost", "bytes")
+
+
+class EvalOut(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in _EVAL_I64 + ("load_pairs", "recv_tokens", "imbalance",
+                                                      "imbalance_recv", "tok_remote_dev",
+                                                      "tok_remote_node")]
+
+
+class CapError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib():
+    """Load libcap_b200.so (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise CapError(f"{LIB_PATH} is missing: run `python -m paper_2607_05116_b200.build` "
+                           "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.cap_workspace_bytes.restype = C.c_size_t
+        L.cap_workspace_bytes.argtypes = [C.c_int, C.c_int32, C.c_int64, C.c_int32, C.c_int32,
+                                          C.c_int32, C.c_int32]
+        L.cap_launch_count.restype = C.c_int64
+        L.cap_version.restype = C.c_char_p
+        vp, i32, i64, f32, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_float, C.c_size_t
+        L.cap_gate_topk.argtypes = [vp, vp, i32, i64, C.POINTER(GateCfg), vp, vp, vp, sz, vp]
+        L.cap_coactivation.argtypes = [vp, vp, i32, i64, i32, i32, vp, vp, vp, sz, vp]
+        L.cap_eval_placements.argtypes = [vp, vp, vp, i32, i64, i32, i32, vp, i32,
+                                          C.POINTER(Topology), vp, C.POINTER(EvalOut), vp, sz, vp]
+        L.cap_prune.argtypes = [vp, vp, vp, i32, i64, i32, i32, vp, C.POINTER(Topology), f32, vp,
+                                C.POINTER(EvalOut), vp, vp, sz, vp]
+        L.cap_dispatch_layout.argtypes = [vp, vp, i64, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
+        L.cap_trace_fused.argtypes = [vp, vp, i32, i64, C.POINTER(GateCfg), vp, vp, vp, vp, vp, vp,
+                                      i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz, vp]
+        L.cap_validate_placements.argtypes = [vp, i32, i32, i32, i32, vp]
+        L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
+        L.cap_kernel_timer_ms.argtypes = [C.c_int]
+        L.cap_kernel_timer_ms.restype = C.c_float
+        _lib = L
+    return _lib
+
+
+def launch_count() -> int:
+    return int(lib().cap_launch_count())
+
+
+def _check(rc, what):
+    if rc != OK:
+        name = {EINVAL: "CAP_EINVAL", EWORKSPACE: "CAP_EWORKSPACE", ECUDA: "CAP_ECUDA"}.get(rc, str(rc))
+        extra = f" (cudaError {lib().cap_last_cuda_error()})" if rc == ECUDA else ""
+        raise CapError(f"{what} -> {name}{extra}")
+
+
+def _ptr(t, dtype=None):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise CapError("cap: tensors must live on a CUDA device (no CPU fallback)")
+    if dtype is not None and t.dtype != dtype:
+        raise CapError(f"cap: expected dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise CapError("cap: tensors must be contiguous")
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def gate_cfg(E, k, scoring=0, renormalize=1, n_group=1, topk_group=1, group_score=0, scale=1.0):
+    return GateCfg(E, k, scoring, renormalize, n_group, topk_group, group_score, scale)
+
+
+def topology(dev_node, cost_local=0, cost_intra=1, cost_inter=1, bytes_per_token=0, N=None):
+    """dev_node: int32 CUDA tensor [D].  N must be given (or is taken from a host copy once)."""
+    D = dev_node.numel()
+    if N is None:
+        N = int(dev_node.max().item()) + 1
+    t = Topology(D, N, dev_node.data_ptr(), cost_local, cost_intra, cost_inter, bytes_per_token)
+    t._keep = dev_node
+    return t
+
+
+def workspace(which, L, T, E, k, D=1, P=0, device="cuda"):
+    n = int(lib().cap_workspace_bytes(which, L, T, E, k, D, P))
+    return torch.empty(max(n, 256), dtype=torch.uint8, device=device)
+
+
+def alloc_eval_out(L, P, D, T=0, per_token=False, device="cuda"):
+    o = SimpleNamespace()
+    for n in _EVAL_I64:
+        setattr(o, n, torch.empty((L, P), dtype=torch.int64, device=device))
+    o.load_pairs = torch.empty((L, P, D), dtype=torch.int64, device=device)
+    o.recv_tokens = torch.empty((L, P, D), dtype=torch.int64, device=device)
+    o.imbalance = torch.empty((L, P), dtype=torch.float64, device=device)
+    o.imbalance_recv = torch.empty((L, P), dtype=torch.float64, device=device)
+    o.tok_remote_dev = torch.empty((L, P, T), dtype=torch.uint8, device=device) if per_token else None
+    o.tok_remote_node = torch.empty((L, P, T), dtype=torch.uint8, device=device) if per_token else None
+    return o
+
+
+def _eval_struct(o):
+    s = EvalOut()
+    for name, _ in EvalOut._fields_:
+        t = getattr(o, name, None)
+        setattr(s, name, None if t is None else t.data_ptr())
+    return s
+
+
+def gate_topk(logits, bias, cfg, idx=None, w=None):
+    L, T, E = logits.shape
+    if idx is None:
+        idx = torch.empty((L, T, cfg.k), dtype=torch.int32, device=logits.device)
+    if w is None:
+        w = torch.empty((L, T, cfg.k), dtype=torch.float32, device=logits.device)
+    rc = lib().cap_gate_topk(_ptr(logits, torch.float32), _ptr(bias, torch.float32), L, T,
+                             C.byref(cfg), _ptr(idx), _ptr(w), None, 0, _stream())
+    _check(rc, "cap_gate_topk")
+    return idx, w
+
+
+def coactivation(idx, kept, E, counts=None, coact=None):
+    L, T, k = idx.shape
+    if counts is None:
+        counts = torch.empty((L, E), dtype=torch.int64, device=idx.device)
+    if coact is None:
+        coact = torch.empty((L, E, E), dtype=torch.int32, device=idx.device)
+    rc = lib().cap_coactivation(_ptr(idx, torch.int32), _ptr(kept, torch.uint8), L, T, k, E,
+                                _ptr(counts), _ptr(coact), None, 0, _stream())
+    _check(rc, "cap_coactivation")
+    return counts, coact
+
+
+def eval_placements(idx, kept, token_src, expert_dev, topo, counts=None, out=None, ws=None,
+                    per_token=False):
+    L, T, k = idx.shape
+    _, P, E = expert_dev.shape
+    if out is None:
+        out = alloc_eval_out(L, P, topo.D, T, per_token, idx.device)
+    if ws is None:
+        ws = workspace(CALL_EVAL_PLACEMENTS, L, T, E, k, topo.D, P, idx.device)
+    s = _eval_struct(out)
+    rc = lib().cap_eval_placements(_ptr(idx, torch.int32), _ptr(kept, torch.uint8),
+                                   _ptr(token_src, torch.int32), L, T, k, E,
+                                   _ptr(expert_dev, torch.int32), P, C.byref(topo),
+                                   _ptr(counts, torch.int64), C.byref(s), _ptr(ws), ws.numel(),
+                                   _stream())
+    _check(rc, "cap_eval_placements")
+    return out
+
+
+def prune(idx, w, token_src, expert_dev, topo, p, kept=None, after=None, near_margin=None,
+          ws=None, want_after=True):
+    L, T, k = idx.shape
+    E = expert_dev.shape[-1]
+    if kept is None:
+        kept = torch.empty((L, T, k), dtype=torch.uint8, device=idx.device)
+    if near_margin is None:
+        near_margin = torch.empty((L,), dtype=torch.int64, device=idx.device)
+    s = None
+    if want_after:
+        if after is None:
+            after = alloc_eval_out(L, 1, topo.D, T, False, idx.device)
+        if ws is None:
+            ws = workspace(CALL_PRUNE, L, T, E, k, topo.D, 1, idx.device)
+        s = _eval_struct(after)
+    rc = lib().cap_prune(_ptr(idx, torch.int32), _ptr(w, torch.float32),
+                         _ptr(token_src, torch.int32), L, T, k, E, _ptr(expert_dev, torch.int32),
+                         C.byref(topo), float(p), _ptr(kept), C.byref(s) if s is not None else None,
+                         _ptr(near_margin), _ptr(ws), 0 if ws is None else ws.numel(), _stream())
+    _check(rc, "cap_prune")
+    return kept, near_margin, after
+
+
+def dispatch_layout(idx, kept, expert_dev, D, want_pos=True, ws=None):
+    T, k = idx.shape
+    E = expert_dev.shape[0]
+    sorted_pairs = torch.empty((T * k,), dtype=torch.int32, device=idx.device)
+    pair_pos = torch.empty((T * k,), dtype=torch.int32, device=idx.device) if want_pos else None
+    offsets = torch.empty((D + 1,), dtype=torch.int64, device=idx.device)
+    if ws is None:
+        ws = workspace(CALL_DISPATCH_LAYOUT, 1, T, E, k, D, 0, idx.device)
+    rc = lib().cap_dispatch_layout(_ptr(idx, torch.int32), _ptr(kept, torch.uint8), T, k, E,
+                                   _ptr(expert_dev, torch.int32), D, _ptr(sorted_pairs),
+                                   _ptr(pair_pos), _ptr(offsets), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "cap_dispatch_layout")
+    return sorted_pairs, offsets, pair_pos
+
+
+class FusedBuffers:
+    """Pre-allocated outputs + workspace of cap_trace_fused for fixed sizes."""
+
+    def __init__(self, L, T, E, k, D, P, device="cuda", per_token=False):
+        self.idx = torch.empty((L, T, k), dtype=torch.int32, device=device)
+        self.w = torch.empty((L, T, k), dtype=torch.float32, device=device)
+        self.counts = torch.empty((L, E), dtype=torch.int64, device=device)
+        self.coact = torch.empty((L, E, E), dtype=torch.int32, device=device)
+        self.out = alloc_eval_out(L, P, D, T, per_token, device)
+        self.ws = workspace(CALL_TRACE_FUSED, L, T, E, k, D, P, device)
+        self.out_struct = _eval_struct(self.out)
+
+
+def trace_fused(logits, bias, cfg, token_src, expert_dev, topo, bufs=None, per_token=False):
+    L, T, E = logits.shape
+    P = expert_dev.shape[1]
+    if bufs is None:
+        bufs = FusedBuffers(L, T, E, cfg.k, topo.D, P, logits.device, per_token)
+    rc = lib().cap_trace_fused(_ptr(logits, torch.float32), _ptr(bias, torch.float32), L, T,
+                               C.byref(cfg), _ptr(bufs.idx), _ptr(bufs.w), _ptr(bufs.counts),
+                               _ptr(bufs.coact), _ptr(token_src, torch.int32),
+                               _ptr(expert_dev, torch.int32), P, C.byref(topo),
+                               C.byref(bufs.out_struct), _ptr(bufs.ws), bufs.ws.numel(), _stream())
+    _check(rc, "cap_trace_fused")
+    return bufs
+
+
+def validate_placements(expert_dev, D):
+    L, P, E = expert_dev.shape
+    return int(lib().cap_validate_placements(_ptr(expert_dev, torch.int32), L, P, E, D, _stream()))
+
+
+def kernel_timer_arm(tag: str, slot: int):
+    _check(lib().cap_kernel_timer_arm(tag.encode(), slot), "cap_kernel_timer_arm")
+
+
+def kernel_timer_ms(slot: int) -> float:
+    return float(lib().cap_kernel_timer_ms(slot))
+
+
+class Pipeline:
+    """The whole hot path for fixed sizes, on resident device buffers: cap_trace_fused (S1+S2+S3
+    over P candidates) -> cap_prune under candidate `chosen` (S4, with the after-metrics) ->
+    cap_dispatch_layout per layer for the same candidate (S5).  Holds every output buffer and
+    workspace, so step() only enqueues kernels."""
+
+    def __init__(self, L, T, gate, D, N, P, dev_node, cost_inter=1, bytes_per_token=0, tau=0.1,
+                 chosen=0, device="cuda"):
+        self.L, self.T, self.P, self.D, self.tau, self.chosen = L, T, P, D, tau, chosen
+        self.gate = gate
+        E, k = gate.E, gate.k
+        self.dev_node = dev_node
+        self.topo = topology(dev_node, 0, 1, cost_inter, bytes_per_token, N=N)
+        self.fb = FusedBuffers(L, T, E, k, D, P, device)
+        self.kept = torch.empty((L, T, k), dtype=torch.uint8, device=device)
+        self.near = torch.empty((L,), dtype=torch.int64, device=device)
+        self.after = alloc_eval_out(L, 1, D, T, False, device)
+        self.after_struct = _eval_struct(self.after)
+        self.ws_prune = workspace(CALL_PRUNE, L, T, E, k, D, 1, device)
+        self.sorted_pairs = torch.empty((L, T * k), dtype=torch.int32, device=device)
+        self.pair_pos = torch.empty((L, T * k), dtype=torch.int32, device=device)
+        self.offsets = torch.empty((L, D + 1), dtype=torch.int64, device=device)
+        self.ws_disp = workspace(CALL_DISPATCH_LAYOUT, 1, T, E, k, D, 0, device)
+        self.pi = torch.empty((L, E), dtype=torch.int32, device=device)
+
+    def step(self, logits, bias, token_src, expert_dev):
+        L, T = self.L, self.T
+        E, k = self.gate.E, self.gate.k
+        trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)
+        self.pi.copy_(expert_dev[:, self.chosen, :])
+        st = _stream()
+        rc = lib().cap_prune(_ptr(self.fb.idx), _ptr(self.fb.w), _ptr(token_src, torch.int32), L, T, k, E,
+                             _ptr(self.pi), C.byref(self.topo), float(self.tau), _ptr(self.kept),
+                             C.byref(self.after_struct), _ptr(self.near), _ptr(self.ws_prune),
+                             self.ws_prune.numel(), st)
+        _check(rc, "cap_prune")
+        for l in range(L):
+            rc = lib().cap_dispatch_layout(_ptr(self.fb.idx[l]), _ptr(self.kept[l]), T, k, E,
+                                           _ptr(self.pi[l]), self.D, _ptr(self.sorted_pairs[l]),
+                                           _ptr(self.pair_pos[l]), _ptr(self.offsets[l]),
+                                           _ptr(self.ws_disp), self.ws_disp.numel(), st)
+            _check(rc, "cap_dispatch_layout")
+        return self
+
+    def result_tensors(self):
+        """Every output of a step (what a host caller reads back)."""
+        o, a = self.fb.out, self.after
+        ts = [self.fb.idx, self.fb.w, self.fb.counts, self.fb.coact, self.kept, self.near,
+              self.sorted_pairs, self.pair_pos, self.offsets]
+        for ns in (o, a):
+            for name, _ in EvalOut._fields_:
+                t = getattr(ns, name, None)
+                if t is not None:
+                    ts.append(t)
+        return ts
+
+
+class HostPipeline:
+    """The same step driven from HOST buffers (the end-to-end call): pinned host inputs are copied
+    to the device, the step runs, every output is copied back to pinned host memory."""
+
+    def __init__(self, pipe: Pipeline, has_bias=False, has_src=False):
+        self.pipe = pipe
+        L, T, P = pipe.L, pipe.T, pipe.P
+        E = pipe.gate.E
+        dev = pipe.kept.device
+        self.d_logits = torch.empty((L, T, E), dtype=torch.float32, device=dev)
+        self.d_maps = torch.empty((L, P, E), dtype=torch.int32, device=dev)
+        self.d_bias = torch.empty((L, E), dtype=torch.float32, device=dev) if has_bias else None
+        self.d_src = torch.empty((L, T), dtype=torch.int32, device=dev) if has_src else None
+        self.h_out = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for t in pipe.result_tensors()]
+        self.d2h_bytes = sum(t.numel() * t.element_size() for t in self.h_out)
+
+    def h2d_bytes(self, logits, maps, bias=None, src=None):
+        return sum(t.numel() * t.element_size() for t in (logits, maps, bias, src) if t is not None)
+
+    def step(self, h_logits, h_maps, h_bias=None, h_src=None):
+        self.d_logits.copy_(h_logits, non_blocking=True)
+        self.d_maps.copy_(h_maps, non_blocking=True)
+        if h_bias is not None:
+            self.d_bias.copy_(h_bias, non_blocking=True)
+        if h_src is not None:
+            self.d_src.copy_(h_src, non_blocking=True)
+        self.pipe.step(self.d_logits, self.d_bias if h_bias is not None else None,
+                       self.d_src if h_src is not None else None, self.d_maps)
+        for h, d in zip(self.h_out, self.pipe.result_tensors()):
+            h.copy_(d, non_blocking=True)
+        return self.h_out

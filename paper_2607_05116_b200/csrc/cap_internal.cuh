@@ -1,0 +1,101 @@
+// Internal declarations shared by the CUDA translation units of libcap_b200.so.
+// Nothing here is shared with oracle/ (the CPU oracle is an independent restatement).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "cap.h"
+
+namespace cap {
+
+// ---- host-side launch bookkeeping -------------------------------------------------------
+void note_launch(int n = 1);            // counts kernels launched (cap_launch_count)
+int check_launch(const char *what);     // cudaGetLastError -> CAP_OK / CAP_ECUDA (records it)
+int sm_count();                         // SMs of the current device (cached)
+
+// Optional profiling aid (cap_kernel_timer_arm): records a cudaEvent pair around the next launch
+// of the kernel with the armed tag.  Costs one table scan per launch when nothing is armed.
+struct KernelTimerScope {
+    KernelTimerScope(const char *tag, cudaStream_t st);
+    ~KernelTimerScope();
+    int slot_;
+    cudaStream_t st_;
+};
+
+#define CAP_TRY(expr)                      \
+    do {                                   \
+        int _rc = (expr);                  \
+        if (_rc != CAP_OK) return _rc;     \
+    } while (0)
+
+// ---- accumulator slots of the evaluation (ws, int64 per (layer, candidate)) --------------
+enum { ACC_DEV = 0, ACC_LOCAL = 1, ACC_SAMENODE = 2, ACC_NODE = 3, ACC_RNODE = 4, ACC_N = 8 };
+
+struct EvalWs {
+    unsigned long long *acc;      // [L][P][ACC_N]
+    unsigned long long *recv;     // [L][P][D]
+    unsigned long long *mcounts;  // [L][E] kept pairs per expert (when the caller gave none)
+};
+
+size_t eval_ws_bytes(int32_t L, int32_t E, int32_t D, int32_t P);
+EvalWs eval_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P);
+
+// ---- stage launchers (arguments already validated) ---------------------------------------
+int launch_gate_topk(const float *logits, const float *bias, int32_t L, int64_t T,
+                     const cap_gate_cfg &cfg, int32_t *idx, float *w, cudaStream_t st);
+int launch_coactivation(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
+                        int32_t E, int64_t *counts, int32_t *coact, cudaStream_t st);
+int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_src, int32_t L,
+                int64_t T, int32_t k, int32_t E, const int32_t *expert_dev, int32_t P,
+                int64_t layer_stride_maps, const cap_topology &topo, const int64_t *counts,
+                const cap_eval_out &out, void *ws, cudaStream_t st);
+int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
+                 int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
+                 const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,
+                 cudaStream_t st);
+size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D);
+int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,
+                    const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
+                    int64_t *offsets, void *ws, cudaStream_t st);
+
+// ---- device helpers ------------------------------------------------------------------------
+// Reproducible fp32 exponential (DESIGN.md R-S1.3): IEEE-exact operations only.
+__device__ __forceinline__ float exp_s(float x)
+{
+    float t = fminf(fmaxf(x, -87.0f), 87.0f);
+    float n = rintf(__fmul_rn(t, 0x1.715476p+0f));
+    float r = __fmaf_rn(n, -0x1.62ep-1f, t);
+    r = __fmaf_rn(n, -0x1.0bfbe8p-15f, r);
+    float p = 0x1.a01a02p-13f;
+    p = __fmaf_rn(p, r, 0x1.6c16c2p-10f);
+    p = __fmaf_rn(p, r, 0x1.111112p-7f);
+    p = __fmaf_rn(p, r, 0x1.555556p-5f);
+    p = __fmaf_rn(p, r, 0x1.555556p-3f);
+    p = __fmaf_rn(p, r, 0x1p-1f);
+    p = __fmaf_rn(p, r, 1.0f);
+    p = __fmaf_rn(p, r, 1.0f);
+    int ni = __float2int_rn(n);
+    return __fmul_rn(p, __int_as_float((ni + 127) << 23));
+}
+
+__device__ __forceinline__ float sig_s(float x)
+{
+    return __fdiv_rn(1.0f, __fadd_rn(1.0f, exp_s(-x)));
+}
+
+// Order-preserving map fp32 -> u32 (larger float <=> larger key); -0 is folded onto +0 so that
+// the two compare equal as IEEE says.  Every finite float gets a key > 0: key 0 means "absent".
+__device__ __forceinline__ uint32_t okey(float x)
+{
+    uint32_t b = __float_as_uint(x);
+    if (b == 0x80000000u) b = 0u;
+    return b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
+}
+
+__device__ __forceinline__ float unkey(uint32_t key)
+{
+    uint32_t b = (key & 0x80000000u) ? (key ^ 0x80000000u) : ~key;
+    return __uint_as_float(b);
+}
+
+}  // namespace cap

@@ -1,0 +1,204 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Integers bit-exact, gate weights within 1e-6 absolute."""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+from oracle import cap_oracle as O                      # noqa: E402
+from paper_2607_05116_b200 import cap                   # noqa: E402
+from paper_2607_05116_b200 import workload as W         # noqa: E402
+from parity_util import (assert_eval_equal, check_all_stages, check_gate, dev, host,  # noqa: E402
+                         topo_of)
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    cap.lib()
+
+
+# ------------------------------------------------------------------ the five BASELINE configs
+def test_config1_tiny_all_stages():
+    cfg = W.CONFIGS["tiny"]
+    check_all_stages(cfg, per_token=True, tag="tiny ")
+    check_all_stages(cfg, random_src=True, per_token=True, tag="tiny/src ")
+
+
+def test_config2_qwen3_two_layers_full_T():
+    cfg = W.CONFIGS["qwen3"]
+    rep = check_all_stages(cfg, layers=(0, 17), tag="qwen3 ")
+    assert rep["w_max_abs_diff"] <= 1e-6
+
+
+def test_config3_target_full_size():
+    cfg = W.CONFIGS["target"]
+    rep = check_all_stages(cfg, tag="target ")
+    print("target report", rep)
+    check_all_stages(cfg, T=4099, random_src=True, per_token=True, tag="target/ragged ")
+
+
+def test_config4_dsv3_two_layers_full_T():
+    cfg = W.CONFIGS["dsv3"]
+    rep = check_all_stages(cfg, layers=(0, 31), tag="dsv3 ")
+    print("dsv3 report", rep)
+
+
+def test_config5_stress_2pow16():
+    cfg = W.CONFIGS["stress"]
+    rep = check_all_stages(cfg, tag="stress ")
+    print("stress report", rep)
+
+
+# ------------------------------------------------------------------ S1 edge cases
+@pytest.mark.parametrize("E,k", [(1, 1), (7, 7), (16, 2), (33, 4), (40, 5), (64, 6), (100, 8), (128, 8),
+                                 (130, 8), (256, 8), (260, 16), (512, 10), (1000, 12), (1024, 16)])
+def test_gate_shapes_and_ties(E, k):
+    rng = np.random.default_rng(E * 31 + k)
+    T = 777
+    x = rng.normal(0, 1, (2, T, E)).astype(np.float32)
+    x[1] = np.round(x[1] * 2) / 2                    # heavy exact ties
+    x[0, :5] = 0.25                                   # all-equal rows
+    x[0, 5, : min(E, 3)] = -0.0                       # -0 / +0
+    x[0, 5, min(E, 3):] = 0.0
+    for gate in (dict(k=k), dict(k=k, renormalize=0), dict(k=k, scale=2.5),
+                 dict(k=k, scoring=1), dict(k=k, scoring=1, renormalize=0)):
+        check_gate(x, None, gate, tag=f"E{E}k{k} {gate} ")
+
+
+@pytest.mark.parametrize("group_score", [0, 1])
+@pytest.mark.parametrize("E,n_group,topk_group,k", [(64, 8, 3, 6), (256, 8, 4, 8), (96, 32, 9, 8), (16, 2, 1, 2)])
+def test_gate_group_limited(E, n_group, topk_group, k, group_score):
+    rng = np.random.default_rng(E + n_group)
+    x = rng.normal(0, 1.3, (2, 500, E)).astype(np.float32)
+    x[1, :100] = np.round(x[1, :100] * 2) / 2
+    bias = rng.uniform(-0.05, 0.05, (2, E)).astype(np.float32)
+    g = dict(k=k, n_group=n_group, topk_group=topk_group, group_score=group_score)
+    check_gate(x, bias, dict(scoring=1, **g))
+    check_gate(x, None, dict(scoring=0, **g))
+
+
+def test_gate_empty_and_single():
+    cfg = cap.gate_cfg(128, 8)
+    idx, w = cap.gate_topk(torch.empty((1, 0, 128), device="cuda"), None, cfg)
+    assert idx.shape == (1, 0, 8)
+    x = np.random.default_rng(0).normal(0, 1, (1, 1, 128)).astype(np.float32)
+    check_gate(x, None, dict(k=8))
+
+
+# ------------------------------------------------------------------ S2/S3/S4/S5 edge cases
+def _trace(rng, L, T, E, k):
+    return np.stack([np.stack([rng.permutation(E)[:k] for _ in range(T)]) for _ in range(L)]).astype(np.int32)
+
+
+@pytest.mark.parametrize("E,k,T", [(8, 3, 5), (16, 2, 1), (24, 5, 1033), (200, 8, 700), (256, 8, 3000), (512, 10, 900)])
+def test_coact_masked_and_shapes(E, k, T):
+    rng = np.random.default_rng(E + T)
+    idx = _trace(rng, 2, T, E, k)
+    kept = (rng.random((2, T, k)) < 0.6).astype(np.uint8)
+    kept[0, 0] = 0
+    for m in (None, kept, np.zeros_like(kept)):
+        cnt_r, C_r = O.coactivation(idx, m, E=E)
+        cnt_d, C_d = cap.coactivation(dev(idx), dev(m), E)
+        assert np.array_equal(host(cnt_d), cnt_r) and np.array_equal(host(C_d), C_r)
+    cnt_d, C_d = cap.coactivation(dev(idx[:, :0]), None, E)          # T = 0 -> zeros
+    assert int(cnt_d.sum()) == 0 and int(C_d.sum()) == 0
+
+
+@pytest.mark.parametrize("E,k,D,N,P,T", [(16, 2, 1, 1, 3, 100), (32, 4, 8, 4, 5, 257), (64, 6, 64, 8, 33, 1000),
+                                         (128, 8, 16, 2, 300, 2048), (512, 10, 64, 8, 70, 500), (1024, 16, 64, 64, 40, 300)])
+def test_eval_generic_unbalanced_maps(E, k, D, N, P, T):
+    rng = np.random.default_rng(E * 7 + D)
+    L = 2
+    idx = _trace(rng, L, T, E, k)
+    kept = (rng.random((L, T, k)) < 0.7).astype(np.uint8)
+    pis = rng.integers(0, D, (L, P, E)).astype(np.int32)
+    pis[0, 0] = 0                                           # everything on device 0
+    dn = np.sort(rng.integers(0, N, D)).astype(np.int32)
+    dn[0], dn[-1] = 0, N - 1
+    src = rng.integers(0, D, (L, T)).astype(np.int32)
+    topo = cap.topology(dev(dn), cost_local=2, cost_intra=3, cost_inter=7, bytes_per_token=4096, N=N)
+    for m, s in ((None, None), (kept, src), (np.zeros_like(kept), src)):
+        ref = O.eval_placements(idx, pis, dn, kept=m, token_src=s, cost_local=2, cost_intra=3,
+                                cost_inter=7, bytes_per_token=4096, per_token=True)
+        got = cap.eval_placements(dev(idx), dev(m), dev(s), dev(pis), topo, per_token=True)
+        assert_eval_equal(got, ref, True, f"E{E} D{D} ")
+    assert cap.validate_placements(dev(pis), D) == cap.OK
+    bad = pis.copy()
+    bad[1, P - 1, E - 1] = D
+    assert cap.validate_placements(dev(bad), D) == cap.EINVAL
+
+
+@pytest.mark.parametrize("k", [1, 3, 8, 16])
+def test_prune_edge_cases(k):
+    rng = np.random.default_rng(100 + k)
+    L, T, E, D = 2, 1500, 64, 16
+    idx = _trace(rng, L, T, E, k)
+    w = rng.random((L, T, k)).astype(np.float32) + np.float32(0.02)
+    w = -np.sort(-w, axis=-1)
+    w = (w / w.sum(-1, keepdims=True, dtype=np.float32)).astype(np.float32)
+    w[0, :50] = np.float32(1.0 / k)                       # exact ratio ties
+    pi = np.stack([rng.permutation(E) % D for _ in range(L)]).astype(np.int32)
+    dn = (np.arange(D) // 4).astype(np.int32)
+    src = rng.integers(0, D, (L, T)).astype(np.int32)
+    for costs in ((0, 1, 4), (1, 1, 1), (0, 0, 3), (2, 1, 5)):
+        topo = cap.topology(dev(dn), *costs, bytes_per_token=64, N=4)
+        for p in (0.0, -1.0, 0.05, 0.3, 0.5, 0.999):
+            for s in (None, src):
+                kept_r, near_r = O.prune(idx, w, pi, dn, p, token_src=s, cost_local=costs[0],
+                                         cost_intra=costs[1], cost_inter=costs[2])
+                kept_d, near_d, aft = cap.prune(dev(idx), dev(w), dev(s), dev(pi), topo, p)
+                assert np.array_equal(host(kept_d), kept_r), (costs, p)
+                assert np.array_equal(host(near_d), near_r), (costs, p)
+                ref = O.eval_placements(idx, pi[:, None], dn, kept=kept_r, token_src=s, cost_local=costs[0],
+                                        cost_intra=costs[1], cost_inter=costs[2], bytes_per_token=64)
+                assert_eval_equal(aft, ref, False, f"after {costs} {p} ")
+
+
+@pytest.mark.parametrize("T,k,E,D", [(1, 1, 4, 2), (5, 3, 8, 4), (2048, 1, 16, 3), (4097, 8, 128, 16), (30000, 10, 512, 64)])
+def test_dispatch_edge_cases(T, k, E, D):
+    rng = np.random.default_rng(T + D)
+    idx = _trace(rng, 1, T, E, k)[0]
+    pi = rng.integers(0, D, E).astype(np.int32)
+    pi[rng.integers(0, E)] = D - 1
+    kept = (rng.random((T, k)) < 0.5).astype(np.uint8)
+    for m in (None, kept, np.zeros_like(kept)):
+        sp_r, off_r, pos_r = O.dispatch_layout(idx, pi, D, kept=m)
+        sp_d, off_d, pos_d = cap.dispatch_layout(dev(idx), dev(m), dev(pi), D)
+        n = int(off_r[-1])
+        assert np.array_equal(host(off_d), off_r)
+        assert np.array_equal(host(sp_d)[:n], sp_r)
+        assert np.array_equal(host(pos_d), pos_r)
+    sp_d, off_d, _ = cap.dispatch_layout(dev(idx[:0]), None, dev(pi), D)
+    assert host(off_d).tolist() == [0] * (D + 1)
+
+
+def test_error_codes():
+    x = torch.zeros((1, 4, 16), device="cuda")
+    b = torch.zeros((1, 16), device="cuda")
+    with pytest.raises(cap.CapError, match="EINVAL"):
+        cap.gate_topk(x, b, cap.gate_cfg(16, 2, scoring=0))            # bias with softmax
+    with pytest.raises(cap.CapError, match="EINVAL"):
+        cap.gate_topk(x, None, cap.gate_cfg(16, 17))
+    with pytest.raises(cap.CapError, match="EINVAL"):
+        cap.gate_topk(x, None, cap.gate_cfg(16, 5, n_group=4, topk_group=1))
+    idx = torch.zeros((1, 4, 2), dtype=torch.int32, device="cuda")
+    w = torch.full((1, 4, 2), 0.5, device="cuda")
+    dn = torch.zeros(4, dtype=torch.int32, device="cuda")
+    pi = torch.zeros((1, 16), dtype=torch.int32, device="cuda")
+    topo = cap.topology(dn, N=1)
+    with pytest.raises(cap.CapError, match="EINVAL"):
+        cap.prune(idx, w, None, pi, topo, 1.0)
+    with pytest.raises(cap.CapError, match="EWORKSPACE"):
+        cap.eval_placements(idx, None, None, pi[None], topo, ws=torch.empty(8, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(cap.CapError, match="CUDA device"):
+        cap.gate_topk(x.cpu(), None, cap.gate_cfg(16, 2))             # no CPU fallback
+
+
+def test_launch_counter_moves():
+    n0 = cap.launch_count()
+    x = torch.zeros((1, 64, 16), device="cuda")
+    cap.gate_topk(x, None, cap.gate_cfg(16, 2))
+    torch.cuda.synchronize()
+    assert cap.launch_count() == n0 + 1
