@@ -169,8 +169,9 @@ int64_t cap_launch_count(void);
 
 /* Profiling aid (not part of the data path; not thread-safe).  cap_kernel_timer_arm(tag, slot)
  * makes the next launch of the kernel tagged `tag` ("gate_topk", "coact", "eval", "eval_finalize",
- * "masked_counts", "prune", "dispatch_hist", "dispatch_scan", "dispatch_scatter", "trace_fused")
- * record a CUDA event pair, owned by the library, around itself on its stream; up to 32 arms
+ * "eval_table", "eval_decode", "masked_counts", "prune", "dispatch_hist", "dispatch_scan",
+ * "dispatch_scatter", "trace_fused")
+ * record a CUDA event pair, owned by the library, around itself on its stream; up to 128 arms
  * may be pending, slot in [0,4096).  cap_kernel_timer_ms(slot) returns the elapsed device time
  * in milliseconds once that work has completed (the caller synchronises), or -1. */
 int cap_kernel_timer_arm(const char *tag, int slot);

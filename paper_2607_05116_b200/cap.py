@@ -19,7 +19,7 @@ EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prun
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms")
 
-KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval", "eval_finalize", "prune",
+KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter")
 
 
@@ -314,6 +314,29 @@ class Pipeline:
             _check(rc, "cap_dispatch_layout")
         return self
 
+    def capture(self, logits, bias, token_src, expert_dev):
+        """Capture one step on these (fixed) input buffers into a CUDA graph: the library only
+        enqueues work on the current stream, so a step is capturable as is.  Returns the graph;
+        replay() re-runs the whole step with no host-side launch cost."""
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            self.step(logits, bias, token_src, expert_dev)      # one-time attribute setup outside capture
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            self.step(logits, bias, token_src, expert_dev)
+        return g
+
+    def capture_fused(self, logits, bias, token_src, expert_dev):
+        """Graph of the cap_trace_fused call alone (S1+S2+S3), for timing the fused pass."""
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)
+        return g
+
     def result_tensors(self):
         """Every output of a step (what a host caller reads back)."""
         o, a = self.fb.out, self.after
@@ -342,6 +365,11 @@ class HostPipeline:
         self.d_src = torch.empty((L, T), dtype=torch.int32, device=dev) if has_src else None
         self.h_out = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for t in pipe.result_tensors()]
         self.d2h_bytes = sum(t.numel() * t.element_size() for t in self.h_out)
+        self.graph = None
+
+    def capture(self):
+        """Capture the device part of the step (on the staging buffers) into a CUDA graph."""
+        self.graph = self.pipe.capture(self.d_logits, self.d_bias, self.d_src, self.d_maps)
 
     def h2d_bytes(self, logits, maps, bias=None, src=None):
         return sum(t.numel() * t.element_size() for t in (logits, maps, bias, src) if t is not None)
@@ -353,8 +381,11 @@ class HostPipeline:
             self.d_bias.copy_(h_bias, non_blocking=True)
         if h_src is not None:
             self.d_src.copy_(h_src, non_blocking=True)
-        self.pipe.step(self.d_logits, self.d_bias if h_bias is not None else None,
-                       self.d_src if h_src is not None else None, self.d_maps)
+        if self.graph is not None:
+            self.graph.replay()
+        else:
+            self.pipe.step(self.d_logits, self.d_bias if h_bias is not None else None,
+                           self.d_src if h_src is not None else None, self.d_maps)
         for h, d in zip(self.h_out, self.pipe.result_tensors()):
             h.copy_(d, non_blocking=True)
         return self.h_out

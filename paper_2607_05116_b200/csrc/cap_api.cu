@@ -37,7 +37,7 @@ int sm_count()
 
 // ---- kernel timer table -------------------------------------------------------------------
 constexpr int KT_SLOTS = 4096;
-constexpr int KT_ARMED = 32;
+constexpr int KT_ARMED = 128;
 struct KtSlot { cudaEvent_t a = nullptr, b = nullptr; int state = 0; };   // state 2 = both recorded
 struct KtArm { char tag[32]; int slot; bool on; };
 static KtSlot g_kt[KT_SLOTS];
@@ -120,6 +120,8 @@ int cap_kernel_timer_arm(const char *tag, int slot)
             return check_launch("event create");
     }
     g_kt[slot].state = 0;
+    for (int i = 0; i < KT_ARMED; ++i)
+        if (g_arm[i].on && g_arm[i].slot == slot && strcmp(g_arm[i].tag, tag) == 0) return CAP_OK;
     for (int i = 0; i < KT_ARMED; ++i) {
         if (!g_arm[i].on) {
             strcpy(g_arm[i].tag, tag);
@@ -158,10 +160,10 @@ size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int3
     case CAP_CALL_EVAL_PLACEMENTS:
     case CAP_CALL_TRACE_FUSED:
         if (D < 1 || P < 0) return 0;
-        return eval_ws_bytes(L, E, D, P);
+        return eval_ws_bytes(L, T, E, k, D, P);
     case CAP_CALL_PRUNE:
         if (D < 1) return 0;
-        return eval_ws_bytes(L, E, D, 1);
+        return eval_ws_bytes(L, T, E, k, D, 1);
     case CAP_CALL_DISPATCH_LAYOUT:
         if (D < 1) return 0;
         return dispatch_ws_bytes(T, k, D);
@@ -198,7 +200,7 @@ int cap_eval_placements(const int32_t *topk_idx, const uint8_t *kept, const int3
     if ((int64_t)L * P > 0 && !expert_dev) return CAP_EINVAL;
     if ((int64_t)L * T > 0 && !topk_idx) return CAP_EINVAL;
     if ((int64_t)L * P >= ((int64_t)1 << 31)) return CAP_EINVAL;
-    if (!ws || ws_bytes < eval_ws_bytes(L, E, topo->D, P)) return CAP_EWORKSPACE;
+    if (!ws || ws_bytes < eval_ws_bytes(L, T, E, k, topo->D, P)) return CAP_EWORKSPACE;
     return launch_eval(topk_idx, kept, token_src, L, T, k, E, expert_dev, P, (int64_t)P * E, *topo,
                        counts, *out, ws, (cudaStream_t)stream);
 }
@@ -212,7 +214,7 @@ int cap_prune(const int32_t *topk_idx, const float *topk_w, const int32_t *token
     if (!(p < 1.0f)) return CAP_EINVAL;   // also rejects NaN
     if (L > 0 && !expert_dev) return CAP_EINVAL;
     if ((int64_t)L * T > 0 && (!topk_idx || !topk_w || !kept)) return CAP_EINVAL;
-    if (after && (!ws || ws_bytes < eval_ws_bytes(L, E, topo->D, 1))) return CAP_EWORKSPACE;
+    if (after && (!ws || ws_bytes < eval_ws_bytes(L, T, E, k, topo->D, 1))) return CAP_EWORKSPACE;
     CAP_TRY(launch_prune(topk_idx, topk_w, token_src, L, T, k, E, expert_dev, *topo, p, kept,
                          near_margin, (cudaStream_t)stream));
     if (after)
@@ -245,7 +247,7 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
     if (L > 0 && (!counts || !coact)) return CAP_EINVAL;
     if ((int64_t)L * P > 0 && !expert_dev) return CAP_EINVAL;
     if ((int64_t)L * P >= ((int64_t)1 << 31)) return CAP_EINVAL;
-    if (!ws || ws_bytes < eval_ws_bytes(L, cfg->E, topo->D, P)) return CAP_EWORKSPACE;
+    if (!ws || ws_bytes < eval_ws_bytes(L, T, cfg->E, cfg->k, topo->D, P)) return CAP_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
     CAP_TRY(launch_gate_topk(logits, bias, L, T, *cfg, topk_idx, topk_w, st));
     CAP_TRY(launch_coactivation(topk_idx, nullptr, L, T, cfg->k, cfg->E, counts, coact, st));

@@ -8,10 +8,10 @@
 
 namespace cap {
 
-size_t eval_ws_bytes(int32_t L, int32_t E, int32_t D, int32_t P)
+size_t eval_ws_bytes(int32_t L, int64_t T, int32_t E, int32_t k, int32_t D, int32_t P)
 {
     size_t n = (size_t)L * P * ACC_N + (size_t)L * P * D + (size_t)L * E;
-    return n * sizeof(unsigned long long) + 256;
+    return n * sizeof(unsigned long long) + 512 + eval_fast_ws_bytes(L, T, k, E, D, P);
 }
 
 EvalWs eval_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P)
@@ -190,11 +190,48 @@ struct FinalParams {
     long long bytes_per_token;
 };
 
-__global__ void eval_finalize_kernel(FinalParams f)
+// One warp per (layer, candidate): lanes stride over the experts (coalesced map and count reads),
+// per-device sums in shared memory, then lanes stride over the devices.
+constexpr int FIN_WARPS = 4;
+__global__ void __launch_bounds__(32 * FIN_WARPS) eval_finalize_kernel(FinalParams f)
 {
-    const int o = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ unsigned long long s_lp[FIN_WARPS][64];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int o = blockIdx.x * FIN_WARPS + warp;
     if (o >= f.L * f.P) return;
     const int layer = o / f.P;
+    unsigned long long *lp = s_lp[warp];
+    lp[lane] = 0ull;
+    lp[lane + 32] = 0ull;
+    __syncwarp();
+    // load_pairs[d] = sum of the (kept) counts of the experts placed on d
+    const int32_t *pi = f.expert_dev + (size_t)o * f.E;
+    const long long *cnt = f.counts + (size_t)layer * f.E;
+    for (int e = lane; e < f.E; e += 32) {
+        const int d = pi[e];
+        const long long c = cnt[e];
+        if (d >= 0 && d < f.D && c) atomicAdd(&lp[d], (unsigned long long)c);
+    }
+    __syncwarp();
+    long long mx = 0, sm = 0, mxr = 0, smr = 0;
+    for (int d = lane; d < f.D; d += 32) {
+        const long long l = (long long)lp[d];
+        const long long r = (long long)f.recv[(size_t)o * f.D + d];
+        if (f.out.load_pairs) f.out.load_pairs[(size_t)o * f.D + d] = l;
+        if (f.out.recv_tokens) f.out.recv_tokens[(size_t)o * f.D + d] = r;
+        mx = max(mx, l);
+        sm += l;
+        mxr = max(mxr, r);
+        smr += r;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, off));
+        mxr = max(mxr, __shfl_xor_sync(0xffffffffu, mxr, off));
+        sm += __shfl_xor_sync(0xffffffffu, sm, off);
+        smr += __shfl_xor_sync(0xffffffffu, smr, off);
+    }
+    if (lane != 0) return;
     const unsigned long long *a = f.acc + (size_t)o * ACC_N;
     const long long dv = (long long)a[ACC_DEV], loc = (long long)a[ACC_LOCAL],
                     same = (long long)a[ACC_SAMENODE];
@@ -209,25 +246,6 @@ __global__ void eval_finalize_kernel(FinalParams f)
         f.out.cost[o] = (long long)f.cost_local * loc + (long long)f.cost_intra * intra +
                         (long long)f.cost_inter * inter;
     if (f.out.bytes) f.out.bytes[o] = rdev * f.bytes_per_token;
-    // load_pairs[d] = sum of the (kept) counts of the experts placed on d
-    long long lp[64];
-    for (int d = 0; d < f.D; ++d) lp[d] = 0;
-    const int32_t *pi = f.expert_dev + (size_t)o * f.E;
-    const long long *cnt = f.counts + (size_t)layer * f.E;
-    for (int e = 0; e < f.E; ++e) {
-        int d = pi[e];
-        if (d >= 0 && d < f.D) lp[d] += cnt[e];
-    }
-    long long mx = 0, sm = 0, mxr = 0, smr = 0;
-    for (int d = 0; d < f.D; ++d) {
-        long long r = (long long)f.recv[(size_t)o * f.D + d];
-        if (f.out.load_pairs) f.out.load_pairs[(size_t)o * f.D + d] = lp[d];
-        if (f.out.recv_tokens) f.out.recv_tokens[(size_t)o * f.D + d] = r;
-        mx = max(mx, lp[d]);
-        sm += lp[d];
-        mxr = max(mxr, r);
-        smr += r;
-    }
     if (f.out.imbalance) f.out.imbalance[o] = sm ? __ddiv_rn((double)(mx * f.D), (double)sm) : 0.0;
     if (f.out.imbalance_recv)
         f.out.imbalance_recv[o] = smr ? __ddiv_rn((double)(mxr * f.D), (double)smr) : 0.0;
@@ -265,6 +283,9 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
             note_launch();
             CAP_TRY(check_launch("masked_counts_kernel"));
         }
+        bool fast = false;
+        if (!token_src && !want_tok)
+            CAP_TRY(launch_eval_fast(idx, kept, L, T, k, E, expert_dev, P, topo, ws, st, &fast));
         int PC = 256;
         while (PC > 32 && eval_smem_bytes(E, D, PC, want_tok) > 200 * 1024) PC >>= 1;
         if (P < PC) PC = ((P + 31) / 32) * 32;
@@ -299,12 +320,14 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
         prm.N = topo.N;
         prm.PC = PC;
         dim3 grid((unsigned)((T + tpb - 1) / tpb), (unsigned)pchunks, (unsigned)L);
-        {
-            KernelTimerScope ts("eval", st);
-            eval_generic_kernel<<<grid, PC < 64 ? 64 : PC, smem, st>>>(prm);
+        if (!fast) {
+            {
+                KernelTimerScope ts("eval", st);
+                eval_generic_kernel<<<grid, PC < 64 ? 64 : PC, smem, st>>>(prm);
+            }
+            note_launch();
+            CAP_TRY(check_launch("eval_generic_kernel"));
         }
-        note_launch();
-        CAP_TRY(check_launch("eval_generic_kernel"));
     }
     FinalParams f;
     f.acc = w.acc;
@@ -324,7 +347,7 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
     const int n = L * P;
     {
         KernelTimerScope ts("eval_finalize", st);
-        eval_finalize_kernel<<<(n + 127) / 128, 128, 0, st>>>(f);
+        eval_finalize_kernel<<<(n + FIN_WARPS - 1) / FIN_WARPS, 32 * FIN_WARPS, 0, st>>>(f);
     }
     note_launch();
     return check_launch("eval_finalize_kernel");

@@ -1,0 +1,583 @@
+// S3 fast path -- bit-sliced scoring of P candidate placements (Eq. 3, Eq. 4, Fig. 6 axes,
+// Tables II-IV).  Used when the token sources are the default contiguous blocks (token_src NULL,
+// reading R5) and no per-token output is wanted; otherwise the generic kernel of cap_eval.cu runs.
+// Method and data layout: cap_eval_fast.cuh and DESIGN.md section 6.
+#include "cap_eval_fast.cuh"
+
+namespace cap {
+
+// ---- host geometry ----------------------------------------------------------------------------------
+static int ceil_log2(long long v)
+{
+    int b = 0;
+    while ((1ll << b) < v) ++b;
+    return b;
+}
+
+bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P,
+                    int target_ctas, size_t smem_budget, EvalFastGeom *g)
+{
+    if (L < 1 || T < 1 || P < 1 || D < 1 || D > 64 || N < 1 || N > 8 || k < 1 || k > 16) return false;
+    g->WD = D <= 8 ? 8 : D <= 16 ? 16 : D <= 32 ? 32 : 64;
+    g->WN = N <= 2 ? 2 : N <= 4 ? 4 : 8;
+    g->KP = (k + 3) & ~3;
+    const int unit = 128 / g->WD;                 // candidates per 16-byte column of the device section
+    const int Pfull = ((P + unit - 1) / unit) * unit;
+    // largest chunk whose table fits: (E + 1) rows of RS * 16 bytes
+    int Pc = Pfull;
+    for (;;) {
+        const int dcol = Pc * g->WD / 128;
+        const int ncol = (Pc * g->WN + 127) / 128;
+        const int R = dcol + ncol;
+        const int RS = R | 1;
+        int S = 1;
+        while (S < 64 && R * (S * 2) <= 320) S *= 2;
+        const size_t tbl = (size_t)(E + 1) * RS * 16;
+        const size_t offs = (size_t)2 * EF_PASSES * S * g->KP * 4;
+        const size_t xch = (size_t)(S / 2) * R * EF_NPL * 16;
+        const size_t smem = tbl + offs + xch + 128;
+        if (smem <= smem_budget && R * 1 <= 320) {
+            g->Pc = Pc;
+            g->DW = dcol * 4;
+            g->NW = ncol * 4;
+            g->R = R;
+            g->RS = RS;
+            g->W = R * 4;
+            g->S = S;
+            g->logS = ceil_log2(S);
+            g->smem = smem;
+            break;
+        }
+        if (Pc <= unit) return false;
+        Pc = ((Pc / 2 + unit - 1) / unit) * unit;
+    }
+    g->PC = (P + g->Pc - 1) / g->Pc;
+    // enough threads to own every (sub-slot, column) pair and to prefetch a block's index entries
+    // with at most EF_PRE registers each (threads beyond R * S only help with the staging)
+    while (g->S > 1 && EF_PASSES * g->S * g->KP > EF_PRE * EF_MAXTHREADS) {
+        g->S /= 2;
+        g->logS -= 1;
+    }
+    const int need_pre = (EF_PASSES * g->S * g->KP + EF_PRE - 1) / EF_PRE;
+    const int need = g->R * g->S > need_pre ? g->R * g->S : need_pre;
+    g->nthreads = ((need + 31) / 32) * 32;
+    if (g->nthreads > EF_MAXTHREADS) return false;
+    const int64_t blk = (int64_t)EF_PASSES * g->S;
+    int64_t want = ((int64_t)target_ctas + (int64_t)g->PC * L - 1) / ((int64_t)g->PC * L);
+    if (want < 1) want = 1;
+    int64_t tpc = (T + want - 1) / want;
+    tpc = ((tpc + blk - 1) / blk) * blk;
+    g->tpc = tpc;
+    g->ncta_t = (int)((T + tpc - 1) / tpc);
+    if (g->ncta_t > 65535) return false;
+    const int64_t cap_run = (int64_t)EF_MAXBLK * blk;
+    // runs split at capacity and at source boundaries
+    const int64_t srcb = ((tpc - 1) * D) / T + 1;      // source boundaries inside a block's range
+    g->maxrec = (int)((tpc + cap_run - 1) / cap_run + (srcb < D - 1 ? srcb : D - 1));
+    if (g->maxrec < 1) g->maxrec = 1;
+    g->NPR = EF_BT + g->logS;
+    g->rec_slots = (size_t)L * g->PC * g->ncta_t * g->maxrec;
+    g->rec_words = g->rec_slots * g->NPR * g->W;
+    g->table_words = (size_t)L * g->PC * (E + 1) * g->RS * 4;
+    return true;
+}
+
+static size_t ef_budget() { return 200 * 1024; }
+
+size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P)
+{
+    size_t best = 0;
+    for (int N = 2; N <= 8; N *= 2) {
+        EvalFastGeom g;
+        if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), ef_budget(), &g)) continue;
+        const size_t b = g.rec_slots * 4 + 256 + g.rec_words * 4 + 256 + g.table_words * 4 + 256;
+        if (b > best) best = b;
+    }
+    return best;
+}
+
+EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
+                              const EvalFastGeom &g)
+{
+    // the fast-path region follows the generic region (acc, recv, mcounts)
+    EvalWs base = eval_ws_carve(ws, L, E, D, P);
+    uintptr_t a = reinterpret_cast<uintptr_t>(base.mcounts + (size_t)L * E);
+    a = (a + 255) & ~(uintptr_t)255;
+    EvalFastWs w;
+    w.rec_src = reinterpret_cast<int32_t *>(a);
+    a += g.rec_slots * 4;
+    a = (a + 255) & ~(uintptr_t)255;
+    w.rec_planes = reinterpret_cast<uint32_t *>(a);
+    a += g.rec_words * 4;
+    a = (a + 255) & ~(uintptr_t)255;
+    w.table = reinterpret_cast<uint32_t *>(a);
+    return w;
+}
+
+// ---- main kernel ---------------------------------------------------------------------------------------
+struct EvalFastParams {
+    const int32_t *idx;          // [L][T][k]
+    const uint8_t *kept;         // [L][T][k] or NULL
+    const int32_t *expert_dev;   // [L][P][E]
+    const int32_t *dev_node;     // [D]
+    int32_t *rec_src;
+    uint32_t *rec_planes;
+    const uint32_t *table;       // [L][PC][E + 1][RS * 4]
+    int64_t T, tpc;
+    int32_t k, E, P, D;
+    int32_t WD, WN, Pc, PC, DW, NW, R, RS, S, logS, ncta_t, maxrec, NPR;
+};
+
+// one thread per table word; grid (words of a table / 256, PC, L)
+__global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
+{
+    const int layer = blockIdx.z, pc = blockIdx.y;
+    const int rowq = q.RS * 4;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (q.E + 1) * rowq) return;
+    const int e = i / rowq, w = i - e * rowq;
+    uint32_t *t = const_cast<uint32_t *>(q.table) + ((size_t)layer * q.PC + pc) * (size_t)(q.E + 1) * rowq;
+    t[i] = ef_table_word(q.expert_dev + ((size_t)layer * q.P) * q.E, q.dev_node, q.E, q.P, q.D, pc * q.Pc,
+                         q.WD, q.WN, q.DW, q.NW, e, w);
+}
+
+// bit-sliced a += b over EF_NPL planes of 4 words
+__device__ __forceinline__ void ef_add_planes(uint4 (&a)[EF_NPL], const uint4 *b, int stride)
+{
+    uint4 carry = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int p = 0; p < EF_NPL; ++p) {
+        const uint4 x = b[(size_t)p * stride];
+        uint4 s, c;
+        CAP_CSA(s.x, c.x, a[p].x, x.x, carry.x);
+        CAP_CSA(s.y, c.y, a[p].y, x.y, carry.y);
+        CAP_CSA(s.z, c.z, a[p].z, x.z, carry.z);
+        CAP_CSA(s.w, c.w, a[p].w, x.w, carry.w);
+        a[p] = s;
+        carry = c;
+    }
+}
+
+template <int KP>
+__device__ __forceinline__ uint4 ef_token_mask(const unsigned char *tblc, const uint32_t *op)
+{
+    uint4 m = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int q = 0; q < KP / 4; ++q) {
+        const uint4 o = *reinterpret_cast<const uint4 *>(op + 4 * q);
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(tblc + o.x);
+        const uint4 v1 = *reinterpret_cast<const uint4 *>(tblc + o.y);
+        const uint4 v2 = *reinterpret_cast<const uint4 *>(tblc + o.z);
+        const uint4 v3 = *reinterpret_cast<const uint4 *>(tblc + o.w);
+        m.x = lop_or3(lop_or3(m.x, v0.x, v1.x), v2.x, v3.x);
+        m.y = lop_or3(lop_or3(m.y, v0.y, v1.y), v2.y, v3.y);
+        m.z = lop_or3(lop_or3(m.z, v0.z, v1.z), v2.z, v3.z);
+        m.w = lop_or3(lop_or3(m.w, v0.w, v1.w), v2.w, v3.w);
+    }
+    return m;
+}
+
+// One block of EF_PASSES tokens per thread: Harley-Seal carry-save tree into planes 0..2, the
+// "eights" carry rippled into planes 3..EF_BT-1.
+#define CAP_EF_WORD(F)                                                                            \
+    do {                                                                                          \
+        uint32_t tA, tB, fA, fB, e8, s;                                                           \
+        CAP_CSA(s, tA, pl[0].F, x[0].F, x[1].F);                                                  \
+        CAP_CSA(s, tB, s, x[2].F, x[3].F);                                                        \
+        CAP_CSA(pl[1].F, fA, pl[1].F, tA, tB);                                                    \
+        CAP_CSA(s, tA, s, x[4].F, x[5].F);                                                        \
+        CAP_CSA(s, tB, s, x[6].F, x[7].F);                                                        \
+        pl[0].F = s;                                                                              \
+        CAP_CSA(pl[1].F, fB, pl[1].F, tA, tB);                                                    \
+        CAP_CSA(pl[2].F, e8, pl[2].F, fA, fB);                                                    \
+        _Pragma("unroll") for (int p = 3; p < EF_BT; ++p) {                                       \
+            const uint32_t c = pl[p].F & e8;                                                      \
+            pl[p].F ^= e8;                                                                        \
+            e8 = c;                                                                               \
+        }                                                                                         \
+    } while (0)
+
+template <int KP>
+__global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams q)
+{
+    extern __shared__ __align__(16) unsigned char ef_sm[];
+    const int tid = threadIdx.x, nthr = blockDim.x;
+    const int layer = blockIdx.z, pc = blockIdx.y;
+    const int E = q.E, D = q.D, k = q.k, S = q.S, R = q.R;
+    const int rowb = q.RS * 16;
+    unsigned char *tbl = ef_sm;
+    uint32_t *offs = reinterpret_cast<uint32_t *>(tbl + (size_t)(E + 1) * rowb);
+    uint4 *xch = reinterpret_cast<uint4 *>(offs + 2 * EF_PASSES * S * KP);
+
+    ef_copy_table(tbl, q.table + ((size_t)layer * q.PC + pc) * (size_t)(E + 1) * q.RS * 4, (E + 1) * q.RS,
+                  tid, nthr);
+
+    const bool active = tid < R * S;
+    const int sub = active ? tid / R : 0;
+    const int col = active ? tid - sub * R : 0;
+    const unsigned char *tblc = tbl + col * 16;
+    const int32_t *idx = q.idx + (size_t)layer * q.T * k;
+    const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
+    const uint32_t zero_row = (uint32_t)E * rowb;
+    const int nent = EF_PASSES * S * KP;          // index entries per block of tokens
+    const int64_t T = q.T;
+    const int64_t t0 = (int64_t)blockIdx.x * q.tpc;
+    const int64_t t1 = min(T, t0 + q.tpc);
+    const size_t slot0 = (((size_t)layer * q.PC + pc) * q.ncta_t + blockIdx.x) * q.maxrec;
+    const int blk_tokens = EF_PASSES * S;
+
+    int nrec = 0;
+    int64_t t = t0;
+    while (t < t1) {
+        // ---- one run: tokens [t, rend) share the source device and fit the thread counters ----
+        const int src = (int)((t * D) / T);
+        const int64_t bnd = ((int64_t)(src + 1) * T + D - 1) / D;
+        int64_t rend = min(t1, bnd);
+        rend = min(rend, t + (int64_t)EF_MAXBLK * blk_tokens);
+        uint4 pl[EF_NPL];
+#pragma unroll
+        for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint4(0u, 0u, 0u, 0u);
+
+        // prefetch registers: entry i of a block = (slot = i / KP, s = i % KP); token = base + slot
+        uint32_t pre[EF_PRE];
+        auto fetch = [&](int64_t base) {
+#pragma unroll
+            for (int j = 0; j < EF_PRE; ++j) {
+                const int i = tid + j * nthr;
+                uint32_t o = zero_row;
+                if (i < nent) {
+                    const int slot = i / KP, s = i - slot * KP;
+                    const int64_t tok = base + slot;
+                    if (tok < rend && s < k) {
+                        const int64_t a = tok * k + s;
+                        const int e = idx[a];
+                        if ((!kept || kept[a]) && (unsigned)e < (unsigned)E) o = (uint32_t)e * rowb;
+                    }
+                }
+                pre[j] = o;
+            }
+        };
+        auto stash = [&](int buf) {
+#pragma unroll
+            for (int j = 0; j < EF_PRE; ++j) {
+                const int i = tid + j * nthr;
+                if (i < nent) offs[buf * nent + i] = pre[j];
+            }
+        };
+        __syncthreads();     // the previous run's readers of offs are done
+        fetch(t);
+        stash(0);
+        __syncthreads();
+        int buf = 0;
+        for (int64_t b = t; b < rend; b += blk_tokens) {
+            const bool more = b + blk_tokens < rend;
+            if (more) fetch(b + blk_tokens);
+            if (active) {
+                uint4 x[EF_PASSES];
+                const uint32_t *ob = offs + buf * nent + sub * KP;
+#pragma unroll
+                for (int ps = 0; ps < EF_PASSES; ++ps) x[ps] = ef_token_mask<KP>(tblc, ob + ps * S * KP);
+                CAP_EF_WORD(x);
+                CAP_EF_WORD(y);
+                CAP_EF_WORD(z);
+                CAP_EF_WORD(w);
+            }
+            if (more) stash(buf ^ 1);
+            __syncthreads();
+            buf ^= 1;
+        }
+        // ---- flush: add the S sub-slots in the bit-sliced domain, write the record ----
+        for (int lvl = 0; lvl < q.logS; ++lvl) {
+            const int half = S >> (lvl + 1);
+            const int stride = half * R;
+            if (active && sub >= half && sub < 2 * half) {
+#pragma unroll
+                for (int p = 0; p < EF_NPL; ++p) xch[(size_t)p * stride + (sub - half) * R + col] = pl[p];
+            }
+            __syncthreads();
+            if (active && sub < half) ef_add_planes(pl, xch + sub * R + col, stride);
+            __syncthreads();
+        }
+        if (active && sub == 0) {
+            uint4 *rp = reinterpret_cast<uint4 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
+#pragma unroll
+            for (int p = 0; p < EF_NPL; ++p)
+                if (p < q.NPR) rp[(size_t)p * R + col] = pl[p];
+        }
+        if (tid == 0) q.rec_src[slot0 + nrec] = src;
+        ++nrec;
+        t = rend;
+    }
+}
+
+// ---- decode: add all records of one record word in the bit-sliced domain, extract once -------------
+struct DecodeParams {
+    const int32_t *rec_src;
+    const uint32_t *rec_planes;
+    const int32_t *dev_node;
+    unsigned long long *acc;    // [L][P][ACC_N]
+    unsigned long long *recv;   // [L][P][D]
+    int32_t P, D, N, WD, WN, Pc, PC, DW, W, NPR, nslots, na;
+};
+
+// acc (na planes) += x (planes 0..EF_NPL-1 of a[], masked), ripple carry
+#define CAP_DEC_ADD(ACC, MASK)                                        \
+    do {                                                              \
+        uint32_t cy = 0u;                                             \
+        _Pragma("unroll") for (int p = 0; p < 32; ++p) {              \
+            if (p < q.na) {                                           \
+                const uint32_t xx = p < EF_NPL ? (a[p < EF_NPL ? p : 0] & (MASK)) : 0u; \
+                const uint32_t s = lop_xor3(ACC[p], xx, cy);          \
+                cy = lop_maj(ACC[p], xx, cy);                         \
+                ACC[p] = s;                                           \
+            }                                                         \
+        }                                                             \
+    } while (0)
+
+#define CAP_DEC_ADD32(ACC)                                            \
+    do {                                                              \
+        uint32_t cy = 0u;                                             \
+        _Pragma("unroll") for (int p = 0; p < 32; ++p) {              \
+            if (p < q.na) {                                           \
+                const uint32_t s = lop_xor3(ACC[p], a[p], cy);        \
+                cy = lop_maj(ACC[p], a[p], cy);                       \
+                ACC[p] = s;                                           \
+            }                                                         \
+        }                                                             \
+    } while (0)
+
+#define CAP_DEC_BFLY(ACC, OFF)                                        \
+    do {                                                              \
+        uint32_t cy = 0u;                                             \
+        _Pragma("unroll") for (int p = 0; p < 32; ++p) {              \
+            if (p < q.na) {                                           \
+                const uint32_t xx = __shfl_xor_sync(0xffffffffu, ACC[p], OFF); \
+                const uint32_t s = lop_xor3(ACC[p], xx, cy);          \
+                cy = lop_maj(ACC[p], xx, cy);                         \
+                ACC[p] = s;                                           \
+            }                                                         \
+        }                                                             \
+    } while (0)
+
+constexpr int DEC_WARPS = 4;
+__global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParams q)
+{
+    __shared__ unsigned long long nodeset[8];
+    __shared__ unsigned char s_dn[64];
+    __shared__ uint32_t s_part[DEC_WARPS - 1][3][32];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int w = blockIdx.x, pc = blockIdx.y, layer = blockIdx.z;
+    if (threadIdx.x < 64) s_dn[threadIdx.x] = (int)threadIdx.x < q.D ? (unsigned char)q.dev_node[threadIdx.x] : 0;
+    if (threadIdx.x >= 64 && threadIdx.x < 72) {
+        const int n = threadIdx.x - 64;
+        unsigned long long m = 0ull;
+        for (int d = 0; d < q.D; ++d)
+            if (q.dev_node[d] == n) m |= 1ull << d;
+        nodeset[n] = m;
+    }
+    __syncthreads();
+    const bool devword = w < q.DW;
+    uint32_t tot[32], loc[32], sam[32];
+#pragma unroll
+    for (int p = 0; p < 32; ++p) tot[p] = loc[p] = sam[p] = 0u;
+    const size_t sbase = ((size_t)layer * q.PC + pc) * q.nslots;
+    constexpr int DEC_SL = 4;     // record slots a thread has in flight
+    for (int s0 = threadIdx.x; s0 < q.nslots; s0 += 32 * DEC_WARPS * DEC_SL) {
+        int srcs[DEC_SL];
+#pragma unroll
+        for (int j = 0; j < DEC_SL; ++j) {
+            const int s = s0 + j * 32 * DEC_WARPS;
+            srcs[j] = s < q.nslots ? q.rec_src[sbase + s] : -1;
+        }
+        uint32_t av[DEC_SL][EF_NPL];
+#pragma unroll
+        for (int j = 0; j < DEC_SL; ++j) {
+            const int s = s0 + j * 32 * DEC_WARPS;
+            const uint32_t *pp = q.rec_planes + ((sbase + s) * (size_t)q.NPR) * q.W + w;
+#pragma unroll
+            for (int p = 0; p < EF_NPL; ++p) av[j][p] = (srcs[j] >= 0 && p < q.NPR) ? pp[(size_t)p * q.W] : 0u;
+        }
+#pragma unroll
+        for (int j = 0; j < DEC_SL; ++j) {
+            if (srcs[j] < 0) continue;
+            const int src = srcs[j];
+            const int node = s_dn[src];
+            uint32_t mloc, msam;
+            if (devword) {
+                mloc = ef_devmask_word(q.WD, w, 1ull << src);
+                msam = ef_devmask_word(q.WD, w, nodeset[node]);
+            } else {
+                mloc = ef_nodemask_word(q.WN, node);
+                msam = 0u;
+            }
+            const uint32_t(&a)[EF_NPL] = av[j];
+            CAP_DEC_ADD(tot, 0xffffffffu);
+            CAP_DEC_ADD(loc, mloc);
+            CAP_DEC_ADD(sam, msam);
+        }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        CAP_DEC_BFLY(tot, off);
+        CAP_DEC_BFLY(loc, off);
+        CAP_DEC_BFLY(sam, off);
+    }
+    // every lane of a warp now holds the warp's sums; warps 1.. hand theirs to warp 0
+    if (warp > 0 && lane < 3) {
+#pragma unroll
+        for (int p = 0; p < 32; ++p) {
+            const uint32_t v = lane == 0 ? tot[p] : lane == 1 ? loc[p] : sam[p];
+            s_part[warp - 1][lane][p] = v;
+        }
+    }
+    __syncthreads();
+    if (warp > 0) return;
+    for (int o = 0; o < DEC_WARPS - 1; ++o) {
+        uint32_t a[32];
+#pragma unroll
+        for (int p = 0; p < 32; ++p) a[p] = s_part[o][0][p];
+        CAP_DEC_ADD32(tot);
+#pragma unroll
+        for (int p = 0; p < 32; ++p) a[p] = s_part[o][1][p];
+        CAP_DEC_ADD32(loc);
+#pragma unroll
+        for (int p = 0; p < 32; ++p) a[p] = s_part[o][2][p];
+        CAP_DEC_ADD32(sam);
+    }
+    unsigned long long vt = 0ull, vl = 0ull, vs = 0ull;
+#pragma unroll
+    for (int p = 0; p < 32; ++p) {
+        if (p < q.na) {
+            vt |= (unsigned long long)((tot[p] >> lane) & 1u) << p;
+            vl |= (unsigned long long)((loc[p] >> lane) & 1u) << p;
+            vs |= (unsigned long long)((sam[p] >> lane) & 1u) << p;
+        }
+    }
+    const int fw = devword ? q.WD : q.WN;                 // field width of this word
+    const int bitpos = (devword ? w : w - q.DW) * 32 + lane;
+    const int pl = bitpos / fw, f = bitpos - pl * fw;
+    const int p = pc * q.Pc + pl;
+    const bool pvalid = pl < q.Pc && p < q.P;
+    if (devword && pvalid && f < q.D) q.recv[((size_t)layer * q.P + p) * q.D + f] = vt;
+    const int gw = fw < 32 ? fw : 32;
+    unsigned long long gt = vt, gl = vl, gs = vs;
+    for (int off = 1; off < gw; off <<= 1) {
+        gt += __shfl_xor_sync(0xffffffffu, gt, off);
+        gl += __shfl_xor_sync(0xffffffffu, gl, off);
+        gs += __shfl_xor_sync(0xffffffffu, gs, off);
+    }
+    if ((lane & (gw - 1)) == 0 && pvalid) {
+        unsigned long long *ac = q.acc + ((size_t)layer * q.P + p) * ACC_N;
+        if (devword) {
+            if (gt) atomicAdd(&ac[ACC_DEV], gt);
+            if (gl) atomicAdd(&ac[ACC_LOCAL], gl);
+            if (gs) atomicAdd(&ac[ACC_SAMENODE], gs);
+        } else {
+            if (gt) atomicAdd(&ac[ACC_NODE], gt);
+            if (gt - gl) atomicAdd(&ac[ACC_RNODE], gt - gl);
+        }
+    }
+}
+
+// ---- launcher ------------------------------------------------------------------------------------------
+template <int KP>
+static int launch_kp(const EvalFastParams &prm, const EvalFastGeom &g, int L, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(eval_fast_kernel<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
+        attr_set = true;
+    }
+    dim3 grid((unsigned)g.ncta_t, (unsigned)g.PC, (unsigned)L);
+    {
+        KernelTimerScope ts("eval", st);
+        eval_fast_kernel<KP><<<grid, g.nthreads, g.smem, st>>>(prm);
+    }
+    note_launch();
+    return check_launch("eval_fast_kernel");
+}
+
+int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
+                     int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                     void *ws, cudaStream_t st, bool *used)
+{
+    *used = false;
+    EvalFastGeom g;
+    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g)) return CAP_OK;
+    EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g);
+    EvalWs base = eval_ws_carve(ws, L, E, topo.D, P);
+    if (cudaMemsetAsync(fw.rec_src, 0xff, g.rec_slots * 4, st) != cudaSuccess)
+        return check_launch("memset rec_src");
+    EvalFastParams prm;
+    prm.idx = idx;
+    prm.kept = kept;
+    prm.expert_dev = expert_dev;
+    prm.dev_node = topo.dev_node;
+    prm.rec_src = fw.rec_src;
+    prm.rec_planes = fw.rec_planes;
+    prm.table = fw.table;
+    prm.T = T;
+    prm.tpc = g.tpc;
+    prm.k = k;
+    prm.E = E;
+    prm.P = P;
+    prm.D = topo.D;
+    prm.WD = g.WD;
+    prm.WN = g.WN;
+    prm.Pc = g.Pc;
+    prm.PC = g.PC;
+    prm.DW = g.DW;
+    prm.NW = g.NW;
+    prm.R = g.R;
+    prm.RS = g.RS;
+    prm.S = g.S;
+    prm.logS = g.logS;
+    prm.ncta_t = g.ncta_t;
+    prm.maxrec = g.maxrec;
+    prm.NPR = g.NPR;
+    {
+        const int nw = (E + 1) * g.RS * 4;
+        KernelTimerScope ts("eval_table", st);
+        eval_table_kernel<<<dim3((unsigned)((nw + 255) / 256), (unsigned)g.PC, (unsigned)L), 256, 0, st>>>(prm);
+    }
+    note_launch();
+    CAP_TRY(check_launch("eval_table_kernel"));
+    int rc;
+    switch (g.KP) {
+    case 4: rc = launch_kp<4>(prm, g, L, st); break;
+    case 8: rc = launch_kp<8>(prm, g, L, st); break;
+    case 12: rc = launch_kp<12>(prm, g, L, st); break;
+    default: rc = launch_kp<16>(prm, g, L, st); break;
+    }
+    CAP_TRY(rc);
+    DecodeParams dq;
+    dq.rec_src = fw.rec_src;
+    dq.rec_planes = fw.rec_planes;
+    dq.dev_node = topo.dev_node;
+    dq.acc = base.acc;
+    dq.recv = base.recv;
+    dq.P = P;
+    dq.D = topo.D;
+    dq.N = topo.N;
+    dq.WD = g.WD;
+    dq.WN = g.WN;
+    dq.Pc = g.Pc;
+    dq.PC = g.PC;
+    dq.DW = g.DW;
+    dq.W = g.W;
+    dq.NPR = g.NPR;
+    dq.nslots = g.ncta_t * g.maxrec;
+    int na = 1;
+    while (na < 32 && (1ll << na) <= T) ++na;
+    dq.na = na;
+    {
+        KernelTimerScope ts("eval_decode", st);
+        eval_decode_kernel<<<dim3((unsigned)g.W, (unsigned)g.PC, (unsigned)L), 32 * DEC_WARPS, 0, st>>>(dq);
+    }
+    note_launch();
+    CAP_TRY(check_launch("eval_decode_kernel"));
+    *used = true;
+    return CAP_OK;
+}
+
+}  // namespace cap

@@ -37,7 +37,7 @@ struct EvalWs {
     unsigned long long *mcounts;  // [L][E] kept pairs per expert (when the caller gave none)
 };
 
-size_t eval_ws_bytes(int32_t L, int32_t E, int32_t D, int32_t P);
+size_t eval_ws_bytes(int32_t L, int64_t T, int32_t E, int32_t k, int32_t D, int32_t P);
 EvalWs eval_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P);
 
 // ---- stage launchers (arguments already validated) ---------------------------------------
@@ -53,6 +53,11 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
                  const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,
                  cudaStream_t st);
+// S3 fast path (cap_eval_fast.cu): *used = false when the sizes do not fit it
+int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
+                     int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                     void *ws, cudaStream_t st, bool *used);
+size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D);
 int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,
                     const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
