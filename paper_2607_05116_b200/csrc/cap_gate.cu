@@ -209,6 +209,9 @@ static int launch_vpl(const GateParams &prm, cudaStream_t st)
 int launch_gate_topk(const float *logits, const float *bias, int32_t L, int64_t T,
                      const cap_gate_cfg &cfg, int32_t *idx, float *w, cudaStream_t st)
 {
+    bool fast = false;
+    CAP_TRY(launch_gate_fast(logits, bias, L, T, cfg, idx, w, st, &fast));
+    if (fast) return CAP_OK;
     GateParams prm;
     prm.logits = logits;
     prm.bias = bias;

@@ -43,6 +43,9 @@ EvalWs eval_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P);
 // ---- stage launchers (arguments already validated) ---------------------------------------
 int launch_gate_topk(const float *logits, const float *bias, int32_t L, int64_t T,
                      const cap_gate_cfg &cfg, int32_t *idx, float *w, cudaStream_t st);
+// S1 fast path (cap_gate_fast.cu): *used = false when the configuration does not fit it
+int launch_gate_fast(const float *logits, const float *bias, int32_t L, int64_t T,
+                     const cap_gate_cfg &cfg, int32_t *idx, float *w, cudaStream_t st, bool *used);
 int launch_coactivation(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                         int32_t E, int64_t *counts, int32_t *coact, cudaStream_t st);
 int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_src, int32_t L,
