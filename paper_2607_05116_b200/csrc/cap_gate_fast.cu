@@ -1,7 +1,7 @@
-// S1 fast path, standalone kernel (Eq. 1): persistent blocks, one producer warp that
-// streams 32-token tiles of logits into a shared-memory ring with TMA bulk copies (one 4E-byte
-// row per copy, rows padded by 16 bytes so that the per-thread 128-bit row reads are
-// bank-conflict free), consumer warps that run the one-thread-per-token selection network of
+// S1 fast path, standalone kernel (Eq. 1): persistent blocks, producer warps that
+// stream 16-token tiles of logits into a shared-memory ring with TMA bulk copies (one copy per
+// tile; rows are dense and the per-thread 128-bit row reads are XOR-swizzled so that they stay
+// bank-conflict free), consumer warps that run the two-lanes-per-token selection network of
 // cap_gate_fast.cuh.  Applies to softmax scoring with renormalised weights, no group limit,
 // k <= 8, E in {64, 128, 256}; everything else takes the generic kernel of cap_gate.cu.
 #include "cap_async.cuh"
@@ -9,9 +9,11 @@
 
 namespace cap {
 
-constexpr int GF_NC = 8;                       // consumer warps
-constexpr int GF_THREADS = 32 * (GF_NC + 1);
-constexpr int GF_MAXST = 16;
+constexpr int GF_NP = 2;                       // producer warps
+constexpr int GF_NC = 14;                      // consumer warps
+constexpr int GF_THREADS = 32 * (GF_NC + GF_NP);
+constexpr int GF_MAXST = 32;
+constexpr int GF_TILE = 16;                    // tokens per tile (one warp, two lanes per token)
 
 struct GateFastParams {
     const float *logits;
@@ -28,8 +30,8 @@ __global__ void __launch_bounds__(GF_THREADS) gate_fast_kernel(GateFastParams q)
 {
     extern __shared__ __align__(128) unsigned char gf_sm[];
     __shared__ uint64_t full_bar[GF_MAXST], empty_bar[GF_MAXST];
-    constexpr int ROWB = E * 4 + 16;
-    constexpr int STAGEB = 32 * ROWB;
+    constexpr int ROWB = E * 4;                  // dense rows; reads are XOR-swizzled per lane
+    constexpr int STAGEB = GF_TILE * ROWB;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nst = q.nst;
     if (threadIdx.x == 0) {
@@ -40,52 +42,55 @@ __global__ void __launch_bounds__(GF_THREADS) gate_fast_kernel(GateFastParams q)
         mbar_fence_init();
     }
     __syncthreads();
-    const int64_t ntiles = (q.LT + 31) >> 5;
+    const int64_t ntiles = (q.LT + GF_TILE - 1) / GF_TILE;
     const int64_t tile0 = (int64_t)blockIdx.x * q.tiles_per_cta;
     int64_t nt = ntiles - tile0;
     if (nt > q.tiles_per_cta) nt = q.tiles_per_cta;
     if (nt <= 0) return;
 
-    if (warp == 0) {
-        // ---- producer ----
-        for (int64_t j = 0; j < nt; ++j) {
-            const int st = (int)(j % nst);
-            if (j >= nst) mbar_wait(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1));
-            const int64_t tok0 = (tile0 + j) << 5;
-            const int rows = (int)min((int64_t)32, q.LT - tok0);
-            if (lane == 0) mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
-            __syncwarp();
-            if (lane < rows)
-                bulk_g2s(gf_sm + (size_t)st * STAGEB + lane * ROWB, q.logits + (tok0 + lane) * E, E * 4,
-                         &full_bar[st]);
+    if (warp < GF_NP) {
+        // ---- producers: warp p streams tiles p, p + NP, ...; one elected lane issues the row copies ----
+        if (lane == 0) {
+            for (int64_t j = warp; j < nt; j += GF_NP) {
+                const int st = (int)(j % nst);
+                if (j >= nst) mbar_wait(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1));
+                const int64_t tok0 = (tile0 + j) * GF_TILE;
+                const int rows = (int)min((int64_t)GF_TILE, q.LT - tok0);
+                mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
+                bulk_g2s(gf_sm + (size_t)st * STAGEB, q.logits + tok0 * E, (uint32_t)rows * E * 4,
+                         &full_bar[st]);           // the tile's rows are contiguous in global memory
+            }
         }
     } else {
-        // ---- consumers: warp c takes tiles c, c + NC, ... ----
-        const int c = warp - 1;
+        // ---- consumers: warp c takes tiles c, c + NC, ...; lanes l and l ^ 16 share token l & 15 ----
+        const int c = warp - GF_NP;
         const int k = q.k;
+        const int h = lane >> 4, tl = lane & 15;
         for (int64_t j = c; j < nt; j += GF_NC) {
             const int st = (int)(j % nst);
             mbar_wait(&full_bar[st], (uint32_t)((j / nst) & 1));
-            const int64_t tok = ((tile0 + j) << 5) + lane;
-            if (tok < q.LT) {
-                const float *row = reinterpret_cast<const float *>(gf_sm + (size_t)st * STAGEB + lane * ROWB);
-                int sel[8];
-                float wv[8];
-                gate_select<E>(row, k, sel);
-                gate_weights_softmax(row, k, sel, q.scale, wv);
+            const int64_t tok = (tile0 + j) * GF_TILE + tl;
+            const bool valid = tok < q.LT;
+            // rows past the end of a ragged last tile were not written: those lanes redo row 0
+            const float *row =
+                reinterpret_cast<const float *>(gf_sm + (size_t)st * STAGEB + (valid ? tl : 0) * ROWB);
+            int sel[8];
+            float wv[4];
+            gate_select_pair<E>(row, h, tl & 7, k, sel);
+            gate_weights_softmax_pair(row, h, k, sel, q.scale, wv);
+            if (valid) {
                 if (q.vec_out) {
-                    int4 *ip = reinterpret_cast<int4 *>(q.idx + tok * 8);
-                    float4 *wp = reinterpret_cast<float4 *>(q.w + tok * 8);
-                    ip[0] = make_int4(sel[0], sel[1], sel[2], sel[3]);
-                    ip[1] = make_int4(sel[4], sel[5], sel[6], sel[7]);
-                    wp[0] = make_float4(wv[0], wv[1], wv[2], wv[3]);
-                    wp[1] = make_float4(wv[4], wv[5], wv[6], wv[7]);
+                    int4 *ip = reinterpret_cast<int4 *>(q.idx + tok * 8 + 4 * h);
+                    float4 *wp = reinterpret_cast<float4 *>(q.w + tok * 8 + 4 * h);
+                    *ip = h ? make_int4(sel[4], sel[5], sel[6], sel[7]) : make_int4(sel[0], sel[1], sel[2], sel[3]);
+                    *wp = make_float4(wv[0], wv[1], wv[2], wv[3]);
                 } else {
 #pragma unroll
-                    for (int s = 0; s < 8; ++s) {
+                    for (int jj = 0; jj < 4; ++jj) {
+                        const int s = 4 * h + jj;
                         if (s < k) {
-                            q.idx[tok * k + s] = sel[s];
-                            q.w[tok * k + s] = wv[s];
+                            q.idx[tok * k + s] = h ? sel[4 + jj] : sel[jj];
+                            q.w[tok * k + s] = wv[jj];
                         }
                     }
                 }
@@ -99,7 +104,7 @@ __global__ void __launch_bounds__(GF_THREADS) gate_fast_kernel(GateFastParams q)
 template <int E>
 static int launch_e(GateFastParams prm, cudaStream_t st)
 {
-    constexpr int STAGEB = 32 * (E * 4 + 16);
+    constexpr int STAGEB = GF_TILE * (E * 4);
     int nst = (200 * 1024) / STAGEB;
     if (nst > GF_MAXST) nst = GF_MAXST;
     prm.nst = nst;
@@ -108,7 +113,7 @@ static int launch_e(GateFastParams prm, cudaStream_t st)
         cudaFuncSetAttribute(gate_fast_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
         attr_set = true;
     }
-    const int64_t ntiles = (prm.LT + 31) >> 5;
+    const int64_t ntiles = (prm.LT + GF_TILE - 1) / GF_TILE;
     int64_t grid = sm_count();
     if (grid > ntiles) grid = ntiles;
     prm.tiles_per_cta = (ntiles + grid - 1) / grid;

@@ -1,16 +1,17 @@
-// S1 fast path (softmax scoring, renormalised weights, no group limit, k <= 8): one THREAD per
-// token.  The token's logits row sits in shared memory (staged by TMA); the thread streams it in
-// groups of 8, sorts each group with a 19-comparator network and merges it into a running sorted
+// S1 fast path (softmax scoring, renormalised weights, no group limit, k <= 8): a PAIR of threads
+// per token.  The token's logits row sits in shared memory (staged by TMA); each thread streams its
+// half of the row in groups of 8, sorts each group with a 19-comparator network and merges it into a running sorted
 // top-8 list (half-cleaner + bitonic merge), all on 32-bit integer keys with min/max only.
 //
 // Keys.  key = order-preserving image of the logit with its low IB = log2(E) bits replaced by
 // (E-1-e): larger key = larger logit, equal truncated logits -> lower expert index first, so one
 // 32-bit comparator orders (value, index) pairs.  Truncation can only mis-order two experts whose
 // keys agree in all upper 32-IB bits; the thread therefore also tracks the 9th largest key and,
-// if any two neighbours among the top 9 share their upper bits, redoes that token with exact
-// full-precision comparisons (k passes of arg-max).  The result is always the exact top-k with
+// if any two neighbours among the top 9 share their upper bits, the warp redoes that token with
+// exact full-precision comparisons (k rounds of warp-wide arg-max).  The result is always the exact top-k with
 // ties toward the lower index (reading R2), the fast path is taken for all but ~0.1% of tokens.
 #pragma once
+#include "cap_async.cuh"
 #include "cap_internal.cuh"
 
 namespace cap {
@@ -63,45 +64,69 @@ __device__ __forceinline__ uint32_t gate_key(float x, int e)
     const float c = __fadd_rn(x, 0.0f);                  // -0 -> +0 (IEEE: they compare equal)
     const uint32_t b = __float_as_uint(c);
     const uint32_t o = b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
-    return (o | GateBits<E>::MASK) ^ (uint32_t)e;        // low bits = MASK - e
+    return (o | GateBits<E>::MASK) ^ (uint32_t)e;        // low bits = MASK - e (a payload, see above)
 }
 
-// Exact top-k of one row by k passes of arg-max on full keys (ties -> lower index).
-// Returns the k indices packed one per byte (E <= 256), slot 0 in the low byte.
+// Exact top-k of one row, computed by the WHOLE warp (all 32 lanes must call it with the same row):
+// lane l holds experts [l E/32, (l+1) E/32) as full 32-bit keys; k rounds of {warp max of the lanes'
+// best keys, warp min over the owners' indices} so that ties go to the lower expert index.
 template <int E>
-__device__ __noinline__ unsigned long long gate_select_exact(const float *row, int k)
+__device__ __noinline__ void gate_select_exact_warp(uint32_t row_smem, int lane, int k, int (&sel)[8])
 {
-    unsigned long long packed = 0ull;
-    uint32_t used[(E + 31) / 32];
+    constexpr int VPL = E / 32;
+    uint32_t key[VPL];
 #pragma unroll
-    for (int i = 0; i < (E + 31) / 32; ++i) used[i] = 0u;
-    for (int s = 0; s < k; ++s) {
-        uint32_t bk = 0u;
-        int bi = 0;
-        for (int e = 0; e < E; ++e) {
-            const uint32_t key = okey(row[e]);
-            const bool free_ = !((used[e >> 5] >> (e & 31)) & 1u);
-            if (free_ && key > bk) { bk = key; bi = e; }
-        }
-        packed |= (unsigned long long)bi << (8 * s);
-        used[bi >> 5] |= 1u << (bi & 31);
+    for (int j = 0; j < VPL; ++j) {
+        float x;
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x) : "r"(row_smem + (uint32_t)(lane * VPL + j) * 4u));
+        key[j] = okey(x);
     }
-    return packed;
+#pragma unroll
+    for (int s = 0; s < 8; ++s) {
+        int wi = 0;
+        if (s < k) {
+            uint32_t bk = 0u;
+            int bi = 0x7fffffff;
+#pragma unroll
+            for (int j = 0; j < VPL; ++j)
+                if (key[j] > bk) { bk = key[j]; bi = lane * VPL + j; }
+            const uint32_t m = __reduce_max_sync(0xffffffffu, bk);
+            wi = __reduce_min_sync(0xffffffffu, bk == m ? bi : 0x7fffffff);
+#pragma unroll
+            for (int j = 0; j < VPL; ++j)
+                if (lane * VPL + j == wi) key[j] = 0u;
+        }
+        sel[s] = wi;
+    }
 }
 
-// Top-k selection of one token.  row: E floats in shared memory, 16-byte aligned.
-// sel[0..k) = expert indices in descending score order.
+// Top-k selection of one token by a PAIR of lanes (lane and lane ^ 16): lane half h streams experts
+// [h E/2, (h+1) E/2) of the row with half-relative index immediates, the two sorted lists are then
+// rebased to full indices and merged (both lanes end with the same result).
+// row: E floats in shared memory, dense (4E-byte rows, tile base 128-byte aligned).  To keep the
+// 128-bit row reads bank-conflict free without padding, lane t reads 16-byte chunk c of its half at
+// chunk position c ^ (t & 7): the keys then carry the index payload of position c, and since the
+// payload never decides a comparison whose outcome is kept (equal upper bits -> exact fallback),
+// the true index is recovered afterwards as payload ^ 4 (t & 7).
+// sel[0..8) = expert indices, descending score.
 template <int E>
-__device__ __forceinline__ void gate_select(const float *row, int k, int (&sel)[8])
+__device__ __forceinline__ void gate_select_pair(const float *row, int h, int t7, int k, int (&sel)[8])
 {
-    static_assert(E % 8 == 0, "E must be a multiple of 8");
+    static_assert(E % 16 == 0 && E >= 32 && E <= 256, "E must be a multiple of 16 in [32, 256]");
     constexpr int IB = GateBits<E>::IB;
+    constexpr int H = E / 2;
+    const uint32_t hb = smem_u32(row + h * H) | ((uint32_t)t7 << 4);   // 128-byte aligned | swizzle
     uint32_t r[8];
     uint32_t r9 = 0u;
 #pragma unroll
-    for (int gi = 0; gi < E / 8; ++gi) {
-        const float4 va = *reinterpret_cast<const float4 *>(row + gi * 8);
-        const float4 vb = *reinterpret_cast<const float4 *>(row + gi * 8 + 4);
+    for (int gi = 0; gi < H / 8; ++gi) {
+        float4 va, vb;
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(va.x), "=f"(va.y), "=f"(va.z), "=f"(va.w)
+                     : "r"(hb ^ (uint32_t)(gi * 32)));
+        asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
+                     : "=f"(vb.x), "=f"(vb.y), "=f"(vb.z), "=f"(vb.w)
+                     : "r"(hb ^ (uint32_t)(gi * 32 + 16)));
         uint32_t g[8];
         g[0] = gate_key<E>(va.x, gi * 8 + 0); g[1] = gate_key<E>(va.y, gi * 8 + 1);
         g[2] = gate_key<E>(va.z, gi * 8 + 2); g[3] = gate_key<E>(va.w, gi * 8 + 3);
@@ -115,44 +140,68 @@ __device__ __forceinline__ void gate_select(const float *row, int k, int (&sel)[
             merge8_desc(r, g, r9);
         }
     }
+    // payload (low bits = MASK - position index) -> full expert index: undo the chunk swizzle
+    // (XOR of bits 2..4), then add h E/2.  MASK - e = ~e on the field, so both are XORs / a subtract.
+    const uint32_t swz = (uint32_t)t7 << 2;
+    const uint32_t adj = (uint32_t)(h * H);
+    uint32_t g[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        r[i] = (r[i] ^ swz) - adj;
+        g[i] = __shfl_xor_sync(0xffffffffu, r[i], 16);
+    }
+    r9 = (r9 ^ swz) - adj;
+    r9 = max(r9, __shfl_xor_sync(0xffffffffu, r9, 16));
+    merge8_desc(r, g, r9);
     // neighbours among the top 9 that agree in every bit above the index field are ambiguous
     bool amb = ((r[7] ^ r9) >> IB) == 0u;
 #pragma unroll
     for (int i = 0; i < 7; ++i) amb |= ((r[i] ^ r[i + 1]) >> IB) == 0u;
-    if (E == 8) amb = false;   // no 9th key
-    static_assert(E <= 256, "packed fallback indices are one byte each");
-    if (amb) {
-        const unsigned long long pk = gate_select_exact<E>(row, k);
 #pragma unroll
-        for (int i = 0; i < 8; ++i) sel[i] = (int)((pk >> (8 * i)) & 0xffull);
-    } else {
+    for (int i = 0; i < 8; ++i) sel[i] = (int)(GateBits<E>::MASK - (r[i] & GateBits<E>::MASK));
+    // ambiguous tokens (rare): the whole warp redoes them one at a time with exact comparisons
+    const int lane = (int)(threadIdx.x & 31u);
+    unsigned todo = __ballot_sync(0xffffffffu, amb) & 0xffffu;     // one lane of each pair
+    const uint32_t row_s = smem_u32(row);
+    while (todo) {
+        const int src = __ffs((int)todo) - 1;
+        todo &= todo - 1u;
+        const uint32_t rs = __shfl_sync(0xffffffffu, row_s, src);
+        int ex[8];
+        gate_select_exact_warp<E>(rs, lane, k, ex);
+        if ((lane & 15) == src) {
 #pragma unroll
-        for (int i = 0; i < 8; ++i) sel[i] = (int)(GateBits<E>::MASK - (r[i] & GateBits<E>::MASK));
+            for (int i = 0; i < 8; ++i) sel[i] = ex[i];
+        }
     }
 }
 
-// Renormalised softmax weights of the selected experts (DESIGN.md R-S1.3): r_s = expS(x_s - x_0),
-// Z summed in slot order, w_s = r_s / Z (* scale).
-__device__ __forceinline__ void gate_weights_softmax(const float *row, int k, const int (&sel)[8],
-                                                     float scale, float (&w)[8])
+// Renormalised softmax weights (DESIGN.md R-S1.3): r_s = expS(x_s - x_0), Z summed in slot order,
+// w_s = r_s / Z (* scale).  Lane half h evaluates slots 4h..4h+3, the pair exchanges them, both sum
+// Z in slot order; w[0..4) = weights of slots 4h..4h+3.
+__device__ __forceinline__ void gate_weights_softmax_pair(const float *row, int h, int k,
+                                                          const int (&sel)[8], float scale, float (&w)[4])
 {
     const float x0 = row[sel[0]];
-    float Z = 0.0f;
+    float mine[4], other[4];
 #pragma unroll
-    for (int s = 0; s < 8; ++s) {
-        if (s < k) {
-            const float rs = exp_s(__fsub_rn(row[sel[s]], x0));
-            w[s] = rs;
-            Z = s == 0 ? rs : __fadd_rn(Z, rs);
-        }
+    for (int j = 0; j < 4; ++j) {
+        const int s = h ? 4 + j : j;
+        const int e = h ? sel[4 + j] : sel[j];
+        mine[j] = s < k ? exp_s(__fsub_rn(row[e], x0)) : 0.0f;
+        other[j] = __shfl_xor_sync(0xffffffffu, mine[j], 16);
+    }
+    float Z = h ? other[0] : mine[0];
+#pragma unroll
+    for (int s = 1; s < 8; ++s) {
+        const float rs = (s < 4) ? (h ? other[s & 3] : mine[s & 3]) : (h ? mine[s & 3] : other[s & 3]);
+        if (s < k) Z = __fadd_rn(Z, rs);
     }
 #pragma unroll
-    for (int s = 0; s < 8; ++s) {
-        if (s < k) {
-            float v = __fdiv_rn(w[s], Z);
-            if (scale != 1.0f) v = __fmul_rn(v, scale);
-            w[s] = v;
-        }
+    for (int j = 0; j < 4; ++j) {
+        float v = __fdiv_rn(mine[j], Z);
+        if (scale != 1.0f) v = __fmul_rn(v, scale);
+        w[j] = v;
     }
 }
 
