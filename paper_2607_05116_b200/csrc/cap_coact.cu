@@ -61,6 +61,9 @@ int launch_coactivation(const int32_t *idx, const uint8_t *kept, int32_t L, int6
     if (cudaMemsetAsync(coact, 0, sizeof(int32_t) * (size_t)L * E * E, st) != cudaSuccess)
         return check_launch("memset coact");
     if (T == 0) return CAP_OK;
+    bool mma = false;
+    CAP_TRY(launch_coact_mma(idx, kept, L, T, k, E, counts, coact, st, &mma));
+    if (mma) return CAP_OK;
     const size_t smem_full = sizeof(int) * ((size_t)E * E + E);
     const int use_smem = smem_full <= 160 * 1024;
     const size_t smem = use_smem ? smem_full : sizeof(int) * (size_t)E;

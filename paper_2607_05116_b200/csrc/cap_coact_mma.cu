@@ -1,0 +1,217 @@
+// S2 fast path -- counts and the E x E co-activation matrix as an exact int8 -> int32 tensor-core
+// contraction C = A^T A of the one-hot routing matrix A [tokens x E] (BASELINE.json
+// north_star (2)).  A is never materialised in HBM: each block synthesises 128-token tiles of A^T
+// ([E rows] x [128 tokens], int8, K-major canonical core-matrix layout) in shared memory straight
+// from the index stream, and one thread issues tcgen05.mma.kind::i8 (M = 128, N = E, K = 32) with
+// the SAME tile as both operands, accumulating in TMEM.  At the end the accumulator is read back
+// with tcgen05.ld and added into the global matrix; symmetry (C[r][c] = C[c][r]) lets lane r write
+// address [c][r], which makes the atomic adds coalesced.  diag(C) gives the counts.
+#include "cap_async.cuh"
+#include "cap_internal.cuh"
+
+namespace cap {
+
+constexpr int CM_TK = 128;          // tokens per tile (4 MMAs of K = 32)
+constexpr int CM_THREADS = 128;
+
+// ---- tcgen05 wrappers ---------------------------------------------------------------------------------
+__device__ __forceinline__ void tmem_alloc(uint32_t *smem_dst, uint32_t ncols)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_dst)),
+                 "r"(ncols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void proxy_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// shared-memory matrix descriptor, K-major, no swizzle: core matrix = 8 rows x 16 bytes (contiguous
+// 128 bytes); lbo = byte step between the two K chunks of one MMA, sbo = byte step between 8-row groups
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo)
+{
+    return (uint64_t)((saddr >> 4) & 0x3fffu) | ((uint64_t)((lbo >> 4) & 0x3fffu) << 16) |
+           ((uint64_t)((sbo >> 4) & 0x3fffu) << 32) | (1ull << 46);
+}
+// D[tmem] (+)= A[smem] * B[smem]^T, int8 x int8 -> int32
+__device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                        uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n\t}" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(
+                     smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]),
+          "=r"(v[15]), "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]),
+          "=r"(v[22]), "=r"(v[23]), "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]),
+          "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+struct CoactMmaParams {
+    const int32_t *idx;        // [L][T][k]
+    const uint8_t *kept;       // [L][T][k] or NULL
+    unsigned long long *counts;   // [L][E]
+    int *coact;                // [L][E][E]
+    int64_t T, tpc;            // tokens per layer, tokens per block
+    int32_t k, E, EP;          // EP = E padded to 128 or 256 (rows of the tile)
+};
+
+template <int EP>
+__global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
+{
+    extern __shared__ __align__(1024) unsigned char cm_sm[];   // two tiles [EP rows][CM_TK tokens] int8
+    __shared__ uint64_t done_bar[2];
+    __shared__ uint32_t s_tmem;
+    constexpr int TILEB = EP * CM_TK;
+    constexpr uint32_t LBO = 128u, SBO = (CM_TK / 16) * 128u;
+    constexpr uint32_t NCOLS = EP == 128 ? 128u : 512u;
+    constexpr uint32_t IDESC = (2u << 4) | ((uint32_t)(EP >> 3) << 17) | (8u << 24);   // S32 acc, u8 x u8, N = EP, M = 128
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int layer = blockIdx.y;
+    const int E = q.E, k = q.k;
+
+    if (warp == 0) tmem_alloc(&s_tmem, NCOLS);
+    if (tid == 0) {
+        mbar_init(&done_bar[0], 1);
+        mbar_init(&done_bar[1], 1);
+        mbar_fence_init();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    const int64_t t0 = (int64_t)blockIdx.x * q.tpc;
+    const int64_t t1 = min(q.T, t0 + q.tpc);
+    const int ntile = t1 > t0 ? (int)((t1 - t0 + CM_TK - 1) / CM_TK) : 0;
+    const int32_t *idx = q.idx + (size_t)layer * q.T * k;
+    const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
+
+    for (int i = 0; i < ntile; ++i) {
+        const int buf = i & 1;
+        unsigned char *tile = cm_sm + (size_t)buf * TILEB;
+        if (i >= 2) mbar_wait(&done_bar[buf], (uint32_t)(((i >> 1) - 1) & 1));   // tile i-2 consumed
+        uint4 *t4 = reinterpret_cast<uint4 *>(tile);
+#pragma unroll
+        for (int j = 0; j < TILEB / 16 / CM_THREADS; ++j) t4[j * CM_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
+        __syncthreads();
+        const int64_t tok = t0 + (int64_t)i * CM_TK + tid;
+        if (tok < t1) {
+            unsigned char *col = tile + (tid >> 4) * LBO + (tid & 15);
+            for (int s = 0; s < k; ++s) {
+                const int64_t a = tok * k + s;
+                const int e = idx[a];
+                if ((!kept || kept[a]) && (unsigned)e < (unsigned)E) col[(e >> 3) * SBO + (e & 7) * 16] = 1;
+            }
+        }
+        proxy_fence_async();       // generic-proxy writes -> visible to the tensor core's async proxy
+        __syncthreads();
+        if (tid == 0) {
+            tc_fence_after();
+            const uint32_t base = smem_u32(tile);
+#pragma unroll
+            for (int j = 0; j < CM_TK / 32; ++j) {
+                const uint64_t b = umma_desc(base + j * 2 * LBO, LBO, SBO);
+                umma_i8(tmem, b, b, IDESC, (uint32_t)((i | j) != 0));
+                if (EP == 256) {
+                    const uint64_t a1 = umma_desc(base + 16 * SBO + j * 2 * LBO, LBO, SBO);
+                    umma_i8(tmem + 256u, a1, b, IDESC, (uint32_t)((i | j) != 0));
+                }
+            }
+            umma_commit(&done_bar[buf]);
+        }
+    }
+    if (ntile > 0) {
+        const int last = ntile - 1;
+        mbar_wait(&done_bar[last & 1], (uint32_t)((last >> 1) & 1));
+        tc_fence_after();
+        int *C = q.coact + (size_t)layer * E * E;
+        unsigned long long *cnt = q.counts + (size_t)layer * E;
+#pragma unroll 1
+        for (int h = 0; h < EP / 128; ++h) {
+            const int r = h * 128 + warp * 32 + lane;          // accumulator row of this thread
+#pragma unroll 1
+            for (int cb = 0; cb < EP / 32; ++cb) {
+                uint32_t v[32];
+                tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(h * 256 + cb * 32), v);
+#pragma unroll
+                for (int j = 0; j < 32; ++j) {
+                    const int c = cb * 32 + j;
+                    if (r < E && c < E && v[j]) {
+                        atomicAdd(&C[(size_t)c * E + r], (int)v[j]);     // C symmetric: [c][r] is coalesced
+                        if (c == r) atomicAdd(&cnt[r], (unsigned long long)v[j]);
+                    }
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, NCOLS);
+}
+
+template <int EP>
+static int launch_ep(const CoactMmaParams &prm, int L, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(coact_mma_kernel<EP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * EP * CM_TK);
+        attr_set = true;
+    }
+    const int64_t nblk = (prm.T + prm.tpc - 1) / prm.tpc;
+    {
+        KernelTimerScope ts("coact", st);
+        coact_mma_kernel<EP><<<dim3((unsigned)nblk, (unsigned)L), CM_THREADS, 2 * EP * CM_TK, st>>>(prm);
+    }
+    note_launch();
+    return check_launch("coact_mma_kernel");
+}
+
+// counts / coact must already be zeroed.  *used = false when E > 256 (generic kernel instead).
+int launch_coact_mma(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k, int32_t E,
+                     int64_t *counts, int32_t *coact, cudaStream_t st, bool *used)
+{
+    *used = false;
+    if (E > 256 || T < 1 || L < 1) return CAP_OK;
+    CoactMmaParams prm;
+    prm.idx = idx;
+    prm.kept = kept;
+    prm.counts = reinterpret_cast<unsigned long long *>(counts);
+    prm.coact = coact;
+    prm.T = T;
+    prm.k = k;
+    prm.E = E;
+    prm.EP = E <= 128 ? 128 : 256;
+    int64_t want = ((int64_t)sm_count() + L - 1) / L;
+    if (want < 1) want = 1;
+    int64_t tpc = (T + want - 1) / want;
+    tpc = ((tpc + CM_TK - 1) / CM_TK) * CM_TK;
+    prm.tpc = tpc;
+    *used = true;
+    return prm.EP == 128 ? launch_ep<128>(prm, L, st) : launch_ep<256>(prm, L, st);
+}
+
+}  // namespace cap

@@ -324,8 +324,8 @@ struct DecodeParams {
 #define CAP_DEC_ADD(ACC, MASK)                                        \
     do {                                                              \
         uint32_t cy = 0u;                                             \
-        _Pragma("unroll") for (int p = 0; p < 32; ++p) {              \
-            if (p < q.na) {                                           \
+        _Pragma("unroll") for (int p = 0; p < NA; ++p) {              \
+            if (p < NA) {                                           \
                 const uint32_t xx = p < EF_NPL ? (a[p < EF_NPL ? p : 0] & (MASK)) : 0u; \
                 const uint32_t s = lop_xor3(ACC[p], xx, cy);          \
                 cy = lop_maj(ACC[p], xx, cy);                         \
@@ -337,8 +337,8 @@ struct DecodeParams {
 #define CAP_DEC_ADD32(ACC)                                            \
     do {                                                              \
         uint32_t cy = 0u;                                             \
-        _Pragma("unroll") for (int p = 0; p < 32; ++p) {              \
-            if (p < q.na) {                                           \
+        _Pragma("unroll") for (int p = 0; p < NA; ++p) {              \
+            if (p < NA) {                                           \
                 const uint32_t s = lop_xor3(ACC[p], a[p], cy);        \
                 cy = lop_maj(ACC[p], a[p], cy);                       \
                 ACC[p] = s;                                           \
@@ -349,8 +349,8 @@ struct DecodeParams {
 #define CAP_DEC_BFLY(ACC, OFF)                                        \
     do {                                                              \
         uint32_t cy = 0u;                                             \
-        _Pragma("unroll") for (int p = 0; p < 32; ++p) {              \
-            if (p < q.na) {                                           \
+        _Pragma("unroll") for (int p = 0; p < NA; ++p) {              \
+            if (p < NA) {                                           \
                 const uint32_t xx = __shfl_xor_sync(0xffffffffu, ACC[p], OFF); \
                 const uint32_t s = lop_xor3(ACC[p], xx, cy);          \
                 cy = lop_maj(ACC[p], xx, cy);                         \
@@ -360,11 +360,12 @@ struct DecodeParams {
     } while (0)
 
 constexpr int DEC_WARPS = 4;
+template <int NA>
 __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParams q)
 {
     __shared__ unsigned long long nodeset[8];
     __shared__ unsigned char s_dn[64];
-    __shared__ uint32_t s_part[DEC_WARPS - 1][3][32];
+    __shared__ uint32_t s_part[DEC_WARPS - 1][3][NA];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int w = blockIdx.x, pc = blockIdx.y, layer = blockIdx.z;
     if (threadIdx.x < 64) s_dn[threadIdx.x] = (int)threadIdx.x < q.D ? (unsigned char)q.dev_node[threadIdx.x] : 0;
@@ -377,11 +378,11 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
     }
     __syncthreads();
     const bool devword = w < q.DW;
-    uint32_t tot[32], loc[32], sam[32];
+    uint32_t tot[NA], loc[NA], sam[NA];
 #pragma unroll
-    for (int p = 0; p < 32; ++p) tot[p] = loc[p] = sam[p] = 0u;
+    for (int p = 0; p < NA; ++p) tot[p] = loc[p] = sam[p] = 0u;
     const size_t sbase = ((size_t)layer * q.PC + pc) * q.nslots;
-    constexpr int DEC_SL = 4;     // record slots a thread has in flight
+    constexpr int DEC_SL = 2;     // record slots a thread has in flight
     for (int s0 = threadIdx.x; s0 < q.nslots; s0 += 32 * DEC_WARPS * DEC_SL) {
         int srcs[DEC_SL];
 #pragma unroll
@@ -425,7 +426,7 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
     // every lane of a warp now holds the warp's sums; warps 1.. hand theirs to warp 0
     if (warp > 0 && lane < 3) {
 #pragma unroll
-        for (int p = 0; p < 32; ++p) {
+        for (int p = 0; p < NA; ++p) {
             const uint32_t v = lane == 0 ? tot[p] : lane == 1 ? loc[p] : sam[p];
             s_part[warp - 1][lane][p] = v;
         }
@@ -433,21 +434,21 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
     __syncthreads();
     if (warp > 0) return;
     for (int o = 0; o < DEC_WARPS - 1; ++o) {
-        uint32_t a[32];
+        uint32_t a[NA];
 #pragma unroll
-        for (int p = 0; p < 32; ++p) a[p] = s_part[o][0][p];
+        for (int p = 0; p < NA; ++p) a[p] = s_part[o][0][p];
         CAP_DEC_ADD32(tot);
 #pragma unroll
-        for (int p = 0; p < 32; ++p) a[p] = s_part[o][1][p];
+        for (int p = 0; p < NA; ++p) a[p] = s_part[o][1][p];
         CAP_DEC_ADD32(loc);
 #pragma unroll
-        for (int p = 0; p < 32; ++p) a[p] = s_part[o][2][p];
+        for (int p = 0; p < NA; ++p) a[p] = s_part[o][2][p];
         CAP_DEC_ADD32(sam);
     }
     unsigned long long vt = 0ull, vl = 0ull, vs = 0ull;
 #pragma unroll
-    for (int p = 0; p < 32; ++p) {
-        if (p < q.na) {
+    for (int p = 0; p < NA; ++p) {
+        {
             vt |= (unsigned long long)((tot[p] >> lane) & 1u) << p;
             vl |= (unsigned long long)((loc[p] >> lane) & 1u) << p;
             vs |= (unsigned long long)((sam[p] >> lane) & 1u) << p;
@@ -572,7 +573,13 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     dq.na = na;
     {
         KernelTimerScope ts("eval_decode", st);
-        eval_decode_kernel<<<dim3((unsigned)g.W, (unsigned)g.PC, (unsigned)L), 32 * DEC_WARPS, 0, st>>>(dq);
+        const dim3 dgrid((unsigned)g.W, (unsigned)g.PC, (unsigned)L);
+        if (na <= 12) eval_decode_kernel<12><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
+        else if (na <= 16) eval_decode_kernel<16><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
+        else if (na <= 20) eval_decode_kernel<20><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
+        else if (na <= 24) eval_decode_kernel<24><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
+        else if (na <= 28) eval_decode_kernel<28><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
+        else eval_decode_kernel<32><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
     }
     note_launch();
     CAP_TRY(check_launch("eval_decode_kernel"));
