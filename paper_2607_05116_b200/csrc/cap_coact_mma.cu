@@ -13,6 +13,7 @@ namespace cap {
 
 constexpr int CM_TK = 128;          // tokens per tile (4 MMAs of K = 32)
 constexpr int CM_THREADS = 128;
+constexpr int CM_NB = 4;            // tiles whose indices are fetched together
 
 // ---- tcgen05 wrappers ---------------------------------------------------------------------------------
 __device__ __forceinline__ void tmem_alloc(uint32_t *smem_dst, uint32_t ncols)
@@ -77,9 +78,10 @@ struct CoactMmaParams {
     int *coact;                // [L][E][E]
     int64_t T, tpc;            // tokens per layer, tokens per block
     int32_t k, E, EP;          // EP = E padded to 128 or 256 (rows of the tile)
+    int32_t pack64;            // E even and coact 8-byte aligned: pairs of counters per 64-bit reduction
 };
 
-template <int EP>
+template <int EP, int KMAX>
 __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
 {
     extern __shared__ __align__(1024) unsigned char cm_sm[];   // two tiles [EP rows][CM_TK tokens] int8
@@ -110,38 +112,80 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
     const int32_t *idx = q.idx + (size_t)layer * q.T * k;
     const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
 
-    for (int i = 0; i < ntile; ++i) {
-        const int buf = i & 1;
-        unsigned char *tile = cm_sm + (size_t)buf * TILEB;
-        if (i >= 2) mbar_wait(&done_bar[buf], (uint32_t)(((i >> 1) - 1) & 1));   // tile i-2 consumed
-        uint4 *t4 = reinterpret_cast<uint4 *>(tile);
+    // The thread's token of each tile: its k expert rows as byte offsets into the tile (-1 = not
+    // kept).  Indices are fetched for CM_NB tiles at a time, so the global-load latency is paid once
+    // per batch instead of once per tile.
+    for (int ib = 0; ib < ntile; ib += CM_NB) {
+        int rowoff[CM_NB][KMAX];
+        // issue every load of the batch first (raw expert ids; -1 = absent), then turn them into offsets
+        const bool vec8 = KMAX == 8 && k == 8 && !kept && (reinterpret_cast<uintptr_t>(idx) & 15u) == 0;
 #pragma unroll
-        for (int j = 0; j < TILEB / 16 / CM_THREADS; ++j) t4[j * CM_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
-        __syncthreads();
-        const int64_t tok = t0 + (int64_t)i * CM_TK + tid;
-        if (tok < t1) {
-            unsigned char *col = tile + (tid >> 4) * LBO + (tid & 15);
-            for (int s = 0; s < k; ++s) {
-                const int64_t a = tok * k + s;
-                const int e = idx[a];
-                if ((!kept || kept[a]) && (unsigned)e < (unsigned)E) col[(e >> 3) * SBO + (e & 7) * 16] = 1;
-            }
-        }
-        proxy_fence_async();       // generic-proxy writes -> visible to the tensor core's async proxy
-        __syncthreads();
-        if (tid == 0) {
-            tc_fence_after();
-            const uint32_t base = smem_u32(tile);
+        for (int u = 0; u < CM_NB; ++u) {
+            const int64_t tok = t0 + (int64_t)(ib + u) * CM_TK + tid;
+            if (vec8) {
+                int4 lo = make_int4(-1, -1, -1, -1), hi = lo;
+                if (tok < t1) {
+                    lo = __ldg(reinterpret_cast<const int4 *>(idx + tok * 8));
+                    hi = __ldg(reinterpret_cast<const int4 *>(idx + tok * 8) + 1);
+                }
+                rowoff[u][0] = lo.x; rowoff[u][1] = lo.y; rowoff[u][2] = lo.z; rowoff[u][3] = lo.w;
+                rowoff[u][4 % KMAX] = hi.x; rowoff[u][5 % KMAX] = hi.y; rowoff[u][6 % KMAX] = hi.z;
+                rowoff[u][7 % KMAX] = hi.w;
+            } else {
 #pragma unroll
-            for (int j = 0; j < CM_TK / 32; ++j) {
-                const uint64_t b = umma_desc(base + j * 2 * LBO, LBO, SBO);
-                umma_i8(tmem, b, b, IDESC, (uint32_t)((i | j) != 0));
-                if (EP == 256) {
-                    const uint64_t a1 = umma_desc(base + 16 * SBO + j * 2 * LBO, LBO, SBO);
-                    umma_i8(tmem + 256u, a1, b, IDESC, (uint32_t)((i | j) != 0));
+                for (int s = 0; s < KMAX; ++s) {
+                    int e = -1;
+                    if (s < k && tok < t1) {
+                        const int64_t a = tok * k + s;
+                        e = __ldg(idx + a);
+                        if (kept && !__ldg(kept + a)) e = -1;
+                    }
+                    rowoff[u][s] = e;
                 }
             }
-            umma_commit(&done_bar[buf]);
+        }
+#pragma unroll
+        for (int u = 0; u < CM_NB; ++u) {
+#pragma unroll
+            for (int s = 0; s < KMAX; ++s) {
+                const int e = rowoff[u][s];
+                rowoff[u][s] = (unsigned)e < (unsigned)E ? (e >> 3) * (int)SBO + (e & 7) * 16 : -1;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < CM_NB; ++u) {
+            const int i = ib + u;
+            if (i >= ntile) break;
+            const int buf = i & 1;
+            unsigned char *tile = cm_sm + (size_t)buf * TILEB;
+            if (i >= 2) mbar_wait(&done_bar[buf], (uint32_t)(((i >> 1) - 1) & 1));   // tile i-2 consumed
+            uint4 *t4 = reinterpret_cast<uint4 *>(tile);
+#pragma unroll
+            for (int j = 0; j < TILEB / 16 / CM_THREADS; ++j)
+                t4[j * CM_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
+            __syncthreads();
+            {
+                unsigned char *col = tile + (tid >> 4) * LBO + (tid & 15);
+#pragma unroll
+                for (int s = 0; s < KMAX; ++s)
+                    if (rowoff[u][s] >= 0) col[rowoff[u][s]] = 1;
+            }
+            proxy_fence_async();   // generic-proxy writes -> visible to the tensor core's async proxy
+            __syncthreads();
+            if (tid == 0) {
+                tc_fence_after();
+                const uint32_t base = smem_u32(tile);
+#pragma unroll
+                for (int j = 0; j < CM_TK / 32; ++j) {
+                    const uint64_t bd = umma_desc(base + j * 2 * LBO, LBO, SBO);
+                    umma_i8(tmem, bd, bd, IDESC, (uint32_t)((i | j) != 0));
+                    if (EP == 256) {
+                        const uint64_t a1 = umma_desc(base + 16 * SBO + j * 2 * LBO, LBO, SBO);
+                        umma_i8(tmem + 256u, a1, bd, IDESC, (uint32_t)((i | j) != 0));
+                    }
+                }
+                umma_commit(&done_bar[buf]);
+            }
         }
     }
     if (ntile > 0) {
@@ -154,16 +198,41 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
         for (int h = 0; h < EP / 128; ++h) {
             const int r = h * 128 + warp * 32 + lane;          // accumulator row of this thread
 #pragma unroll 1
-            for (int cb = 0; cb < EP / 32; ++cb) {
+            for (int cb0 = 0; cb0 < EP / 32; ++cb0) {
+                // blocks start at different column groups so that they do not queue on the same L2 lines
+                const int cb = (cb0 + (int)blockIdx.x) % (EP / 32);
                 uint32_t v[32];
                 tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(h * 256 + cb * 32), v);
+                // C symmetric: the value of (r, c) is added at [c][r], consecutive lanes -> consecutive
+                // addresses.  Two neighbouring int32 counters are added with ONE 64-bit reduction
+                // (counts are < 2^31, so the low word never carries into the high word): even lanes
+                // take even columns, odd lanes odd columns, each packing its own and its neighbour's value.
+                const bool rok = r < E;
+                if (q.pack64) {
+                    int *cp = C + (size_t)(cb * 32) * E + (r & ~1);
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const int c = cb * 32 + j;
-                    if (r < E && c < E && v[j]) {
-                        atomicAdd(&C[(size_t)c * E + r], (int)v[j]);     // C symmetric: [c][r] is coalesced
-                        if (c == r) atomicAdd(&cnt[r], (unsigned long long)v[j]);
+                    for (int j = 0; j < 32; j += 2) {
+                        const uint32_t p0 = __shfl_xor_sync(0xffffffffu, v[j], 1);
+                        const uint32_t p1 = __shfl_xor_sync(0xffffffffu, v[j + 1], 1);
+                        const int jj = j + (lane & 1);
+                        const unsigned long long pk = (lane & 1) ? ((unsigned long long)v[j + 1] << 32) | p1
+                                                                 : ((unsigned long long)p0 << 32) | v[j];
+                        if (rok && cb * 32 + jj < E)
+                            asm volatile("red.global.add.u64 [%0], %1;" ::"l"(cp + (size_t)jj * E), "l"(pk) : "memory");
                     }
+                } else {
+                    int *cp = C + (size_t)(cb * 32) * E + r;
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) {
+                        if (rok && cb * 32 + j < E)
+                            asm volatile("red.global.add.s32 [%0], %1;" ::"l"(cp + (size_t)j * E), "r"(v[j]) : "memory");
+                    }
+                }
+                if (rok && (r >> 5) == cb) {
+                    uint32_t d = 0u;
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) d = (r & 31) == j ? v[j] : d;
+                    atomicAdd(&cnt[r], (unsigned long long)d);
                 }
             }
         }
@@ -173,18 +242,19 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
     if (warp == 0) tmem_dealloc(tmem, NCOLS);
 }
 
-template <int EP>
+template <int EP, int KMAX>
 static int launch_ep(const CoactMmaParams &prm, int L, cudaStream_t st)
 {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(coact_mma_kernel<EP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 2 * EP * CM_TK);
+        cudaFuncSetAttribute(coact_mma_kernel<EP, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             2 * EP * CM_TK);
         attr_set = true;
     }
     const int64_t nblk = (prm.T + prm.tpc - 1) / prm.tpc;
     {
         KernelTimerScope ts("coact", st);
-        coact_mma_kernel<EP><<<dim3((unsigned)nblk, (unsigned)L), CM_THREADS, 2 * EP * CM_TK, st>>>(prm);
+        coact_mma_kernel<EP, KMAX><<<dim3((unsigned)nblk, (unsigned)L), CM_THREADS, 2 * EP * CM_TK, st>>>(prm);
     }
     note_launch();
     return check_launch("coact_mma_kernel");
@@ -205,13 +275,15 @@ int launch_coact_mma(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     prm.k = k;
     prm.E = E;
     prm.EP = E <= 128 ? 128 : 256;
+    prm.pack64 = (E % 2 == 0) && (reinterpret_cast<uintptr_t>(coact) & 7u) == 0;
     int64_t want = ((int64_t)sm_count() + L - 1) / L;
     if (want < 1) want = 1;
     int64_t tpc = (T + want - 1) / want;
     tpc = ((tpc + CM_TK - 1) / CM_TK) * CM_TK;
     prm.tpc = tpc;
     *used = true;
-    return prm.EP == 128 ? launch_ep<128>(prm, L, st) : launch_ep<256>(prm, L, st);
+    if (prm.EP == 128) return k <= 8 ? launch_ep<128, 8>(prm, L, st) : launch_ep<128, 16>(prm, L, st);
+    return k <= 8 ? launch_ep<256, 8>(prm, L, st) : launch_ep<256, 16>(prm, L, st);
 }
 
 }  // namespace cap
