@@ -249,6 +249,11 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
     if ((int64_t)L * P >= ((int64_t)1 << 31)) return CAP_EINVAL;
     if (!ws || ws_bytes < eval_ws_bytes(L, T, cfg->E, cfg->k, topo->D, P)) return CAP_EWORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
+    if (L == 0) return CAP_OK;
+    bool fused = false;
+    CAP_TRY(launch_trace_fused_fast(logits, bias, L, T, *cfg, topk_idx, topk_w, counts, coact, token_src,
+                                    expert_dev, P, *topo, *out, ws, st, &fused));
+    if (fused) return CAP_OK;
     CAP_TRY(launch_gate_topk(logits, bias, L, T, *cfg, topk_idx, topk_w, st));
     CAP_TRY(launch_coactivation(topk_idx, nullptr, L, T, cfg->k, cfg->E, counts, coact, st));
     return launch_eval(topk_idx, nullptr, token_src, L, T, cfg->k, cfg->E, expert_dev, P,

@@ -251,6 +251,44 @@ __global__ void __launch_bounds__(32 * FIN_WARPS) eval_finalize_kernel(FinalPara
         f.out.imbalance_recv[o] = smr ? __ddiv_rn((double)(mxr * f.D), (double)smr) : 0.0;
 }
 
+// last step of every S3 path: per-candidate sums, costs, load_pairs from the counts, imbalance
+int launch_eval_finalize(int32_t L, int32_t E, int32_t P, const int32_t *expert_dev, const cap_topology &topo,
+                         const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st)
+{
+    EvalWs w = eval_ws_carve(ws, L, E, topo.D, P);
+    FinalParams f;
+    f.acc = w.acc;
+    f.recv = w.recv;
+    f.counts = reinterpret_cast<const long long *>(counts);
+    f.expert_dev = expert_dev;
+    f.out = out;
+    f.L = L;
+    f.P = P;
+    f.E = E;
+    f.D = topo.D;
+    f.cost_local = topo.cost_local;
+    f.cost_intra = topo.cost_intra;
+    f.cost_inter = topo.cost_inter;
+    f.bytes_per_token = topo.bytes_per_token;
+    const int n = L * P;
+    {
+        KernelTimerScope ts("eval_finalize", st);
+        eval_finalize_kernel<<<(n + FIN_WARPS - 1) / FIN_WARPS, 32 * FIN_WARPS, 0, st>>>(f);
+    }
+    note_launch();
+    return check_launch("eval_finalize_kernel");
+}
+
+// zero the accumulators of the evaluation workspace (acc, recv and, if wanted, mcounts)
+int eval_zero_ws(int32_t L, int32_t E, int32_t D, int32_t P, bool with_mcounts, void *ws, cudaStream_t st)
+{
+    EvalWs w = eval_ws_carve(ws, L, E, D, P);
+    const size_t zero_bytes = sizeof(unsigned long long) *
+                              ((size_t)L * P * ACC_N + (size_t)L * P * D + (with_mcounts ? (size_t)L * E : 0));
+    if (cudaMemsetAsync(w.acc, 0, zero_bytes, st) != cudaSuccess) return check_launch("memset eval ws");
+    return CAP_OK;
+}
+
 static size_t eval_smem_bytes(int E, int D, int PC, bool want_tok)
 {
     return 64 * 8 + sizeof(int) * (EV_TT * 16 + EV_TT) + sizeof(int) * (size_t)D * PC + EV_TT * 16 + 64 +
@@ -265,9 +303,7 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
     if (L == 0 || P == 0) return CAP_OK;
     const int D = topo.D;
     EvalWs w = eval_ws_carve(ws, L, E, D, P);
-    const size_t zero_bytes = sizeof(unsigned long long) *
-                              ((size_t)L * P * ACC_N + (size_t)L * P * D + (counts ? 0 : (size_t)L * E));
-    if (cudaMemsetAsync(w.acc, 0, zero_bytes, st) != cudaSuccess) return check_launch("memset eval ws");
+    CAP_TRY(eval_zero_ws(L, E, D, P, counts == nullptr, ws, st));
 
     const bool want_tok = out.tok_remote_dev || out.tok_remote_node;
     if (T > 0) {
@@ -329,28 +365,7 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
             CAP_TRY(check_launch("eval_generic_kernel"));
         }
     }
-    FinalParams f;
-    f.acc = w.acc;
-    f.recv = w.recv;
-    f.counts = counts ? reinterpret_cast<const long long *>(counts)
-                      : reinterpret_cast<const long long *>(w.mcounts);
-    f.expert_dev = expert_dev;
-    f.out = out;
-    f.L = L;
-    f.P = P;
-    f.E = E;
-    f.D = D;
-    f.cost_local = topo.cost_local;
-    f.cost_intra = topo.cost_intra;
-    f.cost_inter = topo.cost_inter;
-    f.bytes_per_token = topo.bytes_per_token;
-    const int n = L * P;
-    {
-        KernelTimerScope ts("eval_finalize", st);
-        eval_finalize_kernel<<<(n + FIN_WARPS - 1) / FIN_WARPS, 32 * FIN_WARPS, 0, st>>>(f);
-    }
-    note_launch();
-    return check_launch("eval_finalize_kernel");
+    return launch_eval_finalize(L, E, P, expert_dev, topo, counts ? counts : reinterpret_cast<const int64_t *>(w.mcounts), out, ws, st);
 }
 
 }  // namespace cap

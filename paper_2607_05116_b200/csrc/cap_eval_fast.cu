@@ -93,7 +93,8 @@ size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D,
         const size_t b = g.rec_slots * 4 + 256 + g.rec_words * 4 + 256 + g.table_words * 4 + 256;
         if (b > best) best = b;
     }
-    return best;
+    const size_t fb = fused_ws_bytes(L, T, k, E, D, P);
+    return fb > best ? fb : best;
 }
 
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
@@ -498,59 +499,38 @@ static int launch_kp(const EvalFastParams &prm, const EvalFastGeom &g, int L, cu
     return check_launch("eval_fast_kernel");
 }
 
-int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
-                     int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
-                     void *ws, cudaStream_t st, bool *used)
+// builds the one-hot code tables of all layers and candidate chunks (g.table_words words at fw.table)
+int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *expert_dev, const int32_t *dev_node,
+                    int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st)
 {
-    *used = false;
-    EvalFastGeom g;
-    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g)) return CAP_OK;
-    EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g);
-    EvalWs base = eval_ws_carve(ws, L, E, topo.D, P);
-    if (cudaMemsetAsync(fw.rec_src, 0xff, g.rec_slots * 4, st) != cudaSuccess)
-        return check_launch("memset rec_src");
-    EvalFastParams prm;
-    prm.idx = idx;
-    prm.kept = kept;
+    EvalFastParams prm = {};
     prm.expert_dev = expert_dev;
-    prm.dev_node = topo.dev_node;
-    prm.rec_src = fw.rec_src;
-    prm.rec_planes = fw.rec_planes;
+    prm.dev_node = dev_node;
     prm.table = fw.table;
-    prm.T = T;
-    prm.tpc = g.tpc;
-    prm.k = k;
     prm.E = E;
     prm.P = P;
-    prm.D = topo.D;
+    prm.D = D;
     prm.WD = g.WD;
     prm.WN = g.WN;
     prm.Pc = g.Pc;
     prm.PC = g.PC;
     prm.DW = g.DW;
     prm.NW = g.NW;
-    prm.R = g.R;
     prm.RS = g.RS;
-    prm.S = g.S;
-    prm.logS = g.logS;
-    prm.ncta_t = g.ncta_t;
-    prm.maxrec = g.maxrec;
-    prm.NPR = g.NPR;
+    const int nw = (E + 1) * g.RS * 4;
     {
-        const int nw = (E + 1) * g.RS * 4;
         KernelTimerScope ts("eval_table", st);
         eval_table_kernel<<<dim3((unsigned)((nw + 255) / 256), (unsigned)g.PC, (unsigned)L), 256, 0, st>>>(prm);
     }
     note_launch();
-    CAP_TRY(check_launch("eval_table_kernel"));
-    int rc;
-    switch (g.KP) {
-    case 4: rc = launch_kp<4>(prm, g, L, st); break;
-    case 8: rc = launch_kp<8>(prm, g, L, st); break;
-    case 12: rc = launch_kp<12>(prm, g, L, st); break;
-    default: rc = launch_kp<16>(prm, g, L, st); break;
-    }
-    CAP_TRY(rc);
+    return check_launch("eval_table_kernel");
+}
+
+// adds all records (g.ncta_t * g.maxrec slots per layer and chunk) into acc / recv of the generic workspace
+int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int32_t L, int64_t T, int32_t E,
+                     int32_t P, const cap_topology &topo, cudaStream_t st)
+{
+    EvalWs base = eval_ws_carve(ws, L, E, topo.D, P);
     DecodeParams dq;
     dq.rec_src = fw.rec_src;
     dq.rec_planes = fw.rec_planes;
@@ -582,7 +562,56 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
         else eval_decode_kernel<32><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
     }
     note_launch();
-    CAP_TRY(check_launch("eval_decode_kernel"));
+    return check_launch("eval_decode_kernel");
+}
+
+int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
+                     int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                     void *ws, cudaStream_t st, bool *used)
+{
+    *used = false;
+    EvalFastGeom g;
+    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g)) return CAP_OK;
+    EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g);
+    if (cudaMemsetAsync(fw.rec_src, 0xff, g.rec_slots * 4, st) != cudaSuccess)
+        return check_launch("memset rec_src");
+    CAP_TRY(ef_launch_table(g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st));
+    EvalFastParams prm;
+    prm.idx = idx;
+    prm.kept = kept;
+    prm.expert_dev = expert_dev;
+    prm.dev_node = topo.dev_node;
+    prm.rec_src = fw.rec_src;
+    prm.rec_planes = fw.rec_planes;
+    prm.table = fw.table;
+    prm.T = T;
+    prm.tpc = g.tpc;
+    prm.k = k;
+    prm.E = E;
+    prm.P = P;
+    prm.D = topo.D;
+    prm.WD = g.WD;
+    prm.WN = g.WN;
+    prm.Pc = g.Pc;
+    prm.PC = g.PC;
+    prm.DW = g.DW;
+    prm.NW = g.NW;
+    prm.R = g.R;
+    prm.RS = g.RS;
+    prm.S = g.S;
+    prm.logS = g.logS;
+    prm.ncta_t = g.ncta_t;
+    prm.maxrec = g.maxrec;
+    prm.NPR = g.NPR;
+    int rc;
+    switch (g.KP) {
+    case 4: rc = launch_kp<4>(prm, g, L, st); break;
+    case 8: rc = launch_kp<8>(prm, g, L, st); break;
+    case 12: rc = launch_kp<12>(prm, g, L, st); break;
+    default: rc = launch_kp<16>(prm, g, L, st); break;
+    }
+    CAP_TRY(rc);
+    CAP_TRY(ef_launch_decode(g, fw, ws, L, T, E, P, topo, st));
     *used = true;
     return CAP_OK;
 }

@@ -55,6 +55,11 @@ struct EvalFastWs {
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
                               const EvalFastGeom &g);
 
+int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *expert_dev, const int32_t *dev_node,
+                    int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st);
+int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int32_t L, int64_t T, int32_t E,
+                     int32_t P, const cap_topology &topo, cudaStream_t st);
+
 // ---- device helpers ------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lop_xor3(uint32_t a, uint32_t b, uint32_t c)
 {

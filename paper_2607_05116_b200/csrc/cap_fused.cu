@@ -1,0 +1,605 @@
+// cap_trace_fused fast path: S1 (gate top-k) + S2 (counts / co-activation) + S3 (scoring of P candidate
+// placements) in ONE persistent, warp-specialised kernel that reads the logits exactly once
+// (BASELINE.json north_star, L104/L148, L58/Eq. 3/Eq. 4).  One block per SM, roles:
+//   warp 0        producer: TMA bulk copies of 16-token logits tiles into a shared-memory ring, and
+//                 the one-hot code table of cap_eval_fast.cuh (prebuilt by eval_table_kernel)
+//   warp 1        tensor-core warp: issues tcgen05.mma.kind::i8 on the one-hot tiles (C += A^T A in
+//                 TMEM), recycles the tile buffers
+//   warps 2..9    S1: two lanes per token selection network (cap_gate_fast.cuh); besides top-k
+//                 indices / weights to HBM they leave (a) the token's table-row offsets in a
+//                 shared-memory ring for S3 and (b) its one-hot bytes in the current MMA tile
+//   warps 10..    S3: bit-sliced candidate scoring (cap_eval_fast.cuh) fed from the offsets ring;
+//                 at the end four of them drain the TMEM accumulator into the global matrix.
+// Everything is handed over through mbarriers; only run flushes use a named barrier among the S3
+// warps.  Records / decode / finalize are those of the standalone S3 path.
+#include "cap_async.cuh"
+#include "cap_eval_fast.cuh"
+#include "cap_gate_fast.cuh"
+#include "cap_tc.cuh"
+
+namespace cap {
+
+constexpr int FU_NC = 8;            // S1 warps
+constexpr int FU_S3W0 = 2 + FU_NC;  // first S3 warp
+constexpr int FU_TILE = 16;         // tokens per S1 tile
+constexpr int FU_MT = 64;           // tokens per MMA tile (4 S1 tiles, 2 MMAs of K = 32)
+constexpr int FU_OB = 4;            // S3 offset blocks in the ring
+constexpr int FU_MAXST = 24;        // logits ring stages
+constexpr int FU_MAXTHREADS = 640;
+constexpr int FU_KP = 8;            // offsets per token (k <= 8, padded with the zero row)
+
+struct FusedParams {
+    const float *logits;
+    int32_t *idx;
+    float *w;
+    unsigned long long *counts;   // [L][E], zeroed
+    int *coact;                   // [L][E][E], zeroed
+    const uint32_t *table;        // [L][E + 1][RS * 4]
+    int32_t *rec_src;             // [L][ncta_t][maxrec]
+    uint32_t *rec_planes;         // [L][ncta_t][maxrec][NPR][W]
+    int64_t T;
+    int64_t tiles_per_cta;        // real 16-token tiles per block
+    float scale;
+    int32_t k, D, pack64;
+    int32_t R, RS, S, logS, maxrec, NPR, ncta_t, nst, ns3w;
+};
+
+struct FusedSmem {
+    // byte offsets into the dynamic shared memory
+    uint32_t table, xch, tiles, offs, ring, total;
+};
+
+__host__ __device__ inline FusedSmem fused_smem_layout(int E, int EP, int RS, int R, int S, int nst)
+{
+    FusedSmem m;
+    uint32_t o = 0;
+    m.ring = o;                                   // 128-byte aligned rows for the swizzled reads
+    o += (uint32_t)nst * FU_TILE * E * 4;
+    m.tiles = o;
+    o += 2u * EP * FU_MT;
+    m.table = o;
+    o += (uint32_t)(E + 1) * RS * 16;
+    m.offs = o;
+    o += (uint32_t)FU_OB * EF_PASSES * S * FU_KP * 4;
+    m.xch = o;                                    // level 0 of the sub-slot tree is the largest exchange
+    o += (uint32_t)(S / 2 > 0 ? S / 2 : 1) * R * EF_BT * 16;
+    m.total = o;
+    return m;
+}
+
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+
+// bit-sliced a += b; b has np planes of 4 words (the rest are zero)
+__device__ __forceinline__ void fu_add_planes(uint4 (&a)[EF_NPL], const uint4 *b, int stride, int np)
+{
+    uint4 carry = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+    for (int p = 0; p < EF_NPL; ++p) {
+        const uint4 x = p < np ? b[(size_t)p * stride] : make_uint4(0u, 0u, 0u, 0u);
+        uint4 s, c;
+        CAP_CSA(s.x, c.x, a[p].x, x.x, carry.x);
+        CAP_CSA(s.y, c.y, a[p].y, x.y, carry.y);
+        CAP_CSA(s.z, c.z, a[p].z, x.z, carry.z);
+        CAP_CSA(s.w, c.w, a[p].w, x.w, carry.w);
+        a[p] = s;
+        carry = c;
+    }
+}
+
+// OR of the FU_KP table rows of one token at this thread's column
+__device__ __forceinline__ uint4 fu_token_mask(const unsigned char *tblc, const uint32_t *op)
+{
+    const uint4 oa = *reinterpret_cast<const uint4 *>(op);
+    const uint4 ob = *reinterpret_cast<const uint4 *>(op + 4);
+    const uint4 v0 = *reinterpret_cast<const uint4 *>(tblc + oa.x);
+    const uint4 v1 = *reinterpret_cast<const uint4 *>(tblc + oa.y);
+    const uint4 v2 = *reinterpret_cast<const uint4 *>(tblc + oa.z);
+    const uint4 v3 = *reinterpret_cast<const uint4 *>(tblc + oa.w);
+    const uint4 v4 = *reinterpret_cast<const uint4 *>(tblc + ob.x);
+    const uint4 v5 = *reinterpret_cast<const uint4 *>(tblc + ob.y);
+    const uint4 v6 = *reinterpret_cast<const uint4 *>(tblc + ob.z);
+    const uint4 v7 = *reinterpret_cast<const uint4 *>(tblc + ob.w);
+    uint4 m;
+    m.x = lop_or3(lop_or3(lop_or3(v0.x, v1.x, v2.x), v3.x, v4.x), lop_or3(v5.x, v6.x, v7.x), 0u);
+    m.y = lop_or3(lop_or3(lop_or3(v0.y, v1.y, v2.y), v3.y, v4.y), lop_or3(v5.y, v6.y, v7.y), 0u);
+    m.z = lop_or3(lop_or3(lop_or3(v0.z, v1.z, v2.z), v3.z, v4.z), lop_or3(v5.z, v6.z, v7.z), 0u);
+    m.w = lop_or3(lop_or3(lop_or3(v0.w, v1.w, v2.w), v3.w, v4.w), lop_or3(v5.w, v6.w, v7.w), 0u);
+    return m;
+}
+
+// half a Harley-Seal block: four token masks into planes 0/1, carry of weight 4 out
+#define CAP_FU_HALF(F, X0, X1, X2, X3, OUT4)            \
+    do {                                                \
+        uint32_t tA, tB, s;                             \
+        CAP_CSA(s, tA, pl[0].F, (X0).F, (X1).F);        \
+        CAP_CSA(s, tB, s, (X2).F, (X3).F);              \
+        pl[0].F = s;                                    \
+        CAP_CSA(pl[1].F, OUT4, pl[1].F, tA, tB);        \
+    } while (0)
+// weight-4 carries of the two halves into plane 2, weight-8 carry rippled into planes 3..EF_BT-1
+#define CAP_FU_TOP(F, FA, FB)                           \
+    do {                                                \
+        uint32_t e8;                                    \
+        CAP_CSA(pl[2].F, e8, pl[2].F, FA, FB);          \
+        _Pragma("unroll") for (int p = 3; p < EF_BT; ++p) { \
+            const uint32_t c = pl[p].F & e8;            \
+            pl[p].F ^= e8;                              \
+            e8 = c;                                     \
+        }                                               \
+    } while (0)
+
+template <int E>
+__global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedParams q)
+{
+    extern __shared__ __align__(1024) unsigned char fu_sm[];
+    __shared__ uint64_t full_bar[FU_MAXST], empty_bar[FU_MAXST];
+    __shared__ uint64_t offs_full[FU_OB], offs_empty[FU_OB];
+    __shared__ uint64_t tile_full[2], tile_ready[2], mma_done[2];
+    __shared__ uint64_t tbl_bar, acc_done;
+    __shared__ uint32_t s_tmem;
+    constexpr int EP = E <= 128 ? 128 : 256;
+    constexpr uint32_t LBO = 128u, SBO = (FU_MT / 16) * 128u;
+    constexpr uint32_t NCOLS = EP == 128 ? 128u : 512u;
+    constexpr uint32_t IDESC = (2u << 4) | ((uint32_t)(EP >> 3) << 17) | (8u << 24);
+    constexpr int TILE_BYTES = FU_TILE * E * 4;
+    constexpr int MT_TILES = FU_MT / FU_TILE;          // S1 tiles per MMA tile
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int layer = blockIdx.y;
+    const int S = q.S, R = q.R, nst = q.nst, k = q.k;
+    const int BT = EF_PASSES * S;                       // tokens per S3 block
+    const int TPB = BT / FU_TILE;                       // S1 tiles per S3 block
+    const FusedSmem lay = fused_smem_layout(E, EP, q.RS, R, S, nst);
+    unsigned char *ring = fu_sm + lay.ring;
+    unsigned char *tiles = fu_sm + lay.tiles;
+    unsigned char *tbl = fu_sm + lay.table;
+    uint32_t *offs = reinterpret_cast<uint32_t *>(fu_sm + lay.offs);
+    uint4 *xch = reinterpret_cast<uint4 *>(fu_sm + lay.xch);
+    const int rowb = q.RS * 16;
+    const uint32_t zero_row = (uint32_t)E * rowb;
+    const int ns3 = q.ns3w * 32;
+
+    // ---- this block's token range (whole 16-token tiles of one layer) ----
+    const int64_t T = q.T;
+    const int64_t ltiles = (T + FU_TILE - 1) / FU_TILE;
+    const int64_t tile0 = (int64_t)blockIdx.x * q.tiles_per_cta;
+    int64_t nt64 = ltiles - tile0;
+    if (nt64 > q.tiles_per_cta) nt64 = q.tiles_per_cta;
+    const int nt = nt64 > 0 ? (int)nt64 : 0;
+    const int pad = TPB > MT_TILES ? TPB : MT_TILES;
+    const int ntp = ((nt + pad - 1) / pad) * pad;       // with ghost tiles: whole S3 blocks and MMA tiles
+    const int nb = ntp / TPB, nm = ntp / MT_TILES;
+    const int64_t t0 = tile0 * FU_TILE;
+    const int64_t t1 = min(T, t0 + (int64_t)nt * FU_TILE);
+    const float *logits = q.logits + (size_t)layer * T * E;
+    int32_t *gidx = q.idx + (size_t)layer * T * k;
+    float *gw = q.w + (size_t)layer * T * k;
+
+    // ---- set-up ----
+    if (tid == 0) {
+        for (int s = 0; s < nst; ++s) {
+            mbar_init(&full_bar[s], 1);
+            mbar_init(&empty_bar[s], 1);
+        }
+        for (int s = 0; s < FU_OB; ++s) {
+            mbar_init(&offs_full[s], TPB);
+            mbar_init(&offs_empty[s], q.ns3w);
+        }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&tile_full[s], MT_TILES);
+            mbar_init(&tile_ready[s], 1);
+            mbar_init(&mma_done[s], 1);
+        }
+        mbar_init(&tbl_bar, 1);
+        mbar_init(&acc_done, 1);
+        mbar_fence_init();
+    }
+    if (warp == 1) tmem_alloc(&s_tmem, NCOLS);
+    {
+        uint4 *z = reinterpret_cast<uint4 *>(tiles);
+        for (int i = tid; i < 2 * EP * FU_MT / 16; i += blockDim.x) z[i] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    proxy_fence_async();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    if (warp == 0) {
+        // ================= producer =================
+        if (lane == 0 && nt > 0) {
+            mbar_expect_tx(&tbl_bar, (uint32_t)(E + 1) * rowb);
+            bulk_g2s(tbl, q.table + (size_t)layer * (E + 1) * q.RS * 4, (uint32_t)(E + 1) * rowb, &tbl_bar);
+            for (int j = 0; j < nt; ++j) {
+                const int st = j % nst;
+                if (j >= nst) mbar_wait(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1));
+                const int64_t tok0 = t0 + (int64_t)j * FU_TILE;
+                const int rows = (int)min((int64_t)FU_TILE, T - tok0);
+                mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
+                bulk_g2s(ring + (size_t)st * TILE_BYTES, logits + tok0 * E, (uint32_t)rows * E * 4, &full_bar[st]);
+            }
+        }
+    } else if (warp == 1) {
+        // ================= tensor-core warp =================
+        for (int m = 0; m < nm; ++m) {
+            const int tb = m & 1;
+            unsigned char *tile = tiles + (size_t)tb * EP * FU_MT;
+            mbar_wait(&tile_full[tb], (uint32_t)((m >> 1) & 1));
+            tc_fence_after();
+            if (lane == 0) {
+                const uint32_t base = smem_u32(tile);
+#pragma unroll
+                for (int j = 0; j < FU_MT / 32; ++j) {
+                    const uint64_t bd = umma_desc(base + j * 2 * LBO, LBO, SBO);
+                    umma_i8(tmem, bd, bd, IDESC, (uint32_t)((m | j) != 0));
+                    if (EP == 256) {
+                        const uint64_t a1 = umma_desc(base + 16 * SBO + j * 2 * LBO, LBO, SBO);
+                        umma_i8(tmem + 256u, a1, bd, IDESC, (uint32_t)((m | j) != 0));
+                    }
+                }
+                umma_commit(&mma_done[tb]);
+                if (m == nm - 1) umma_commit(&acc_done);
+            }
+            __syncwarp();
+            if (m + 2 < nm) {
+                // recycle the buffer for MMA tile m + 2: wait until the tensor core has read it, clear it
+                mbar_wait(&mma_done[tb], (uint32_t)((m >> 1) & 1));
+                uint4 *z = reinterpret_cast<uint4 *>(tile);
+                for (int i = lane; i < EP * FU_MT / 16; i += 32) z[i] = make_uint4(0u, 0u, 0u, 0u);
+                proxy_fence_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&tile_ready[tb]);
+            }
+        }
+    } else if (warp < FU_S3W0) {
+        // ================= S1: gate top-k, two lanes per token =================
+        const int c = warp - 2;
+        const int h = lane >> 4, tl = lane & 15;
+        for (int j = c; j < ntp; j += FU_NC) {
+            const bool ghost = j >= nt;
+            const int st = j % nst;
+            const int64_t tok = t0 + (int64_t)j * FU_TILE + tl;
+            const bool valid = !ghost && tok < T;
+            int sel[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) sel[i] = 0;
+            if (!ghost) {
+                // this warp alternates on a stage with one other warp: first make sure that warp's
+                // tile (the previous use of the stage) has been consumed, then wait for ours
+                const int u = j / nst;
+                if (u >= 1) mbar_wait(&empty_bar[st], (uint32_t)((u - 1) & 1));
+                mbar_wait(&full_bar[st], (uint32_t)(u & 1));
+                const float *row = reinterpret_cast<const float *>(ring + (size_t)st * TILE_BYTES +
+                                                                   (size_t)(tok < T ? tl : 0) * E * 4);
+                float wv[4];
+                gate_select_pair<E>(row, h, tl & 7, k, sel);
+                gate_weights_softmax_pair(row, h, k, sel, q.scale, wv);
+                if (valid) {
+                    if (k == 8) {
+                        *reinterpret_cast<int4 *>(gidx + tok * 8 + 4 * h) =
+                            h ? make_int4(sel[4], sel[5], sel[6], sel[7]) : make_int4(sel[0], sel[1], sel[2], sel[3]);
+                        *reinterpret_cast<float4 *>(gw + tok * 8 + 4 * h) = make_float4(wv[0], wv[1], wv[2], wv[3]);
+                    } else {
+#pragma unroll
+                        for (int jj = 0; jj < 4; ++jj) {
+                            const int s = 4 * h + jj;
+                            if (s < k) {
+                                gidx[tok * k + s] = h ? sel[4 + jj] : sel[jj];
+                                gw[tok * k + s] = wv[jj];
+                            }
+                        }
+                    }
+                }
+            }
+            // ---- table-row offsets for S3 ----
+            const int b = j / TPB, ob = b % FU_OB;
+            if (b >= FU_OB) mbar_wait(&offs_empty[ob], (uint32_t)(((b / FU_OB) - 1) & 1));
+            {
+                uint4 o4;
+                uint32_t ov[4];
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    const int s = 4 * h + jj;
+                    const int e = h ? sel[4 + jj] : sel[jj];
+                    ov[jj] = (valid && s < k) ? (uint32_t)e * rowb : zero_row;
+                }
+                o4 = make_uint4(ov[0], ov[1], ov[2], ov[3]);
+                const int slot = (j % TPB) * FU_TILE + tl;
+                *reinterpret_cast<uint4 *>(offs + ((size_t)ob * BT + slot) * FU_KP + 4 * h) = o4;
+            }
+            // ---- one-hot bytes for the co-activation MMA ----
+            const int m = j / MT_TILES, tb = m & 1;
+            if (m >= 2) mbar_wait(&tile_ready[tb], (uint32_t)(((m >> 1) - 1) & 1));
+            if (valid) {
+                const int tp = (j % MT_TILES) * FU_TILE + tl;
+                unsigned char *col = tiles + (size_t)tb * EP * FU_MT + (tp >> 4) * LBO + (tp & 15);
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) {
+                    const int s = 4 * h + jj;
+                    const int e = h ? sel[4 + jj] : sel[jj];
+                    if (s < k) col[(e >> 3) * SBO + (e & 7) * 16] = 1;
+                }
+            }
+            proxy_fence_async();
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&offs_full[ob]);
+                mbar_arrive(&tile_full[tb]);
+                if (!ghost) mbar_arrive(&empty_bar[st]);
+            }
+        }
+    } else {
+        // ================= S3: bit-sliced candidate scoring =================
+        const int t3 = tid - FU_S3W0 * 32;
+        const bool active = t3 < R * S;
+        const int sub = active ? t3 / R : 0;
+        const int col = active ? t3 - sub * R : 0;
+        const unsigned char *tblc = tbl + col * 16;
+        const int D = q.D;
+        const size_t slot0 = ((size_t)layer * q.ncta_t + blockIdx.x) * q.maxrec;
+        const int64_t cap_run = (int64_t)(EF_MAXBLK - 2) * BT;
+        if (nt > 0) mbar_wait(&tbl_bar, 0u);
+        uint4 pl[EF_NPL];
+#pragma unroll
+        for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint4(0u, 0u, 0u, 0u);
+        int nrec = 0, src = 0;
+        int64_t rend = t0;               // end of the current run (none yet)
+        bool have_run = false;
+
+        auto flush = [&]() {
+            // add the S sub-slots in the bit-sliced domain (tree through shared memory), write the record
+            for (int lvl = 0; lvl < q.logS; ++lvl) {
+                const int half = S >> (lvl + 1);
+                const int stride = half * R;
+                const int np = EF_BT + lvl;
+                if (active && sub >= half && sub < 2 * half) {
+#pragma unroll
+                    for (int p = 0; p < EF_NPL; ++p)
+                        if (p < np) xch[(size_t)p * stride + (sub - half) * R + col] = pl[p];
+                }
+                named_bar_sync(1, ns3);
+                if (active && sub < half) fu_add_planes(pl, xch + sub * R + col, stride, np);
+                named_bar_sync(1, ns3);
+            }
+            if (active && sub == 0) {
+                uint4 *rp = reinterpret_cast<uint4 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
+#pragma unroll
+                for (int p = 0; p < EF_NPL; ++p)
+                    if (p < q.NPR) rp[(size_t)p * R + col] = pl[p];
+            }
+            if (t3 == 0) q.rec_src[slot0 + nrec] = src;
+            ++nrec;
+#pragma unroll
+            for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint4(0u, 0u, 0u, 0u);
+        };
+
+        for (int b = 0; b < nb; ++b) {
+            const int ob = b % FU_OB;
+            mbar_wait(&offs_full[ob], (uint32_t)((b / FU_OB) & 1));
+            const int64_t bt0 = t0 + (int64_t)b * BT;
+            const int64_t bend = min(bt0 + BT, t1);
+            const uint32_t *obuf = offs + ((size_t)ob * BT + sub) * FU_KP;
+            int64_t cur = bt0;
+            while (cur < bend) {
+                if (cur >= rend) {
+                    if (have_run) flush();
+                    src = (int)((cur * D) / T);
+                    const int64_t bnd = ((int64_t)(src + 1) * T + D - 1) / D;
+                    rend = min(bnd, cur + cap_run);
+                    have_run = true;
+                }
+                const int64_t seg = min(bend, rend);
+                const bool whole = cur == bt0 && seg == bend;     // tokens past t1 carry the zero row
+                if (active) {
+                    uint4 x0, x1, x2, x3;
+                    uint32_t fAx, fAy, fAz, fAw, fBx, fBy, fBz, fBw;
+#define CAP_FU_LOAD(X, PS)                                                               \
+    do {                                                                                 \
+        X = fu_token_mask(tblc, obuf + (size_t)(PS) * S * FU_KP);                        \
+        if (!whole) {                                                                    \
+            const int64_t tk = bt0 + (PS) * S + sub;                                     \
+            if (tk < cur || tk >= seg) X = make_uint4(0u, 0u, 0u, 0u);                   \
+        }                                                                                \
+    } while (0)
+                    CAP_FU_LOAD(x0, 0); CAP_FU_LOAD(x1, 1); CAP_FU_LOAD(x2, 2); CAP_FU_LOAD(x3, 3);
+                    CAP_FU_HALF(x, x0, x1, x2, x3, fAx); CAP_FU_HALF(y, x0, x1, x2, x3, fAy);
+                    CAP_FU_HALF(z, x0, x1, x2, x3, fAz); CAP_FU_HALF(w, x0, x1, x2, x3, fAw);
+                    CAP_FU_LOAD(x0, 4); CAP_FU_LOAD(x1, 5); CAP_FU_LOAD(x2, 6); CAP_FU_LOAD(x3, 7);
+                    CAP_FU_HALF(x, x0, x1, x2, x3, fBx); CAP_FU_HALF(y, x0, x1, x2, x3, fBy);
+                    CAP_FU_HALF(z, x0, x1, x2, x3, fBz); CAP_FU_HALF(w, x0, x1, x2, x3, fBw);
+                    CAP_FU_TOP(x, fAx, fBx); CAP_FU_TOP(y, fAy, fBy);
+                    CAP_FU_TOP(z, fAz, fBz); CAP_FU_TOP(w, fAw, fBw);
+#undef CAP_FU_LOAD
+                }
+                cur = seg;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&offs_empty[ob]);
+        }
+        if (have_run) flush();
+
+        // ---- drain the co-activation accumulator (four S3 warps, one TMEM lane quadrant each) ----
+        const int w3 = warp - FU_S3W0;
+        if (w3 < 4 && nm > 0) {
+            mbar_wait(&acc_done, 0u);
+            tc_fence_after();
+            const int quad = warp & 3;
+            int *C = q.coact + (size_t)layer * E * E;
+            unsigned long long *cnt = q.counts + (size_t)layer * E;
+#pragma unroll 1
+            for (int hh = 0; hh < EP / 128; ++hh) {
+                const int r = hh * 128 + quad * 32 + lane;
+#pragma unroll 1
+                for (int cb = 0; cb < EP / 32; ++cb) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)(hh * 256 + cb * 32), v);
+                    const bool rok = r < E;
+                    if (q.pack64) {
+                        int *cp = C + (size_t)(cb * 32) * E + (r & ~1);
+#pragma unroll
+                        for (int j = 0; j < 32; j += 2) {
+                            const uint32_t p0 = __shfl_xor_sync(0xffffffffu, v[j], 1);
+                            const uint32_t p1 = __shfl_xor_sync(0xffffffffu, v[j + 1], 1);
+                            const int jj = j + (lane & 1);
+                            const unsigned long long pk = (lane & 1) ? ((unsigned long long)v[j + 1] << 32) | p1
+                                                                     : ((unsigned long long)p0 << 32) | v[j];
+                            if (rok && cb * 32 + jj < E)
+                                asm volatile("red.global.add.u64 [%0], %1;" ::"l"(cp + (size_t)jj * E), "l"(pk) : "memory");
+                        }
+                    } else {
+                        int *cp = C + (size_t)(cb * 32) * E + r;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j)
+                            if (rok && cb * 32 + j < E)
+                                asm volatile("red.global.add.s32 [%0], %1;" ::"l"(cp + (size_t)j * E), "r"(v[j]) : "memory");
+                    }
+                    if (rok && (r >> 5) == cb) {
+                        uint32_t d = 0u;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) d = (r & 31) == j ? v[j] : d;
+                        atomicAdd(&cnt[r], (unsigned long long)d);
+                    }
+                }
+            }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) tmem_dealloc(tmem, NCOLS);
+}
+
+// ---- host side ------------------------------------------------------------------------------------------
+struct FusedGeom {
+    EvalFastGeom g;      // table / column geometry of the S3 part; ncta_t, maxrec, rec_* hold the fused values
+    int nst, ns3w, nthreads, EP;
+    int64_t tiles_per_cta;
+    size_t smem;
+};
+
+static bool fused_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P, FusedGeom *f)
+{
+    if (E != 64 && E != 128 && E != 256) return false;
+    if (k > 8 || L < 1 || T < 1 || P < 1) return false;
+    EvalFastGeom &g = f->g;
+    if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), 150 * 1024, &g)) return false;
+    if (g.PC != 1 || g.S < 4) return false;
+    f->EP = E <= 128 ? 128 : 256;
+    f->ns3w = (g.R * g.S + 31) / 32;
+    f->nthreads = 32 * (FU_S3W0 + f->ns3w);
+    if (f->nthreads > FU_MAXTHREADS) return false;
+    const size_t budget = 224 * 1024;
+    int nst = FU_MAXST;
+    for (; nst >= 8; nst -= 4)
+        if (fused_smem_layout(E, f->EP, g.RS, g.R, g.S, nst).total <= budget) break;
+    if (nst < 8) return false;
+    f->nst = nst;
+    f->smem = fused_smem_layout(E, f->EP, g.RS, g.R, g.S, nst).total;
+    const int64_t ltiles = (T + FU_TILE - 1) / FU_TILE;
+    int64_t want = sm_count() / L;
+    if (want < 1) want = 1;
+    f->tiles_per_cta = (ltiles + want - 1) / want;
+    g.ncta_t = (int)((ltiles + f->tiles_per_cta - 1) / f->tiles_per_cta);
+    if (g.ncta_t > 65535) return false;
+    const int64_t tpc = f->tiles_per_cta * FU_TILE;
+    const int64_t BT = (int64_t)EF_PASSES * g.S;
+    const int64_t cap_run = (int64_t)(EF_MAXBLK - 2) * BT;
+    int64_t srcb = ((tpc - 1) * D) / T + 1;
+    if (srcb > D - 1) srcb = D - 1;
+    g.maxrec = (int)((tpc + cap_run - 1) / cap_run + srcb + 1);
+    g.tpc = tpc;
+    g.NPR = EF_BT + g.logS;
+    g.rec_slots = (size_t)L * g.ncta_t * g.maxrec;
+    g.rec_words = g.rec_slots * g.NPR * g.W;
+    g.table_words = (size_t)L * (E + 1) * g.RS * 4;
+    return true;
+}
+
+size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P)
+{
+    size_t best = 0;
+    for (int N = 2; N <= 8; N *= 2) {
+        FusedGeom f;
+        if (!fused_geom(L, T, k, E, D, N, P, &f)) continue;
+        const size_t b = f.g.rec_slots * 4 + 256 + f.g.rec_words * 4 + 256 + f.g.table_words * 4 + 256;
+        if (b > best) best = b;
+    }
+    return best;
+}
+
+template <int E>
+static int launch_fused_e(const FusedParams &prm, const FusedGeom &f, int L, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(trace_fused_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
+        attr_set = true;
+    }
+    {
+        KernelTimerScope ts("trace_fused", st);
+        trace_fused_kernel<E><<<dim3((unsigned)f.g.ncta_t, (unsigned)L), f.nthreads, f.smem, st>>>(prm);
+    }
+    note_launch();
+    return check_launch("trace_fused_kernel");
+}
+
+int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
+                            int32_t *idx, float *w, int64_t *counts, int32_t *coact, const int32_t *token_src,
+                            const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                            const cap_eval_out &out, void *ws, cudaStream_t st, bool *used)
+{
+    *used = false;
+    if (cfg.scoring != 0 || cfg.renormalize != 1 || cfg.n_group != 1 || cfg.k > 8 || bias != nullptr) return CAP_OK;
+    if (token_src != nullptr || out.tok_remote_dev || out.tok_remote_node) return CAP_OK;
+    if (!counts || !coact || L < 1 || T < 1 || P < 1) return CAP_OK;
+    if ((reinterpret_cast<uintptr_t>(logits) | reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u)
+        return CAP_OK;
+    FusedGeom f;
+    if (!fused_geom(L, T, cfg.k, cfg.E, topo.D, topo.N, P, &f)) return CAP_OK;
+    const int E = cfg.E;
+    EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, f.g);
+    if (cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)L * E, st) != cudaSuccess ||
+        cudaMemsetAsync(coact, 0, sizeof(int32_t) * (size_t)L * E * E, st) != cudaSuccess ||
+        cudaMemsetAsync(fw.rec_src, 0xff, f.g.rec_slots * 4, st) != cudaSuccess)
+        return check_launch("memset fused");
+    CAP_TRY(eval_zero_ws(L, E, topo.D, P, false, ws, st));
+    CAP_TRY(ef_launch_table(f.g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st));
+    FusedParams prm;
+    prm.logits = logits;
+    prm.idx = idx;
+    prm.w = w;
+    prm.counts = reinterpret_cast<unsigned long long *>(counts);
+    prm.coact = coact;
+    prm.table = fw.table;
+    prm.rec_src = fw.rec_src;
+    prm.rec_planes = fw.rec_planes;
+    prm.T = T;
+    prm.tiles_per_cta = f.tiles_per_cta;
+    prm.scale = cfg.scale;
+    prm.k = cfg.k;
+    prm.D = topo.D;
+    prm.pack64 = (E % 2 == 0) && (reinterpret_cast<uintptr_t>(coact) & 7u) == 0;
+    prm.R = f.g.R;
+    prm.RS = f.g.RS;
+    prm.S = f.g.S;
+    prm.logS = f.g.logS;
+    prm.maxrec = f.g.maxrec;
+    prm.NPR = f.g.NPR;
+    prm.ncta_t = f.g.ncta_t;
+    prm.nst = f.nst;
+    prm.ns3w = f.ns3w;
+    int rc;
+    switch (E) {
+    case 64: rc = launch_fused_e<64>(prm, f, L, st); break;
+    case 128: rc = launch_fused_e<128>(prm, f, L, st); break;
+    default: rc = launch_fused_e<256>(prm, f, L, st); break;
+    }
+    CAP_TRY(rc);
+    CAP_TRY(ef_launch_decode(f.g, fw, ws, L, T, E, P, topo, st));
+    CAP_TRY(launch_eval_finalize(L, E, P, expert_dev, topo, counts, out, ws, st));
+    *used = true;
+    return CAP_OK;
+}
+
+}  // namespace cap

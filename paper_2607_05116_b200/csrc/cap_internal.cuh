@@ -55,6 +55,15 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
                 int64_t T, int32_t k, int32_t E, const int32_t *expert_dev, int32_t P,
                 int64_t layer_stride_maps, const cap_topology &topo, const int64_t *counts,
                 const cap_eval_out &out, void *ws, cudaStream_t st);
+int launch_eval_finalize(int32_t L, int32_t E, int32_t P, const int32_t *expert_dev, const cap_topology &topo,
+                         const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st);
+int eval_zero_ws(int32_t L, int32_t E, int32_t D, int32_t P, bool with_mcounts, void *ws, cudaStream_t st);
+// fused S1+S2+S3 kernel (cap_fused.cu): *used = false when the configuration does not fit it
+int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
+                            int32_t *idx, float *w, int64_t *counts, int32_t *coact, const int32_t *token_src,
+                            const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                            const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
+size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
                  const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,
