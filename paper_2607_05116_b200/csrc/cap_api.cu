@@ -215,12 +215,8 @@ int cap_prune(const int32_t *topk_idx, const float *topk_w, const int32_t *token
     if (L > 0 && !expert_dev) return CAP_EINVAL;
     if ((int64_t)L * T > 0 && (!topk_idx || !topk_w || !kept)) return CAP_EINVAL;
     if (after && (!ws || ws_bytes < eval_ws_bytes(L, T, E, k, topo->D, 1))) return CAP_EWORKSPACE;
-    CAP_TRY(launch_prune(topk_idx, topk_w, token_src, L, T, k, E, expert_dev, *topo, p, kept,
-                         near_margin, (cudaStream_t)stream));
-    if (after)
-        return launch_eval(topk_idx, kept, token_src, L, T, k, E, expert_dev, 1, (int64_t)E, *topo,
-                           nullptr, *after, ws, (cudaStream_t)stream);
-    return CAP_OK;
+    return launch_prune(topk_idx, topk_w, token_src, L, T, k, E, expert_dev, *topo, p, kept, near_margin, after,
+                        ws, (cudaStream_t)stream);
 }
 
 int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T, int32_t k,

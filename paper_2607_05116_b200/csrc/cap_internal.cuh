@@ -67,7 +67,7 @@ size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int
 int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
                  const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,
-                 cudaStream_t st);
+                 const cap_eval_out *after, void *ws, cudaStream_t st);
 // S3 fast path (cap_eval_fast.cu): *used = false when the sizes do not fit it
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                      int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,

@@ -1,7 +1,14 @@
-// S4 -- communication-aware pruning (Eq. 6 and its greedy solver).  One thread per
-// token: aggregate the slot weights per destination device in slot order (fp32), price each
-// device by topology relative to the token's source, keep devices by descending a_d/c_d until
-// the kept weight reaches 1-p.  Every fp32 step is a single IEEE operation (readings R7-R10).
+// S4 -- communication-aware pruning (Eq. 6 and its greedy solver), fused with the
+// evaluation of the pruned trace under the same placement ("new volume and load").  One thread per
+// token, everything in registers (fully unrolled over the k slots, no indexed local arrays):
+//   1. aggregate the slot weights per destination device in slot order (fp32, single IEEE adds),
+//   2. price each device by topology relative to the token's source (readings R7, R13),
+//   3. rank the devices by a_d / c_d descending, ties -> lower device id (R10),
+//   4. keep devices in rank order while the kept weight is below 1 - p (R8, R9),
+//   5. kept[t][s] = 1 iff the slot's device was kept; near-margin tokens are counted (R-S4.7).
+// When the caller wants the after-metrics, the same thread also adds the token's kept device set
+// into the block's evaluation accumulators (distinct devices / nodes, local, same-node, received
+// tokens per device, kept pairs per expert), which are flushed with a few atomics per block.
 #include <math_constants.h>
 
 #include "cap_internal.cuh"
@@ -16,124 +23,274 @@ struct PruneParams {
     const int32_t *dev_node;
     uint8_t *kept;
     unsigned long long *near_margin;   // [L] or NULL
+    // evaluation of the kept trace (all NULL when not wanted)
+    unsigned long long *acc;      // [L][ACC_N]
+    unsigned long long *recv;     // [L][D]
+    unsigned long long *mcounts;  // [L][E]
+    uint8_t *tok_rdev, *tok_rnode;   // [L][T] or NULL
     int64_t T;
-    int32_t k, E, D, cost_local, cost_intra, cost_inter;
+    int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec;
     float p;
 };
 
 template <int KMAX>
 __global__ void __launch_bounds__(256) prune_kernel(PruneParams prm)
 {
-    extern __shared__ int s_map[];     // [E] expert -> device of this layer, then [D] dev -> node
+    extern __shared__ int s_map[];     // [E] expert -> device, [64] device -> node, [64] recv, [E] counts
+    __shared__ unsigned long long s_nodemask[64];
+    __shared__ unsigned long long s_acc[ACC_N];
     const int layer = blockIdx.y;
     const int E = prm.E, D = prm.D, k = prm.k;
     int *s_dn = s_map + E;
-    for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = prm.expert_dev[(size_t)layer * E + i];
-    for (int i = threadIdx.x; i < D; i += blockDim.x) s_dn[i] = prm.dev_node[i];
+    int *s_recv = s_dn + 64;
+    int *s_cnt = s_recv + 64;
+    const bool want_eval = prm.acc != nullptr;
+    for (int i = threadIdx.x; i < E; i += blockDim.x) {
+        s_map[i] = prm.expert_dev[(size_t)layer * E + i];
+        s_cnt[i] = 0;
+    }
+    if (threadIdx.x < 64) {
+        s_dn[threadIdx.x] = (int)threadIdx.x < D ? prm.dev_node[threadIdx.x] : 0;
+        s_recv[threadIdx.x] = 0;
+        unsigned long long m = 0ull;
+        if ((int)threadIdx.x < prm.N)
+            for (int d = 0; d < D; ++d)
+                if (prm.dev_node[d] == (int)threadIdx.x) m |= 1ull << d;
+        s_nodemask[threadIdx.x] = m;
+    }
+    if (threadIdx.x < ACC_N) s_acc[threadIdx.x] = 0ull;
     __syncthreads();
 
     const int64_t T = prm.T;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int near = 0;
+    unsigned a_dev = 0, a_loc = 0, a_same = 0, a_node = 0, a_rnode = 0;
     if (t < T) {
         const int64_t base = ((int64_t)layer * T + t) * k;
-        if (prm.p <= 0.0f) {
-            for (int s = 0; s < k; ++s) prm.kept[base + s] = 1;
+        int e[KMAX], d[KMAX];
+        float wv[KMAX];
+        if (KMAX == 8 && prm.vec) {
+            const int4 i0 = __ldg(reinterpret_cast<const int4 *>(prm.idx + base));
+            const int4 i1 = __ldg(reinterpret_cast<const int4 *>(prm.idx + base) + 1);
+            const float4 w0 = __ldg(reinterpret_cast<const float4 *>(prm.w + base));
+            const float4 w1 = __ldg(reinterpret_cast<const float4 *>(prm.w + base) + 1);
+            e[0] = i0.x; e[1] = i0.y; e[2] = i0.z; e[3] = i0.w;
+            e[4 % KMAX] = i1.x; e[5 % KMAX] = i1.y; e[6 % KMAX] = i1.z; e[7 % KMAX] = i1.w;
+            wv[0] = w0.x; wv[1] = w0.y; wv[2] = w0.z; wv[3] = w0.w;
+            wv[4 % KMAX] = w1.x; wv[5 % KMAX] = w1.y; wv[6 % KMAX] = w1.z; wv[7 % KMAX] = w1.w;
         } else {
-            const int src = prm.token_src ? prm.token_src[(int64_t)layer * T + t] : (int)((t * D) / T);
+#pragma unroll
+            for (int s = 0; s < KMAX; ++s) {
+                e[s] = s < k ? __ldg(prm.idx + base + s) : 0;
+                wv[s] = s < k ? __ldg(prm.w + base + s) : 0.0f;
+            }
+        }
+#pragma unroll
+        for (int s = 0; s < KMAX; ++s) {
+            const int ee = (unsigned)e[s] < (unsigned)E ? e[s] : 0;
+            d[s] = s < k ? (s_map[ee] & 63) : -1 - s;      // absent slots: distinct negative ids
+            e[s] = ee;
+        }
+        unsigned long long keepmask = 0ull;
+        if (prm.p <= 0.0f) {
+#pragma unroll
+            for (int s = 0; s < KMAX; ++s)
+                if (s < k) keepmask |= 1ull << d[s];
+        } else {
+            const int src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63) : (int)((t * D) / T);
             const int srcn = s_dn[src];
-            int dev[KMAX], sdev[KMAX];
-            float a[KMAX], ratio[KMAX];
+            // 1. per-device weight at the device's first slot, added in slot order
+            bool rep[KMAX];
+            float a[KMAX];
+#pragma unroll
+            for (int s = 0; s < KMAX; ++s) {
+                rep[s] = s < k;
+                a[s] = wv[s];
+            }
+#pragma unroll
+            for (int s = 1; s < KMAX; ++s) {
+#pragma unroll
+                for (int j = 0; j < s; ++j) {
+                    if (s < k && rep[j] && d[j] == d[s]) {
+                        a[j] = __fadd_rn(a[j], wv[s]);
+                        rep[s] = false;
+                    }
+                }
+            }
+            // 2. cost ratio of every represented device
+            float ratio[KMAX];
             int m = 0;
 #pragma unroll
             for (int s = 0; s < KMAX; ++s) {
-                if (s < k) {
-                    const int d = s_map[prm.idx[base + s]];
-                    sdev[s] = d;
-                    const float ws = prm.w[base + s];
-                    int j = 0;
-                    while (j < m && dev[j] != d) ++j;
-                    if (j == m) { dev[m] = d; a[m] = ws; ++m; }
-                    else a[j] = __fadd_rn(a[j], ws);
-                }
+                const int dd = d[s] & 63;
+                const int c = (dd == src) ? prm.cost_local : (s_dn[dd] == srcn) ? prm.cost_intra : prm.cost_inter;
+                ratio[s] = (c == 0) ? CUDART_INF_F : __fdiv_rn(a[s], (float)c);
+                m += rep[s] ? 1 : 0;
             }
-            for (int j = 0; j < m; ++j) {
-                const int d = dev[j];
-                const int c = (d == src) ? prm.cost_local : (s_dn[d] == srcn) ? prm.cost_intra : prm.cost_inter;
-                ratio[j] = (c == 0) ? CUDART_INF_F : __fdiv_rn(a[j], (float)c);
+            // 3. rank: devices with a larger ratio, or an equal ratio and a lower id, come first
+            int rank[KMAX];
+#pragma unroll
+            for (int s = 0; s < KMAX; ++s) {
+                int r = 0;
+#pragma unroll
+                for (int j = 0; j < KMAX; ++j)
+                    if (j != s && rep[j] && (ratio[j] > ratio[s] || (ratio[j] == ratio[s] && d[j] < d[s]))) ++r;
+                rank[s] = r;
             }
-            // order by ratio descending, ties -> lower device id (insertion sort, m <= k)
-            for (int i = 1; i < m; ++i) {
-                const int d = dev[i];
-                const float r = ratio[i], av = a[i];
-                int j = i - 1;
-                while (j >= 0 && (ratio[j] < r || (ratio[j] == r && dev[j] > d))) {
-                    dev[j + 1] = dev[j]; ratio[j + 1] = ratio[j]; a[j + 1] = a[j];
-                    --j;
-                }
-                dev[j + 1] = d; ratio[j + 1] = r; a[j + 1] = av;
-            }
+            // 4. greedy in rank order
             const float target = __fsub_rn(1.0f, prm.p);
-            float cum = 0.0f;
-            int nk = 0;
-            unsigned long long keepmask = 0ull;
-            for (int i = 0; i < m; ++i) {
-                if (fabsf(__fsub_rn(cum, target)) < 1e-6f) near = 1;
-                if (cum >= target) break;
-                keepmask |= 1ull << dev[i];
-                cum = __fadd_rn(cum, a[i]);
-                nk = i + 1;
+            float cum = 0.0f, r_last = 0.0f, r_cut = 0.0f;
+            bool stopped = false;
+#pragma unroll
+            for (int r = 0; r < KMAX; ++r) {
+                if (r < m && !stopped) {
+                    float Ar = 0.0f, Rr = 0.0f;
+                    int dr = 0;
+#pragma unroll
+                    for (int s = 0; s < KMAX; ++s)
+                        if (rep[s] && rank[s] == r) { Ar = a[s]; Rr = ratio[s]; dr = d[s]; }
+                    if (fabsf(__fsub_rn(cum, target)) < 1e-6f) near = 1;
+                    if (cum >= target) {
+                        stopped = true;
+                        r_cut = Rr;
+                    } else {
+                        keepmask |= 1ull << dr;
+                        cum = __fadd_rn(cum, Ar);
+                        r_last = Rr;
+                    }
+                }
             }
-            if (nk < m) {
-                const float r1 = ratio[nk - 1], r2 = ratio[nk];
-                if (r1 != CUDART_INF_F && r2 != CUDART_INF_F && __fsub_rn(r1, r2) < 1e-6f) near = 1;
+            if (stopped && r_last != CUDART_INF_F && r_cut != CUDART_INF_F && __fsub_rn(r_last, r_cut) < 1e-6f)
+                near = 1;
+        }
+        // 5. kept mask per slot
+        if (KMAX == 8 && k == 8 && prm.vec) {
+            unsigned lo = 0, hi = 0;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                lo |= (unsigned)((keepmask >> d[s]) & 1ull) << (8 * s);
+                hi |= (unsigned)((keepmask >> d[(4 + s) % KMAX]) & 1ull) << (8 * s);
             }
+            *reinterpret_cast<uint2 *>(prm.kept + base) = make_uint2(lo, hi);
+        } else {
 #pragma unroll
             for (int s = 0; s < KMAX; ++s)
-                if (s < k) prm.kept[base + s] = (uint8_t)((keepmask >> sdev[s]) & 1ull);
+                if (s < k) prm.kept[base + s] = (uint8_t)((keepmask >> d[s]) & 1ull);
+        }
+        // evaluation of the kept trace under this placement (P = 1)
+        if (want_eval) {
+            const int src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63) : (int)((t * D) / T);
+            const int srcn = s_dn[src];
+            unsigned long long nodebits = 0ull;
+#pragma unroll
+            for (int s = 0; s < KMAX; ++s) {
+                if (s < k && ((keepmask >> d[s]) & 1ull)) {
+                    nodebits |= 1ull << s_dn[d[s]];
+                    atomicAdd(&s_cnt[e[s]], 1);
+                }
+            }
+            unsigned long long mm = keepmask;
+            while (mm) {
+                const int dd = __ffsll((long long)mm) - 1;
+                mm &= mm - 1;
+                atomicAdd(&s_recv[dd], 1);
+            }
+            a_dev = __popcll(keepmask);
+            a_loc = (unsigned)((keepmask >> src) & 1ull);
+            a_same = __popcll(keepmask & s_nodemask[srcn]);
+            a_node = __popcll(nodebits);
+            a_rnode = a_node - (unsigned)((nodebits >> srcn) & 1ull);
+            if (prm.tok_rdev) prm.tok_rdev[(int64_t)layer * T + t] = (uint8_t)(a_dev - a_loc);
+            if (prm.tok_rnode) prm.tok_rnode[(int64_t)layer * T + t] = (uint8_t)a_rnode;
         }
     }
     if (prm.near_margin) {
         const unsigned b = __ballot_sync(0xffffffffu, near != 0);
         if ((threadIdx.x & 31) == 0 && b) atomicAdd(&prm.near_margin[layer], (unsigned long long)__popc(b));
     }
+    if (want_eval) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) {
+            a_dev += __shfl_xor_sync(0xffffffffu, a_dev, off);
+            a_loc += __shfl_xor_sync(0xffffffffu, a_loc, off);
+            a_same += __shfl_xor_sync(0xffffffffu, a_same, off);
+            a_node += __shfl_xor_sync(0xffffffffu, a_node, off);
+            a_rnode += __shfl_xor_sync(0xffffffffu, a_rnode, off);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            atomicAdd(&s_acc[ACC_DEV], (unsigned long long)a_dev);
+            atomicAdd(&s_acc[ACC_LOCAL], (unsigned long long)a_loc);
+            atomicAdd(&s_acc[ACC_SAMENODE], (unsigned long long)a_same);
+            atomicAdd(&s_acc[ACC_NODE], (unsigned long long)a_node);
+            atomicAdd(&s_acc[ACC_RNODE], (unsigned long long)a_rnode);
+        }
+        __syncthreads();
+        if (threadIdx.x < ACC_N && s_acc[threadIdx.x])
+            atomicAdd(&prm.acc[(size_t)layer * ACC_N + threadIdx.x], s_acc[threadIdx.x]);
+        if ((int)threadIdx.x < D && s_recv[threadIdx.x])
+            atomicAdd(&prm.recv[(size_t)layer * D + threadIdx.x], (unsigned long long)s_recv[threadIdx.x]);
+        for (int i = threadIdx.x; i < E; i += blockDim.x)
+            if (s_cnt[i]) atomicAdd(&prm.mcounts[(size_t)layer * E + i], (unsigned long long)s_cnt[i]);
+    }
 }
 
+// Prune and, when `after` is given, evaluate the kept trace (P = 1): ws is the evaluation workspace.
 int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
                  const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,
-                 cudaStream_t st)
+                 const cap_eval_out *after, void *ws, cudaStream_t st)
 {
     if (L == 0) return CAP_OK;
     if (near_margin &&
         cudaMemsetAsync(near_margin, 0, sizeof(int64_t) * (size_t)L, st) != cudaSuccess)
         return check_launch("memset near_margin");
-    if (T == 0) return CAP_OK;
     PruneParams prm;
-    prm.idx = idx;
-    prm.w = w;
-    prm.token_src = token_src;
-    prm.expert_dev = expert_dev;
-    prm.dev_node = topo.dev_node;
-    prm.kept = kept;
-    prm.near_margin = reinterpret_cast<unsigned long long *>(near_margin);
-    prm.T = T;
-    prm.k = k;
-    prm.E = E;
-    prm.D = topo.D;
-    prm.cost_local = topo.cost_local;
-    prm.cost_intra = topo.cost_intra;
-    prm.cost_inter = topo.cost_inter;
-    prm.p = p;
-    dim3 grid((unsigned)((T + 255) / 256), (unsigned)L);
-    const size_t smem = sizeof(int) * ((size_t)E + topo.D);
-    {
-        KernelTimerScope ts("prune", st);
-        if (k <= 8) prune_kernel<8><<<grid, 256, smem, st>>>(prm);
-        else prune_kernel<16><<<grid, 256, smem, st>>>(prm);
+    prm.acc = prm.recv = prm.mcounts = nullptr;
+    prm.tok_rdev = prm.tok_rnode = nullptr;
+    if (after) {
+        CAP_TRY(eval_zero_ws(L, E, topo.D, 1, true, ws, st));
+        EvalWs ew = eval_ws_carve(ws, L, E, topo.D, 1);
+        prm.acc = ew.acc;
+        prm.recv = ew.recv;
+        prm.mcounts = ew.mcounts;
+        prm.tok_rdev = after->tok_remote_dev;
+        prm.tok_rnode = after->tok_remote_node;
     }
-    note_launch();
-    return check_launch("prune_kernel");
+    if (T > 0) {
+        prm.idx = idx;
+        prm.w = w;
+        prm.token_src = token_src;
+        prm.expert_dev = expert_dev;
+        prm.dev_node = topo.dev_node;
+        prm.kept = kept;
+        prm.near_margin = reinterpret_cast<unsigned long long *>(near_margin);
+        prm.T = T;
+        prm.k = k;
+        prm.E = E;
+        prm.D = topo.D;
+        prm.N = topo.N;
+        prm.cost_local = topo.cost_local;
+        prm.cost_intra = topo.cost_intra;
+        prm.cost_inter = topo.cost_inter;
+        prm.p = p;
+        prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
+                  (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
+        dim3 grid((unsigned)((T + 255) / 256), (unsigned)L);
+        const size_t smem = sizeof(int) * ((size_t)2 * E + 128);
+        {
+            KernelTimerScope ts("prune", st);
+            if (k <= 8) prune_kernel<8><<<grid, 256, smem, st>>>(prm);
+            else prune_kernel<16><<<grid, 256, smem, st>>>(prm);
+        }
+        note_launch();
+        CAP_TRY(check_launch("prune_kernel"));
+    }
+    if (after) {
+        EvalWs ew = eval_ws_carve(ws, L, E, topo.D, 1);
+        return launch_eval_finalize(L, E, 1, expert_dev, topo, reinterpret_cast<const int64_t *>(ew.mcounts), *after,
+                                    ws, st);
+    }
+    return CAP_OK;
 }
 
 }  // namespace cap
