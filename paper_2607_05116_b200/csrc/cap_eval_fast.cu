@@ -127,6 +127,10 @@ struct EvalFastParams {
     int64_t T, tpc;
     int32_t k, E, P, D;
     int32_t WD, WN, Pc, PC, DW, NW, R, RS, S, logS, ncta_t, maxrec, NPR;
+    // optional fills done by the table kernel (saves separate memset nodes): 32-bit words
+    uint32_t *fill_ptr[4];
+    unsigned long long fill_words[4];
+    uint32_t fill_val[4];
 };
 
 // one thread per table word; grid (words of a table / 256, PC, L)
@@ -135,6 +139,14 @@ __global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
     const int layer = blockIdx.z, pc = blockIdx.y;
     const int rowq = q.RS * 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    {
+        const unsigned long long nthr = (unsigned long long)gridDim.x * gridDim.y * gridDim.z * blockDim.x;
+        const unsigned long long me = ((unsigned long long)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) *
+                                          blockDim.x + threadIdx.x;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            for (unsigned long long x = me; x < q.fill_words[j]; x += nthr) q.fill_ptr[j][x] = q.fill_val[j];
+    }
     if (i >= (q.E + 1) * rowq) return;
     const int e = i / rowq, w = i - e * rowq;
     uint32_t *t = const_cast<uint32_t *>(q.table) + ((size_t)layer * q.PC + pc) * (size_t)(q.E + 1) * rowq;
@@ -501,9 +513,14 @@ static int launch_kp(const EvalFastParams &prm, const EvalFastGeom &g, int L, cu
 
 // builds the one-hot code tables of all layers and candidate chunks (g.table_words words at fw.table)
 int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *expert_dev, const int32_t *dev_node,
-                    int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st)
+                    int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st, const EfFill *fills, int nfill)
 {
     EvalFastParams prm = {};
+    for (int j = 0; j < 4; ++j) {
+        prm.fill_ptr[j] = j < nfill ? reinterpret_cast<uint32_t *>(fills[j].ptr) : nullptr;
+        prm.fill_words[j] = j < nfill ? fills[j].bytes / 4 : 0;
+        prm.fill_val[j] = j < nfill ? fills[j].value : 0u;
+    }
     prm.expert_dev = expert_dev;
     prm.dev_node = dev_node;
     prm.table = fw.table;
@@ -573,10 +590,9 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     EvalFastGeom g;
     if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g)) return CAP_OK;
     EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g);
-    if (cudaMemsetAsync(fw.rec_src, 0xff, g.rec_slots * 4, st) != cudaSuccess)
-        return check_launch("memset rec_src");
-    CAP_TRY(ef_launch_table(g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st));
-    EvalFastParams prm;
+    const EfFill fill = {fw.rec_src, g.rec_slots * 4, 0xffffffffu};
+    CAP_TRY(ef_launch_table(g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st, &fill, 1));
+    EvalFastParams prm = {};
     prm.idx = idx;
     prm.kept = kept;
     prm.expert_dev = expert_dev;

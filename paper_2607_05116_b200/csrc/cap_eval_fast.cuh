@@ -55,8 +55,14 @@ struct EvalFastWs {
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
                               const EvalFastGeom &g);
 
+// a buffer the table kernel fills with a 32-bit value on the side (bytes must be a multiple of 4)
+struct EfFill {
+    void *ptr;
+    size_t bytes;
+    uint32_t value;
+};
 int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *expert_dev, const int32_t *dev_node,
-                    int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st);
+                    int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st, const EfFill *fills, int nfill);
 int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int32_t L, int64_t T, int32_t E,
                      int32_t P, const cap_topology &topo, cudaStream_t st);
 

@@ -559,12 +559,15 @@ int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, i
     if (!fused_geom(L, T, cfg.k, cfg.E, topo.D, topo.N, P, &f)) return CAP_OK;
     const int E = cfg.E;
     EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, f.g);
-    if (cudaMemsetAsync(counts, 0, sizeof(int64_t) * (size_t)L * E, st) != cudaSuccess ||
-        cudaMemsetAsync(coact, 0, sizeof(int32_t) * (size_t)L * E * E, st) != cudaSuccess ||
-        cudaMemsetAsync(fw.rec_src, 0xff, f.g.rec_slots * 4, st) != cudaSuccess)
-        return check_launch("memset fused");
-    CAP_TRY(eval_zero_ws(L, E, topo.D, P, false, ws, st));
-    CAP_TRY(ef_launch_table(f.g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st));
+    // every buffer the pass accumulates into is cleared by the table kernel itself (no memset nodes)
+    EvalWs base = eval_ws_carve(ws, L, E, topo.D, P);
+    const EfFill fills[4] = {
+        {counts, sizeof(int64_t) * (size_t)L * E, 0u},
+        {coact, sizeof(int32_t) * (size_t)L * E * E, 0u},
+        {fw.rec_src, f.g.rec_slots * 4, 0xffffffffu},
+        {base.acc, sizeof(unsigned long long) * ((size_t)L * P * ACC_N + (size_t)L * P * topo.D), 0u},
+    };
+    CAP_TRY(ef_launch_table(f.g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st, fills, 4));
     FusedParams prm;
     prm.logits = logits;
     prm.idx = idx;
