@@ -117,13 +117,17 @@ def algorithmic_bytes(cfg, has_src=False):
     LT = L * T
     ev_out = L * P * (8 * 8 + 2 * 8 * D + 2 * 8)
     return {
-        "trace_fused": LT * (4 * E + 8 * k) + L * P * E * 4 + L * (4 * E * E + 8 * E) + ev_out,
+        # 4E + 8k bytes per token (logits in, top-k indices and weights out)
+        "trace_fused": LT * (4 * E + 8 * k),
         "gate_topk": LT * (4 * E + 8 * k),
         "coact": LT * 4 * k + L * (4 * E * E + 8 * E),
         "eval": LT * (4 * k + (4 if has_src else 0)) + L * P * E * 4,
         "prune": LT * (8 * k + k),
         "dispatch_hist": LT * 4 * k + LT * k,
         "dispatch_scatter": LT * (4 * k + k + 4 * k + 4 * k),
+        "eval_table": L * P * E * 4,
+        "eval_decode": ev_out,
+        "eval_finalize": L * P * E * 4 + ev_out,
     }
 
 
@@ -264,11 +268,13 @@ def run_cap(args, cfg, W):
     # ---- warm-up; find the dominant kernel with the library's per-kernel event timers ----------
     tags = list(cap.KERNEL_TAGS)
     tot = {t: 0.0 for t in tags}
-    for i in range(max(args.warmup, 3)):
+    for i in range(max(args.warmup, 3) + 1):
         for j, t in enumerate(tags):
             cap.kernel_timer_arm(t, j)
         dstep(i)
         torch.cuda.synchronize()
+        if i == 0:
+            continue                    # first step pays one-time module loading: not representative
         for j, t in enumerate(tags):
             ms = cap.kernel_timer_ms(j)
             if ms > 0:
@@ -304,6 +310,17 @@ def run_cap(args, cfg, W):
     launches = cap.launch_count() - n0
     dom_ms = [cap.kernel_timer_ms(100 + i) for i in range(args.steps)]
     dom_ms = [v for v in dom_ms if v > 0]
+    dom_how = "library CUDA-event pair around the kernel in K directly launched steps"
+    if dominant == "trace_fused":
+        # direct launches from Python leave the GPU idle between kernels, which the event pair would
+        # count; the library's profiling entry launches the fused kernel alone K times back to back
+        # (rotating over the input sets, > L2) between two events on the launching stream
+        kms = cap.profile_fused_kernel([d[0] for d in d_sets], gate, d_sets[0][2], pipe.topo, pipe.fb,
+                                       max(args.steps, 8))
+        if kms is not None:
+            dom_ms = [kms]
+            dom_how = ("cap_profile_fused_kernel: the fused kernel alone, K back-to-back launches rotating "
+                       "over the input sets, one CUDA-event pair on the launching stream")
     # the fused call alone (S1+S2+S3: every kernel and memset of cap_trace_fused), graph replays
     ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     for i in range(3):
@@ -359,7 +376,8 @@ def run_cap(args, cfg, W):
             "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak,
                          "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
                          "traffic": None, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
-                         "kernel_ms": dom_avg, "algorithmic_bytes": ab.get(dominant),
+                         "kernel_ms": dom_avg, "kernel_ms_how": dom_how,
+                         "algorithmic_bytes": ab.get(dominant),
                          "fused_call_ms": ms_fused,
                          "fused_call_gbs": ab["trace_fused"] / (ms_fused * 1e-3) / 1e9,
                          "fused_call_frac": ab["trace_fused"] / (ms_fused * 1e-3) / 1e9 / peak,

@@ -177,6 +177,20 @@ int64_t cap_launch_count(void);
 int cap_kernel_timer_arm(const char *tag, int slot);
 float cap_kernel_timer_ms(int slot);
 
+/* Profiling aid, synchronous, host pointers where noted: builds the candidate tables once, then
+ * launches ONLY the fused S1+S2+S3 kernel of cap_trace_fused n_rep times back to back on `stream`
+ * (launch i reads logits_list[i % n_list], so that inputs larger than L2 can be rotated) between two
+ * library-owned CUDA events, and stores the average device time per launch in *avg_ms (host).
+ * logits_list is a HOST array of n_list device pointers.  The outputs are left un-finalised (the
+ * accumulators hold n_rep passes).  CAP_EINVAL when the configuration is not served by the fused
+ * kernel (it is for softmax scoring with renormalisation, no group limit, k <= 8, E in {64,128,256},
+ * token_src NULL, candidates fitting one table).  Other arguments as in cap_trace_fused. */
+int cap_profile_fused_kernel(const float *const *logits_list, int32_t n_list, int32_t n_rep, int32_t L,
+                             int64_t T, const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w,
+                             int64_t *counts, int32_t *coact, const int32_t *expert_dev, int32_t P,
+                             const cap_topology *topo, const cap_eval_out *out, void *ws, size_t ws_bytes,
+                             void *stream, float *avg_ms);
+
 /* Library version string (static storage). */
 const char *cap_version(void);
 

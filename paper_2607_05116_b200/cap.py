@@ -17,7 +17,7 @@ OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
            "cap_dispatch_layout", "cap_trace_fused", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
-           "cap_kernel_timer_arm", "cap_kernel_timer_ms")
+           "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter")
@@ -76,6 +76,9 @@ def lib():
         L.cap_trace_fused.argtypes = [vp, vp, i32, i64, C.POINTER(GateCfg), vp, vp, vp, vp, vp, vp,
                                       i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz, vp]
         L.cap_validate_placements.argtypes = [vp, i32, i32, i32, i32, vp]
+        L.cap_profile_fused_kernel.argtypes = [C.POINTER(C.c_void_p), i32, i32, i32, i64, C.POINTER(GateCfg), vp, vp,
+                                               vp, vp, vp, i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz,
+                                               vp, C.POINTER(C.c_float)]
         L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
         L.cap_kernel_timer_ms.argtypes = [C.c_int]
         L.cap_kernel_timer_ms.restype = C.c_float
@@ -255,6 +258,24 @@ def trace_fused(logits, bias, cfg, token_src, expert_dev, topo, bufs=None, per_t
                                C.byref(bufs.out_struct), _ptr(bufs.ws), bufs.ws.numel(), _stream())
     _check(rc, "cap_trace_fused")
     return bufs
+
+
+def profile_fused_kernel(logits_list, cfg, expert_dev, topo, bufs, n_rep):
+    """Average device time (ms) of the fused S1+S2+S3 kernel alone over n_rep back-to-back launches
+    rotating over logits_list; returns None if the configuration is not served by the fused kernel."""
+    L, T, E = logits_list[0].shape
+    P = expert_dev.shape[1]
+    arr = (C.c_void_p * len(logits_list))(*[t.data_ptr() for t in logits_list])
+    ms = C.c_float(0.0)
+    rc = lib().cap_profile_fused_kernel(arr, len(logits_list), n_rep, L, T, C.byref(cfg), _ptr(bufs.idx),
+                                        _ptr(bufs.w), _ptr(bufs.counts), _ptr(bufs.coact),
+                                        _ptr(expert_dev, torch.int32), P, C.byref(topo),
+                                        C.byref(bufs.out_struct), _ptr(bufs.ws), bufs.ws.numel(), _stream(),
+                                        C.byref(ms))
+    if rc == EINVAL:
+        return None
+    _check(rc, "cap_profile_fused_kernel")
+    return float(ms.value)
 
 
 def validate_placements(expert_dev, D):

@@ -256,6 +256,23 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
                        (int64_t)P * cfg->E, *topo, counts, *out, ws, st);
 }
 
+int cap_profile_fused_kernel(const float *const *logits_list, int32_t n_list, int32_t n_rep, int32_t L,
+                             int64_t T, const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w,
+                             int64_t *counts, int32_t *coact, const int32_t *expert_dev, int32_t P,
+                             const cap_topology *topo, const cap_eval_out *out, void *ws, size_t ws_bytes,
+                             void *stream, float *avg_ms)
+{
+    if (!logits_list || n_list < 1 || n_rep < 1 || !avg_ms) return CAP_EINVAL;
+    if (!gate_ok(cfg) || !sizes_ok(L, T, cfg->E, cfg->k) || !topo_ok(topo) || P < 1 || !out || L < 1 || T < 1)
+        return CAP_EINVAL;
+    if (!topk_idx || !topk_w || !counts || !coact || !expert_dev) return CAP_EINVAL;
+    if (!ws || ws_bytes < eval_ws_bytes(L, T, cfg->E, cfg->k, topo->D, P)) return CAP_EWORKSPACE;
+    bool used = false;
+    CAP_TRY(profile_trace_fused_kernel(logits_list, n_list, n_rep, avg_ms, L, T, *cfg, topk_idx, topk_w, counts,
+                                       coact, expert_dev, P, *topo, *out, ws, (cudaStream_t)stream, &used));
+    return used ? CAP_OK : CAP_EINVAL;
+}
+
 int cap_validate_placements(const int32_t *expert_dev, int32_t L, int32_t P, int32_t E, int32_t D,
                             void *stream)
 {

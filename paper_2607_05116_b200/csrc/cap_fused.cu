@@ -544,17 +544,14 @@ static int launch_fused_e(const FusedParams &prm, const FusedGeom &f, int L, cud
     return check_launch("trace_fused_kernel");
 }
 
-int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
-                            int32_t *idx, float *w, int64_t *counts, int32_t *coact, const int32_t *token_src,
-                            const int32_t *expert_dev, int32_t P, const cap_topology &topo,
-                            const cap_eval_out &out, void *ws, cudaStream_t st, bool *used)
+// nrep > 0: profiling mode -- after the table build, launch ONLY the fused kernel nrep times back to
+// back (input i = logits_list[i % nlist]) between two events and return the average in *avg_ms.
+static int fused_core(const float *const *logits_list, int nlist, int nrep, float *avg_ms, int32_t L, int64_t T,
+                      const cap_gate_cfg &cfg, int32_t *idx, float *w, int64_t *counts, int32_t *coact,
+                      const int32_t *expert_dev, int32_t P, const cap_topology &topo, const cap_eval_out &out,
+                      void *ws, cudaStream_t st, bool *used)
 {
     *used = false;
-    if (cfg.scoring != 0 || cfg.renormalize != 1 || cfg.n_group != 1 || cfg.k > 8 || bias != nullptr) return CAP_OK;
-    if (token_src != nullptr || out.tok_remote_dev || out.tok_remote_node) return CAP_OK;
-    if (!counts || !coact || L < 1 || T < 1 || P < 1) return CAP_OK;
-    if ((reinterpret_cast<uintptr_t>(logits) | reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u)
-        return CAP_OK;
     FusedGeom f;
     if (!fused_geom(L, T, cfg.k, cfg.E, topo.D, topo.N, P, &f)) return CAP_OK;
     const int E = cfg.E;
@@ -569,7 +566,7 @@ int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, i
     };
     CAP_TRY(ef_launch_table(f.g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st, fills, 4));
     FusedParams prm;
-    prm.logits = logits;
+    prm.logits = logits_list[0];
     prm.idx = idx;
     prm.w = w;
     prm.counts = reinterpret_cast<unsigned long long *>(counts);
@@ -592,17 +589,71 @@ int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, i
     prm.ncta_t = f.g.ncta_t;
     prm.nst = f.nst;
     prm.ns3w = f.ns3w;
-    int rc;
-    switch (E) {
-    case 64: rc = launch_fused_e<64>(prm, f, L, st); break;
-    case 128: rc = launch_fused_e<128>(prm, f, L, st); break;
-    default: rc = launch_fused_e<256>(prm, f, L, st); break;
+    cudaEvent_t ea = nullptr, eb = nullptr;
+    if (nrep > 0) {
+        if (cudaEventCreate(&ea) != cudaSuccess || cudaEventCreate(&eb) != cudaSuccess) return check_launch("event");
+        cudaEventRecord(ea, st);
     }
-    CAP_TRY(rc);
+    const int reps = nrep > 0 ? nrep : 1;
+    for (int i = 0; i < reps; ++i) {
+        prm.logits = logits_list[i % nlist];
+        int rc;
+        switch (E) {
+        case 64: rc = launch_fused_e<64>(prm, f, L, st); break;
+        case 128: rc = launch_fused_e<128>(prm, f, L, st); break;
+        default: rc = launch_fused_e<256>(prm, f, L, st); break;
+        }
+        CAP_TRY(rc);
+    }
+    if (nrep > 0) {
+        cudaEventRecord(eb, st);
+        if (cudaEventSynchronize(eb) != cudaSuccess) return check_launch("event sync");
+        float ms = 0.0f;
+        cudaEventElapsedTime(&ms, ea, eb);
+        cudaEventDestroy(ea);
+        cudaEventDestroy(eb);
+        if (avg_ms) *avg_ms = ms / (float)nrep;
+        *used = true;
+        return CAP_OK;        // accumulators hold nrep passes: profiling only, outputs are not finalised
+    }
     CAP_TRY(ef_launch_decode(f.g, fw, ws, L, T, E, P, topo, st));
     CAP_TRY(launch_eval_finalize(L, E, P, expert_dev, topo, counts, out, ws, st));
     *used = true;
     return CAP_OK;
+}
+
+static bool fused_args_ok(const float *logits, const float *bias, const cap_gate_cfg &cfg, int32_t *idx, float *w,
+                          int64_t *counts, int32_t *coact, const int32_t *token_src, const cap_eval_out &out,
+                          int32_t L, int64_t T, int32_t P)
+{
+    if (cfg.scoring != 0 || cfg.renormalize != 1 || cfg.n_group != 1 || cfg.k > 8 || bias != nullptr) return false;
+    if (token_src != nullptr || out.tok_remote_dev || out.tok_remote_node) return false;
+    if (!counts || !coact || L < 1 || T < 1 || P < 1) return false;
+    if ((reinterpret_cast<uintptr_t>(logits) | reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u)
+        return false;
+    return true;
+}
+
+int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
+                            int32_t *idx, float *w, int64_t *counts, int32_t *coact, const int32_t *token_src,
+                            const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                            const cap_eval_out &out, void *ws, cudaStream_t st, bool *used)
+{
+    *used = false;
+    if (!fused_args_ok(logits, bias, cfg, idx, w, counts, coact, token_src, out, L, T, P)) return CAP_OK;
+    return fused_core(&logits, 1, 0, nullptr, L, T, cfg, idx, w, counts, coact, expert_dev, P, topo, out, ws, st, used);
+}
+
+int profile_trace_fused_kernel(const float *const *logits_list, int nlist, int nrep, float *avg_ms, int32_t L,
+                               int64_t T, const cap_gate_cfg &cfg, int32_t *idx, float *w, int64_t *counts,
+                               int32_t *coact, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                               const cap_eval_out &out, void *ws, cudaStream_t st, bool *used)
+{
+    *used = false;
+    for (int i = 0; i < nlist; ++i)
+        if (!fused_args_ok(logits_list[i], nullptr, cfg, idx, w, counts, coact, nullptr, out, L, T, P)) return CAP_OK;
+    return fused_core(logits_list, nlist, nrep, avg_ms, L, T, cfg, idx, w, counts, coact, expert_dev, P, topo, out,
+                      ws, st, used);
 }
 
 }  // namespace cap

@@ -63,6 +63,10 @@ int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, i
                             int32_t *idx, float *w, int64_t *counts, int32_t *coact, const int32_t *token_src,
                             const int32_t *expert_dev, int32_t P, const cap_topology &topo,
                             const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
+int profile_trace_fused_kernel(const float *const *logits_list, int nlist, int nrep, float *avg_ms, int32_t L,
+                               int64_t T, const cap_gate_cfg &cfg, int32_t *idx, float *w, int64_t *counts,
+                               int32_t *coact, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
+                               const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
 size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
