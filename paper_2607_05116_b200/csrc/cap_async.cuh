@@ -51,6 +51,12 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
     }
 }
 
+// for waits that are expected to last microseconds: poll rarely, leave the issue slots to working warps
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity, unsigned ns)
+{
+    while (!mbar_try_wait(bar, parity)) __nanosleep(ns);
+}
+
 // TMA bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned) global -> shared,
 // completing `bytes` of transaction count on `bar`.
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)

@@ -8,10 +8,14 @@
 //   warps 2..9    S1: two lanes per token selection network (cap_gate_fast.cuh); besides top-k
 //                 indices / weights to HBM they leave (a) the token's table-row offsets in a
 //                 shared-memory ring for S3 and (b) its one-hot bytes in the current MMA tile
-//   warps 10..    S3: bit-sliced candidate scoring (cap_eval_fast.cuh) fed from the offsets ring;
-//                 at the end four of them drain the TMEM accumulator into the global matrix.
+//                 (when their tiles are done, four of them drain the TMEM accumulator into the
+//                 global matrix, one lane quadrant each)
+//   warps 10..    S3: bit-sliced candidate scoring (cap_eval_fast.cuh) fed from the offsets ring.
 // Everything is handed over through mbarriers; only run flushes use a named barrier among the S3
 // warps.  Records / decode / finalize are those of the standalone S3 path.
+#include <cstdio>
+#include <cstdlib>
+
 #include "cap_async.cuh"
 #include "cap_eval_fast.cuh"
 #include "cap_gate_fast.cuh"
@@ -214,7 +218,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             bulk_g2s(tbl, q.table + (size_t)layer * (E + 1) * q.RS * 4, (uint32_t)(E + 1) * rowb, &tbl_bar);
             for (int j = 0; j < nt; ++j) {
                 const int st = j % nst;
-                if (j >= nst) mbar_wait(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1));
+                if (j >= nst) mbar_wait_relaxed(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1), 256);
                 const int64_t tok0 = t0 + (int64_t)j * FU_TILE;
                 const int rows = (int)min((int64_t)FU_TILE, T - tok0);
                 mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
@@ -226,7 +230,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
         for (int m = 0; m < nm; ++m) {
             const int tb = m & 1;
             unsigned char *tile = tiles + (size_t)tb * EP * FU_MT;
-            mbar_wait(&tile_full[tb], (uint32_t)((m >> 1) & 1));
+            mbar_wait_relaxed(&tile_full[tb], (uint32_t)((m >> 1) & 1), 256);
             tc_fence_after();
             if (lane == 0) {
                 const uint32_t base = smem_u32(tile);
@@ -330,6 +334,49 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 if (!ghost) mbar_arrive(&empty_bar[st]);
             }
         }
+        // ---- drain the co-activation accumulator: S1 warps 0..3, one TMEM lane quadrant each ----
+        if (c < 4 && nm > 0) {
+            mbar_wait_relaxed(&acc_done, 0u, 128);
+            tc_fence_after();
+            const int quad = warp & 3;
+            int *C = q.coact + (size_t)layer * E * E;
+            unsigned long long *cnt = q.counts + (size_t)layer * E;
+#pragma unroll 1
+            for (int hh = 0; hh < EP / 128; ++hh) {
+                const int r = hh * 128 + quad * 32 + lane;
+#pragma unroll 1
+                for (int cb = 0; cb < EP / 32; ++cb) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)(hh * 256 + cb * 32), v);
+                    const bool rok = r < E;
+                    if (q.pack64) {
+                        int *cp = C + (size_t)(cb * 32) * E + (r & ~1);
+#pragma unroll
+                        for (int j = 0; j < 32; j += 2) {
+                            const uint32_t p0 = __shfl_xor_sync(0xffffffffu, v[j], 1);
+                            const uint32_t p1 = __shfl_xor_sync(0xffffffffu, v[j + 1], 1);
+                            const int jj = j + (lane & 1);
+                            const unsigned long long pk = (lane & 1) ? ((unsigned long long)v[j + 1] << 32) | p1
+                                                                     : ((unsigned long long)p0 << 32) | v[j];
+                            if (rok && cb * 32 + jj < E)
+                                asm volatile("red.global.add.u64 [%0], %1;" ::"l"(cp + (size_t)jj * E), "l"(pk) : "memory");
+                        }
+                    } else {
+                        int *cp = C + (size_t)(cb * 32) * E + r;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j)
+                            if (rok && cb * 32 + j < E)
+                                asm volatile("red.global.add.s32 [%0], %1;" ::"l"(cp + (size_t)j * E), "r"(v[j]) : "memory");
+                    }
+                    if (rok && (r >> 5) == cb) {
+                        uint32_t d = 0u;
+#pragma unroll
+                        for (int j = 0; j < 32; ++j) d = (r & 31) == j ? v[j] : d;
+                        atomicAdd(&cnt[r], (unsigned long long)d);
+                    }
+                }
+            }
+        }
     } else {
         // ================= S3: bit-sliced candidate scoring =================
         const int t3 = tid - FU_S3W0 * 32;
@@ -377,7 +424,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
 
         for (int b = 0; b < nb; ++b) {
             const int ob = b % FU_OB;
-            mbar_wait(&offs_full[ob], (uint32_t)((b / FU_OB) & 1));
+            mbar_wait_relaxed(&offs_full[ob], (uint32_t)((b / FU_OB) & 1), 128);
             const int64_t bt0 = t0 + (int64_t)b * BT;
             const int64_t bend = min(bt0 + BT, t1);
             const uint32_t *obuf = offs + ((size_t)ob * BT + sub) * FU_KP;
@@ -420,50 +467,6 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
         }
         if (have_run) flush();
 
-        // ---- drain the co-activation accumulator (four S3 warps, one TMEM lane quadrant each) ----
-        const int w3 = warp - FU_S3W0;
-        if (w3 < 4 && nm > 0) {
-            mbar_wait(&acc_done, 0u);
-            tc_fence_after();
-            const int quad = warp & 3;
-            int *C = q.coact + (size_t)layer * E * E;
-            unsigned long long *cnt = q.counts + (size_t)layer * E;
-#pragma unroll 1
-            for (int hh = 0; hh < EP / 128; ++hh) {
-                const int r = hh * 128 + quad * 32 + lane;
-#pragma unroll 1
-                for (int cb = 0; cb < EP / 32; ++cb) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)(hh * 256 + cb * 32), v);
-                    const bool rok = r < E;
-                    if (q.pack64) {
-                        int *cp = C + (size_t)(cb * 32) * E + (r & ~1);
-#pragma unroll
-                        for (int j = 0; j < 32; j += 2) {
-                            const uint32_t p0 = __shfl_xor_sync(0xffffffffu, v[j], 1);
-                            const uint32_t p1 = __shfl_xor_sync(0xffffffffu, v[j + 1], 1);
-                            const int jj = j + (lane & 1);
-                            const unsigned long long pk = (lane & 1) ? ((unsigned long long)v[j + 1] << 32) | p1
-                                                                     : ((unsigned long long)p0 << 32) | v[j];
-                            if (rok && cb * 32 + jj < E)
-                                asm volatile("red.global.add.u64 [%0], %1;" ::"l"(cp + (size_t)jj * E), "l"(pk) : "memory");
-                        }
-                    } else {
-                        int *cp = C + (size_t)(cb * 32) * E + r;
-#pragma unroll
-                        for (int j = 0; j < 32; ++j)
-                            if (rok && cb * 32 + j < E)
-                                asm volatile("red.global.add.s32 [%0], %1;" ::"l"(cp + (size_t)j * E), "r"(v[j]) : "memory");
-                    }
-                    if (rok && (r >> 5) == cb) {
-                        uint32_t d = 0u;
-#pragma unroll
-                        for (int j = 0; j < 32; ++j) d = (r & 31) == j ? v[j] : d;
-                        atomicAdd(&cnt[r], (unsigned long long)d);
-                    }
-                }
-            }
-        }
     }
     tc_fence_before();
     __syncthreads();
@@ -480,20 +483,31 @@ struct FusedGeom {
 
 static bool fused_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P, FusedGeom *f)
 {
-    if (E != 64 && E != 128 && E != 256) return false;
-    if (k > 8 || L < 1 || T < 1 || P < 1) return false;
+#define FG_FAIL(why) do { if (getenv("CAP_DEBUG")) fprintf(stderr, "fused_geom: %s\n", why); return false; } while (0)
+    if (E != 64 && E != 128 && E != 256) FG_FAIL("E");
+    if (k > 8 || L < 1 || T < 1 || P < 1) FG_FAIL("sizes");
     EvalFastGeom &g = f->g;
-    if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), 150 * 1024, &g)) return false;
-    if (g.PC != 1 || g.S < 4) return false;
+    if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), 150 * 1024, &g)) FG_FAIL("eval geom");
+    if (g.PC != 1 || g.S < 4) FG_FAIL("PC/S");
     f->EP = E <= 128 ? 128 : 256;
+    // fewer token sub-slots (S) shrink the offsets ring and the exchange area: trade them for ring stages
+    const size_t budget = 224 * 1024;
+    int nst = 0, bestS = 0, bestLog = 0, bestNst = 0;
+    for (int S = g.S, lg = g.logS; S >= 4; S /= 2, lg -= 1) {
+        int n = FU_MAXST;
+        for (; n >= 8; n -= 4)
+            if (fused_smem_layout(E, f->EP, g.RS, g.R, S, n).total <= budget) break;
+        if (n < 8) continue;
+        if (bestS == 0) { bestS = S; bestLog = lg; bestNst = n; }          // most sub-slots that fit at all
+        if (n >= 12 && S >= 8) { bestS = S; bestLog = lg; bestNst = n; break; }   // double-buffered S1 warps
+    }
+    if (bestS == 0) FG_FAIL("smem");
+    g.S = bestS;
+    g.logS = bestLog;
+    nst = bestNst;
     f->ns3w = (g.R * g.S + 31) / 32;
     f->nthreads = 32 * (FU_S3W0 + f->ns3w);
-    if (f->nthreads > FU_MAXTHREADS) return false;
-    const size_t budget = 224 * 1024;
-    int nst = FU_MAXST;
-    for (; nst >= 8; nst -= 4)
-        if (fused_smem_layout(E, f->EP, g.RS, g.R, g.S, nst).total <= budget) break;
-    if (nst < 8) return false;
+    if (f->nthreads > FU_MAXTHREADS) FG_FAIL("threads");
     f->nst = nst;
     f->smem = fused_smem_layout(E, f->EP, g.RS, g.R, g.S, nst).total;
     const int64_t ltiles = (T + FU_TILE - 1) / FU_TILE;

@@ -202,3 +202,49 @@ def test_launch_counter_moves():
     cap.gate_topk(x, None, cap.gate_cfg(16, 2))
     torch.cuda.synchronize()
     assert cap.launch_count() == n0 + 1
+
+
+# ------------------------------------------------------------------ fast paths on other shapes
+# The fused S1+S2+S3 kernel, the bit-sliced S3 path, the tcgen05 S2 path and the register-only S4
+# kernel are selected by shape; these cases walk their templates (E = 64 / 128 / 256, field widths
+# 8..64, node widths 2..8, k < 8) and their ragged edges (T not a multiple of the 16-token tile, of
+# the 64-token scoring block or of the source-device segments; single tokens; several layers).
+_FAST_SHAPES = [
+    dict(base="target", T=4099),
+    dict(base="target", T=1), dict(base="target", T=15), dict(base="target", T=16), dict(base="target", T=17),
+    dict(base="target", T=1000, k=3, P=17),
+    dict(base="target", T=3001, E=64, k=4, D=8, N=2, P=40, clusters=(8, 8, 0.5)),
+    dict(base="target", T=2500, E=256, k=8, D=32, N=4, P=24, clusters=(32, 8, 0.5)),
+    dict(base="target", T=2049, D=64, N=8, P=8),
+    dict(base="target", T=777, D=1, N=1, P=5),
+    dict(base="target", T=5000, D=4, N=4, P=300),
+    dict(base="qwen3", T=1500, L=3),
+    dict(base="target", T=70000, P=64),
+]
+
+
+@pytest.mark.parametrize("shape", _FAST_SHAPES, ids=lambda s: "-".join(f"{k}{v}" for k, v in s.items() if k != "clusters"))
+def test_fast_paths_shapes(shape):
+    kw = dict(shape)
+    cfg = W.CONFIGS[kw.pop("base")].with_(**kw)
+    layers = tuple(range(cfg.L))
+    check_all_stages(cfg, layers=layers, tag=f"{shape} ")
+    if cfg.T >= 16:
+        check_all_stages(cfg, layers=layers[:1], random_src=True, per_token=True, tag=f"{shape}/src ")
+
+
+@pytest.mark.parametrize("shape", [_FAST_SHAPES[0], _FAST_SHAPES[6], _FAST_SHAPES[7], _FAST_SHAPES[11]],
+                         ids=["E128", "E64", "E256", "L3"])
+def test_fused_kernel_serves_these_shapes(shape):
+    """cap_trace_fused must run its single fused kernel here (the kernel timer tagged 'trace_fused' only
+    fires for it), not the three-kernel fallback."""
+    kw = dict(shape)
+    cfg = W.CONFIGS[kw.pop("base")].with_(**kw)
+    from parity_util import layers_inputs
+    logits, bias, cand = layers_inputs(cfg, tuple(range(cfg.L)), cfg.T)
+    dn_d = dev(W.dev_node(cfg))
+    topo = topo_of(cfg, dn_d)
+    cap.kernel_timer_arm("trace_fused", 7)
+    cap.trace_fused(dev(logits), dev(bias), cap.gate_cfg(cfg.E, **cfg.gate), None, dev(cand), topo)
+    torch.cuda.synchronize()
+    assert cap.kernel_timer_ms(7) > 0.0
