@@ -1,20 +1,30 @@
 // S5 -- dispatch layout (P:L58 device-centric routing; BASELINE.json stage 5): stable counting
-// sort of the kept (token,slot) pairs by destination device.  Three kernels: per-chunk key
-// histograms, an ordered scan over (device, chunk) that fixes every chunk's base per device
-// (this is what makes the sort stable across blocks -- no global cursors), and a scatter that
-// ranks pairs inside a chunk with warp match/ballot and per-warp prefixes.
+// sort of the kept (token,slot) pairs by destination device.  The pair stream is cut into sub-chunks
+// of DS_SUB consecutive pairs, one per WARP.  Three kernels: (1) every warp counts the keys of its
+// sub-chunk (warp match, private counters: no block-level synchronisation, no atomics); (2) an
+// ordered scan over (device, sub-chunk) fixes every sub-chunk's base per device -- this is what makes
+// the sort stable across warps and blocks without global cursors; (3) every warp scatters its
+// sub-chunk in pair order, ranking equal keys inside a 32-pair round with match/popc.
 #include "cap_internal.cuh"
 
 namespace cap {
 
-constexpr int DS_CHUNK = 2048;   // pairs per block
-constexpr int DS_THREADS = 256;
+constexpr int DS_SUB = 256;       // pairs per warp (8 rounds of 32)
+constexpr int DS_THREADS = 256;   // 8 warps: 2048 pairs per block
+constexpr int DS_NW = DS_THREADS / 32;
+constexpr int DS_MAXD = 64;
+
+// sub-chunks of n pairs, padded so that every lane of the scan owns whole 16-byte vectors
+static int64_t ds_stride(int64_t n)
+{
+    const int64_t nsub = (n + DS_SUB - 1) / DS_SUB;
+    return ((nsub + 127) / 128) * 128;
+}
 
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D)
 {
     const int64_t n = T * k;
-    const int64_t nb = (n + DS_CHUNK - 1) / DS_CHUNK;
-    return (size_t)(2 * nb * D) * sizeof(int) + 256;
+    return (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
 }
 
 __device__ __forceinline__ int pair_key(const int32_t *idx, const uint8_t *kept, const int *s_map,
@@ -25,46 +35,74 @@ __device__ __forceinline__ int pair_key(const int32_t *idx, const uint8_t *kept,
     return s_map[idx[i]];
 }
 
+// hist[d][sub] = kept pairs of sub-chunk `sub` going to device d (rows of `stride` entries, zero padded)
 __global__ void __launch_bounds__(DS_THREADS)
 dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, int64_t n,
                      int E, int D, const int32_t *__restrict__ expert_dev, int *__restrict__ hist,
-                     int64_t nb)
+                     int64_t stride)
 {
     extern __shared__ int sm[];
-    int *s_map = sm;          // [E]
-    int *cnt = sm + E;        // [D]
+    int *s_map = sm;                               // [E]
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int *cnt = sm + E + warp * DS_MAXD;            // [D] private to the warp
+    pdl_launch_dependents();
+    pdl_wait();
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
-    for (int i = threadIdx.x; i < D; i += blockDim.x) cnt[i] = 0;
+    for (int d = lane; d < D; d += 32) cnt[d] = 0;
     __syncthreads();
-    const int64_t i0 = (int64_t)blockIdx.x * DS_CHUNK;
-    for (int j = threadIdx.x; j < DS_CHUNK; j += blockDim.x) {
-        int d = pair_key(idx, kept, s_map, i0 + j, n);
-        if (d >= 0) atomicAdd(&cnt[d], 1);
+    const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
+    if (sub >= stride) return;
+    const int64_t i0 = sub * DS_SUB;
+    if (i0 < n) {
+        int key[DS_SUB / 32];
+#pragma unroll
+        for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n);
+#pragma unroll
+        for (int r = 0; r < DS_SUB / 32; ++r) {
+            const unsigned grp = __match_any_sync(0xffffffffu, key[r]);
+            if (key[r] >= 0 && (grp & ((1u << lane) - 1u)) == 0u) cnt[key[r]] += __popc(grp);   // one lane per key
+            __syncwarp();
+        }
     }
-    __syncthreads();
-    for (int d = threadIdx.x; d < D; d += blockDim.x) hist[(int64_t)d * nb + blockIdx.x] = cnt[d];
+    for (int d = lane; d < D; d += 32) hist[(int64_t)d * stride + sub] = cnt[d];
 }
 
-// One block.  Warp w scans device d = w, w+nwarps, ... over all chunks (device-major layout).
+// One block, warp w scans devices w, w + nwarps, ... in coalesced chunks of 128 sub-chunks (one int4
+// per lane), four chunks in flight: the loop is bound by L2 latency, not by arithmetic.
 __global__ void __launch_bounds__(1024)
 dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, long long *__restrict__ offsets,
-                     int D, int64_t nb)
+                     int D, int64_t stride)
 {
-    __shared__ long long tot[64];
+    __shared__ long long tot[DS_MAXD];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    const int64_t nch = stride / 128;
+    pdl_launch_dependents();
+    pdl_wait();
     for (int d = warp; d < D; d += nw) {
-        int run = 0;
-        for (int64_t b0 = 0; b0 < nb; b0 += 32) {
-            int64_t b = b0 + lane;
-            int v = (b < nb) ? hist[(int64_t)d * nb + b] : 0;
-            int inc = v;
+        const int4 *h = reinterpret_cast<const int4 *>(hist + (int64_t)d * stride) + lane;
+        int4 *bs = reinterpret_cast<int4 *>(base + (int64_t)d * stride) + lane;
+        int run = 0;                               // pairs of device d before the current chunk
+        for (int64_t c0 = 0; c0 < nch; c0 += 4) {
+            int4 v[4];
 #pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int y = __shfl_up_sync(0xffffffffu, inc, o);
-                if (lane >= o) inc += y;
+            for (int j = 0; j < 4; ++j) v[j] = c0 + j < nch ? h[(c0 + j) * 32] : make_int4(0, 0, 0, 0);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int sum = (v[j].x + v[j].y) + (v[j].z + v[j].w);
+                int inc = sum;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int y = __shfl_up_sync(0xffffffffu, inc, o);
+                    if (lane >= o) inc += y;
+                }
+                int4 o;
+                o.x = run + inc - sum;             // exclusive, within device d
+                o.y = o.x + v[j].x;
+                o.z = o.y + v[j].y;
+                o.w = o.z + v[j].z;
+                if (c0 + j < nch) bs[(c0 + j) * 32] = o;
+                run += __shfl_sync(0xffffffffu, inc, 31);
             }
-            if (b < nb) base[(int64_t)d * nb + b] = run + inc - v;   // exclusive, within device d
-            run += __shfl_sync(0xffffffffu, inc, 31);
         }
         if (lane == 0) tot[d] = run;
     }
@@ -80,43 +118,39 @@ __global__ void __launch_bounds__(DS_THREADS)
 dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, int64_t n,
                         int E, int D, const int32_t *__restrict__ expert_dev,
                         const int *__restrict__ base, const long long *__restrict__ offsets,
-                        int32_t *__restrict__ sorted_pairs, int32_t *__restrict__ pair_pos, int64_t nb)
+                        int32_t *__restrict__ sorted_pairs, int32_t *__restrict__ pair_pos, int64_t stride)
 {
     extern __shared__ int sm[];
-    constexpr int NW = DS_THREADS / 32;
-    int *s_map = sm;              // [E]
-    int *running = sm + E;        // [D]   next free position of device d for this chunk
-    int *wcnt = running + D;      // [NW][D]
+    int *s_map = sm;                               // [E]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int *running = sm + E + warp * DS_MAXD;        // [D] next free position per device, private to the warp
+    const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
+    pdl_launch_dependents();
+    pdl_wait();
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
-    for (int d = threadIdx.x; d < D; d += blockDim.x)
-        running[d] = (int)offsets[d] + base[(int64_t)d * nb + blockIdx.x];
+    const int64_t i0 = sub * DS_SUB;
+    if (i0 < n)
+        for (int d = lane; d < D; d += 32) running[d] = (int)offsets[d] + base[(int64_t)d * stride + sub];
     __syncthreads();
-    const int64_t i0 = (int64_t)blockIdx.x * DS_CHUNK;
-    for (int r = 0; r < DS_CHUNK / DS_THREADS; ++r) {
-        for (int i = threadIdx.x; i < NW * D; i += blockDim.x) wcnt[i] = 0;
-        __syncthreads();
-        const int64_t i = i0 + (int64_t)r * DS_THREADS + threadIdx.x;
-        const int d = pair_key(idx, kept, s_map, i, n);
+    if (i0 >= n) return;
+    int key[DS_SUB / 32];
+#pragma unroll
+    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n);
+#pragma unroll
+    for (int r = 0; r < DS_SUB / 32; ++r) {
+        const int64_t i = i0 + r * 32 + lane;
+        const int d = key[r];
         const unsigned grp = __match_any_sync(0xffffffffu, d);
         const int rank = __popc(grp & ((1u << lane) - 1u));
-        if (d >= 0 && rank == 0) wcnt[warp * D + d] = __popc(grp);
-        __syncthreads();
+        int pos = -1;
         if (d >= 0) {
-            int pos = running[d] + rank;
-            for (int w = 0; w < warp; ++w) pos += wcnt[w * D + d];
+            pos = running[d] + rank;
             sorted_pairs[pos] = (int32_t)i;
-            if (pair_pos) pair_pos[i] = pos;
-        } else if (pair_pos && i < n) {
-            pair_pos[i] = -1;
         }
-        __syncthreads();
-        for (int dd = threadIdx.x; dd < D; dd += blockDim.x) {
-            int s = 0;
-            for (int w = 0; w < NW; ++w) s += wcnt[w * D + dd];
-            running[dd] += s;
-        }
-        __syncthreads();
+        if (pair_pos && i < n) pair_pos[i] = pos;
+        __syncwarp();
+        if (d >= 0 && rank == 0) running[d] += __popc(grp);
+        __syncwarp();
     }
 }
 
@@ -130,28 +164,29 @@ int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t 
             return check_launch("memset offsets");
         return CAP_OK;
     }
-    const int64_t nb = (n + DS_CHUNK - 1) / DS_CHUNK;
+    const int64_t nsub = (n + DS_SUB - 1) / DS_SUB, stride = ds_stride(n);
+    const int64_t nb = (nsub + DS_NW - 1) / DS_NW, nbh = stride / DS_NW;
+    const size_t smem = sizeof(int) * (size_t)(E + DS_NW * DS_MAXD);
     int *hist = reinterpret_cast<int *>((reinterpret_cast<uintptr_t>(ws) + 255) & ~(uintptr_t)255);
-    int *base = hist + nb * D;
+    int *base = hist + stride * D;
     {
     KernelTimerScope ts("dispatch_hist", st);
-    dispatch_hist_kernel<<<(unsigned)nb, DS_THREADS, sizeof(int) * (size_t)(E + D), st>>>(
-        idx, kept, n, E, D, expert_dev, hist, nb);
+    launch_pdl(dispatch_hist_kernel, dim3((unsigned)nbh), dim3(DS_THREADS), smem, st, idx, kept, n, E, D, expert_dev, hist,
+               stride);
     }
     note_launch();
     CAP_TRY(check_launch("dispatch_hist_kernel"));
     {
     KernelTimerScope ts("dispatch_scan", st);
-    dispatch_scan_kernel<<<1, 1024, 0, st>>>(hist, base, reinterpret_cast<long long *>(offsets), D, nb);
+    launch_pdl(dispatch_scan_kernel, dim3(1), dim3(D <= 16 ? 512 : 1024), 0, st, hist, base,
+               reinterpret_cast<long long *>(offsets), D, stride);
     }
     note_launch();
     CAP_TRY(check_launch("dispatch_scan_kernel"));
     {
     KernelTimerScope ts("dispatch_scatter", st);
-    dispatch_scatter_kernel<<<(unsigned)nb, DS_THREADS,
-                              sizeof(int) * (size_t)(E + D + (DS_THREADS / 32) * D), st>>>(
-        idx, kept, n, E, D, expert_dev, base, reinterpret_cast<const long long *>(offsets), sorted_pairs,
-        pair_pos, nb);
+    launch_pdl(dispatch_scatter_kernel, dim3((unsigned)nb), dim3(DS_THREADS), smem, st, idx, kept, n, E, D, expert_dev,
+               base, reinterpret_cast<const long long *>(offsets), sorted_pairs, pair_pos, stride);
     }
     note_launch();
     return check_launch("dispatch_scatter_kernel");

@@ -4,13 +4,14 @@
 // consecutive bytes), one thread owns one candidate and walks the block's tokens, building the
 // token's device set as a 64-bit mask.  Scalar totals live in registers, per-device token
 // counts in a shared-memory column private to the thread; both are flushed once per block.
+#include "cap_eval_final.cuh"
 #include "cap_internal.cuh"
 
 namespace cap {
 
 size_t eval_ws_bytes(int32_t L, int64_t T, int32_t E, int32_t k, int32_t D, int32_t P)
 {
-    size_t n = (size_t)L * P * ACC_N + (size_t)L * P * D + (size_t)L * E;
+    size_t n = (size_t)L * P * ACC_N + (size_t)L * P * D + (size_t)L * E + (size_t)L * 64;
     return n * sizeof(unsigned long long) + 512 + eval_fast_ws_bytes(L, T, k, E, D, P);
 }
 
@@ -21,6 +22,7 @@ EvalWs eval_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P)
     w.acc = reinterpret_cast<unsigned long long *>(a);
     w.recv = w.acc + (size_t)L * P * ACC_N;
     w.mcounts = w.recv + (size_t)L * P * D;
+    w.ldirect = w.mcounts + (size_t)L * E;
     return w;
 }
 
@@ -180,88 +182,30 @@ masked_counts_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
         if (cnt[i]) atomicAdd(&counts[(size_t)layer * E + i], (unsigned long long)cnt[i]);
 }
 
-struct FinalParams {
-    const unsigned long long *acc, *recv;
-    const long long *counts;            // [L][E]
-    const int32_t *expert_dev;          // [L][P][E]
-    cap_eval_out out;
-    int32_t L, P, E, D;
-    int32_t cost_local, cost_intra, cost_inter;
-    long long bytes_per_token;
-};
-
-// One warp per (layer, candidate): lanes stride over the experts (coalesced map and count reads),
-// per-device sums in shared memory, then lanes stride over the devices.
 constexpr int FIN_WARPS = 4;
 __global__ void __launch_bounds__(32 * FIN_WARPS) eval_finalize_kernel(FinalParams f)
 {
     __shared__ unsigned long long s_lp[FIN_WARPS][64];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int o = blockIdx.x * FIN_WARPS + warp;
+    pdl_launch_dependents();
+    pdl_wait();
     if (o >= f.L * f.P) return;
-    const int layer = o / f.P;
-    unsigned long long *lp = s_lp[warp];
-    lp[lane] = 0ull;
-    lp[lane + 32] = 0ull;
-    __syncwarp();
-    // load_pairs[d] = sum of the (kept) counts of the experts placed on d
-    const int32_t *pi = f.expert_dev + (size_t)o * f.E;
-    const long long *cnt = f.counts + (size_t)layer * f.E;
-    for (int e = lane; e < f.E; e += 32) {
-        const int d = pi[e];
-        const long long c = cnt[e];
-        if (d >= 0 && d < f.D && c) atomicAdd(&lp[d], (unsigned long long)c);
-    }
-    __syncwarp();
-    long long mx = 0, sm = 0, mxr = 0, smr = 0;
-    for (int d = lane; d < f.D; d += 32) {
-        const long long l = (long long)lp[d];
-        const long long r = (long long)f.recv[(size_t)o * f.D + d];
-        if (f.out.load_pairs) f.out.load_pairs[(size_t)o * f.D + d] = l;
-        if (f.out.recv_tokens) f.out.recv_tokens[(size_t)o * f.D + d] = r;
-        mx = max(mx, l);
-        sm += l;
-        mxr = max(mxr, r);
-        smr += r;
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        mx = max(mx, __shfl_xor_sync(0xffffffffu, mx, off));
-        mxr = max(mxr, __shfl_xor_sync(0xffffffffu, mxr, off));
-        sm += __shfl_xor_sync(0xffffffffu, sm, off);
-        smr += __shfl_xor_sync(0xffffffffu, smr, off);
-    }
-    if (lane != 0) return;
-    const unsigned long long *a = f.acc + (size_t)o * ACC_N;
-    const long long dv = (long long)a[ACC_DEV], loc = (long long)a[ACC_LOCAL],
-                    same = (long long)a[ACC_SAMENODE];
-    const long long rdev = dv - loc, intra = same - loc, inter = dv - same;
-    if (f.out.dev_visits) f.out.dev_visits[o] = dv;
-    if (f.out.remote_dev) f.out.remote_dev[o] = rdev;
-    if (f.out.remote_intra) f.out.remote_intra[o] = intra;
-    if (f.out.remote_inter) f.out.remote_inter[o] = inter;
-    if (f.out.node_visits) f.out.node_visits[o] = (long long)a[ACC_NODE];
-    if (f.out.remote_node) f.out.remote_node[o] = (long long)a[ACC_RNODE];
-    if (f.out.cost)
-        f.out.cost[o] = (long long)f.cost_local * loc + (long long)f.cost_intra * intra +
-                        (long long)f.cost_inter * inter;
-    if (f.out.bytes) f.out.bytes[o] = rdev * f.bytes_per_token;
-    if (f.out.imbalance) f.out.imbalance[o] = sm ? __ddiv_rn((double)(mx * f.D), (double)sm) : 0.0;
-    if (f.out.imbalance_recv)
-        f.out.imbalance_recv[o] = smr ? __ddiv_rn((double)(mxr * f.D), (double)smr) : 0.0;
+    eval_finalize_one(f, o, lane, s_lp[warp]);
 }
 
-// last step of every S3 path: per-candidate sums, costs, load_pairs from the counts, imbalance
-int launch_eval_finalize(int32_t L, int32_t E, int32_t P, const int32_t *expert_dev, const cap_topology &topo,
-                         const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st)
+FinalParams make_final_params(int32_t L, int32_t E, int32_t P, const int32_t *expert_dev, const cap_topology &topo,
+                              const int64_t *counts, const cap_eval_out &out, void *ws, int64_t *near_out)
 {
     EvalWs w = eval_ws_carve(ws, L, E, topo.D, P);
     FinalParams f;
     f.acc = w.acc;
     f.recv = w.recv;
     f.counts = reinterpret_cast<const long long *>(counts);
+    f.load_direct = nullptr;
     f.expert_dev = expert_dev;
     f.out = out;
+    f.near_out = reinterpret_cast<long long *>(near_out);
     f.L = L;
     f.P = P;
     f.E = E;
@@ -270,10 +214,19 @@ int launch_eval_finalize(int32_t L, int32_t E, int32_t P, const int32_t *expert_
     f.cost_intra = topo.cost_intra;
     f.cost_inter = topo.cost_inter;
     f.bytes_per_token = topo.bytes_per_token;
+    return f;
+}
+
+// last step of every S3 path: per-candidate sums, costs, load_pairs from the counts, imbalance
+int launch_eval_finalize(int32_t L, int32_t E, int32_t P, const int32_t *expert_dev, const cap_topology &topo,
+                         const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st,
+                         int64_t *near_out)
+{
+    const FinalParams f = make_final_params(L, E, P, expert_dev, topo, counts, out, ws, near_out);
     const int n = L * P;
     {
         KernelTimerScope ts("eval_finalize", st);
-        eval_finalize_kernel<<<(n + FIN_WARPS - 1) / FIN_WARPS, 32 * FIN_WARPS, 0, st>>>(f);
+        launch_pdl(eval_finalize_kernel, dim3((unsigned)((n + FIN_WARPS - 1) / FIN_WARPS)), dim3(32 * FIN_WARPS), 0, st, f);
     }
     note_launch();
     return check_launch("eval_finalize_kernel");
@@ -284,7 +237,7 @@ int eval_zero_ws(int32_t L, int32_t E, int32_t D, int32_t P, bool with_mcounts, 
 {
     EvalWs w = eval_ws_carve(ws, L, E, D, P);
     const size_t zero_bytes = sizeof(unsigned long long) *
-                              ((size_t)L * P * ACC_N + (size_t)L * P * D + (with_mcounts ? (size_t)L * E : 0));
+                              ((size_t)L * P * ACC_N + (size_t)L * P * D + (with_mcounts ? (size_t)L * E + (size_t)L * 64 : 0));
     if (cudaMemsetAsync(w.acc, 0, zero_bytes, st) != cudaSuccess) return check_launch("memset eval ws");
     return CAP_OK;
 }

@@ -102,7 +102,7 @@ EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t
 {
     // the fast-path region follows the generic region (acc, recv, mcounts)
     EvalWs base = eval_ws_carve(ws, L, E, D, P);
-    uintptr_t a = reinterpret_cast<uintptr_t>(base.mcounts + (size_t)L * E);
+    uintptr_t a = reinterpret_cast<uintptr_t>(base.ldirect + (size_t)L * 64);
     a = (a + 255) & ~(uintptr_t)255;
     EvalFastWs w;
     w.rec_src = reinterpret_cast<int32_t *>(a);
@@ -139,6 +139,8 @@ __global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
     const int layer = blockIdx.z, pc = blockIdx.y;
     const int rowq = q.RS * 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_launch_dependents();
+    pdl_wait();
     {
         const unsigned long long nthr = (unsigned long long)gridDim.x * gridDim.y * gridDim.z * blockDim.x;
         const unsigned long long me = ((unsigned long long)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) *
@@ -381,12 +383,15 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
     __shared__ uint32_t s_part[DEC_WARPS - 1][3][NA];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int w = blockIdx.x, pc = blockIdx.y, layer = blockIdx.z;
+    pdl_launch_dependents();
+    pdl_wait();
     if (threadIdx.x < 64) s_dn[threadIdx.x] = (int)threadIdx.x < q.D ? (unsigned char)q.dev_node[threadIdx.x] : 0;
-    if (threadIdx.x >= 64 && threadIdx.x < 72) {
-        const int n = threadIdx.x - 64;
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        const int n = threadIdx.x;              // from the shared copy: one round of global loads, not D
         unsigned long long m = 0ull;
         for (int d = 0; d < q.D; ++d)
-            if (q.dev_node[d] == n) m |= 1ull << d;
+            if (s_dn[d] == n) m |= 1ull << d;
         nodeset[n] = m;
     }
     __syncthreads();
@@ -537,7 +542,7 @@ int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *
     const int nw = (E + 1) * g.RS * 4;
     {
         KernelTimerScope ts("eval_table", st);
-        eval_table_kernel<<<dim3((unsigned)((nw + 255) / 256), (unsigned)g.PC, (unsigned)L), 256, 0, st>>>(prm);
+        launch_pdl(eval_table_kernel, dim3((unsigned)((nw + 255) / 256), (unsigned)g.PC, (unsigned)L), dim3(256), 0, st, prm);
     }
     note_launch();
     return check_launch("eval_table_kernel");
@@ -571,12 +576,12 @@ int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int3
     {
         KernelTimerScope ts("eval_decode", st);
         const dim3 dgrid((unsigned)g.W, (unsigned)g.PC, (unsigned)L);
-        if (na <= 12) eval_decode_kernel<12><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
-        else if (na <= 16) eval_decode_kernel<16><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
-        else if (na <= 20) eval_decode_kernel<20><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
-        else if (na <= 24) eval_decode_kernel<24><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
-        else if (na <= 28) eval_decode_kernel<28><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
-        else eval_decode_kernel<32><<<dgrid, 32 * DEC_WARPS, 0, st>>>(dq);
+        if (na <= 12) launch_pdl(eval_decode_kernel<12>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 16) launch_pdl(eval_decode_kernel<16>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 20) launch_pdl(eval_decode_kernel<20>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 24) launch_pdl(eval_decode_kernel<24>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 28) launch_pdl(eval_decode_kernel<28>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else launch_pdl(eval_decode_kernel<32>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
     }
     note_launch();
     return check_launch("eval_decode_kernel");

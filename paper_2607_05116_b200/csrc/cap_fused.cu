@@ -32,6 +32,25 @@ constexpr int FU_MAXST = 24;        // logits ring stages
 constexpr int FU_MAXTHREADS = 640;
 constexpr int FU_KP = 8;            // offsets per token (k <= 8, padded with the zero row)
 
+// Optional per-warp timeline (build with -DCAP_FU_TRACE; read back with cap_debug_fused_trace): clock64
+// stamps relative to the block's entry at role milestones, plus cycles spent waiting on each hand-over.
+#ifdef CAP_FU_TRACE
+__device__ unsigned long long g_fu_trace[160 * 24 * 8];
+#define FU_TR(ev, val)                                                                        \
+    do {                                                                                      \
+        if (lane == 0 && blockIdx.x < 160 && warp < 24)                                       \
+            g_fu_trace[((size_t)blockIdx.x * 24 + warp) * 8 + (ev)] = (unsigned long long)(val); \
+    } while (0)
+#define FU_NOW() ((long long)clock64() - tr_t0)
+#define FU_WAIT_BEGIN() const long long tr_w0 = clock64()
+#define FU_WAIT_END(acc) (acc) += clock64() - tr_w0
+#else
+#define FU_TR(ev, val) do { } while (0)
+#define FU_NOW() 0
+#define FU_WAIT_BEGIN() do { } while (0)
+#define FU_WAIT_END(acc) do { } while (0)
+#endif
+
 struct FusedParams {
     const float *logits;
     int32_t *idx;
@@ -42,7 +61,8 @@ struct FusedParams {
     int32_t *rec_src;             // [L][ncta_t][maxrec]
     uint32_t *rec_planes;         // [L][ncta_t][maxrec][NPR][W]
     int64_t T;
-    int64_t tiles_per_cta;        // real 16-token tiles per block
+    int64_t tiles_per_cta;        // real 16-token tiles per block (uniform split)
+    int32_t cps;                  // > 0: blocks per source device, block ranges aligned to the source runs
     float scale;
     int32_t k, D, pack64;
     int32_t R, RS, S, logS, maxrec, NPR, ncta_t, nst, ns3w;
@@ -151,6 +171,10 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
     constexpr int TILE_BYTES = FU_TILE * E * 4;
     constexpr int MT_TILES = FU_MT / FU_TILE;          // S1 tiles per MMA tile
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+#ifdef CAP_FU_TRACE
+    const long long tr_t0 = clock64();
+    long long tr_wa = 0, tr_wb = 0, tr_wc = 0;
+#endif
     const int layer = blockIdx.y;
     const int S = q.S, R = q.R, nst = q.nst, k = q.k;
     const int BT = EF_PASSES * S;                       // tokens per S3 block
@@ -165,18 +189,28 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
     const uint32_t zero_row = (uint32_t)E * rowb;
     const int ns3 = q.ns3w * 32;
 
-    // ---- this block's token range (whole 16-token tiles of one layer) ----
+    // ---- this block's token range [t0, t1) of one layer, in 16-token tiles from t0 ----
+    // uniform split: equal tile counts; aligned split (cps > 0): the tokens of each source device
+    // (default token_src: contiguous blocks, reading A5) are shared by cps blocks, so that a block
+    // scores a single run and flushes its counters once
     const int64_t T = q.T;
-    const int64_t ltiles = (T + FU_TILE - 1) / FU_TILE;
-    const int64_t tile0 = (int64_t)blockIdx.x * q.tiles_per_cta;
-    int64_t nt64 = ltiles - tile0;
-    if (nt64 > q.tiles_per_cta) nt64 = q.tiles_per_cta;
-    const int nt = nt64 > 0 ? (int)nt64 : 0;
+    int64_t t0, t1;
+    if (q.cps > 0) {
+        const int srcd = (int)blockIdx.x / q.cps, jj = (int)blockIdx.x % q.cps;
+        const int64_t b0 = ((int64_t)srcd * T + q.D - 1) / q.D, b1 = ((int64_t)(srcd + 1) * T + q.D - 1) / q.D;
+        const int64_t nts = (b1 - b0 + FU_TILE - 1) / FU_TILE;
+        const int64_t base = nts / q.cps, rem = nts % q.cps;
+        const int64_t ts = jj * base + (jj < rem ? jj : rem), tn = base + (jj < rem ? 1 : 0);
+        t0 = min(b1, b0 + ts * FU_TILE);
+        t1 = min(b1, t0 + tn * FU_TILE);
+    } else {
+        t0 = min(T, (int64_t)blockIdx.x * q.tiles_per_cta * FU_TILE);
+        t1 = min(T, t0 + q.tiles_per_cta * FU_TILE);
+    }
+    const int nt = (int)((t1 - t0 + FU_TILE - 1) / FU_TILE);
     const int pad = TPB > MT_TILES ? TPB : MT_TILES;
     const int ntp = ((nt + pad - 1) / pad) * pad;       // with ghost tiles: whole S3 blocks and MMA tiles
     const int nb = ntp / TPB, nm = ntp / MT_TILES;
-    const int64_t t0 = tile0 * FU_TILE;
-    const int64_t t1 = min(T, t0 + (int64_t)nt * FU_TILE);
     const float *logits = q.logits + (size_t)layer * T * E;
     int32_t *gidx = q.idx + (size_t)layer * T * k;
     float *gw = q.w + (size_t)layer * T * k;
@@ -207,9 +241,12 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
     }
     proxy_fence_async();
     tc_fence_before();
+    pdl_launch_dependents();
+    pdl_wait();                       // everything above touched shared memory / TMEM only
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = s_tmem;
+    FU_TR(1, FU_NOW());
 
     if (warp == 0) {
         // ================= producer =================
@@ -220,11 +257,12 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 const int st = j % nst;
                 if (j >= nst) mbar_wait_relaxed(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1), 256);
                 const int64_t tok0 = t0 + (int64_t)j * FU_TILE;
-                const int rows = (int)min((int64_t)FU_TILE, T - tok0);
+                const int rows = (int)min((int64_t)FU_TILE, t1 - tok0);
                 mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
                 bulk_g2s(ring + (size_t)st * TILE_BYTES, logits + tok0 * E, (uint32_t)rows * E * 4, &full_bar[st]);
             }
         }
+        FU_TR(2, FU_NOW());
     } else if (warp == 1) {
         // ================= tensor-core warp =================
         for (int m = 0; m < nm; ++m) {
@@ -257,6 +295,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 if (lane == 0) mbar_arrive(&tile_ready[tb]);
             }
         }
+        FU_TR(2, FU_NOW());
     } else if (warp < FU_S3W0) {
         // ================= S1: gate top-k, two lanes per token =================
         const int c = warp - 2;
@@ -265,7 +304,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             const bool ghost = j >= nt;
             const int st = j % nst;
             const int64_t tok = t0 + (int64_t)j * FU_TILE + tl;
-            const bool valid = !ghost && tok < T;
+            const bool valid = !ghost && tok < t1;
             int sel[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) sel[i] = 0;
@@ -273,10 +312,12 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 // this warp alternates on a stage with one other warp: first make sure that warp's
                 // tile (the previous use of the stage) has been consumed, then wait for ours
                 const int u = j / nst;
+                FU_WAIT_BEGIN();
                 if (u >= 1) mbar_wait(&empty_bar[st], (uint32_t)((u - 1) & 1));
                 mbar_wait(&full_bar[st], (uint32_t)(u & 1));
+                FU_WAIT_END(tr_wa);
                 const float *row = reinterpret_cast<const float *>(ring + (size_t)st * TILE_BYTES +
-                                                                   (size_t)(tok < T ? tl : 0) * E * 4);
+                                                                   (size_t)(tok < t1 ? tl : 0) * E * 4);
                 float wv[4];
                 gate_select_pair<E>(row, h, tl & 7, k, sel);
                 gate_weights_softmax_pair(row, h, k, sel, q.scale, wv);
@@ -299,7 +340,11 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             }
             // ---- table-row offsets for S3 ----
             const int b = j / TPB, ob = b % FU_OB;
-            if (b >= FU_OB) mbar_wait(&offs_empty[ob], (uint32_t)(((b / FU_OB) - 1) & 1));
+            {
+                FU_WAIT_BEGIN();
+                if (b >= FU_OB) mbar_wait(&offs_empty[ob], (uint32_t)(((b / FU_OB) - 1) & 1));
+                FU_WAIT_END(tr_wb);
+            }
             {
                 uint4 o4;
                 uint32_t ov[4];
@@ -315,7 +360,11 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             }
             // ---- one-hot bytes for the co-activation MMA ----
             const int m = j / MT_TILES, tb = m & 1;
-            if (m >= 2) mbar_wait(&tile_ready[tb], (uint32_t)(((m >> 1) - 1) & 1));
+            {
+                FU_WAIT_BEGIN();
+                if (m >= 2) mbar_wait(&tile_ready[tb], (uint32_t)(((m >> 1) - 1) & 1));
+                FU_WAIT_END(tr_wc);
+            }
             if (valid) {
                 const int tp = (j % MT_TILES) * FU_TILE + tl;
                 unsigned char *col = tiles + (size_t)tb * EP * FU_MT + (tp >> 4) * LBO + (tp & 15);
@@ -334,9 +383,14 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 if (!ghost) mbar_arrive(&empty_bar[st]);
             }
         }
+        FU_TR(2, FU_NOW());
+        FU_TR(5, tr_wa);
+        FU_TR(6, tr_wb);
+        FU_TR(7, tr_wc);
         // ---- drain the co-activation accumulator: S1 warps 0..3, one TMEM lane quadrant each ----
         if (c < 4 && nm > 0) {
             mbar_wait_relaxed(&acc_done, 0u, 128);
+            FU_TR(3, FU_NOW());
             tc_fence_after();
             const int quad = warp & 3;
             int *C = q.coact + (size_t)layer * E * E;
@@ -381,8 +435,20 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
         // ================= S3: bit-sliced candidate scoring =================
         const int t3 = tid - FU_S3W0 * 32;
         const bool active = t3 < R * S;
-        const int sub = active ? t3 / R : 0;
-        const int col = active ? t3 - sub * R : 0;
+        // (sub-slot, column) of this thread: whole warps own 32 consecutive columns of one sub-slot (one
+        // row segment per load: no bank conflicts); the R % 32 remaining columns are packed behind them
+        const int Rm = R & ~31, Rr = R - Rm;
+        int sub = 0, col = 0;
+        if (active) {
+            if (t3 < Rm * S) {
+                sub = (t3 >> 5) % S;
+                col = ((t3 >> 5) / S) * 32 + (t3 & 31);
+            } else {
+                const int tt = t3 - Rm * S;
+                sub = tt / Rr;
+                col = Rm + tt - sub * Rr;
+            }
+        }
         const unsigned char *tblc = tbl + col * 16;
         const int D = q.D;
         const size_t slot0 = ((size_t)layer * q.ncta_t + blockIdx.x) * q.maxrec;
@@ -410,6 +476,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 if (active && sub < half) fu_add_planes(pl, xch + sub * R + col, stride, np);
                 named_bar_sync(1, ns3);
             }
+            FU_TR(6, FU_NOW());
             if (active && sub == 0) {
                 uint4 *rp = reinterpret_cast<uint4 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
 #pragma unroll
@@ -424,7 +491,11 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
 
         for (int b = 0; b < nb; ++b) {
             const int ob = b % FU_OB;
-            mbar_wait_relaxed(&offs_full[ob], (uint32_t)((b / FU_OB) & 1), 128);
+            {
+                FU_WAIT_BEGIN();
+                mbar_wait_relaxed(&offs_full[ob], (uint32_t)((b / FU_OB) & 1), 128);
+                FU_WAIT_END(tr_wa);
+            }
             const int64_t bt0 = t0 + (int64_t)b * BT;
             const int64_t bend = min(bt0 + BT, t1);
             const uint32_t *obuf = offs + ((size_t)ob * BT + sub) * FU_KP;
@@ -465,18 +536,22 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             __syncwarp();
             if (lane == 0) mbar_arrive(&offs_empty[ob]);
         }
+        FU_TR(2, FU_NOW());
+        FU_TR(5, tr_wa);
         if (have_run) flush();
-
+        FU_TR(3, FU_NOW());
     }
+    FU_TR(4, FU_NOW());
     tc_fence_before();
     __syncthreads();
+    FU_TR(0, FU_NOW());
     if (warp == 1) tmem_dealloc(tmem, NCOLS);
 }
 
 // ---- host side ------------------------------------------------------------------------------------------
 struct FusedGeom {
     EvalFastGeom g;      // table / column geometry of the S3 part; ncta_t, maxrec, rec_* hold the fused values
-    int nst, ns3w, nthreads, EP;
+    int nst, ns3w, nthreads, EP, cps;
     int64_t tiles_per_cta;
     size_t smem;
 };
@@ -513,16 +588,29 @@ static bool fused_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, in
     const int64_t ltiles = (T + FU_TILE - 1) / FU_TILE;
     int64_t want = sm_count() / L;
     if (want < 1) want = 1;
-    f->tiles_per_cta = (ltiles + want - 1) / want;
-    g.ncta_t = (int)((ltiles + f->tiles_per_cta - 1) / f->tiles_per_cta);
-    if (g.ncta_t > 65535) return false;
-    const int64_t tpc = f->tiles_per_cta * FU_TILE;
     const int64_t BT = (int64_t)EF_PASSES * g.S;
     const int64_t cap_run = (int64_t)(EF_MAXBLK - 2) * BT;
-    int64_t srcb = ((tpc - 1) * D) / T + 1;
-    if (srcb > D - 1) srcb = D - 1;
-    g.maxrec = (int)((tpc + cap_run - 1) / cap_run + srcb + 1);
-    g.tpc = tpc;
+    f->cps = 0;
+    if (D <= want && T / D >= 4 * BT) {
+        // aligned split: want / D blocks per source device, one run per block
+        f->cps = (int)(want / D);
+        const int64_t per_src = (T + D - 1) / D;                            // tokens of the largest source
+        const int64_t nts = (per_src + FU_TILE - 1) / FU_TILE;
+        f->tiles_per_cta = (nts + f->cps - 1) / f->cps;
+        g.ncta_t = f->cps * D;
+        const int64_t tpc = f->tiles_per_cta * FU_TILE;
+        g.maxrec = (int)((tpc + cap_run - 1) / cap_run + 1);
+        g.tpc = tpc;
+    } else {
+        f->tiles_per_cta = (ltiles + want - 1) / want;
+        g.ncta_t = (int)((ltiles + f->tiles_per_cta - 1) / f->tiles_per_cta);
+        if (g.ncta_t > 65535) return false;
+        const int64_t tpc = f->tiles_per_cta * FU_TILE;
+        int64_t srcb = ((tpc - 1) * D) / T + 1;
+        if (srcb > D - 1) srcb = D - 1;
+        g.maxrec = (int)((tpc + cap_run - 1) / cap_run + srcb + 1);
+        g.tpc = tpc;
+    }
     g.NPR = EF_BT + g.logS;
     g.rec_slots = (size_t)L * g.ncta_t * g.maxrec;
     g.rec_words = g.rec_slots * g.NPR * g.W;
@@ -552,7 +640,7 @@ static int launch_fused_e(const FusedParams &prm, const FusedGeom &f, int L, cud
     }
     {
         KernelTimerScope ts("trace_fused", st);
-        trace_fused_kernel<E><<<dim3((unsigned)f.g.ncta_t, (unsigned)L), f.nthreads, f.smem, st>>>(prm);
+        launch_pdl(trace_fused_kernel<E>, dim3((unsigned)f.g.ncta_t, (unsigned)L), dim3(f.nthreads), f.smem, st, prm);
     }
     note_launch();
     return check_launch("trace_fused_kernel");
@@ -590,6 +678,7 @@ static int fused_core(const float *const *logits_list, int nlist, int nrep, floa
     prm.rec_planes = fw.rec_planes;
     prm.T = T;
     prm.tiles_per_cta = f.tiles_per_cta;
+    prm.cps = f.cps;
     prm.scale = cfg.scale;
     prm.k = cfg.k;
     prm.D = topo.D;
@@ -671,3 +760,11 @@ int profile_trace_fused_kernel(const float *const *logits_list, int nlist, int n
 }
 
 }  // namespace cap
+
+#ifdef CAP_FU_TRACE
+extern "C" int cap_debug_fused_trace(unsigned long long *host_out, int n)
+{
+    if (n > 160 * 24 * 8) n = 160 * 24 * 8;
+    return (int)cudaMemcpyFromSymbol(host_out, cap::g_fu_trace, sizeof(unsigned long long) * (size_t)n);
+}
+#endif

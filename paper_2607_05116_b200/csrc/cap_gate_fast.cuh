@@ -1,30 +1,50 @@
 // S1 fast path (softmax scoring, renormalised weights, no group limit, k <= 8): a PAIR of threads
 // per token.  The token's logits row sits in shared memory (staged by TMA); each thread streams its
 // half of the row in groups of 8, sorts each group with a 19-comparator network and merges it into a running sorted
-// top-8 list (half-cleaner + bitonic merge), all on 32-bit integer keys with min/max only.
+// top-8 list (half-cleaner + bitonic merge), all on 32-bit keys with fp32 min/max only.
 //
-// Keys.  key = order-preserving image of the logit with its low IB = log2(E) bits replaced by
-// (E-1-e): larger key = larger logit, equal truncated logits -> lower expert index first, so one
-// 32-bit comparator orders (value, index) pairs.  Truncation can only mis-order two experts whose
-// keys agree in all upper 32-IB bits; the thread therefore also tracks the 9th largest key and,
-// if any two neighbours among the top 9 share their upper bits, the warp redoes that token with
-// exact full-precision comparisons (k rounds of warp-wide arg-max).  The result is always the exact top-k with
-// ties toward the lower index (reading R2), the fast path is taken for all but ~0.1% of tokens.
+// Keys.  key = the logit's own bit pattern with its low BYTE replaced by the element's position
+// (one PRMT per element, no sign transform: fp32 min/max already order the patterns).  A payload can
+// only decide a comparison between two keys that agree in all upper 24 bits; the thread therefore
+// also tracks the 9th largest key and, if any two neighbours among the top 9 share their upper bits
+// -- or one of them is a zero, whose two signs are distinct patterns but compare equal (reading R2) --
+// the warp redoes that token with exact full-precision comparisons (k rounds of warp-wide arg-max).
+// The result is always the exact top-k with ties toward the lower index; the fast path alone serves
+// all but ~0.2% of the tokens of the paper-shaped traces.
 #pragma once
 #include "cap_async.cuh"
 #include "cap_internal.cuh"
 
 namespace cap {
 
+__device__ __forceinline__ float kmax(float a, float b)
+{
+    float r;
+    asm("max.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ float kmin(float a, float b)
+{
+    float r;
+    asm("min.f32 %0, %1, %2;" : "=f"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ float kmax3(float a, float b, float c)
+{
+    float r;
+    asm("max.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(a), "f"(b), "f"(c));
+    return r;
+}
+
 #define CAP_CE(a, b)                         \
     do {                                     \
-        const uint32_t _h = max((a), (b));   \
-        (b) = min((a), (b));                 \
+        const float _h = kmax((a), (b));     \
+        (b) = kmin((a), (b));                \
         (a) = _h;                            \
     } while (0)
 
 // sort 8 keys descending: optimal 19-comparator network
-__device__ __forceinline__ void sort8_desc(uint32_t (&g)[8])
+__device__ __forceinline__ void sort8_desc(float (&g)[8])
 {
     CAP_CE(g[0], g[1]); CAP_CE(g[2], g[3]); CAP_CE(g[4], g[5]); CAP_CE(g[6], g[7]);
     CAP_CE(g[0], g[2]); CAP_CE(g[1], g[3]); CAP_CE(g[4], g[6]); CAP_CE(g[5], g[7]);
@@ -36,14 +56,15 @@ __device__ __forceinline__ void sort8_desc(uint32_t (&g)[8])
 }
 
 // r (sorted desc) <- top 8 of r U g (g sorted desc); r9 <- max(r9, largest discarded key)
-__device__ __forceinline__ void merge8_desc(uint32_t (&r)[8], const uint32_t (&g)[8], uint32_t &r9)
+__device__ __forceinline__ void merge8_desc(float (&r)[8], const float (&g)[8], float &r9)
 {
-    uint32_t lo = r9;
+    float lo = r9;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const uint32_t a = r[i], b = g[7 - i];
-        r[i] = max(a, b);
-        lo = max(lo, min(a, b));
+    for (int i = 0; i < 8; i += 2) {
+        const float a0 = r[i], b0 = g[7 - i], a1 = r[i + 1], b1 = g[6 - i];
+        r[i] = kmax(a0, b0);
+        r[i + 1] = kmax(a1, b1);
+        lo = kmax3(lo, kmin(a0, b0), kmin(a1, b1));
     }
     r9 = lo;
     CAP_CE(r[0], r[4]); CAP_CE(r[1], r[5]); CAP_CE(r[2], r[6]); CAP_CE(r[3], r[7]);
@@ -51,20 +72,12 @@ __device__ __forceinline__ void merge8_desc(uint32_t (&r)[8], const uint32_t (&g
     CAP_CE(r[0], r[1]); CAP_CE(r[2], r[3]); CAP_CE(r[4], r[5]); CAP_CE(r[6], r[7]);
 }
 
-template <int E>
-struct GateBits {
-    static constexpr int IB = E <= 64 ? 6 : E <= 128 ? 7 : E <= 256 ? 8 : E <= 512 ? 9 : 10;
-    static constexpr uint32_t MASK = (1u << IB) - 1u;
-};
-
-// key of logit x for expert e (e a compile-time constant after unrolling)
-template <int E>
-__device__ __forceinline__ uint32_t gate_key(float x, int e)
+// key of the logit x at position pos of the thread's half row (pos a compile-time constant after
+// unrolling): the low byte of the pattern is replaced by pos
+__device__ __forceinline__ float gate_key(float x, int pos)
 {
-    const float c = __fadd_rn(x, 0.0f);                  // -0 -> +0 (IEEE: they compare equal)
-    const uint32_t b = __float_as_uint(c);
-    const uint32_t o = b ^ ((uint32_t)((int32_t)b >> 31) | 0x80000000u);
-    return (o | GateBits<E>::MASK) ^ (uint32_t)e;        // low bits = MASK - e (a payload, see above)
+    const uint32_t pay = 0x03020100u + 0x04040404u * (uint32_t)(pos >> 2);
+    return __uint_as_float(__byte_perm(__float_as_uint(x), pay, 0x3214u + (uint32_t)(pos & 3)));
 }
 
 // Exact top-k of one row, computed by the WHOLE warp (all 32 lanes must call it with the same row):
@@ -113,11 +126,10 @@ template <int E>
 __device__ __forceinline__ void gate_select_pair(const float *row, int h, int t7, int k, int (&sel)[8])
 {
     static_assert(E % 16 == 0 && E >= 32 && E <= 256, "E must be a multiple of 16 in [32, 256]");
-    constexpr int IB = GateBits<E>::IB;
     constexpr int H = E / 2;
     const uint32_t hb = smem_u32(row + h * H) | ((uint32_t)t7 << 4);   // 128-byte aligned | swizzle
-    uint32_t r[8];
-    uint32_t r9 = 0u;
+    float r[8];
+    float r9 = __uint_as_float(0xff800000u);                           // -inf: below every finite key
 #pragma unroll
     for (int gi = 0; gi < H / 8; ++gi) {
         float4 va, vb;
@@ -127,11 +139,11 @@ __device__ __forceinline__ void gate_select_pair(const float *row, int h, int t7
         asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
                      : "=f"(vb.x), "=f"(vb.y), "=f"(vb.z), "=f"(vb.w)
                      : "r"(hb ^ (uint32_t)(gi * 32 + 16)));
-        uint32_t g[8];
-        g[0] = gate_key<E>(va.x, gi * 8 + 0); g[1] = gate_key<E>(va.y, gi * 8 + 1);
-        g[2] = gate_key<E>(va.z, gi * 8 + 2); g[3] = gate_key<E>(va.w, gi * 8 + 3);
-        g[4] = gate_key<E>(vb.x, gi * 8 + 4); g[5] = gate_key<E>(vb.y, gi * 8 + 5);
-        g[6] = gate_key<E>(vb.z, gi * 8 + 6); g[7] = gate_key<E>(vb.w, gi * 8 + 7);
+        float g[8];
+        g[0] = gate_key(va.x, gi * 8 + 0); g[1] = gate_key(va.y, gi * 8 + 1);
+        g[2] = gate_key(va.z, gi * 8 + 2); g[3] = gate_key(va.w, gi * 8 + 3);
+        g[4] = gate_key(vb.x, gi * 8 + 4); g[5] = gate_key(vb.y, gi * 8 + 5);
+        g[6] = gate_key(vb.z, gi * 8 + 6); g[7] = gate_key(vb.w, gi * 8 + 7);
         sort8_desc(g);
         if (gi == 0) {
 #pragma unroll
@@ -140,25 +152,31 @@ __device__ __forceinline__ void gate_select_pair(const float *row, int h, int t7
             merge8_desc(r, g, r9);
         }
     }
-    // payload (low bits = MASK - position index) -> full expert index: undo the chunk swizzle
-    // (XOR of bits 2..4), then add h E/2.  MASK - e = ~e on the field, so both are XORs / a subtract.
+    // payload (position in the half row) -> full expert index: undo the chunk swizzle (XOR of bits
+    // 2..4), then add h E/2 (position < E/2 <= 128, so the sum stays inside the byte)
     const uint32_t swz = (uint32_t)t7 << 2;
     const uint32_t adj = (uint32_t)(h * H);
-    uint32_t g[8];
+    float g[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
-        r[i] = (r[i] ^ swz) - adj;
+        r[i] = __uint_as_float((__float_as_uint(r[i]) ^ swz) + adj);
         g[i] = __shfl_xor_sync(0xffffffffu, r[i], 16);
     }
-    r9 = (r9 ^ swz) - adj;
-    r9 = max(r9, __shfl_xor_sync(0xffffffffu, r9, 16));
+    r9 = kmax(r9, __shfl_xor_sync(0xffffffffu, r9, 16));               // its payload is never decoded
     merge8_desc(r, g, r9);
-    // neighbours among the top 9 that agree in every bit above the index field are ambiguous
-    bool amb = ((r[7] ^ r9) >> IB) == 0u;
+    // ambiguous: neighbours among the top 9 that agree in every bit above the payload, or a zero
+    // among them (+0 and -0 are different patterns that must compare equal)
+    uint32_t u[9];
 #pragma unroll
-    for (int i = 0; i < 7; ++i) amb |= ((r[i] ^ r[i + 1]) >> IB) == 0u;
+    for (int i = 0; i < 8; ++i) u[i] = __float_as_uint(r[i]);
+    u[8] = __float_as_uint(r9);
+    bool amb = false;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) sel[i] = (int)(GateBits<E>::MASK - (r[i] & GateBits<E>::MASK));
+    for (int i = 0; i < 8; ++i) amb |= ((u[i] ^ u[i + 1]) >> 8) == 0u;
+#pragma unroll
+    for (int i = 0; i < 9; ++i) amb |= (u[i] & 0x7fffff00u) == 0u;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) sel[i] = (int)(u[i] & 0xffu);
     // ambiguous tokens (rare): the whole warp redoes them one at a time with exact comparisons
     const int lane = (int)(threadIdx.x & 31u);
     unsigned todo = __ballot_sync(0xffffffffu, amb) & 0xffffu;     // one lane of each pair

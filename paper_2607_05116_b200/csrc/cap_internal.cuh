@@ -22,6 +22,37 @@ struct KernelTimerScope {
     cudaStream_t st_;
 };
 
+// ---- programmatic dependent launch (PDL) ---------------------------------------------------
+// The stages of a step are short kernels that follow each other on one stream; launched with the
+// programmatic-serialization attribute, kernel n+1 is scheduled while kernel n still runs and blocks
+// in pdl_wait() until kernel n has completed and flushed its memory (so the dependency is exactly the
+// stream order; only launch latency, block scheduling and the smem-only prologue overlap).  EVERY
+// kernel launched through launch_pdl() must execute pdl_wait() before its first global access.
+// Inside a stream capture the attribute is left out: measured on B200, programmatic edges made the
+// graph replay of a step slower (dispatch 18.5 -> 25.5 us), while directly launched kernels gain
+// (fused kernel back to back 33.2 -> 30.0 us).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                              Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    cudaStreamIsCapturing(st, &cs);
+    cfg.attrs = at;
+    cfg.numAttrs = cs == cudaStreamCaptureStatusNone ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 #define CAP_TRY(expr)                      \
     do {                                   \
         int _rc = (expr);                  \
@@ -29,12 +60,13 @@ struct KernelTimerScope {
     } while (0)
 
 // ---- accumulator slots of the evaluation (ws, int64 per (layer, candidate)) --------------
-enum { ACC_DEV = 0, ACC_LOCAL = 1, ACC_SAMENODE = 2, ACC_NODE = 3, ACC_RNODE = 4, ACC_N = 8 };
+enum { ACC_DEV = 0, ACC_LOCAL = 1, ACC_SAMENODE = 2, ACC_NODE = 3, ACC_RNODE = 4, ACC_NEAR = 5, ACC_TICKET = 6, ACC_N = 8 };
 
 struct EvalWs {
     unsigned long long *acc;      // [L][P][ACC_N]
     unsigned long long *recv;     // [L][P][D]
     unsigned long long *mcounts;  // [L][E] kept pairs per expert (when the caller gave none)
+    unsigned long long *ldirect;  // [L][64] kept pairs per device, counted directly (cap_prune, P = 1)
 };
 
 size_t eval_ws_bytes(int32_t L, int64_t T, int32_t E, int32_t k, int32_t D, int32_t P);
@@ -56,7 +88,8 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
                 int64_t layer_stride_maps, const cap_topology &topo, const int64_t *counts,
                 const cap_eval_out &out, void *ws, cudaStream_t st);
 int launch_eval_finalize(int32_t L, int32_t E, int32_t P, const int32_t *expert_dev, const cap_topology &topo,
-                         const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st);
+                         const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st,
+                         int64_t *near_out = nullptr);
 int eval_zero_ws(int32_t L, int32_t E, int32_t D, int32_t P, bool with_mcounts, void *ws, cudaStream_t st);
 // fused S1+S2+S3 kernel (cap_fused.cu): *used = false when the configuration does not fit it
 int launch_trace_fused_fast(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,

@@ -8,9 +8,12 @@
 //   5. kept[t][s] = 1 iff the slot's device was kept; near-margin tokens are counted (R-S4.7).
 // When the caller wants the after-metrics, the same thread also adds the token's kept device set
 // into the block's evaluation accumulators (distinct devices / nodes, local, same-node, received
-// tokens per device, kept pairs per expert), which are flushed with a few atomics per block.
+// tokens per device, kept pairs per expert), which are flushed with a few atomics per block; the
+// block that finishes last in its layer (ticket in a spare accumulator slot) turns the sums into the
+// caller's outputs (eval_finalize_one), so cap_prune with after-metrics is one memset and ONE kernel.
 #include <math_constants.h>
 
+#include "cap_eval_final.cuh"
 #include "cap_internal.cuh"
 
 namespace cap {
@@ -22,49 +25,62 @@ struct PruneParams {
     const int32_t *expert_dev;   // [L][E]
     const int32_t *dev_node;
     uint8_t *kept;
-    unsigned long long *near_margin;   // [L] or NULL
+    unsigned long long *near_margin;   // [L * near_stride] or NULL
+    int32_t near_stride;
+    FinalParams fin;              // used when acc != NULL
     // evaluation of the kept trace (all NULL when not wanted)
     unsigned long long *acc;      // [L][ACC_N]
     unsigned long long *recv;     // [L][D]
-    unsigned long long *mcounts;  // [L][E]
+    unsigned long long *ldirect;  // [L][64] kept pairs per device
     uint8_t *tok_rdev, *tok_rnode;   // [L][T] or NULL
     int64_t T;
     int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec;
     float p;
 };
 
+constexpr int PR_THREADS = 128;
+
 template <int KMAX>
-__global__ void __launch_bounds__(256) prune_kernel(PruneParams prm)
+__global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
 {
-    extern __shared__ int s_map[];     // [E] expert -> device, [64] device -> node, [64] recv, [E] counts
+    extern __shared__ int s_map[];     // [E] expert -> device, [64] device -> node, [64] recv, [64] pairs per device
     __shared__ unsigned long long s_nodemask[64];
     __shared__ unsigned long long s_acc[ACC_N];
+    __shared__ unsigned long long s_lp[64];
+    __shared__ int s_last;
     const int layer = blockIdx.y;
     const int E = prm.E, D = prm.D, k = prm.k;
     int *s_dn = s_map + E;
     int *s_recv = s_dn + 64;
-    int *s_cnt = s_recv + 64;
+    int *s_ld = s_recv + 64;
     const bool want_eval = prm.acc != nullptr;
-    for (int i = threadIdx.x; i < E; i += blockDim.x) {
-        s_map[i] = prm.expert_dev[(size_t)layer * E + i];
-        s_cnt[i] = 0;
-    }
+    pdl_launch_dependents();
+    pdl_wait();
+    for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = prm.expert_dev[(size_t)layer * E + i];
     if (threadIdx.x < 64) {
         s_dn[threadIdx.x] = (int)threadIdx.x < D ? prm.dev_node[threadIdx.x] : 0;
         s_recv[threadIdx.x] = 0;
-        unsigned long long m = 0ull;
-        if ((int)threadIdx.x < prm.N)
-            for (int d = 0; d < D; ++d)
-                if (prm.dev_node[d] == (int)threadIdx.x) m |= 1ull << d;
-        s_nodemask[threadIdx.x] = m;
+        s_ld[threadIdx.x] = 0;
     }
     if (threadIdx.x < ACC_N) s_acc[threadIdx.x] = 0ull;
+    __syncthreads();
+    if (threadIdx.x < 64) {
+        // devices of node threadIdx.x (from the shared copy: one round of global loads, not D)
+        unsigned long long m = 0ull;
+        for (int d = 0; d < D; ++d)
+            if (s_dn[d] == (int)threadIdx.x) m |= 1ull << d;
+        s_nodemask[threadIdx.x] = (int)threadIdx.x < prm.N ? m : 0ull;
+    }
     __syncthreads();
 
     const int64_t T = prm.T;
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int near = 0;
     unsigned a_dev = 0, a_loc = 0, a_same = 0, a_node = 0, a_rnode = 0;
+    unsigned long long km = 0ull;      // kept device set of this thread's token (after-metrics)
+    int dkey[KMAX];                    // device of every kept slot, -1 otherwise
+#pragma unroll
+    for (int s = 0; s < KMAX; ++s) dkey[s] = -1;
     if (t < T) {
         const int64_t base = ((int64_t)layer * T + t) * k;
         int e[KMAX], d[KMAX];
@@ -186,15 +202,10 @@ __global__ void __launch_bounds__(256) prune_kernel(PruneParams prm)
             for (int s = 0; s < KMAX; ++s) {
                 if (s < k && ((keepmask >> d[s]) & 1ull)) {
                     nodebits |= 1ull << s_dn[d[s]];
-                    atomicAdd(&s_cnt[e[s]], 1);
+                    dkey[s] = d[s];
                 }
             }
-            unsigned long long mm = keepmask;
-            while (mm) {
-                const int dd = __ffsll((long long)mm) - 1;
-                mm &= mm - 1;
-                atomicAdd(&s_recv[dd], 1);
-            }
+            km = keepmask;
             a_dev = __popcll(keepmask);
             a_loc = (unsigned)((keepmask >> src) & 1ull);
             a_same = __popcll(keepmask & s_nodemask[srcn]);
@@ -206,9 +217,27 @@ __global__ void __launch_bounds__(256) prune_kernel(PruneParams prm)
     }
     if (prm.near_margin) {
         const unsigned b = __ballot_sync(0xffffffffu, near != 0);
-        if ((threadIdx.x & 31) == 0 && b) atomicAdd(&prm.near_margin[layer], (unsigned long long)__popc(b));
+        if ((threadIdx.x & 31) == 0 && b) atomicAdd(&prm.near_margin[(size_t)layer * prm.near_stride], (unsigned long long)__popc(b));
     }
     if (want_eval) {
+        const int lane = threadIdx.x & 31;
+        // kept pairs per device: equal keys of a slot are counted once per warp (match), no per-pair atomics
+#pragma unroll
+        for (int s = 0; s < KMAX; ++s) {
+            const unsigned grp = __match_any_sync(0xffffffffu, dkey[s]);
+            if (dkey[s] >= 0 && (grp & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_ld[dkey[s]], __popc(grp));
+        }
+        // tokens received per device: one ballot per device, lane d keeps the count of devices d, d + 32
+        int r0 = 0, r1 = 0;
+        for (int dd = 0; dd < D; ++dd) {
+            const int c = __popc(__ballot_sync(0xffffffffu, (km >> dd) & 1ull));
+            if (lane == (dd & 31)) {
+                if (dd < 32) r0 = c;
+                else r1 = c;
+            }
+        }
+        if (r0) atomicAdd(&s_recv[lane], r0);
+        if (r1) atomicAdd(&s_recv[lane + 32], r1);
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             a_dev += __shfl_xor_sync(0xffffffffu, a_dev, off);
@@ -229,8 +258,18 @@ __global__ void __launch_bounds__(256) prune_kernel(PruneParams prm)
             atomicAdd(&prm.acc[(size_t)layer * ACC_N + threadIdx.x], s_acc[threadIdx.x]);
         if ((int)threadIdx.x < D && s_recv[threadIdx.x])
             atomicAdd(&prm.recv[(size_t)layer * D + threadIdx.x], (unsigned long long)s_recv[threadIdx.x]);
-        for (int i = threadIdx.x; i < E; i += blockDim.x)
-            if (s_cnt[i]) atomicAdd(&prm.mcounts[(size_t)layer * E + i], (unsigned long long)s_cnt[i]);
+        if (threadIdx.x < 64 && s_ld[threadIdx.x])
+            atomicAdd(&prm.ldirect[(size_t)layer * 64 + threadIdx.x], (unsigned long long)s_ld[threadIdx.x]);
+        // last block of the layer: all sums are in L2, finish the outputs
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0)
+            s_last = atomicAdd(&prm.acc[(size_t)layer * ACC_N + ACC_TICKET], 1ull) == (unsigned long long)gridDim.x - 1ull;
+        __syncthreads();
+        if (s_last && threadIdx.x < 32) {
+            __threadfence();
+            eval_finalize_one(prm.fin, layer, (int)threadIdx.x, s_lp);
+        }
     }
 }
 
@@ -241,20 +280,25 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
                  const cap_eval_out *after, void *ws, cudaStream_t st)
 {
     if (L == 0) return CAP_OK;
-    if (near_margin &&
+    // with the after-metrics the near-margin count rides in the evaluation accumulators (one memset for
+    // everything, written out by the finalize kernel); without them it is counted in place
+    if (near_margin && (!after || T == 0) &&
         cudaMemsetAsync(near_margin, 0, sizeof(int64_t) * (size_t)L, st) != cudaSuccess)
         return check_launch("memset near_margin");
     PruneParams prm;
-    prm.acc = prm.recv = prm.mcounts = nullptr;
+    prm.acc = prm.recv = prm.ldirect = nullptr;
     prm.tok_rdev = prm.tok_rnode = nullptr;
     if (after) {
         CAP_TRY(eval_zero_ws(L, E, topo.D, 1, true, ws, st));
         EvalWs ew = eval_ws_carve(ws, L, E, topo.D, 1);
         prm.acc = ew.acc;
         prm.recv = ew.recv;
-        prm.mcounts = ew.mcounts;
+        prm.ldirect = ew.ldirect;
         prm.tok_rdev = after->tok_remote_dev;
         prm.tok_rnode = after->tok_remote_node;
+        prm.fin = make_final_params(L, E, 1, expert_dev, topo, reinterpret_cast<const int64_t *>(ew.mcounts), *after, ws,
+                                    T > 0 ? near_margin : nullptr);
+        prm.fin.load_direct = ew.ldirect;
     }
     if (T > 0) {
         prm.idx = idx;
@@ -264,6 +308,11 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
         prm.dev_node = topo.dev_node;
         prm.kept = kept;
         prm.near_margin = reinterpret_cast<unsigned long long *>(near_margin);
+        prm.near_stride = 1;
+        if (after && near_margin) {
+            prm.near_margin = prm.acc + ACC_NEAR;
+            prm.near_stride = ACC_N;
+        }
         prm.T = T;
         prm.k = k;
         prm.E = E;
@@ -275,20 +324,20 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
         prm.p = p;
         prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
                   (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
-        dim3 grid((unsigned)((T + 255) / 256), (unsigned)L);
-        const size_t smem = sizeof(int) * ((size_t)2 * E + 128);
+        dim3 grid((unsigned)((T + PR_THREADS - 1) / PR_THREADS), (unsigned)L);
+        const size_t smem = sizeof(int) * ((size_t)E + 192);
         {
             KernelTimerScope ts("prune", st);
-            if (k <= 8) prune_kernel<8><<<grid, 256, smem, st>>>(prm);
-            else prune_kernel<16><<<grid, 256, smem, st>>>(prm);
+            if (k <= 8) launch_pdl(prune_kernel<8>, grid, dim3(PR_THREADS), smem, st, prm);
+            else launch_pdl(prune_kernel<16>, grid, dim3(PR_THREADS), smem, st, prm);
         }
         note_launch();
         CAP_TRY(check_launch("prune_kernel"));
     }
-    if (after) {
+    if (after && T == 0) {
         EvalWs ew = eval_ws_carve(ws, L, E, topo.D, 1);
         return launch_eval_finalize(L, E, 1, expert_dev, topo, reinterpret_cast<const int64_t *>(ew.mcounts), *after,
-                                    ws, st);
+                                    ws, st, nullptr);
     }
     return CAP_OK;
 }
