@@ -29,7 +29,7 @@ constexpr int FU_TILE = 16;         // tokens per S1 tile
 constexpr int FU_MT = 64;           // tokens per MMA tile (4 S1 tiles, 2 MMAs of K = 32)
 constexpr int FU_OB = 4;            // S3 offset blocks in the ring
 constexpr int FU_MAXST = 24;        // logits ring stages
-constexpr int FU_MAXTHREADS = 640;
+constexpr int FU_MAXTHREADS = 896;
 constexpr int FU_KP = 8;            // offsets per token (k <= 8, padded with the zero row)
 
 // Optional per-warp timeline (build with -DCAP_FU_TRACE; read back with cap_debug_fused_trace): clock64
@@ -96,41 +96,37 @@ __device__ __forceinline__ void named_bar_sync(int id, int nthreads)
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
 }
 
-// bit-sliced a += b; b has np planes of 4 words (the rest are zero)
-__device__ __forceinline__ void fu_add_planes(uint4 (&a)[EF_NPL], const uint4 *b, int stride, int np)
+// bit-sliced a += b; b has np planes of 2 words (the rest are zero)
+__device__ __forceinline__ void fu_add_planes(uint2 (&a)[EF_NPL], const uint2 *b, int stride, int np)
 {
-    uint4 carry = make_uint4(0u, 0u, 0u, 0u);
+    uint2 carry = make_uint2(0u, 0u);
 #pragma unroll
     for (int p = 0; p < EF_NPL; ++p) {
-        const uint4 x = p < np ? b[(size_t)p * stride] : make_uint4(0u, 0u, 0u, 0u);
-        uint4 s, c;
+        const uint2 x = p < np ? b[(size_t)p * stride] : make_uint2(0u, 0u);
+        uint2 s, c;
         CAP_CSA(s.x, c.x, a[p].x, x.x, carry.x);
         CAP_CSA(s.y, c.y, a[p].y, x.y, carry.y);
-        CAP_CSA(s.z, c.z, a[p].z, x.z, carry.z);
-        CAP_CSA(s.w, c.w, a[p].w, x.w, carry.w);
         a[p] = s;
         carry = c;
     }
 }
 
-// OR of the FU_KP table rows of one token at this thread's column
-__device__ __forceinline__ uint4 fu_token_mask(const unsigned char *tblc, const uint32_t *op)
+// OR of the FU_KP table rows of one token at this thread's 8-byte column
+__device__ __forceinline__ uint2 fu_token_mask(const unsigned char *tblc, const uint32_t *op)
 {
     const uint4 oa = *reinterpret_cast<const uint4 *>(op);
     const uint4 ob = *reinterpret_cast<const uint4 *>(op + 4);
-    const uint4 v0 = *reinterpret_cast<const uint4 *>(tblc + oa.x);
-    const uint4 v1 = *reinterpret_cast<const uint4 *>(tblc + oa.y);
-    const uint4 v2 = *reinterpret_cast<const uint4 *>(tblc + oa.z);
-    const uint4 v3 = *reinterpret_cast<const uint4 *>(tblc + oa.w);
-    const uint4 v4 = *reinterpret_cast<const uint4 *>(tblc + ob.x);
-    const uint4 v5 = *reinterpret_cast<const uint4 *>(tblc + ob.y);
-    const uint4 v6 = *reinterpret_cast<const uint4 *>(tblc + ob.z);
-    const uint4 v7 = *reinterpret_cast<const uint4 *>(tblc + ob.w);
-    uint4 m;
+    const uint2 v0 = *reinterpret_cast<const uint2 *>(tblc + oa.x);
+    const uint2 v1 = *reinterpret_cast<const uint2 *>(tblc + oa.y);
+    const uint2 v2 = *reinterpret_cast<const uint2 *>(tblc + oa.z);
+    const uint2 v3 = *reinterpret_cast<const uint2 *>(tblc + oa.w);
+    const uint2 v4 = *reinterpret_cast<const uint2 *>(tblc + ob.x);
+    const uint2 v5 = *reinterpret_cast<const uint2 *>(tblc + ob.y);
+    const uint2 v6 = *reinterpret_cast<const uint2 *>(tblc + ob.z);
+    const uint2 v7 = *reinterpret_cast<const uint2 *>(tblc + ob.w);
+    uint2 m;
     m.x = lop_or3(lop_or3(lop_or3(v0.x, v1.x, v2.x), v3.x, v4.x), lop_or3(v5.x, v6.x, v7.x), 0u);
     m.y = lop_or3(lop_or3(lop_or3(v0.y, v1.y, v2.y), v3.y, v4.y), lop_or3(v5.y, v6.y, v7.y), 0u);
-    m.z = lop_or3(lop_or3(lop_or3(v0.z, v1.z, v2.z), v3.z, v4.z), lop_or3(v5.z, v6.z, v7.z), 0u);
-    m.w = lop_or3(lop_or3(lop_or3(v0.w, v1.w, v2.w), v3.w, v4.w), lop_or3(v5.w, v6.w, v7.w), 0u);
     return m;
 }
 
@@ -184,7 +180,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
     unsigned char *tiles = fu_sm + lay.tiles;
     unsigned char *tbl = fu_sm + lay.table;
     uint32_t *offs = reinterpret_cast<uint32_t *>(fu_sm + lay.offs);
-    uint4 *xch = reinterpret_cast<uint4 *>(fu_sm + lay.xch);
+    uint2 *xch = reinterpret_cast<uint2 *>(fu_sm + lay.xch);
     const int rowb = q.RS * 16;
     const uint32_t zero_row = (uint32_t)E * rowb;
     const int ns3 = q.ns3w * 32;
@@ -433,11 +429,14 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
         }
     } else {
         // ================= S3: bit-sliced candidate scoring =================
+        // a thread owns one 8-byte column (2 words) of one token sub-slot: twice the threads of a 16-byte
+        // split, half the registers each -- more row loads in flight per SM (the loop waits on LDS latency)
         const int t3 = tid - FU_S3W0 * 32;
-        const bool active = t3 < R * S;
+        const int R2 = 2 * R;
+        const bool active = t3 < R2 * S;
         // (sub-slot, column) of this thread: whole warps own 32 consecutive columns of one sub-slot (one
         // row segment per load: no bank conflicts); the R % 32 remaining columns are packed behind them
-        const int Rm = R & ~31, Rr = R - Rm;
+        const int Rm = R2 & ~31, Rr = R2 - Rm;
         int sub = 0, col = 0;
         if (active) {
             if (t3 < Rm * S) {
@@ -449,14 +448,14 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 col = Rm + tt - sub * Rr;
             }
         }
-        const unsigned char *tblc = tbl + col * 16;
+        const unsigned char *tblc = tbl + col * 8;
         const int D = q.D;
         const size_t slot0 = ((size_t)layer * q.ncta_t + blockIdx.x) * q.maxrec;
         const int64_t cap_run = (int64_t)(EF_MAXBLK - 2) * BT;
         if (nt > 0) mbar_wait(&tbl_bar, 0u);
-        uint4 pl[EF_NPL];
+        uint2 pl[EF_NPL];
 #pragma unroll
-        for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint4(0u, 0u, 0u, 0u);
+        for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint2(0u, 0u);
         int nrec = 0, src = 0;
         int64_t rend = t0;               // end of the current run (none yet)
         bool have_run = false;
@@ -465,28 +464,28 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             // add the S sub-slots in the bit-sliced domain (tree through shared memory), write the record
             for (int lvl = 0; lvl < q.logS; ++lvl) {
                 const int half = S >> (lvl + 1);
-                const int stride = half * R;
+                const int stride = half * R2;
                 const int np = EF_BT + lvl;
                 if (active && sub >= half && sub < 2 * half) {
 #pragma unroll
                     for (int p = 0; p < EF_NPL; ++p)
-                        if (p < np) xch[(size_t)p * stride + (sub - half) * R + col] = pl[p];
+                        if (p < np) xch[(size_t)p * stride + (sub - half) * R2 + col] = pl[p];
                 }
                 named_bar_sync(1, ns3);
-                if (active && sub < half) fu_add_planes(pl, xch + sub * R + col, stride, np);
+                if (active && sub < half) fu_add_planes(pl, xch + sub * R2 + col, stride, np);
                 named_bar_sync(1, ns3);
             }
             FU_TR(6, FU_NOW());
             if (active && sub == 0) {
-                uint4 *rp = reinterpret_cast<uint4 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
+                uint2 *rp = reinterpret_cast<uint2 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
 #pragma unroll
                 for (int p = 0; p < EF_NPL; ++p)
-                    if (p < q.NPR) rp[(size_t)p * R + col] = pl[p];
+                    if (p < q.NPR) rp[(size_t)p * R2 + col] = pl[p];
             }
             if (t3 == 0) q.rec_src[slot0 + nrec] = src;
             ++nrec;
 #pragma unroll
-            for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint4(0u, 0u, 0u, 0u);
+            for (int p = 0; p < EF_NPL; ++p) pl[p] = make_uint2(0u, 0u);
         };
 
         for (int b = 0; b < nb; ++b) {
@@ -511,24 +510,21 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 const int64_t seg = min(bend, rend);
                 const bool whole = cur == bt0 && seg == bend;     // tokens past t1 carry the zero row
                 if (active) {
-                    uint4 x0, x1, x2, x3;
-                    uint32_t fAx, fAy, fAz, fAw, fBx, fBy, fBz, fBw;
+                    uint2 x0, x1, x2, x3;
+                    uint32_t fAx, fAy, fBx, fBy;
 #define CAP_FU_LOAD(X, PS)                                                               \
     do {                                                                                 \
         X = fu_token_mask(tblc, obuf + (size_t)(PS) * S * FU_KP);                        \
         if (!whole) {                                                                    \
             const int64_t tk = bt0 + (PS) * S + sub;                                     \
-            if (tk < cur || tk >= seg) X = make_uint4(0u, 0u, 0u, 0u);                   \
+            if (tk < cur || tk >= seg) X = make_uint2(0u, 0u);                           \
         }                                                                                \
     } while (0)
                     CAP_FU_LOAD(x0, 0); CAP_FU_LOAD(x1, 1); CAP_FU_LOAD(x2, 2); CAP_FU_LOAD(x3, 3);
                     CAP_FU_HALF(x, x0, x1, x2, x3, fAx); CAP_FU_HALF(y, x0, x1, x2, x3, fAy);
-                    CAP_FU_HALF(z, x0, x1, x2, x3, fAz); CAP_FU_HALF(w, x0, x1, x2, x3, fAw);
                     CAP_FU_LOAD(x0, 4); CAP_FU_LOAD(x1, 5); CAP_FU_LOAD(x2, 6); CAP_FU_LOAD(x3, 7);
                     CAP_FU_HALF(x, x0, x1, x2, x3, fBx); CAP_FU_HALF(y, x0, x1, x2, x3, fBy);
-                    CAP_FU_HALF(z, x0, x1, x2, x3, fBz); CAP_FU_HALF(w, x0, x1, x2, x3, fBw);
                     CAP_FU_TOP(x, fAx, fBx); CAP_FU_TOP(y, fAy, fBy);
-                    CAP_FU_TOP(z, fAz, fBz); CAP_FU_TOP(w, fAw, fBw);
 #undef CAP_FU_LOAD
                 }
                 cur = seg;
@@ -573,6 +569,7 @@ static bool fused_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, in
         for (; n >= 8; n -= 4)
             if (fused_smem_layout(E, f->EP, g.RS, g.R, S, n).total <= budget) break;
         if (n < 8) continue;
+        if (32 * (FU_S3W0 + (2 * g.R * S + 31) / 32) > FU_MAXTHREADS) continue;
         if (bestS == 0) { bestS = S; bestLog = lg; bestNst = n; }          // most sub-slots that fit at all
         if (n >= 12 && S >= 8) { bestS = S; bestLog = lg; bestNst = n; break; }   // double-buffered S1 warps
     }
@@ -580,7 +577,7 @@ static bool fused_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, in
     g.S = bestS;
     g.logS = bestLog;
     nst = bestNst;
-    f->ns3w = (g.R * g.S + 31) / 32;
+    f->ns3w = (2 * g.R * g.S + 31) / 32;
     f->nthreads = 32 * (FU_S3W0 + f->ns3w);
     if (f->nthreads > FU_MAXTHREADS) FG_FAIL("threads");
     f->nst = nst;
