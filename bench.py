@@ -43,6 +43,20 @@ def _peaks():
     return FALLBACK_HBM_GBS, "fallback"
 
 
+def _ncu_traffic(kernel, workload):
+    """dram bytes read + written per launch of `kernel` from the committed `ncu --set full` capture
+    (profiles/ncu_traffic.txt: lines `kernel workload bytes source`), or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.txt")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            t = line.split()
+            if len(t) >= 3 and not line.startswith("#") and t[0] == kernel and t[1] == workload:
+                return int(t[2])
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,"
@@ -375,7 +389,7 @@ def run_cap(args, cfg, W):
             "clocks": clocks,
             "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak,
                          "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                         "traffic": None, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
+                         "traffic": _ncu_traffic(dominant, args.config), "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
                          "kernel_ms": dom_avg, "kernel_ms_how": dom_how,
                          "algorithmic_bytes": ab.get(dominant),
                          "fused_call_ms": ms_fused,
