@@ -34,6 +34,8 @@ constexpr int FU_KP = 8;            // offsets per token (k <= 8, padded with th
 
 // Optional per-warp timeline (build with -DCAP_FU_TRACE; read back with cap_debug_fused_trace): clock64
 // stamps relative to the block's entry at role milestones, plus cycles spent waiting on each hand-over.
+// -DCAP_FU_NO_S1 / -DCAP_FU_NO_S3 compile the S1 selection / the S3 scoring out (outputs are then wrong):
+// the ablation builds behind the decomposition quoted in profiles/r1c_fused.md and DESIGN.md 6.3.
 #ifdef CAP_FU_TRACE
 __device__ unsigned long long g_fu_trace[160 * 24 * 8];
 #define FU_TR(ev, val)                                                                        \
@@ -315,8 +317,14 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 const float *row = reinterpret_cast<const float *>(ring + (size_t)st * TILE_BYTES +
                                                                    (size_t)(tok < t1 ? tl : 0) * E * 4);
                 float wv[4];
+#ifdef CAP_FU_NO_S1      // ablation build: no selection arithmetic (arbitrary distinct experts)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) sel[i] = (tl * 8 + i + j) & (E - 1);
+                wv[0] = wv[1] = wv[2] = wv[3] = row[h];
+#else
                 gate_select_pair<E>(row, h, tl & 7, k, sel);
                 gate_weights_softmax_pair(row, h, k, sel, q.scale, wv);
+#endif
                 if (valid) {
                     if (k == 8) {
                         *reinterpret_cast<int4 *>(gidx + tok * 8 + 4 * h) =
@@ -509,7 +517,11 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
                 }
                 const int64_t seg = min(bend, rend);
                 const bool whole = cur == bt0 && seg == bend;     // tokens past t1 carry the zero row
+#ifdef CAP_FU_NO_S3      // ablation build: no candidate scoring
+                if (false) {
+#else
                 if (active) {
+#endif
                     uint2 x0, x1, x2, x3;
                     uint32_t fAx, fAy, fBx, fBy;
 #define CAP_FU_LOAD(X, PS)                                                               \
