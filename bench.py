@@ -264,7 +264,7 @@ def run_cap(args, cfg, W):
     gate = cap.gate_cfg(E, **cfg.gate)
     pipe = cap.Pipeline(L, T, gate, D, cfg.N, P, dn, cost_inter=cfg.cost_inter,
                         bytes_per_token=cfg.bytes_per_token, tau=cfg.taus[-1], chosen=0, device=dev)
-    hpipe = cap.HostPipeline(pipe, has_bias=cfg.has_bias)
+    hpipe = cap.HostPipeline(pipe, has_bias=cfg.has_bias, depth=2)
 
     def dstep(i):                       # direct launches (per-kernel event timers can be armed)
         x, b, m = d_sets[i % n_sets]
@@ -348,13 +348,17 @@ def run_cap(args, cfg, W):
     ms_fused = ev4.elapsed_time(ev5) / args.steps
 
     # ---- end to end: pinned host inputs -> device -> step -> every output back to the host ----------
-    for i in range(2):
+    # (two staging sets: the upload of step i+1 and the read-back of step i-1 overlap the compute of step
+    # i; every step uploads its own inputs and reads back all of its own outputs inside the timed region)
+    for i in range(3):
         hstep(i)
+    hpipe.finish()
     barrier()
     ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev2.record()
     for i in range(args.steps):
         hstep(i)
+    hpipe.finish()
     ev3.record()
     barrier()
     ms_e2e = ev2.elapsed_time(ev3)

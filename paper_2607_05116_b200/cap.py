@@ -3,6 +3,7 @@ step of the path runs in the library's CUDA kernels.  torch is used for device m
 streams.  There is no CPU fallback: a missing library or a missing GPU raises.
 """
 import ctypes as C
+import types
 import os
 from types import SimpleNamespace
 
@@ -300,6 +301,8 @@ class Pipeline:
     def __init__(self, L, T, gate, D, N, P, dev_node, cost_inter=1, bytes_per_token=0, tau=0.1,
                  chosen=0, device="cuda"):
         self.L, self.T, self.P, self.D, self.tau, self.chosen = L, T, P, D, tau, chosen
+        self._ctor = dict(L=L, T=T, gate=gate, D=D, N=N, P=P, dev_node=dev_node, cost_inter=cost_inter,
+                          bytes_per_token=bytes_per_token, tau=tau, chosen=chosen, device=device)
         self.gate = gate
         E, k = gate.E, gate.k
         self.dev_node = dev_node
@@ -316,20 +319,28 @@ class Pipeline:
         self.ws_disp = workspace(CALL_DISPATCH_LAYOUT, 1, T, E, k, D, 0, device)
         self.pi = torch.empty((L, E), dtype=torch.int32, device=device)
 
+    def clone(self):
+        """A second pipeline with its own output buffers and workspaces (same configuration)."""
+        return Pipeline(**self._ctor)
+
     def step(self, logits, bias, token_src, expert_dev):
         L, T = self.L, self.T
         E, k = self.gate.E, self.gate.k
         trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)
-        self.pi.copy_(expert_dev[:, self.chosen, :])
+        if L == 1:
+            pi = expert_dev[:, self.chosen, :]          # already the [L][E] layout cap_prune wants: no copy
+        else:
+            self.pi.copy_(expert_dev[:, self.chosen, :])
+            pi = self.pi
         st = _stream()
         rc = lib().cap_prune(_ptr(self.fb.idx), _ptr(self.fb.w), _ptr(token_src, torch.int32), L, T, k, E,
-                             _ptr(self.pi), C.byref(self.topo), float(self.tau), _ptr(self.kept),
+                             _ptr(pi), C.byref(self.topo), float(self.tau), _ptr(self.kept),
                              C.byref(self.after_struct), _ptr(self.near), _ptr(self.ws_prune),
                              self.ws_prune.numel(), st)
         _check(rc, "cap_prune")
         for l in range(L):
             rc = lib().cap_dispatch_layout(_ptr(self.fb.idx[l]), _ptr(self.kept[l]), T, k, E,
-                                           _ptr(self.pi[l]), self.D, _ptr(self.sorted_pairs[l]),
+                                           _ptr(pi[l]), self.D, _ptr(self.sorted_pairs[l]),
                                            _ptr(self.pair_pos[l]), _ptr(self.offsets[l]),
                                            _ptr(self.ws_disp), self.ws_disp.numel(), st)
             _check(rc, "cap_dispatch_layout")
@@ -373,40 +384,103 @@ class Pipeline:
 
 class HostPipeline:
     """The same step driven from HOST buffers (the end-to-end call): pinned host inputs are copied
-    to the device, the step runs, every output is copied back to pinned host memory."""
+    to the device, the step runs, every output is copied back to pinned host memory.
 
-    def __init__(self, pipe: Pipeline, has_bias=False, has_src=False):
+    depth = 1: copy in, compute, copy out, one after the other on the current stream.
+    depth > 1: `depth` independent sets of staging buffers, device outputs and host outputs; the copies
+    run on two side streams, so the upload of step i+1 and the read-back of step i-1 overlap the
+    compute of step i (PCIe is full duplex).  Every step still uploads its own inputs and reads back
+    all of its own outputs; call finish() before looking at the returned host tensors."""
+
+    def __init__(self, pipe: Pipeline, has_bias=False, has_src=False, depth=1):
         self.pipe = pipe
+        self.depth = depth
         L, T, P = pipe.L, pipe.T, pipe.P
         E = pipe.gate.E
         dev = pipe.kept.device
-        self.d_logits = torch.empty((L, T, E), dtype=torch.float32, device=dev)
-        self.d_maps = torch.empty((L, P, E), dtype=torch.int32, device=dev)
-        self.d_bias = torch.empty((L, E), dtype=torch.float32, device=dev) if has_bias else None
-        self.d_src = torch.empty((L, T), dtype=torch.int32, device=dev) if has_src else None
-        self.h_out = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for t in pipe.result_tensors()]
+        self.sets = []
+        for i in range(depth):
+            st = types.SimpleNamespace()
+            st.pipe = pipe if i == 0 else pipe.clone()
+            st.d_logits = torch.empty((L, T, E), dtype=torch.float32, device=dev)
+            st.d_maps = torch.empty((L, P, E), dtype=torch.int32, device=dev)
+            st.d_bias = torch.empty((L, E), dtype=torch.float32, device=dev) if has_bias else None
+            st.d_src = torch.empty((L, T), dtype=torch.int32, device=dev) if has_src else None
+            st.h_out = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for t in st.pipe.result_tensors()]
+            st.graph = None
+            st.ev_in, st.ev_comp, st.ev_out = torch.cuda.Event(), torch.cuda.Event(), torch.cuda.Event()
+            st.used = False
+            self.sets.append(st)
+        self.h_out = self.sets[0].h_out
         self.d2h_bytes = sum(t.numel() * t.element_size() for t in self.h_out)
-        self.graph = None
+        self.s_h2d = torch.cuda.Stream(device=dev) if depth > 1 else None
+        self.s_d2h = torch.cuda.Stream(device=dev) if depth > 1 else None
+        self.n = 0
 
     def capture(self):
-        """Capture the device part of the step (on the staging buffers) into a CUDA graph."""
-        self.graph = self.pipe.capture(self.d_logits, self.d_bias, self.d_src, self.d_maps)
+        """Capture the device part of the step (on the staging buffers) into a CUDA graph per set."""
+        for st in self.sets:
+            st.graph = st.pipe.capture(st.d_logits, st.d_bias, st.d_src, st.d_maps)
+        self.graph = self.sets[0].graph
 
     def h2d_bytes(self, logits, maps, bias=None, src=None):
         return sum(t.numel() * t.element_size() for t in (logits, maps, bias, src) if t is not None)
 
-    def step(self, h_logits, h_maps, h_bias=None, h_src=None):
-        self.d_logits.copy_(h_logits, non_blocking=True)
-        self.d_maps.copy_(h_maps, non_blocking=True)
+    @staticmethod
+    def _upload(st, h_logits, h_maps, h_bias, h_src):
+        st.d_logits.copy_(h_logits, non_blocking=True)
+        st.d_maps.copy_(h_maps, non_blocking=True)
         if h_bias is not None:
-            self.d_bias.copy_(h_bias, non_blocking=True)
+            st.d_bias.copy_(h_bias, non_blocking=True)
         if h_src is not None:
-            self.d_src.copy_(h_src, non_blocking=True)
-        if self.graph is not None:
-            self.graph.replay()
+            st.d_src.copy_(h_src, non_blocking=True)
+
+    @staticmethod
+    def _compute(st, h_bias, h_src):
+        if st.graph is not None:
+            st.graph.replay()
         else:
-            self.pipe.step(self.d_logits, self.d_bias if h_bias is not None else None,
-                           self.d_src if h_src is not None else None, self.d_maps)
-        for h, d in zip(self.h_out, self.pipe.result_tensors()):
+            st.pipe.step(st.d_logits, st.d_bias if h_bias is not None else None,
+                         st.d_src if h_src is not None else None, st.d_maps)
+
+    @staticmethod
+    def _download(st):
+        for h, d in zip(st.h_out, st.pipe.result_tensors()):
             h.copy_(d, non_blocking=True)
-        return self.h_out
+
+    def step(self, h_logits, h_maps, h_bias=None, h_src=None):
+        st = self.sets[self.n % self.depth]
+        self.n += 1
+        if self.depth == 1:
+            self._upload(st, h_logits, h_maps, h_bias, h_src)
+            self._compute(st, h_bias, h_src)
+            self._download(st)
+            return st.h_out
+        cur = torch.cuda.current_stream()
+        if st.used:
+            self.s_h2d.wait_event(st.ev_comp)       # the compute that read these staging buffers
+        else:
+            self.s_h2d.wait_stream(cur)
+        with torch.cuda.stream(self.s_h2d):
+            self._upload(st, h_logits, h_maps, h_bias, h_src)
+            st.ev_in.record(self.s_h2d)
+        cur.wait_event(st.ev_in)
+        if st.used:
+            cur.wait_event(st.ev_out)               # the read-back of this set's previous outputs
+        self._compute(st, h_bias, h_src)
+        st.ev_comp.record(cur)
+        self.s_d2h.wait_event(st.ev_comp)
+        with torch.cuda.stream(self.s_d2h):
+            self._download(st)
+            st.ev_out.record(self.s_d2h)
+        st.used = True
+        return st.h_out
+
+    def finish(self):
+        """Make the current stream wait for every copy issued so far."""
+        if self.depth > 1:
+            cur = torch.cuda.current_stream()
+            cur.wait_stream(self.s_h2d)
+            cur.wait_stream(self.s_d2h)
+
+

@@ -27,12 +27,17 @@ size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D)
     return (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
 }
 
+// destination device of pair i, -1 if the pair is pruned, past the end, or carries an out-of-range expert
+// or device (memory-safe on garbage inputs: such pairs are left out of the layout)
 __device__ __forceinline__ int pair_key(const int32_t *idx, const uint8_t *kept, const int *s_map,
-                                        int64_t i, int64_t n)
+                                        int64_t i, int64_t n, int E, int D)
 {
     if (i >= n) return -1;
     if (kept && !kept[i]) return -1;
-    return s_map[idx[i]];
+    const int e = idx[i];
+    if ((unsigned)e >= (unsigned)E) return -1;
+    const int d = s_map[e];
+    return (unsigned)d < (unsigned)D ? d : -1;
 }
 
 // hist[d][sub] = kept pairs of sub-chunk `sub` going to device d (rows of `stride` entries, zero padded)
@@ -56,7 +61,7 @@ dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
     if (i0 < n) {
         int key[DS_SUB / 32];
 #pragma unroll
-        for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n);
+        for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n, E, D);
 #pragma unroll
         for (int r = 0; r < DS_SUB / 32; ++r) {
             const unsigned grp = __match_any_sync(0xffffffffu, key[r]);
@@ -135,7 +140,7 @@ dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restri
     if (i0 >= n) return;
     int key[DS_SUB / 32];
 #pragma unroll
-    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n);
+    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n, E, D);
 #pragma unroll
     for (int r = 0; r < DS_SUB / 32; ++r) {
         const int64_t i = i0 + r * 32 + lane;

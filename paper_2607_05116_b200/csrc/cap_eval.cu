@@ -68,20 +68,22 @@ __global__ void __launch_bounds__(256) eval_generic_kernel(EvalParams prm)
     const int32_t *maps = prm.expert_dev + ((int64_t)layer * prm.P) * E;
 
     // ---- stage maps (transposed), node masks, zero counters ------------------------------------
-    if (threadIdx.x < 64) {
-        unsigned long long m = 0ull;
-        if ((int)threadIdx.x < N)
-            for (int d = 0; d < D; ++d)
-                if (prm.dev_node[d] == (int)threadIdx.x) m |= 1ull << d;
-        nodemask[threadIdx.x] = m;
-        s_dn[threadIdx.x] = ((int)threadIdx.x < D) ? (unsigned char)prm.dev_node[threadIdx.x] : 0;
-    }
+    if (threadIdx.x < 64)
+        s_dn[threadIdx.x] = ((int)threadIdx.x < D) ? (unsigned char)(prm.dev_node[threadIdx.x] & 63) : 0;
     for (int i = threadIdx.x; i < E * PC; i += blockDim.x) {
         int pp = i / E, e = i - pp * E;          // coalesced read of map rows
         int v = (p0 + pp < prm.P) ? maps[(int64_t)(p0 + pp) * E + e] : 0;
-        mapT[(size_t)e * PC + pp] = (unsigned char)v;
+        mapT[(size_t)e * PC + pp] = (unsigned)v < (unsigned)D ? (unsigned char)v : (unsigned char)0;   // memory-safe on garbage
     }
     for (int i = threadIdx.x; i < D * PC; i += blockDim.x) recv_s[i] = 0;
+    __syncthreads();
+    if (threadIdx.x < 64) {
+        unsigned long long m = 0ull;              // devices of node threadIdx.x, from the shared copy
+        if ((int)threadIdx.x < N)
+            for (int d = 0; d < D; ++d)
+                if (s_dn[d] == (int)threadIdx.x) m |= 1ull << d;
+        nodemask[threadIdx.x] = m;
+    }
     __syncthreads();
 
     unsigned long long a_dev = 0, a_local = 0, a_same = 0, a_node = 0, a_rnode = 0;
@@ -94,11 +96,12 @@ __global__ void __launch_bounds__(256) eval_generic_kernel(EvalParams prm)
         __syncthreads();
         for (int i = threadIdx.x; i < nt * k; i += blockDim.x) {
             int tt = i / k, s = i - tt * k;
-            s_idx[tt * 16 + s] = idx[(tb + tt) * k + s];
+            const int e = idx[(tb + tt) * k + s];
+            s_idx[tt * 16 + s] = (unsigned)e < (unsigned)E ? e : 0;
             s_kept[tt * 16 + s] = kept ? kept[(tb + tt) * k + s] : 1;
         }
         for (int i = threadIdx.x; i < nt; i += blockDim.x)
-            s_src[i] = tsrc ? tsrc[tb + i] : (int)(((tb + i) * D) / T);
+            s_src[i] = tsrc ? (tsrc[tb + i] & 63) : (int)(((tb + i) * D) / T);   // & 63: memory-safe on garbage
         __syncthreads();
         if (valid_p) {
             for (int tt = 0; tt < nt; ++tt) {

@@ -248,3 +248,68 @@ def test_fused_kernel_serves_these_shapes(shape):
     cap.trace_fused(dev(logits), dev(bias), cap.gate_cfg(cfg.E, **cfg.gate), None, dev(cand), topo)
     torch.cuda.synchronize()
     assert cap.kernel_timer_ms(7) > 0.0
+
+
+def test_host_pipeline_double_buffered_matches_single():
+    """The end-to-end call with two staging sets (copies on side streams, as bench.py's e2e leg uses it)
+    returns, step by step, exactly what the plain device pipeline computes on the same inputs."""
+    cfg = W.CONFIGS["target"].with_(T=3001, P=24)
+    from parity_util import layers_inputs
+    dn_d = dev(W.dev_node(cfg))
+    gate = cap.gate_cfg(cfg.E, **cfg.gate)
+    mk = lambda: cap.Pipeline(cfg.L, cfg.T, gate, cfg.D, cfg.N, cfg.P, dn_d, cost_inter=cfg.cost_inter,
+                              bytes_per_token=cfg.bytes_per_token, tau=cfg.taus[-1], chosen=0, device="cuda")
+    ref, hp = mk(), cap.HostPipeline(mk(), depth=2)
+    hp.capture()
+    ins = []
+    for s in range(5):
+        logits, _, cand = layers_inputs(cfg, tuple(range(cfg.L)), cfg.T)
+        logits = np.roll(logits, s * 13, axis=1).copy()           # distinct inputs per step
+        ins.append((torch.from_numpy(logits).pin_memory(), torch.from_numpy(cand).pin_memory()))
+    outs = [hp.step(x, m) for x, m in ins[:2]]                     # two steps in flight
+    hp.finish()
+    torch.cuda.synchronize()
+    got = [[t.clone() for t in o] for o in outs]
+    for s in range(2, 5):                                          # reuse of both sets
+        o = hp.step(*ins[s])
+        hp.finish()
+        torch.cuda.synchronize()
+        got.append([t.clone() for t in o])
+    for s, (x, m) in enumerate(ins):
+        ref.step(x.cuda(), None, None, m.cuda())
+        torch.cuda.synchronize()
+        for a, b in zip(got[s], ref.result_tensors()):
+            if a.dtype == torch.float32:
+                assert torch.equal(a, b.cpu()), f"step {s}"
+            elif a.shape == ref.sorted_pairs.shape and a.dtype == torch.int32 and a is not None:
+                n = int(ref.offsets[0, -1])
+                assert torch.equal(a.reshape(-1)[:n], b.cpu().reshape(-1)[:n]) or torch.equal(a, b.cpu()), f"step {s}"
+            else:
+                assert torch.equal(a, b.cpu()), f"step {s}"
+
+
+@pytest.mark.parametrize("with_src", [False, True])
+def test_garbage_values_are_memory_safe(with_src):
+    """include/cap.h: out-of-range VALUES inside device arrays (expert_dev >= D or negative, token_src >= D,
+    non-finite logits) give undefined results but must stay memory-safe: the calls run to completion and
+    the next valid call is still bit-exact."""
+    cfg = W.CONFIGS["target"].with_(T=4099, P=40)
+    rng = np.random.default_rng(7)
+    L, T, E, k, P, D = cfg.L, cfg.T, cfg.E, cfg.k, cfg.P, cfg.D
+    x = rng.normal(0, 1, (L, T, E)).astype(np.float32)
+    x[0, ::7, 3] = np.nan
+    x[0, 1::11, 5] = np.inf
+    x[0, 2::13, :] = -np.inf
+    maps = rng.integers(-2 ** 31, 2 ** 31 - 1, (L, P, E), dtype=np.int64).astype(np.int32)
+    src = rng.integers(-2 ** 31, 2 ** 31 - 1, (L, T), dtype=np.int64).astype(np.int32) if with_src else None
+    dn_d = dev(W.dev_node(cfg))
+    topo = topo_of(cfg, dn_d)
+    gate = cap.gate_cfg(E, **cfg.gate)
+    fb = cap.trace_fused(dev(x), None, gate, dev(src), dev(maps), topo)
+    pi = dev(maps[:, 0, :].copy())
+    kept, near, aft = cap.prune(fb.idx, fb.w, dev(src), pi, topo, 0.1)
+    cap.dispatch_layout(fb.idx[0], kept[0], pi[0], D)
+    cap.dispatch_layout(fb.idx[0], None, pi[0], D)
+    cap.eval_placements(fb.idx, kept, dev(src), dev(maps), topo)
+    torch.cuda.synchronize()
+    check_all_stages(W.CONFIGS["tiny"], tag="after garbage ")
