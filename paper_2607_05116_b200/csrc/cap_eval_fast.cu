@@ -139,8 +139,11 @@ __global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
     const int layer = blockIdx.z, pc = blockIdx.y;
     const int rowq = q.RS * 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ unsigned char s_node[64];
     pdl_launch_dependents();
     pdl_wait();
+    if (threadIdx.x < 64) s_node[threadIdx.x] = (int)threadIdx.x < q.D ? (unsigned char)q.dev_node[threadIdx.x] : 0;
+    __syncthreads();
     {
         const unsigned long long nthr = (unsigned long long)gridDim.x * gridDim.y * gridDim.z * blockDim.x;
         const unsigned long long me = ((unsigned long long)(blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x) *
@@ -152,7 +155,7 @@ __global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
     if (i >= (q.E + 1) * rowq) return;
     const int e = i / rowq, w = i - e * rowq;
     uint32_t *t = const_cast<uint32_t *>(q.table) + ((size_t)layer * q.PC + pc) * (size_t)(q.E + 1) * rowq;
-    t[i] = ef_table_word(q.expert_dev + ((size_t)layer * q.P) * q.E, q.dev_node, q.E, q.P, q.D, pc * q.Pc,
+    t[i] = ef_table_word(q.expert_dev + ((size_t)layer * q.P) * q.E, s_node, q.E, q.P, q.D, pc * q.Pc,
                          q.WD, q.WN, q.DW, q.NW, e, w);
 }
 
@@ -414,7 +417,9 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
             const int s = s0 + j * 32 * DEC_WARPS;
             const uint32_t *pp = q.rec_planes + ((sbase + s) * (size_t)q.NPR) * q.W + w;
 #pragma unroll
-            for (int p = 0; p < EF_NPL; ++p) av[j][p] = (srcs[j] >= 0 && p < q.NPR) ? pp[(size_t)p * q.W] : 0u;
+            // not conditional on srcs[j]: the loads go out together with the header loads (unused slots hold
+            // stale planes, skipped below)
+            for (int p = 0; p < EF_NPL; ++p) av[j][p] = (s < q.nslots && p < q.NPR) ? pp[(size_t)p * q.W] : 0u;
         }
 #pragma unroll
         for (int j = 0; j < DEC_SL; ++j) {

@@ -108,41 +108,38 @@ __device__ __forceinline__ uint32_t ef_nodemask_word(int WN, int node)
 }
 
 // One word of the code table: row e (e == E is the all-zero row), word w of candidate chunk
-// [p0, p0 + Pc).  Words [0, DW) hold device codes, [DW, DW + NW) node codes.
+// [p0, p0 + Pc).  Words [0, DW) hold device codes, [DW, DW + NW) node codes.  node_of: node code of
+// every device (a shared-memory copy).  The map entries of a word (up to 16 candidates) are fetched
+// with independent loads first -- the [P][E] maps are read with a stride of E, one L2 round trip each.
 __device__ __forceinline__ uint32_t ef_table_word(const int32_t *__restrict__ maps /*[P][E]*/,
-                                                  const int32_t *__restrict__ dev_node, int E, int P,
+                                                  const unsigned char *node_of, int E, int P,
                                                   int D, int p0, int WD, int WN, int DW, int NW, int e,
                                                   int w)
 {
-    uint32_t word = 0u;
     if (e >= E || w >= DW + NW) return 0u;
-    if (w < DW) {
+    const bool devw = w < DW;
+    const int fpw = devw ? (WD == 64 ? 1 : 32 / WD) : 32 / WN;          // candidates in this word (<= 16)
+    const int pb = p0 + (devw ? (WD == 64 ? (w >> 1) : w * fpw) : (w - DW) * fpw);
+    int dv[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+        const int p = pb + j;
+        dv[j] = (j < fpw && p < P) ? maps[(size_t)p * E + e] : -1;
+    }
+    uint32_t word = 0u;
+    if (devw) {
         if (WD == 64) {
-            const int p = p0 + (w >> 1);
-            if (p < P) {
-                const int d = maps[(size_t)p * E + e];
-                if ((unsigned)d < (unsigned)D && (d >> 5) == (w & 1)) word = 1u << (d & 31);
-            }
+            const int d = dv[0];
+            if ((unsigned)d < (unsigned)D && (d >> 5) == (w & 1)) word = 1u << (d & 31);
         } else {
-            const int fpw = 32 / WD;
-            for (int j = 0; j < fpw; ++j) {
-                const int p = p0 + w * fpw + j;
-                if (p < P) {
-                    const int d = maps[(size_t)p * E + e];
-                    if ((unsigned)d < (unsigned)D) word |= 1u << (j * WD + d);
-                }
-            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if (j < fpw && (unsigned)dv[j] < (unsigned)D) word |= 1u << (j * WD + dv[j]);
         }
     } else {
-        const int fpw = 32 / WN;
-        const int wn = w - DW;
-        for (int j = 0; j < fpw; ++j) {
-            const int p = p0 + wn * fpw + j;
-            if (p < P) {
-                const int d = maps[(size_t)p * E + e];
-                if ((unsigned)d < (unsigned)D) word |= 1u << (j * WN + (dev_node[d] & (WN - 1)));
-            }
-        }
+#pragma unroll
+        for (int j = 0; j < 16; ++j)
+            if (j < fpw && (unsigned)dv[j] < (unsigned)D) word |= 1u << (j * WN + (node_of[dv[j]] & (WN - 1)));
     }
     return word;
 }
