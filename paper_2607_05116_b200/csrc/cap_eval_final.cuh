@@ -27,13 +27,18 @@ FinalParams make_final_params(int32_t L, int32_t E, int32_t P, const int32_t *ex
 __device__ __forceinline__ void eval_finalize_one(const FinalParams &f, int o, int lane, unsigned long long *lp)
 {
     const int layer = o / f.P;
-    lp[lane] = 0ull;
-    lp[lane + 32] = 0ull;
-    __syncwarp();
+    // every global load of this candidate goes out first (independent: one L2 round trip for all of them)
+    const long long r0 = lane < f.D ? (long long)__ldcg(f.recv + (size_t)o * f.D + lane) : 0ll;
+    const long long r1 = lane + 32 < f.D ? (long long)__ldcg(f.recv + (size_t)o * f.D + lane + 32) : 0ll;
+    const unsigned long long *a = f.acc + (size_t)o * ACC_N;
+    const unsigned long long av = lane < ACC_N ? __ldcg(a + lane) : 0ull;
     if (f.load_direct) {
         lp[lane] = __ldcg(f.load_direct + (size_t)o * 64 + lane);
         lp[lane + 32] = __ldcg(f.load_direct + (size_t)o * 64 + lane + 32);
     } else {
+        lp[lane] = 0ull;
+        lp[lane + 32] = 0ull;
+        __syncwarp();
         // load_pairs[d] = sum of the (kept) counts of the experts placed on d
         const int32_t *pi = f.expert_dev + (size_t)o * f.E;
         const long long *cnt = f.counts + (size_t)layer * f.E;
@@ -47,7 +52,7 @@ __device__ __forceinline__ void eval_finalize_one(const FinalParams &f, int o, i
     long long mx = 0, sm = 0, mxr = 0, smr = 0;
     for (int d = lane; d < f.D; d += 32) {
         const long long l = (long long)lp[d];
-        const long long r = (long long)__ldcg(f.recv + (size_t)o * f.D + d);
+        const long long r = d < 32 ? r0 : r1;
         if (f.out.load_pairs) f.out.load_pairs[(size_t)o * f.D + d] = l;
         if (f.out.recv_tokens) f.out.recv_tokens[(size_t)o * f.D + d] = r;
         mx = max(mx, l);
@@ -62,18 +67,19 @@ __device__ __forceinline__ void eval_finalize_one(const FinalParams &f, int o, i
         sm += __shfl_xor_sync(0xffffffffu, sm, off);
         smr += __shfl_xor_sync(0xffffffffu, smr, off);
     }
+    const long long dv = (long long)__shfl_sync(0xffffffffu, av, ACC_DEV), loc = (long long)__shfl_sync(0xffffffffu, av, ACC_LOCAL),
+                    same = (long long)__shfl_sync(0xffffffffu, av, ACC_SAMENODE);
+    const long long a_node = (long long)__shfl_sync(0xffffffffu, av, ACC_NODE), a_rnode = (long long)__shfl_sync(0xffffffffu, av, ACC_RNODE),
+                    a_near = (long long)__shfl_sync(0xffffffffu, av, ACC_NEAR);
     if (lane != 0) return;
-    const unsigned long long *a = f.acc + (size_t)o * ACC_N;
-    const long long dv = (long long)__ldcg(a + ACC_DEV), loc = (long long)__ldcg(a + ACC_LOCAL),
-                    same = (long long)__ldcg(a + ACC_SAMENODE);
     const long long rdev = dv - loc, intra = same - loc, inter = dv - same;
-    if (f.near_out) f.near_out[o] = (long long)__ldcg(a + ACC_NEAR);
+    if (f.near_out) f.near_out[o] = a_near;
     if (f.out.dev_visits) f.out.dev_visits[o] = dv;
     if (f.out.remote_dev) f.out.remote_dev[o] = rdev;
     if (f.out.remote_intra) f.out.remote_intra[o] = intra;
     if (f.out.remote_inter) f.out.remote_inter[o] = inter;
-    if (f.out.node_visits) f.out.node_visits[o] = (long long)__ldcg(a + ACC_NODE);
-    if (f.out.remote_node) f.out.remote_node[o] = (long long)__ldcg(a + ACC_RNODE);
+    if (f.out.node_visits) f.out.node_visits[o] = a_node;
+    if (f.out.remote_node) f.out.remote_node[o] = a_rnode;
     if (f.out.cost)
         f.out.cost[o] = (long long)f.cost_local * loc + (long long)f.cost_intra * intra +
                         (long long)f.cost_inter * inter;
