@@ -27,14 +27,19 @@ size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D)
     return (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
 }
 
-// destination device of pair i, -1 if the pair is pruned, past the end, or carries an out-of-range expert
-// or device (memory-safe on garbage inputs: such pairs are left out of the layout)
-__device__ __forceinline__ int pair_key(const int32_t *idx, const uint8_t *kept, const int *s_map,
-                                        int64_t i, int64_t n, int E, int D)
+// expert of pair i, -1 if the pair is pruned or past the end (both loads are issued unconditionally and
+// before the placement map is staged: one memory round trip instead of three)
+__device__ __forceinline__ int pair_expert(const int32_t *idx, const uint8_t *kept, int64_t i, int64_t n)
 {
     if (i >= n) return -1;
-    if (kept && !kept[i]) return -1;
     const int e = idx[i];
+    const int kp = kept ? (int)kept[i] : 1;
+    return kp ? e : -1;
+}
+// destination device of an expert, -1 for "no pair" or an out-of-range expert or device (memory-safe on
+// garbage inputs: such pairs are left out of the layout)
+__device__ __forceinline__ int expert_key(int e, const int *s_map, int E, int D)
+{
     if ((unsigned)e >= (unsigned)E) return -1;
     const int d = s_map[e];
     return (unsigned)d < (unsigned)D ? d : -1;
@@ -52,16 +57,18 @@ dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
     int *cnt = sm + E + warp * DS_MAXD;            // [D] private to the warp
     pdl_launch_dependents();
     pdl_wait();
+    const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
+    const int64_t i0 = sub * DS_SUB;
+    int key[DS_SUB / 32];
+#pragma unroll
+    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_expert(idx, kept, i0 + r * 32 + lane, n);
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
     for (int d = lane; d < D; d += 32) cnt[d] = 0;
     __syncthreads();
-    const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
     if (sub >= stride) return;
-    const int64_t i0 = sub * DS_SUB;
     if (i0 < n) {
-        int key[DS_SUB / 32];
 #pragma unroll
-        for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n, E, D);
+        for (int r = 0; r < DS_SUB / 32; ++r) key[r] = expert_key(key[r], s_map, E, D);
 #pragma unroll
         for (int r = 0; r < DS_SUB / 32; ++r) {
             const unsigned grp = __match_any_sync(0xffffffffu, key[r]);
@@ -73,7 +80,7 @@ dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
 }
 
 // One block, warp w scans devices w, w + nwarps, ... in coalesced chunks of 128 sub-chunks (one int4
-// per lane), four chunks in flight: the loop is bound by L2 latency, not by arithmetic.
+// per lane), eight chunks in flight: the loop is bound by L2 latency, not by arithmetic.
 __global__ void __launch_bounds__(1024)
 dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, long long *__restrict__ offsets,
                      int D, int64_t stride)
@@ -87,12 +94,12 @@ dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, long 
         const int4 *h = reinterpret_cast<const int4 *>(hist + (int64_t)d * stride) + lane;
         int4 *bs = reinterpret_cast<int4 *>(base + (int64_t)d * stride) + lane;
         int run = 0;                               // pairs of device d before the current chunk
-        for (int64_t c0 = 0; c0 < nch; c0 += 4) {
-            int4 v[4];
+        for (int64_t c0 = 0; c0 < nch; c0 += 8) {
+            int4 v[8];
 #pragma unroll
-            for (int j = 0; j < 4; ++j) v[j] = c0 + j < nch ? h[(c0 + j) * 32] : make_int4(0, 0, 0, 0);
+            for (int j = 0; j < 8; ++j) v[j] = c0 + j < nch ? h[(c0 + j) * 32] : make_int4(0, 0, 0, 0);
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
+            for (int j = 0; j < 8; ++j) {
                 const int sum = (v[j].x + v[j].y) + (v[j].z + v[j].w);
                 int inc = sum;
 #pragma unroll
@@ -132,15 +139,17 @@ dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restri
     const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
     pdl_launch_dependents();
     pdl_wait();
-    for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
     const int64_t i0 = sub * DS_SUB;
+    int key[DS_SUB / 32];
+#pragma unroll
+    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_expert(idx, kept, i0 + r * 32 + lane, n);
+    for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
     if (i0 < n)
         for (int d = lane; d < D; d += 32) running[d] = (int)offsets[d] + base[(int64_t)d * stride + sub];
     __syncthreads();
     if (i0 >= n) return;
-    int key[DS_SUB / 32];
 #pragma unroll
-    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_key(idx, kept, s_map, i0 + r * 32 + lane, n, E, D);
+    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = expert_key(key[r], s_map, E, D);
 #pragma unroll
     for (int r = 0; r < DS_SUB / 32; ++r) {
         const int64_t i = i0 + r * 32 + lane;

@@ -56,6 +56,17 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
     const bool want_eval = prm.acc != nullptr;
     pdl_launch_dependents();
     pdl_wait();
+    // this thread's token (vector path): in flight while the maps are staged
+    const int64_t tq = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int4 q_i0 = make_int4(0, 0, 0, 0), q_i1 = q_i0;
+    float4 q_w0 = make_float4(0.f, 0.f, 0.f, 0.f), q_w1 = q_w0;
+    if (KMAX == 8 && prm.vec && tq < prm.T) {
+        const int64_t qb = ((int64_t)layer * prm.T + tq) * k;
+        q_i0 = __ldg(reinterpret_cast<const int4 *>(prm.idx + qb));
+        q_i1 = __ldg(reinterpret_cast<const int4 *>(prm.idx + qb) + 1);
+        q_w0 = __ldg(reinterpret_cast<const float4 *>(prm.w + qb));
+        q_w1 = __ldg(reinterpret_cast<const float4 *>(prm.w + qb) + 1);
+    }
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = prm.expert_dev[(size_t)layer * E + i];
     if (threadIdx.x < 64) {
         s_dn[threadIdx.x] = (int)threadIdx.x < D ? prm.dev_node[threadIdx.x] : 0;
@@ -86,10 +97,8 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
         int e[KMAX], d[KMAX];
         float wv[KMAX];
         if (KMAX == 8 && prm.vec) {
-            const int4 i0 = __ldg(reinterpret_cast<const int4 *>(prm.idx + base));
-            const int4 i1 = __ldg(reinterpret_cast<const int4 *>(prm.idx + base) + 1);
-            const float4 w0 = __ldg(reinterpret_cast<const float4 *>(prm.w + base));
-            const float4 w1 = __ldg(reinterpret_cast<const float4 *>(prm.w + base) + 1);
+            const int4 i0 = q_i0, i1 = q_i1;
+            const float4 w0 = q_w0, w1 = q_w1;
             e[0] = i0.x; e[1] = i0.y; e[2] = i0.z; e[3] = i0.w;
             e[4 % KMAX] = i1.x; e[5 % KMAX] = i1.y; e[6 % KMAX] = i1.z; e[7 % KMAX] = i1.w;
             wv[0] = w0.x; wv[1] = w0.y; wv[2] = w0.z; wv[3] = w0.w;
