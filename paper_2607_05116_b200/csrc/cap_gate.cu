@@ -88,6 +88,31 @@ __global__ void __launch_bounds__(256) gate_topk_kernel(GateParams prm)
         if (prm.n_group > 1) {
             const int gsz = E / prm.n_group;
             uint32_t gk = 0u;       // lane g holds the key of group g's score
+            // Segmented path: with 4 consecutive experts per register block and group sizes that divide 128,
+            // a register block lies inside one group and a group occupies gsz / 4 consecutive lanes of one
+            // block: top-2 per block in registers, then a butterfly inside the lane segment (all groups at
+            // once) instead of one warp-wide reduction per group.
+            const int seg = gsz >> 2;
+            const bool segmented = CW == 4 && (gsz & 3) == 0 && gsz <= 128 && (128 % gsz) == 0;
+            if (segmented) {
+                if constexpr (CW == 4) {
+                    const int gb = (lane * gsz) >> 7, gl = ((lane * gsz) & 127) >> 2;   // block / first lane of group `lane`
+#pragma unroll
+                    for (int c = 0; c < VPL / 4; ++c) {
+                        const uint32_t a = key[4 * c], b = key[4 * c + 1], cc = key[4 * c + 2], d = key[4 * c + 3];
+                        const uint32_t h1 = max(a, b), l1 = min(a, b), h2 = max(cc, d), l2 = min(cc, d);
+                        uint32_t m1 = max(h1, h2), m2 = max(min(h1, h2), max(l1, l2));   // two largest elements
+                        for (int o = 1; o < seg; o <<= 1) {
+                            const uint32_t o1 = __shfl_xor_sync(FULL, m1, o), o2 = __shfl_xor_sync(FULL, m2, o);
+                            m2 = max(min(m1, o1), max(m2, o2));
+                            m1 = max(m1, o1);
+                        }
+                        const uint32_t score = prm.group_score == 1 ? okey(__fadd_rn(unkey(m1), unkey(m2))) : m1;
+                        const uint32_t v = __shfl_sync(FULL, score, gl & 31);
+                        if (lane < prm.n_group && gb == c) gk = v;
+                    }
+                }
+            } else
             for (int g = 0; g < prm.n_group; ++g) {
                 const int lo = g * gsz, hi = lo + gsz;
                 uint32_t lm = 0u;
