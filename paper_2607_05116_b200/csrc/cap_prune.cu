@@ -34,7 +34,7 @@ struct PruneParams {
     unsigned long long *ldirect;  // [L][64] kept pairs per device
     uint8_t *tok_rdev, *tok_rnode;   // [L][T] or NULL
     int64_t T;
-    int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec;
+    int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec, small;
     float p;
 };
 
@@ -116,13 +116,17 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             d[s] = s < k ? (s_map[ee] & 63) : -1 - s;      // absent slots: distinct negative ids
             e[s] = ee;
         }
+        // source device of the token (reading A5): explicit, or contiguous blocks floor(t D / T); the 32-bit
+        // quotient is exact whenever T D < 2^32 (one short division instead of a 64-bit one)
+        const int tok_src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63)
+                            : prm.small ? (int)(((unsigned)t * (unsigned)D) / (unsigned)T) : (int)((t * D) / T);
         unsigned long long keepmask = 0ull;
         if (prm.p <= 0.0f) {
 #pragma unroll
             for (int s = 0; s < KMAX; ++s)
                 if (s < k) keepmask |= 1ull << d[s];
         } else {
-            const int src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63) : (int)((t * D) / T);
+            const int src = tok_src;
             const int srcn = s_dn[src];
             // 1. per-device weight at the device's first slot, added in slot order
             bool rep[KMAX];
@@ -135,11 +139,10 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
 #pragma unroll
             for (int s = 1; s < KMAX; ++s) {
 #pragma unroll
-                for (int j = 0; j < s; ++j) {
-                    if (s < k && rep[j] && d[j] == d[s]) {
-                        a[j] = __fadd_rn(a[j], wv[s]);
-                        rep[s] = false;
-                    }
+                for (int j = 0; j < s; ++j) {          // selects, not branches: the warp's tokens diverge everywhere
+                    const bool hit = (s < k) & rep[j] & (d[j] == d[s]);
+                    a[j] = hit ? __fadd_rn(a[j], wv[s]) : a[j];
+                    rep[s] = rep[s] & !hit;
                 }
             }
             // 2. cost ratio of every represented device
@@ -159,7 +162,7 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
                 int r = 0;
 #pragma unroll
                 for (int j = 0; j < KMAX; ++j)
-                    if (j != s && rep[j] && (ratio[j] > ratio[s] || (ratio[j] == ratio[s] && d[j] < d[s]))) ++r;
+                    if (j != s) r += (int)(rep[j] & ((ratio[j] > ratio[s]) | ((ratio[j] == ratio[s]) & (d[j] < d[s]))));
                 rank[s] = r;
             }
             // 4. greedy in rank order
@@ -168,22 +171,24 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             bool stopped = false;
 #pragma unroll
             for (int r = 0; r < KMAX; ++r) {
-                if (r < m && !stopped) {
-                    float Ar = 0.0f, Rr = 0.0f;
-                    int dr = 0;
+                float Ar = 0.0f, Rr = 0.0f;
+                int dr = 0;
 #pragma unroll
-                    for (int s = 0; s < KMAX; ++s)
-                        if (rep[s] && rank[s] == r) { Ar = a[s]; Rr = ratio[s]; dr = d[s]; }
-                    if (fabsf(__fsub_rn(cum, target)) < 1e-6f) near = 1;
-                    if (cum >= target) {
-                        stopped = true;
-                        r_cut = Rr;
-                    } else {
-                        keepmask |= 1ull << dr;
-                        cum = __fadd_rn(cum, Ar);
-                        r_last = Rr;
-                    }
+                for (int s = 0; s < KMAX; ++s) {
+                    const bool sel = rep[s] & (rank[s] == r);
+                    Ar = sel ? a[s] : Ar;
+                    Rr = sel ? ratio[s] : Rr;
+                    dr = sel ? d[s] : dr;
                 }
+                const bool act = (r < m) & !stopped;
+                const bool reached = cum >= target;
+                near |= (int)(act & (fabsf(__fsub_rn(cum, target)) < 1e-6f));
+                const bool stop_now = act & reached, keep_now = act & !reached;
+                r_cut = stop_now ? Rr : r_cut;
+                keepmask |= keep_now ? (1ull << dr) : 0ull;
+                cum = keep_now ? __fadd_rn(cum, Ar) : cum;
+                r_last = keep_now ? Rr : r_last;
+                stopped = stopped | stop_now;
             }
             if (stopped && r_last != CUDART_INF_F && r_cut != CUDART_INF_F && __fsub_rn(r_last, r_cut) < 1e-6f)
                 near = 1;
@@ -204,7 +209,7 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
         }
         // evaluation of the kept trace under this placement (P = 1)
         if (want_eval) {
-            const int src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63) : (int)((t * D) / T);
+            const int src = tok_src;
             const int srcn = s_dn[src];
             unsigned long long nodebits = 0ull;
 #pragma unroll
@@ -331,6 +336,7 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
         prm.cost_intra = topo.cost_intra;
         prm.cost_inter = topo.cost_inter;
         prm.p = p;
+        prm.small = (unsigned long long)T * (unsigned long long)topo.D < (1ull << 32);
         prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
                   (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
         dim3 grid((unsigned)((T + PR_THREADS - 1) / PR_THREADS), (unsigned)L);
