@@ -158,12 +158,15 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             // 3. rank: devices with a larger ratio, or an equal ratio and a lower id, come first
             int rank[KMAX];
 #pragma unroll
-            for (int s = 0; s < KMAX; ++s) {
-                int r = 0;
+            for (int s = 0; s < KMAX; ++s) rank[s] = 0;
 #pragma unroll
-                for (int j = 0; j < KMAX; ++j)
-                    if (j != s) r += (int)(rep[j] & ((ratio[j] > ratio[s]) | ((ratio[j] == ratio[s]) & (d[j] < d[s]))));
-                rank[s] = r;
+            for (int s = 1; s < KMAX; ++s) {
+#pragma unroll
+                for (int j = 0; j < s; ++j) {          // each pair once: exactly one of two represented devices comes first
+                    const bool jfirst = (ratio[j] > ratio[s]) | ((ratio[j] == ratio[s]) & (d[j] < d[s]));
+                    rank[s] += (int)(rep[j] & jfirst);
+                    rank[j] += (int)(rep[s] & !jfirst);
+                }
             }
             // 4. greedy in rank order
             const float target = __fsub_rn(1.0f, prm.p);
