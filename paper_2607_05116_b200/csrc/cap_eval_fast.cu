@@ -77,7 +77,7 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     if (g->maxrec < 1) g->maxrec = 1;
     g->NPR = EF_BT + g->logS;
     g->rec_slots = (size_t)L * g->PC * g->ncta_t * g->maxrec;
-    g->rec_words = g->rec_slots * g->NPR * g->W;
+    g->rec_words = g->rec_slots * (size_t)EF_RECW * g->W;
     g->table_words = (size_t)L * g->PC * (E + 1) * g->RS * 4;
     return true;
 }
@@ -317,10 +317,20 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
             __syncthreads();
         }
         if (active && sub == 0) {
-            uint4 *rp = reinterpret_cast<uint4 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
+            uint32_t *rp = q.rec_planes + ((slot0 + nrec) * (size_t)(R * 4) + (size_t)col * 4) * EF_RECW;
+            uint32_t v[EF_RECW];
 #pragma unroll
-            for (int p = 0; p < EF_NPL; ++p)
-                if (p < q.NPR) rp[(size_t)p * R + col] = pl[p];
+            for (int p = 0; p < EF_RECW; ++p) v[p] = (p < EF_NPL && p < q.NPR) ? pl[p < EF_NPL ? p : 0].x : 0u;
+            ef_store_word_planes(rp, v);
+#pragma unroll
+            for (int p = 0; p < EF_RECW; ++p) v[p] = (p < EF_NPL && p < q.NPR) ? pl[p < EF_NPL ? p : 0].y : 0u;
+            ef_store_word_planes(rp + EF_RECW, v);
+#pragma unroll
+            for (int p = 0; p < EF_RECW; ++p) v[p] = (p < EF_NPL && p < q.NPR) ? pl[p < EF_NPL ? p : 0].z : 0u;
+            ef_store_word_planes(rp + 2 * EF_RECW, v);
+#pragma unroll
+            for (int p = 0; p < EF_RECW; ++p) v[p] = (p < EF_NPL && p < q.NPR) ? pl[p < EF_NPL ? p : 0].w : 0u;
+            ef_store_word_planes(rp + 3 * EF_RECW, v);
         }
         if (tid == 0) q.rec_src[slot0 + nrec] = src;
         ++nrec;
@@ -415,11 +425,20 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
 #pragma unroll
         for (int j = 0; j < DEC_SL; ++j) {
             const int s = s0 + j * 32 * DEC_WARPS;
-            const uint32_t *pp = q.rec_planes + ((sbase + s) * (size_t)q.NPR) * q.W + w;
+            // one 64-byte run per (slot, word); not conditional on srcs[j]: the loads go out together with the
+            // header loads (unused slots hold stale planes, skipped below)
+            const uint4 *pp = reinterpret_cast<const uint4 *>(q.rec_planes + ((sbase + s) * (size_t)q.W + w) * EF_RECW);
+            uint32_t t16[EF_RECW];
 #pragma unroll
-            // not conditional on srcs[j]: the loads go out together with the header loads (unused slots hold
-            // stale planes, skipped below)
-            for (int p = 0; p < EF_NPL; ++p) av[j][p] = (s < q.nslots && p < q.NPR) ? pp[(size_t)p * q.W] : 0u;
+            for (int i = 0; i < EF_RECW / 4; ++i) {
+                const uint4 x = s < q.nslots ? pp[i] : make_uint4(0u, 0u, 0u, 0u);
+                t16[4 * i] = x.x;
+                t16[4 * i + 1] = x.y;
+                t16[4 * i + 2] = x.z;
+                t16[4 * i + 3] = x.w;
+            }
+#pragma unroll
+            for (int p = 0; p < EF_NPL; ++p) av[j][p] = t16[p];
         }
 #pragma unroll
         for (int j = 0; j < DEC_SL; ++j) {

@@ -18,6 +18,7 @@ namespace cap {
 
 constexpr int EF_BT = 8;        // planes a thread accumulates between flushes (counts < 256)
 constexpr int EF_NPL = 14;      // planes after the sub-slot tree (S <= 64)
+constexpr int EF_RECW = 16;     // record layout [word][EF_RECW planes]: a word's planes are one 64-byte run
 constexpr int EF_PASSES = 8;    // tokens per thread per block of the CSA tree
 constexpr int EF_MAXBLK = 31;   // blocks per run: 248 inputs per thread < 2^EF_BT
 constexpr int EF_PRE = 16;      // prefetched index entries per thread
@@ -49,7 +50,7 @@ size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D,
 
 struct EvalFastWs {
     int32_t *rec_src;       // [L][PC][ncta_t][maxrec], -1 = unused
-    uint32_t *rec_planes;   // [L][PC][ncta_t][maxrec][NPR][W]
+    uint32_t *rec_planes;   // [L][PC][ncta_t][maxrec][W][EF_RECW] (word-major: the decode reads 64-byte runs)
     uint32_t *table;        // [L][PC][E + 1][RS * 4] one-hot code table
 };
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
@@ -92,6 +93,14 @@ __device__ __forceinline__ uint32_t lop_or3(uint32_t a, uint32_t b, uint32_t c)
         (c) = lop_maj(_a, _b, _x);            \
         (s) = lop_xor3(_a, _b, _x);           \
     } while (0)
+
+// planes of one record word (EF_NPL values, the rest of the EF_RECW-word run zero) as four 16-byte stores
+__device__ __forceinline__ void ef_store_word_planes(uint32_t *dst, const uint32_t (&v)[EF_RECW])
+{
+    uint4 *d4 = reinterpret_cast<uint4 *>(dst);
+#pragma unroll
+    for (int i = 0; i < EF_RECW / 4; ++i) d4[i] = make_uint4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+}
 
 // Word mask of the bit positions of record word w whose device belongs to `set` (bit d = device d).
 __device__ __forceinline__ uint32_t ef_devmask_word(int WD, int w, unsigned long long set)

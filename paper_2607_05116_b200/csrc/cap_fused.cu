@@ -61,7 +61,7 @@ struct FusedParams {
     int *coact;                   // [L][E][E], zeroed
     const uint32_t *table;        // [L][E + 1][RS * 4]
     int32_t *rec_src;             // [L][ncta_t][maxrec]
-    uint32_t *rec_planes;         // [L][ncta_t][maxrec][NPR][W]
+    uint32_t *rec_planes;         // [L][ncta_t][maxrec][W][EF_RECW]
     int64_t T;
     int64_t tiles_per_cta;        // real 16-token tiles per block (uniform split)
     int32_t cps;                  // > 0: blocks per source device, block ranges aligned to the source runs
@@ -485,10 +485,15 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
             }
             FU_TR(6, FU_NOW());
             if (active && sub == 0) {
-                uint2 *rp = reinterpret_cast<uint2 *>(q.rec_planes + (slot0 + nrec) * (size_t)q.NPR * (R * 4));
+                // word-major record: the planes of a word are one 64-byte run (what the decode kernel reads)
+                uint32_t *rp = q.rec_planes + ((slot0 + nrec) * (size_t)(R * 4) + (size_t)col * 2) * EF_RECW;
+                uint32_t v[EF_RECW];
 #pragma unroll
-                for (int p = 0; p < EF_NPL; ++p)
-                    if (p < q.NPR) rp[(size_t)p * R2 + col] = pl[p];
+                for (int p = 0; p < EF_RECW; ++p) v[p] = (p < EF_NPL && p < q.NPR) ? pl[p < EF_NPL ? p : 0].x : 0u;
+                ef_store_word_planes(rp, v);
+#pragma unroll
+                for (int p = 0; p < EF_RECW; ++p) v[p] = (p < EF_NPL && p < q.NPR) ? pl[p < EF_NPL ? p : 0].y : 0u;
+                ef_store_word_planes(rp + EF_RECW, v);
             }
             if (t3 == 0) q.rec_src[slot0 + nrec] = src;
             ++nrec;
@@ -622,7 +627,7 @@ static bool fused_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, in
     }
     g.NPR = EF_BT + g.logS;
     g.rec_slots = (size_t)L * g.ncta_t * g.maxrec;
-    g.rec_words = g.rec_slots * g.NPR * g.W;
+    g.rec_words = g.rec_slots * (size_t)EF_RECW * g.W;
     g.table_words = (size_t)L * (E + 1) * g.RS * 4;
     return true;
 }
