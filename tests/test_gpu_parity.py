@@ -1,6 +1,7 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
 the same seeded inputs.  Integers bit-exact, gate weights within 1e-6 absolute."""
 import numpy as np
+from types import SimpleNamespace
 import pytest
 import torch
 
@@ -313,3 +314,96 @@ def test_garbage_values_are_memory_safe(with_src):
     cap.eval_placements(fb.idx, kept, dev(src), dev(maps), topo)
     torch.cuda.synchronize()
     check_all_stages(W.CONFIGS["tiny"], tag="after garbage ")
+
+
+def test_config5_maximum_size_sampled_and_invariants():
+    """Config 5 at the top of its T sweep (2^22 tokens, E=512, top-10, 64 devices over 8 nodes): 8.6 GB of
+    logits, 41.9 M (token, slot) pairs.  The oracle cannot run the whole trace, so: sampled tokens are
+    checked element by element against it (S1 indices / weights, S3 per-token remote devices / nodes, S4
+    kept masks), and the aggregates through properties that hold at any size (BASELINE.json invariants:
+    sum of counts = T k, C symmetric with diag = counts and off-diagonal row sums = (k-1) counts; S3 totals
+    equal the sums of the per-token outputs; S5 is a stable permutation of the kept pairs grouped by
+    device).  Inputs are generated on the GPU (torch, seeded): same distribution family as the stress
+    config (N(0,1) + Zipf-like bias), sized so the host generator is not the bottleneck."""
+    cfg = W.CONFIGS["stress"]
+    L, T, E, k, D, N = 1, 1 << 22, cfg.E, cfg.k, cfg.D, cfg.N
+    g = torch.Generator(device="cuda").manual_seed(20260705)
+    x = torch.randn((L, T, E), device="cuda", generator=g, dtype=torch.float32)
+    x += (0.25 * torch.log1p(torch.arange(E, device="cuda", dtype=torch.float32)).flip(0))[None, None, :]
+    gate = cap.gate_cfg(E, **cfg.gate)
+    dn = W.dev_node(cfg)
+    dn_d = dev(dn)
+    topo = topo_of(cfg, dn_d)
+    rng = np.random.default_rng(5)
+    sample = np.unique(np.concatenate([np.arange(0, 48), np.arange(T - 48, T),
+                                       rng.integers(0, T, 4000)])).astype(np.int64)
+    samp_d = torch.from_numpy(sample).cuda()
+
+    # S1 on everything, oracle on the sample
+    idx_d, w_d = cap.gate_topk(x, None, gate)
+    xs = x[0, samp_d].cpu().numpy()[None]
+    idx_r, w_r = O.gate_topk(xs, None, **cfg.gate)
+    assert np.array_equal(idx_d[0, samp_d].cpu().numpy()[None], idx_r)
+    assert float(np.abs(w_d[0, samp_d].cpu().numpy()[None].astype(np.float64) - w_r).max()) <= 1e-6
+    del x
+    torch.cuda.empty_cache()
+
+    # S2: invariants + an independent count
+    cnt_d, C_d = cap.coactivation(idx_d, None, E)
+    cnt_t = torch.bincount(idx_d.reshape(-1).long(), minlength=E)
+    assert torch.equal(cnt_d[0], cnt_t) and int(cnt_d.sum()) == T * k
+    Cl = C_d[0].long()
+    assert torch.equal(Cl, Cl.t()) and torch.equal(torch.diagonal(Cl), cnt_d[0])
+    assert torch.equal(Cl.sum(1) - torch.diagonal(Cl), (k - 1) * cnt_d[0])
+
+    # S3: P = 48 candidates with per-token outputs; sampled tokens against the oracle, totals against the sums
+    P = 48
+    cand = W.candidates(cfg, 0, P)[None]
+    cand_d = dev(cand)
+    ev = cap.eval_placements(idx_d, None, None, cand_d, topo, counts=cnt_d, per_token=True)
+    src_s = ((sample * D) // T).astype(np.int32)[None]
+    ev_r = O.eval_placements(idx_r, cand, dn, token_src=src_s, cost_inter=cfg.cost_inter,
+                             bytes_per_token=cfg.bytes_per_token, per_token=True)
+    assert np.array_equal(ev.tok_remote_dev[0][:, samp_d].cpu().numpy(), ev_r.tok_remote_dev[0])
+    assert np.array_equal(ev.tok_remote_node[0][:, samp_d].cpu().numpy(), ev_r.tok_remote_node[0])
+    assert torch.equal(ev.remote_dev[0], ev.tok_remote_dev[0].long().sum(1))
+    assert torch.equal(ev.remote_node[0], ev.tok_remote_node[0].long().sum(1))
+    assert torch.equal(ev.dev_visits[0], ev.recv_tokens[0].sum(1))
+    assert bool((ev.load_pairs[0].sum(1) == T * k).all())
+    assert torch.equal(ev.bytes[0], ev.remote_dev[0] * cfg.bytes_per_token)
+    assert torch.equal(ev.remote_dev[0], ev.remote_intra[0] + ev.remote_inter[0])
+    # the fast (bit-sliced) path without per-token outputs gives the same totals
+    ev2 = cap.eval_placements(idx_d, None, None, cand_d, topo, counts=cnt_d)
+    for name in ("dev_visits", "remote_dev", "remote_intra", "remote_inter", "node_visits", "remote_node", "cost",
+                 "bytes", "load_pairs", "recv_tokens"):
+        assert torch.equal(getattr(ev, name), getattr(ev2, name)), name
+    del ev, ev2
+    torch.cuda.empty_cache()
+
+    # S4: sampled tokens against the oracle; after-metrics against an evaluation of the kept trace
+    pi = cand[:, 2, :].copy()
+    pi_d = dev(pi)
+    tau = cfg.taus[-1]
+    kept_d, near_d, aft = cap.prune(idx_d, w_d, None, pi_d, topo, tau)
+    w_s = w_d[0, samp_d].cpu().numpy()[None]
+    kept_r, near_r = O.prune(idx_r, w_s, pi, dn, tau, token_src=src_s, cost_inter=cfg.cost_inter)
+    assert np.array_equal(kept_d[0, samp_d].cpu().numpy()[None], kept_r)
+    ev_k = cap.eval_placements(idx_d, kept_d, None, pi_d[:, None, :].contiguous(), topo)
+    assert_eval_equal(aft, SimpleNamespace(**{n: host(getattr(ev_k, n)) for n in
+                                              ("dev_visits", "remote_dev", "remote_intra", "remote_inter", "node_visits",
+                                               "remote_node", "cost", "bytes", "load_pairs", "recv_tokens", "imbalance",
+                                               "imbalance_recv")}), False, "2^22 after-prune ")
+
+    # S5: stable permutation of the kept pairs grouped by device
+    sp, off, pos = cap.dispatch_layout(idx_d[0], kept_d[0], pi_d[0], D)
+    n_kept = int(kept_d.sum())
+    assert int(off[0]) == 0 and int(off[-1]) == n_kept
+    spv = sp[:n_kept].long()
+    keys = pi_d[0].long()[idx_d[0].reshape(-1).long()[spv]]
+    assert bool((keys[1:] >= keys[:-1]).all())                                   # grouped by device
+    assert torch.equal(torch.bincount(keys, minlength=D).cumsum(0), off[1:])     # offsets = prefix of the counts
+    same = keys[1:] == keys[:-1]
+    assert bool((spv[1:][same] > spv[:-1][same]).all())                          # ascending inside a device: stable
+    assert bool(kept_d.reshape(-1)[spv].all())                                   # only kept pairs
+    assert torch.equal(pos.long()[spv], torch.arange(n_kept, device="cuda"))     # inverse permutation
+    assert int((pos >= 0).sum()) == n_kept
