@@ -441,3 +441,150 @@ int capo_dispatch_layout(const int32_t *idx, const uint8_t *kept, int64_t T, int
     offsets[D] = pos;
     return CAPO_OK;
 }
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-1  co-activation probabilities and Algorithm 1.
+ *
+ * p_ij: "the ratio between the number of times they are selected
+ * together and the total number of times either of them is selected" ->
+ * reading R3 (Jaccard): p_ij = C_ij / (n_i + n_j - C_ij), 0 when the
+ * denominator is 0, p_ii = 0 (never used: every sum below is over j != i or
+ * over members of a group that e does not belong to).  Integers converted to
+ * double exactly, one IEEE divide.
+ *
+ * Algorithm 1, followed line by line (capo_alg1 below):
+ *   line 1   deg[i] = sum_{j != i} p_ij             (ascending j, fp64)
+ *   line 2-3 G[g] = {} ; U = {all}
+ *   line 4   pi = experts sorted by deg descending  (ties -> lower index, R23)
+ *   line 5-7 for g = 1..k: seed G[g] with pi[g]
+ *   line 8   while U not empty                      (starts at g = 1, R16)
+ *   line 9-10  e* = argmax_{e in U} sum_{v in G[g]} p_ev   (sum in the order the
+ *              members joined G[g]; ties -> lower index, R23)
+ *   line 11-12 if that score is 0: e* = the r-th smallest element of U with
+ *              r = rnd[step] mod |U| ("uniformly at random"; the random
+ *              numbers are an INPUT, one per growth step, so that no generator
+ *              is shared with the CUDA path; rnd == NULL reads as zeros)
+ *   line 13  move e* from U to G[g]
+ *   line 14  g = (g mod k) + 1
+ * n must be a multiple of k ("each GPU hosts the same number of experts",
+ * P:L160): the round-robin then fills every group to exactly n/k.
+ *
+ * Stage 2: "treat each GPU group as a coarse-grained unit, compute the
+ * co-activation strength between groups, and apply the same grouping principle
+ * again to assign GPU groups to nodes" -> reading R24: strength
+ * W[a][b] = sum_{i in G[a]} sum_{j in G[b]} p_ij (i ascending outer, j
+ * ascending inner, fp64), W[a][a] = 0; then capo_alg1 with n = D units, k = N.
+ *
+ * Outputs: expert_group [L][E] (stage 1), group_node [L][D] (stage 2), and the
+ * placement expert_dev [L][E] on the regular topology dev_node[d] = d / (D/N):
+ * group a becomes device group_node[a]*(D/N) + (rank at which a joined its node).
+ * p_out [L][E][E] (nullable) receives the probabilities.
+ * rnd [L][E + D] uint32 (nullable): stage 1 step s reads rnd[s], stage 2 step s
+ * reads rnd[E + s].
+ *
+ * Pins (tests/test_oracle_pins.py): SURVEY worked example p_01 = 1/4, p_04 =
+ * 2/3 by hand; k = 1, k = n closed forms; exact recovery of planted clusters
+ * (block-diagonal C) and of planted node structure; an exact-rational
+ * (fractions.Fraction) replay of the listing on tiny inputs; devices per token
+ * below the sequential placement on the clustered trace (the paper's claim).
+ * ------------------------------------------------------------------------- */
+static void capo_alg1(int32_t n, int32_t k, const double *Pm, const uint32_t *rnd,
+                      int32_t *grp, int32_t *ord)
+{
+    double *deg = (double *)malloc(sizeof(double) * (size_t)n);
+    int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)n);
+    int32_t *G = (int32_t *)malloc(sizeof(int32_t) * (size_t)n * (size_t)k); /* G[g][0..size) */
+    int32_t *size = (int32_t *)calloc((size_t)k, sizeof(int32_t));
+    uint8_t *inU = (uint8_t *)malloc((size_t)n);
+    for (int32_t i = 0; i < n; ++i) {                       /* line 1 */
+        double s = 0.0;
+        for (int32_t j = 0; j < n; ++j)
+            if (j != i) s += Pm[(size_t)i * n + j];
+        deg[i] = s;
+        inU[i] = 1;                                         /* line 3 */
+        pi[i] = i;
+    }
+    for (int32_t a = 1; a < n; ++a) {                       /* line 4: stable insertion sort */
+        int32_t x = pi[a];
+        int32_t b = a - 1;
+        while (b >= 0 && deg[pi[b]] < deg[x]) { pi[b + 1] = pi[b]; --b; }
+        pi[b + 1] = x;
+    }
+    int32_t nU = n;
+    for (int32_t g = 0; g < k; ++g) {                       /* lines 5-7 */
+        int32_t s = pi[g];
+        ord[s] = size[g];
+        G[(size_t)g * n + size[g]++] = s;
+        grp[s] = g;
+        inU[s] = 0;
+        --nU;
+    }
+    int32_t g = 0, step = 0;
+    while (nU > 0) {                                        /* line 8 */
+        int32_t best = -1;
+        double bests = 0.0;
+        for (int32_t e = 0; e < n; ++e) {                   /* lines 9-10 */
+            if (!inU[e]) continue;
+            double sc = 0.0;
+            for (int32_t m = 0; m < size[g]; ++m) sc += Pm[(size_t)e * n + G[(size_t)g * n + m]];
+            if (best < 0 || sc > bests) { best = e; bests = sc; }
+        }
+        if (bests == 0.0) {                                 /* lines 11-12 */
+            uint32_t r = (rnd ? rnd[step] : 0u) % (uint32_t)nU;
+            for (int32_t e = 0; e < n; ++e) {
+                if (!inU[e]) continue;
+                if (r == 0) { best = e; break; }
+                --r;
+            }
+        }
+        ord[best] = size[g];                                /* line 13 */
+        G[(size_t)g * n + size[g]++] = best;
+        grp[best] = g;
+        inU[best] = 0;
+        --nU;
+        g = (g + 1) % k;                                    /* line 14 */
+        ++step;
+    }
+    free(deg); free(pi); free(G); free(size); free(inU);
+}
+
+int capo_coact_placement(const int64_t *counts, const int32_t *coact, int32_t L, int32_t E,
+                         int32_t D, int32_t N, const uint32_t *rnd, double *p_out,
+                         int32_t *expert_group, int32_t *group_node, int32_t *expert_dev)
+{
+    if (L < 0 || E < 1 || D < 1 || N < 1 || E % D != 0 || D % N != 0) return CAPO_EINVAL;
+    double *Pm = (double *)malloc(sizeof(double) * (size_t)E * (size_t)E);
+    double *W = (double *)malloc(sizeof(double) * (size_t)D * (size_t)D);
+    int32_t *ord = (int32_t *)malloc(sizeof(int32_t) * (size_t)E);
+    int32_t *ord2 = (int32_t *)malloc(sizeof(int32_t) * (size_t)D);
+    for (int32_t l = 0; l < L; ++l) {
+        const int64_t *n = counts + (size_t)l * E;
+        const int32_t *C = coact + (size_t)l * E * E;
+        int32_t *grp = expert_group + (size_t)l * E;
+        int32_t *gn = group_node + (size_t)l * D;
+        for (int32_t i = 0; i < E; ++i)
+            for (int32_t j = 0; j < E; ++j) {
+                int64_t den = n[i] + n[j] - (int64_t)C[(size_t)i * E + j];
+                Pm[(size_t)i * E + j] =
+                    (i == j || den == 0) ? 0.0 : (double)C[(size_t)i * E + j] / (double)den;
+            }
+        if (p_out) memcpy(p_out + (size_t)l * E * E, Pm, sizeof(double) * (size_t)E * (size_t)E);
+        capo_alg1(E, D, Pm, rnd ? rnd + (size_t)l * (size_t)(E + D) : NULL, grp, ord);
+        for (int32_t a = 0; a < D; ++a)
+            for (int32_t b = 0; b < D; ++b) {
+                double s = 0.0;
+                if (a != b)
+                    for (int32_t i = 0; i < E; ++i) {
+                        if (grp[i] != a) continue;
+                        for (int32_t j = 0; j < E; ++j)
+                            if (grp[j] == b) s += Pm[(size_t)i * E + j];
+                    }
+                W[(size_t)a * D + b] = s;
+            }
+        capo_alg1(D, N, W, rnd ? rnd + (size_t)l * (size_t)(E + D) + E : NULL, gn, ord2);
+        for (int32_t e = 0; e < E; ++e)
+            expert_dev[(size_t)l * E + e] = gn[grp[e]] * (D / N) + ord2[grp[e]];
+    }
+    free(Pm); free(W); free(ord); free(ord2);
+    return CAPO_OK;
+}

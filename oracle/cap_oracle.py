@@ -164,3 +164,24 @@ def trace_fused(logits, bias, gate, expert_dev, dev_node, *, token_src=None, cos
                          cost_intra=cost_intra, cost_inter=cost_inter,
                          bytes_per_token=bytes_per_token, per_token=per_token)
     return idx, w, counts, coact, ev
+
+
+def coact_placement(counts, coact, *, D, N, rnd=None, want_p=False):
+    """NEXT-1: Jaccard p_ij + Algorithm 1 (device groups, then node groups).
+
+    counts [L,E] int64, coact [L,E,E] int32, rnd [L,E+D] uint32 or None ->
+    (expert_group [L,E], group_node [L,D], expert_dev [L,E], p [L,E,E] fp64 or None)."""
+    counts = _c(counts, np.int64)
+    coact = _c(coact, np.int32)
+    L, E = counts.shape
+    rnd = _c(rnd, np.uint32)
+    p = np.empty((L, E, E), np.float64) if want_p else None
+    expert_group = np.empty((L, E), np.int32)
+    group_node = np.empty((L, D), np.int32)
+    expert_dev = np.empty((L, E), np.int32)
+    rc = lib().capo_coact_placement(_p(counts), _p(coact), C.c_int32(L), C.c_int32(E), C.c_int32(D),
+                                    C.c_int32(N), _p(rnd), _p(p), _p(expert_group), _p(group_node),
+                                    _p(expert_dev))
+    if rc != 0:
+        raise ValueError(f"capo_coact_placement -> {rc}")
+    return expert_group, group_node, expert_dev, p

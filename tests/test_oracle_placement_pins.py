@@ -1,0 +1,193 @@
+"""Pins of the oracle's NEXT-1 function: Jaccard co-activation probabilities
+(reading R3) and Algorithm 1 in both stages.  Each pin is
+something other than the oracle itself: hand values, closed-form special cases, exact recovery of
+planted structure, an exact-rational replay of the listing, and the paper's claim that the
+placement lowers devices per token."""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from paper_2607_05116_b200 import workload as W
+
+
+def planted(E, D, N, rng, strong=40, weak=3):
+    """Counts / co-activation with planted device clusters (size E/D) grouped into planted nodes.
+    One "hub" expert per cluster co-activates more strongly with its cluster mates and one hub
+    cluster per node co-activates (weakly) across nodes, so that the top-D weighted degrees are
+    one expert per cluster and the top-N group strengths one cluster per node: Algorithm 1 seeds
+    with the largest degrees, and two seeds inside one cluster could not recover it.
+    Returns (counts, C, cluster_of_expert, node_of_cluster)."""
+    perm = rng.permutation(E)
+    cl = np.empty(E, np.int64)
+    cl[perm] = np.arange(E) // (E // D)
+    cperm = rng.permutation(D)
+    nd = np.empty(D, np.int64)
+    nd[cperm] = np.arange(D) // (D // N)
+    hub_e = {int(perm[c * (E // D)]) for c in range(D)}
+    hub_c = {int(cperm[m * (D // N)]) for m in range(N)}
+    Cm = np.zeros((E, E), np.int64)
+    for i in range(E):
+        for j in range(E):
+            if i == j:
+                continue
+            if cl[i] == cl[j]:
+                Cm[i, j] = strong + (20 if (i in hub_e or j in hub_e) else 0)
+            elif nd[cl[i]] == nd[cl[j]]:
+                Cm[i, j] = weak
+            else:
+                Cm[i, j] = 1 if (int(cl[i]) in hub_c or int(cl[j]) in hub_c) else 0
+    n = Cm.sum(1) + 5
+    Cm[np.arange(E), np.arange(E)] = n
+    return n[None].astype(np.int64), Cm[None].astype(np.int32), cl, nd
+
+
+def same_partition(a, b):
+    m = {}
+    for x, y in zip(a.tolist(), b.tolist()):
+        if m.setdefault(x, y) != y:
+            return False
+    return len(set(m.values())) == len(m)
+
+
+def test_jaccard_worked_example(oracle, golden):
+    """SURVEY 8(c) worked example: counts [3,2,2,1,2,1,1,0]; p_01 = 1/(3+2-1), p_04 = 2/(3+2-2),
+    p_07 = 0 (expert 7 never selected), p symmetric with zero diagonal."""
+    idx = np.array(golden["worked_example"]["idx"], np.int32)[None]
+    cnt, C = oracle.coactivation(idx, E=8)
+    *_, p = oracle.coact_placement(cnt, C, D=4, N=2, want_p=True)
+    p = p[0]
+    assert p[0, 1] == 0.25 and p[0, 4] == 2.0 / 3.0 and p[0, 7] == 0.0 and p[7, 7] == 0.0
+    assert p[1, 6] == 1.0 / 2.0                      # C=1, n=2,1 -> 1/(2+1-1)
+    np.testing.assert_array_equal(p, p.T)
+    assert np.all(np.diag(p) == 0.0) and np.all((p >= 0) & (p <= 1))
+
+
+def test_jaccard_zero_denominator(oracle):
+    cnt = np.zeros((1, 4), np.int64)
+    C = np.zeros((1, 4, 4), np.int32)
+    g, gn, ed, p = oracle.coact_placement(cnt, C, D=2, N=1, want_p=True)
+    assert np.all(p == 0.0)
+    # all scores are 0 -> every growth step takes the random branch; with rnd = None (zeros) the
+    # lowest unassigned expert joins: seeds 0,1 then 2 -> g0, 3 -> g1
+    assert g.tolist() == [[0, 1, 0, 1]] and gn.tolist() == [[0, 0]] and ed.tolist() == [[0, 1, 0, 1]]
+
+
+def test_random_branch_uses_supplied_numbers(oracle):
+    """Zero matrix, E=6, D=2: seeds 0,1; U = {2,3,4,5}.  rnd = [3, 1, 6, 9]: step 0 picks the
+    3 mod 4 = 3rd of {2,3,4,5} = 5 -> g0; step 1: 1 mod 3 -> {2,3,4}[1] = 3 -> g1; step 2:
+    6 mod 2 = 0 -> 2 -> g0; step 3: 9 mod 1 = 0 -> 4 -> g1."""
+    cnt = np.zeros((1, 6), np.int64)
+    C = np.zeros((1, 6, 6), np.int32)
+    rnd = np.array([[3, 1, 6, 9, 0, 0, 0, 0]], np.uint32)
+    g, _, _, _ = oracle.coact_placement(cnt, C, D=2, N=1, rnd=rnd)
+    assert g.tolist() == [[0, 1, 0, 1, 1, 0]]
+
+
+def test_k_equals_one_and_k_equals_n(oracle):
+    rng = np.random.default_rng(3)
+    n, C, _, _ = planted(12, 4, 2, rng)
+    g, gn, ed, p = oracle.coact_placement(n, C, D=1, N=1, want_p=True)
+    assert np.all(g == 0) and np.all(ed == 0)
+    # D = E: every expert is a seed; group index = rank by weighted degree (desc, ties -> lower)
+    A = rng.integers(0, 30, (12, 12))
+    A = np.triu(A, 1)
+    A = A + A.T
+    nn = A.sum(1) + 1
+    A[np.arange(12), np.arange(12)] = nn
+    g, gn, ed, p = oracle.coact_placement(nn[None].astype(np.int64), A[None].astype(np.int32),
+                                          D=12, N=1, want_p=True)
+    deg = np.array([sum(p[0, i, j] for j in range(12) if j != i) for i in range(12)])
+    order = sorted(range(12), key=lambda i: (-deg[i], i))
+    assert [int(g[0, e]) for e in order] == list(range(12))
+
+
+@pytest.mark.parametrize("E,D,N", [(16, 4, 2), (64, 8, 2), (128, 16, 4)])
+def test_planted_clusters_and_nodes_recovered(oracle, E, D, N):
+    """Block structure: co-activation >= 40 inside a cluster, 3 between clusters of one node,
+    <= 1 across nodes, seeds forced into distinct clusters / nodes by the hubs.  The greedy step
+    of a group then always sees its own cluster mates with the largest score, so stage 1 returns
+    the clusters and stage 2 the nodes."""
+    rng = np.random.default_rng(E)
+    n, C, cl, nd = planted(E, D, N, rng)
+    g, gn, ed, _ = oracle.coact_placement(n, C, D=D, N=N)
+    assert same_partition(g[0], cl)
+    assert np.bincount(g[0], minlength=D).tolist() == [E // D] * D
+    assert same_partition(gn[0][g[0]], nd[cl])
+    # final placement: a permutation-balanced map on the regular topology
+    assert np.bincount(ed[0], minlength=D).tolist() == [E // D] * D
+    np.testing.assert_array_equal(ed[0] // (D // N), gn[0][g[0]])
+    assert same_partition(ed[0], g[0])
+
+
+def alg1_exact(P, k, rnd):
+    """Algorithm 1 replayed in exact rational arithmetic."""
+    n = len(P)
+    deg = [sum(P[i][j] for j in range(n) if j != i) for i in range(n)]
+    pi = sorted(range(n), key=lambda i: (-deg[i], i))
+    G = [[pi[g]] for g in range(k)]
+    U = sorted(set(range(n)) - set(pi[:k]))
+    g, step = 0, 0
+    while U:
+        sc = {e: sum(P[e][v] for v in G[g]) for e in U}
+        best = max(U, key=lambda e: (sc[e], -e))
+        if sc[best] == 0:
+            best = U[int(rnd[step]) % len(U)]
+        G[g].append(best)
+        U.remove(best)
+        g = (g + 1) % k
+        step += 1
+    return G
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_algorithm1_vs_exact_rational_replay(oracle, seed):
+    """Tiny random traces: the fp64 oracle takes the same decisions as the listing evaluated with
+    fractions.Fraction (random integer matrices have no rational near-ties at 1e-16)."""
+    rng = np.random.default_rng(100 + seed)
+    E, D, N, k, T = 12, 4, 2, 3, 40 + 10 * seed
+    idx = np.stack([rng.choice(E - 2, k, replace=False) for _ in range(T)]).astype(np.int32)[None]
+    cnt, C = oracle.coactivation(idx, E=E)          # experts E-2, E-1 never selected -> zero rows
+    rnd = rng.integers(0, 2**32, (1, E + D), dtype=np.uint64).astype(np.uint32)
+    g, gn, ed, p = oracle.coact_placement(cnt, C, D=D, N=N, rnd=rnd, want_p=True)
+    n = cnt[0].tolist()
+    Cm = C[0].tolist()
+    P = [[Fraction(0) if (i == j or n[i] + n[j] - Cm[i][j] == 0)
+          else Fraction(Cm[i][j], n[i] + n[j] - Cm[i][j]) for j in range(E)] for i in range(E)]
+    np.testing.assert_allclose(p[0], np.array([[float(x) for x in r] for r in P]), rtol=0, atol=1e-16)
+    G = alg1_exact(P, D, rnd[0, :E])
+    for a, members in enumerate(G):
+        assert all(g[0, e] == a for e in members)
+    Wm = [[sum(P[i][j] for i in sorted(G[a]) for j in sorted(G[b])) if a != b else Fraction(0)
+           for b in range(D)] for a in range(D)]
+    G2 = alg1_exact(Wm, N, rnd[0, E:])
+    for nd, members in enumerate(G2):
+        for r, a in enumerate(members):
+            assert gn[0, a] == nd
+            assert all(ed[0, e] == nd * (D // N) + r for e in G[a])
+
+
+def test_placement_lowers_devices_per_token(oracle, golden):
+    """P:L162, Table III: grouping co-activated experts lowers the devices each token visits
+    (paper: 5.33-5.35 -> 4.14-4.49 at E=128, k=8, D=8).  On the Qwen3-shaped synthetic trace the
+    Algorithm 1 placement must beat the sequential one clearly and stay balanced in size."""
+    cfg = W.CONFIGS["qwen3"].with_(T=16384)
+    x = W.logits(cfg, 0)[None]
+    idx, _ = oracle.gate_topk(x, k=cfg.k)
+    cnt, C = oracle.coactivation(idx, E=cfg.E)
+    g, gn, ed, _ = oracle.coact_placement(cnt, C, D=cfg.D, N=cfg.N)
+    seq = (np.arange(cfg.E) // (cfg.E // cfg.D)).astype(np.int32)
+    ev = oracle.eval_placements(idx, np.stack([seq, ed[0]])[None], W.dev_node(cfg))
+    dpt = ev.dev_visits[0] / cfg.T
+    assert np.bincount(ed[0], minlength=cfg.D).tolist() == [cfg.E // cfg.D] * cfg.D
+    lo, hi = golden["paper_table3_default"]["cap_devices_per_token_range"]
+    assert dpt[1] < dpt[0] - 0.4 and lo - 0.6 < dpt[1] < hi + 0.6
+
+
+def test_placement_einval(oracle):
+    cnt = np.zeros((1, 6), np.int64)
+    C = np.zeros((1, 6, 6), np.int32)
+    with pytest.raises(ValueError):
+        oracle.coact_placement(cnt, C, D=4, N=1)      # E % D != 0
+    with pytest.raises(ValueError):
+        oracle.coact_placement(cnt, C, D=3, N=2)      # D % N != 0
