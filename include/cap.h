@@ -48,6 +48,7 @@ extern "C" {
 #define CAP_CALL_PRUNE 3
 #define CAP_CALL_DISPATCH_LAYOUT 4
 #define CAP_CALL_TRACE_FUSED 5
+#define CAP_CALL_COACT_PLACEMENT 6   /* T, k, P ignored */
 
 /* Gate configuration (Eq. 1; scoring / group-limited routing / tie rule from
  * BASELINE.json, readings R1, R2, R14, R21). */
@@ -152,6 +153,31 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
                     const int32_t *expert_dev, int32_t P, const cap_topology *topo,
                     const cap_eval_out *out, void *ws, size_t ws_bytes, void *stream);
 
+/* Co-activation driven expert placement: SURVEY 8(f) rank 1, the consumer of cap_coactivation's
+ * outputs.  P:L148 defines the co-activation probability ("the ratio between the number of times
+ * they are selected together and the total number of times either of them is selected"; reading R3:
+ * p_ij = C_ij / (n_i + n_j - C_ij), 0 when the denominator is 0, p_ii = 0, fp64, one IEEE divide);
+ * P:L106-144 is Algorithm 1 (weighted degrees, the D largest as seeds -- ties to the lower index,
+ * R23 --, then round-robin growth from g = 1, each step taking the unassigned expert with the
+ * largest sum of p to the group's members, summed in joining order, ties to the lower index; a zero
+ * best score takes the r-th smallest unassigned expert, r = rnd[step] mod |U|); P:L162-164 applies
+ * it again to the device groups with strength W[a][b] = sum_{i in G[a]} sum_{j in G[b]} p_ij
+ * (ascending i outer, ascending j inner, R24) to form N node groups.
+ *   counts [L][E] int64, coact [L][E][E] int32: as written by cap_coactivation / cap_trace_fused.
+ *   rnd [L][E + D] uint32, nullable (= zeros): stage 1 growth step s reads rnd[s], stage 2 step s
+ *     reads rnd[E + s]; only consumed on the zero-score branch (line 12 of the listing).
+ *   p_out [L][E][E] fp64, nullable: the probabilities.
+ *   expert_group [L][E]: stage-1 group of each expert; group_node [L][D]: node of each group;
+ *   expert_dev [L][E]: the placement on the regular topology dev_node[d] = d / (D/N): group a
+ *     is device group_node[a] * (D/N) + (rank at which a joined its node group, seed = 0).
+ * Requires E % D == 0 and D % N == 0 ("each GPU hosts the same number of experts"), else
+ * CAP_EINVAL.  Workspace: cap_workspace_bytes(CAP_CALL_COACT_PLACEMENT, L, 0, E, 1, D, 0).
+ * All outputs are reproducible bit for bit (fixed summation orders). */
+int cap_coact_placement(const int64_t *counts, const int32_t *coact, int32_t L, int32_t E, int32_t D,
+                        int32_t N, const uint32_t *rnd, double *p_out, int32_t *expert_group,
+                        int32_t *group_node, int32_t *expert_dev, void *ws, size_t ws_bytes,
+                        void *stream);
+
 /* Bytes of workspace the given call needs for these sizes (0 on invalid sizes). */
 size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int32_t k,
                            int32_t D, int32_t P);
@@ -170,7 +196,7 @@ int64_t cap_launch_count(void);
 /* Profiling aid (not part of the data path; not thread-safe).  cap_kernel_timer_arm(tag, slot)
  * makes the next launch of the kernel tagged `tag` ("gate_topk", "coact", "eval", "eval_finalize",
  * "eval_table", "eval_decode", "masked_counts", "prune", "dispatch_hist", "dispatch_scan",
- * "dispatch_scatter", "trace_fused")
+ * "dispatch_scatter", "trace_fused", "coact_placement")
  * record a CUDA event pair, owned by the library, around itself on its stream; up to 128 arms
  * may be pending, slot in [0,4096).  cap_kernel_timer_ms(slot) returns the elapsed device time
  * in milliseconds once that work has completed (the caller synchronises), or -1. */

@@ -12,16 +12,17 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcap_b200.so")
 
-CALL_GATE_TOPK, CALL_COACTIVATION, CALL_EVAL_PLACEMENTS, CALL_PRUNE, CALL_DISPATCH_LAYOUT, CALL_TRACE_FUSED = range(6)
+(CALL_GATE_TOPK, CALL_COACTIVATION, CALL_EVAL_PLACEMENTS, CALL_PRUNE, CALL_DISPATCH_LAYOUT, CALL_TRACE_FUSED,
+ CALL_COACT_PLACEMENT) = range(7)
 OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
-           "cap_dispatch_layout", "cap_trace_fused", "cap_workspace_bytes",
+           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
-               "dispatch_hist", "dispatch_scan", "dispatch_scatter")
+               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement")
 
 
 class GateCfg(C.Structure):
@@ -77,6 +78,7 @@ def lib():
         L.cap_trace_fused.argtypes = [vp, vp, i32, i64, C.POINTER(GateCfg), vp, vp, vp, vp, vp, vp,
                                       i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz, vp]
         L.cap_validate_placements.argtypes = [vp, i32, i32, i32, i32, vp]
+        L.cap_coact_placement.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.cap_profile_fused_kernel.argtypes = [C.POINTER(C.c_void_p), i32, i32, i32, i64, C.POINTER(GateCfg), vp, vp,
                                                vp, vp, vp, i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz,
                                                vp, C.POINTER(C.c_float)]
@@ -232,6 +234,25 @@ def dispatch_layout(idx, kept, expert_dev, D, want_pos=True, ws=None):
                                    _ptr(pair_pos), _ptr(offsets), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_dispatch_layout")
     return sorted_pairs, offsets, pair_pos
+
+
+def coact_placement(counts, coact, D, N, rnd=None, want_p=False, ws=None):
+    """cap_coact_placement: Jaccard p_ij + Algorithm 1 (device groups, then node groups).
+    counts [L,E] int64, coact [L,E,E] int32, rnd [L,E+D] int32-typed bits or None ->
+    (expert_group [L,E], group_node [L,D], expert_dev [L,E], p [L,E,E] fp64 or None)."""
+    L, E = counts.shape
+    dev = counts.device
+    p = torch.empty((L, E, E), dtype=torch.float64, device=dev) if want_p else None
+    expert_group = torch.empty((L, E), dtype=torch.int32, device=dev)
+    group_node = torch.empty((L, D), dtype=torch.int32, device=dev)
+    expert_dev = torch.empty((L, E), dtype=torch.int32, device=dev)
+    if ws is None:
+        ws = workspace(CALL_COACT_PLACEMENT, L, 0, E, 1, D, 0, device=dev)
+    rc = lib().cap_coact_placement(_ptr(counts, torch.int64), _ptr(coact, torch.int32), L, E, D, N,
+                                   _ptr(rnd, torch.int32), _ptr(p), _ptr(expert_group), _ptr(group_node),
+                                   _ptr(expert_dev), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "cap_coact_placement")
+    return expert_group, group_node, expert_dev, p
 
 
 class FusedBuffers:

@@ -57,6 +57,13 @@ def test_host_side_einval_without_gpu(lib):
                                    C.byref(out), None, 0, None) == cap.EINVAL            # D = 0
     assert lib.cap_dispatch_layout(None, None, 4, 2, 16, None, 65, None, None, None, None, 0, None) == cap.EINVAL
     assert lib.cap_validate_placements(None, 1, 1, 16, 0, None) == cap.EINVAL
+    pl = lambda E, D, N, ws=None, n=0: lib.cap_coact_placement(None, None, 1, E, D, N, None, None, None, None,
+                                                               None, ws, n, None)
+    assert pl(6, 4, 1) == cap.EINVAL and pl(6, 3, 2) == cap.EINVAL and pl(2048, 4, 1) == cap.EINVAL
+    assert pl(128, 65, 1) == cap.EINVAL and pl(16, 4, 2) == cap.EINVAL                 # NULL arrays
+    assert lib.cap_coact_placement(None, None, 0, 16, 4, 2, None, None, None, None, None, None, 0,
+                                   None) == cap.EWORKSPACE
+    assert lib.cap_workspace_bytes(cap.CALL_COACT_PLACEMENT, 2, 0, 128, 1, 16, 0) >= 2 * 8 * (128 * 128 + 16 * 128 + 256)
 
 
 def test_binding_refuses_cpu_tensors(lib):
