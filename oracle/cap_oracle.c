@@ -588,3 +588,53 @@ int capo_coact_placement(const int64_t *counts, const int32_t *coact, int32_t L,
     free(Pm); free(W); free(ord); free(ord2);
     return CAPO_OK;
 }
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-3  the pairwise communication objective, Eq. 2-3
+ * (P:L152-158), for P candidate placements, from the co-activation statistics
+ * alone (no pass over the trace):
+ *   C(pi) = sum_{i<j} p_ij d(pi(i), pi(j)),
+ *   d = 0 same device, cost_intra (the paper's 1) same node, cost_inter (c) else.
+ * Two weights: the integer co-activation counts C_ij (obj_count, int64, exact)
+ * and the probabilities p_ij of P:L148 / R3 (obj_prob, fp64, summed over i
+ * ascending, then j ascending).  Eq. 5: combined = lambda * obj_prob +
+ * (1 - lambda) * B(pi) with B the caller's imbalance array (Eq. 4, an output
+ * of S3); written only when imbalance != NULL.
+ * expert_dev [L][P][E], dev_node [D]; outputs [L][P], any may be NULL.
+ * Pins: all experts on one device -> 0; one expert per device on one node with
+ * cost 1 -> sum_{i<j} C_ij = (sum_i (k-1) n_i) / 2 (S2's invariant); the
+ * worked example by hand; the cluster-aligned placement scores below the
+ * sequential one; brute force over pairs in Python.
+ * ------------------------------------------------------------------------- */
+int capo_pairwise_objective(const int64_t *counts, const int32_t *coact, int32_t L, int32_t E,
+                            const int32_t *expert_dev, int32_t P, int32_t D, const int32_t *dev_node,
+                            int32_t cost_intra, int32_t cost_inter, double lambda,
+                            const double *imbalance, int64_t *obj_count, double *obj_prob,
+                            double *combined)
+{
+    if (L < 0 || E < 1 || P < 0 || D < 1) return CAPO_EINVAL;
+    for (int32_t l = 0; l < L; ++l) {
+        const int64_t *n = counts + (size_t)l * E;
+        const int32_t *C = coact + (size_t)l * E * E;
+        for (int32_t p = 0; p < P; ++p) {
+            const int32_t *pi = expert_dev + ((size_t)l * P + p) * E;
+            int64_t oc = 0;
+            double op = 0.0;
+            for (int32_t i = 0; i < E; ++i)
+                for (int32_t j = i + 1; j < E; ++j) {
+                    int32_t di = pi[i], dj = pi[j];
+                    int32_t d = di == dj ? 0 : (dev_node[di] == dev_node[dj] ? cost_intra : cost_inter);
+                    int64_t c = C[(size_t)i * E + j];
+                    int64_t den = n[i] + n[j] - c;
+                    double pij = den == 0 ? 0.0 : (double)c / (double)den;
+                    oc += c * (int64_t)d;
+                    op += pij * (double)d;
+                }
+            size_t o = (size_t)l * P + p;
+            if (obj_count) obj_count[o] = oc;
+            if (obj_prob) obj_prob[o] = op;
+            if (combined && imbalance) combined[o] = lambda * op + (1.0 - lambda) * imbalance[o];
+        }
+    }
+    return CAPO_OK;
+}

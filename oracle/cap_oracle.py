@@ -185,3 +185,26 @@ def coact_placement(counts, coact, *, D, N, rnd=None, want_p=False):
     if rc != 0:
         raise ValueError(f"capo_coact_placement -> {rc}")
     return expert_group, group_node, expert_dev, p
+
+
+def pairwise_objective(counts, coact, expert_dev, dev_node, *, cost_intra=1, cost_inter=1, lam=0.5,
+                       imbalance=None):
+    """NEXT-3: Eq. 2-3 for P candidates from (counts, coact).  expert_dev [L,P,E] ->
+    (obj_count [L,P] int64, obj_prob [L,P] fp64, combined [L,P] fp64 or None)."""
+    counts = _c(counts, np.int64)
+    coact = _c(coact, np.int32)
+    expert_dev = _c(expert_dev, np.int32)
+    dev_node = _c(dev_node, np.int32)
+    L, P, E = expert_dev.shape
+    D = dev_node.shape[0]
+    imbalance = _c(imbalance, np.float64)
+    oc = np.empty((L, P), np.int64)
+    op = np.empty((L, P), np.float64)
+    cb = np.empty((L, P), np.float64) if imbalance is not None else None
+    rc = lib().capo_pairwise_objective(_p(counts), _p(coact), C.c_int32(L), C.c_int32(E), _p(expert_dev),
+                                       C.c_int32(P), C.c_int32(D), _p(dev_node), C.c_int32(cost_intra),
+                                       C.c_int32(cost_inter), C.c_double(lam), _p(imbalance), _p(oc),
+                                       _p(op), _p(cb))
+    if rc != 0:
+        raise ValueError(f"capo_pairwise_objective -> {rc}")
+    return oc, op, cb

@@ -191,3 +191,63 @@ def test_placement_einval(oracle):
         oracle.coact_placement(cnt, C, D=4, N=1)      # E % D != 0
     with pytest.raises(ValueError):
         oracle.coact_placement(cnt, C, D=3, N=2)      # D % N != 0
+
+
+# ------------------------------------------------------------------ NEXT-3: pairwise objective, Eq. 2-3
+def test_objective_worked_example_by_hand(oracle, golden):
+    """Worked example, Eq. 2-3 with costs 1 / 4, summed by hand over the ten co-activated
+    pairs: pi_A: (0,2) 2*1 + (0,4) 2*4 + (0,5) 4 + (1,2) 1 + (1,3) 1 + (1,6) 4 + (2,4) 4 + (3,6) 4 = 28;
+    pi_B: 1 + 8 + 0 + 1 + 4 + 4 + 4 + 4 + 1 + 1 = 28.  Probabilities (Jaccard) under pi_A:
+    2/3 + 4*2/3 + 4/3 + 1/3 + 1/2 + 4/2 + 4/3 + 4*1 = 19/3 + 6.5."""
+    g = golden["worked_example"]
+    cnt = np.array(g["counts"], np.int64)[None]
+    C = np.array(g["coact"], np.int32)[None]
+    maps = np.array([g["pi_A"], g["pi_B"]], np.int32)[None]
+    oc, op, cb = oracle.pairwise_objective(cnt, C, maps, np.array(g["dev_node"], np.int32), cost_intra=1,
+                                           cost_inter=4, lam=0.25,
+                                           imbalance=np.array([[g["eval_A"]["imbalance"], 2.0]]))
+    assert oc.tolist() == [[28, 28]]
+    assert abs(op[0, 0] - (19.0 / 3.0 + 6.5)) < 1e-14
+    assert abs(cb[0, 0] - (0.25 * (19.0 / 3.0 + 6.5) + 0.75 * 5.0 / 3.0)) < 1e-14      # Eq. 5
+
+
+def test_objective_closed_forms_and_brute_force(oracle):
+    rng = np.random.default_rng(11)
+    E, k, T, D = 24, 4, 300, 6
+    idx = np.stack([rng.choice(E, k, replace=False) for _ in range(T)]).astype(np.int32)[None]
+    cnt, C = oracle.coactivation(idx, E=E)
+    dn = np.array([0, 0, 0, 1, 1, 1], np.int32)
+    one_dev = np.zeros(E, np.int32)
+    ident = np.arange(E, dtype=np.int32)
+    rnd = rng.integers(0, D, E).astype(np.int32)
+    # all experts on one device: nothing is cut
+    oc, op, _ = oracle.pairwise_objective(cnt, C, np.stack([one_dev, rnd])[None], dn, cost_intra=1, cost_inter=5)
+    assert oc[0, 0] == 0 and op[0, 0] == 0.0
+    # brute force over pairs for the random map
+    n, Cm = cnt[0], C[0].astype(np.int64)
+    want_c, want_p = 0, 0.0
+    for i in range(E):
+        for j in range(i + 1, E):
+            d = 0 if rnd[i] == rnd[j] else (1 if dn[rnd[i]] == dn[rnd[j]] else 5)
+            want_c += int(Cm[i, j]) * d
+            den = n[i] + n[j] - Cm[i, j]
+            want_p += (Cm[i, j] / den if den else 0.0) * d
+    assert oc[0, 1] == want_c and abs(op[0, 1] - want_p) <= 1e-12 * want_p
+    # one expert per device, one node, cost 1: every co-activated pair is cut once:
+    # sum_{i<j} C_ij = sum_i (k-1) n_i / 2 = T k (k-1) / 2   (S2's row-sum invariant)
+    oc, _, _ = oracle.pairwise_objective(cnt, C, ident[None, None], np.zeros(E, np.int32))
+    assert oc[0, 0] == T * k * (k - 1) // 2
+
+
+def test_objective_prefers_cluster_aligned_placement(oracle):
+    """Eq. 2 is the proxy the placement minimises: on the clustered trace the planted cluster-aligned
+    candidate (workload candidate 2) and Algorithm 1's placement score below the sequential map."""
+    cfg = W.CONFIGS["target"].with_(T=8192)
+    idx, _ = oracle.gate_topk(W.logits(cfg, 0)[None], k=cfg.k)
+    cnt, C = oracle.coactivation(idx, E=cfg.E)
+    cand = W.candidates(cfg, 0)[:3]
+    _, _, ed, _ = oracle.coact_placement(cnt, C, D=cfg.D, N=cfg.N)
+    maps = np.concatenate([cand, ed])[None]
+    oc, op, _ = oracle.pairwise_objective(cnt, C, maps, W.dev_node(cfg), cost_intra=1, cost_inter=cfg.cost_inter)
+    assert oc[0, 2] < oc[0, 0] and op[0, 2] < op[0, 0]
+    assert oc[0, 3] < oc[0, 0] and op[0, 3] < op[0, 0]
