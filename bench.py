@@ -364,6 +364,21 @@ def run_cap(args, cfg, W):
     ms_e2e = ev2.elapsed_time(ev3)
     clocks = sampler.stop() if rank == 0 else None
 
+    # ---- SURVEY 8(f) rank 1, outside every timed region above: cap_coact_placement (Jaccard p_ij +
+    # Algorithm 1, both stages) on the counts / co-activation matrices the last step left on the device
+    dstep(0)
+    ws_pl = cap.workspace(cap.CALL_COACT_PLACEMENT, L, 0, E, 1, D, 0, device=dev)
+    for _ in range(3):
+        cap.coact_placement(pipe.fb.counts, pipe.fb.coact, D, cfg.N, ws=ws_pl)
+    torch.cuda.synchronize()
+    ev6, ev7 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev6.record()
+    for _ in range(10):
+        cap.coact_placement(pipe.fb.counts, pipe.fb.coact, D, cfg.N, ws=ws_pl)
+    ev7.record()
+    torch.cuda.synchronize()
+    us_place = ev6.elapsed_time(ev7) / 10 * 1e3
+
     if world > 1:
         tt = torch.tensor([ms, ms_e2e], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -402,6 +417,10 @@ def run_cap(args, cfg, W):
                          "kernel_ms_warmup_share": {t: round(v / max(sum(tot.values()), 1e-9), 4)
                                                     for t, v in tot.items() if v > 0}},
         }
+        out["next"] = {"coact_placement": {
+            "us_per_call": us_place, "layers": L, "greedy_steps_per_layer": (E - D) + (D - cfg.N),
+            "what": "cap_coact_placement (P:L106-144, L148, L162-164) on the step's counts / coact; latency-bound "
+                    "sequential greedy, one CTA per layer; not part of `value`"}}
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = time_oracle(cfg, W, args.cpu_seconds)
         print(json.dumps(out))

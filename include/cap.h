@@ -178,6 +178,26 @@ int cap_coact_placement(const int64_t *counts, const int32_t *coact, int32_t L, 
                         int32_t *group_node, int32_t *expert_dev, void *ws, size_t ws_bytes,
                         void *stream);
 
+/* Pairwise communication objective of P:L152-158 (Eq. 2-3) for P candidate placements, computed from
+ * the co-activation statistics alone: C(pi) = sum_{i<j} w_ij d(pi(i), pi(j)) with
+ * d = 0 on the same device, topo->cost_intra (the paper's 1) on the same node, topo->cost_inter (the
+ * paper's c) across nodes (cost_local is not used), for two weights:
+ *   obj_count [L][P] int64: w_ij = C_ij (exact);
+ *   obj_prob  [L][P] fp64:  w_ij = p_ij = C_ij / (n_i + n_j - C_ij) (R3; 0 when the denominator
+ *     is 0).  Summation order is the kernel's (fixed, so results repeat run to run); the definition's
+ *     i-then-j order differs by at most (E^2 / 2) ulp relative, all terms being non-negative: compare
+ *     with relative tolerance 1e-10.
+ *   combined  [L][P] fp64, nullable: Eq. 5, lambda * obj_prob + (1 - lambda) * imbalance, with
+ *     imbalance [L][P] fp64 (B(pi) of Eq. 4, e.g. cap_eval_out.imbalance); CAP_EINVAL if combined is
+ *     given without imbalance.
+ * counts [L][E] int64 and coact [L][E][E] int32 as written by cap_coactivation; expert_dev [L][P][E]
+ * (values outside [0, D) are clamped: memory-safe, result undefined).  Any output may be NULL.  No
+ * workspace. */
+int cap_pairwise_objective(const int64_t *counts, const int32_t *coact, int32_t L, int32_t E,
+                           const int32_t *expert_dev, int32_t P, const cap_topology *topo, double lambda,
+                           const double *imbalance, int64_t *obj_count, double *obj_prob, double *combined,
+                           void *stream);
+
 /* Bytes of workspace the given call needs for these sizes (0 on invalid sizes). */
 size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int32_t k,
                            int32_t D, int32_t P);
@@ -196,7 +216,7 @@ int64_t cap_launch_count(void);
 /* Profiling aid (not part of the data path; not thread-safe).  cap_kernel_timer_arm(tag, slot)
  * makes the next launch of the kernel tagged `tag` ("gate_topk", "coact", "eval", "eval_finalize",
  * "eval_table", "eval_decode", "masked_counts", "prune", "dispatch_hist", "dispatch_scan",
- * "dispatch_scatter", "trace_fused", "coact_placement")
+ * "dispatch_scatter", "trace_fused", "coact_placement", "objective")
  * record a CUDA event pair, owned by the library, around itself on its stream; up to 128 arms
  * may be pending, slot in [0,4096).  cap_kernel_timer_ms(slot) returns the elapsed device time
  * in milliseconds once that work has completed (the caller synchronises), or -1. */

@@ -17,12 +17,12 @@ LIB_PATH = os.path.join(_HERE, "libcap_b200.so")
 OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
-           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_workspace_bytes",
+           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
-               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement")
+               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective")
 
 
 class GateCfg(C.Structure):
@@ -78,6 +78,8 @@ def lib():
         L.cap_trace_fused.argtypes = [vp, vp, i32, i64, C.POINTER(GateCfg), vp, vp, vp, vp, vp, vp,
                                       i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz, vp]
         L.cap_validate_placements.argtypes = [vp, i32, i32, i32, i32, vp]
+        L.cap_pairwise_objective.argtypes = [vp, vp, i32, i32, vp, i32, C.POINTER(Topology), C.c_double, vp, vp, vp,
+                                             vp, vp]
         L.cap_coact_placement.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.cap_profile_fused_kernel.argtypes = [C.POINTER(C.c_void_p), i32, i32, i32, i64, C.POINTER(GateCfg), vp, vp,
                                                vp, vp, vp, i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz,
@@ -253,6 +255,21 @@ def coact_placement(counts, coact, D, N, rnd=None, want_p=False, ws=None):
                                    _ptr(expert_dev), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_coact_placement")
     return expert_group, group_node, expert_dev, p
+
+
+def pairwise_objective(counts, coact, expert_dev, topo, lam=0.5, imbalance=None):
+    """cap_pairwise_objective: Eq. 2-3 for P candidates from (counts, coact); Eq. 5 when imbalance is given.
+    expert_dev [L,P,E] int32 -> (obj_count [L,P] int64, obj_prob [L,P] fp64, combined [L,P] fp64 or None)."""
+    L, P, E = expert_dev.shape
+    dev = counts.device
+    oc = torch.empty((L, P), dtype=torch.int64, device=dev)
+    op = torch.empty((L, P), dtype=torch.float64, device=dev)
+    cb = torch.empty((L, P), dtype=torch.float64, device=dev) if imbalance is not None else None
+    rc = lib().cap_pairwise_objective(_ptr(counts, torch.int64), _ptr(coact, torch.int32), L, E,
+                                      _ptr(expert_dev, torch.int32), P, C.byref(topo), float(lam),
+                                      _ptr(imbalance, torch.float64), _ptr(oc), _ptr(op), _ptr(cb), _stream())
+    _check(rc, "cap_pairwise_objective")
+    return oc, op, cb
 
 
 class FusedBuffers:

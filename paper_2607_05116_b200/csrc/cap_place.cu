@@ -17,33 +17,26 @@
 namespace cap {
 namespace {
 
-struct Best {
-    double v;
-    int e;
-};
-
-__device__ __forceinline__ Best better(Best a, Best b)   // larger score, ties -> lower index (R23)
+// Arg-max of non-negative doubles over a warp, ties -> lowest lane (= lowest index, R23).  The bit
+// pattern of a non-negative double orders like the value, so the maximum is two 32-bit REDUX
+// operations (high word, then low word among the lanes that hold the largest high word) and one
+// ballot.  Lanes outside U pass hi = -1.  Returns the winning lane; *mh / *ml = the maximum's words.
+__device__ __forceinline__ int warp_argmax(int hi, unsigned lo, int *mh, unsigned *ml)
 {
-    return (b.v > a.v || (b.v == a.v && b.e < a.e)) ? b : a;
-}
-
-__device__ __forceinline__ Best warp_best(Best x)
-{
-#pragma unroll
-    for (int o = 16; o; o >>= 1) {
-        Best y;
-        y.v = __shfl_xor_sync(0xffffffffu, x.v, o);
-        y.e = __shfl_xor_sync(0xffffffffu, x.e, o);
-        x = better(x, y);
-    }
-    return x;
+    int h = __reduce_max_sync(0xffffffffu, hi);
+    unsigned l = __reduce_max_sync(0xffffffffu, hi == h ? lo : 0u);
+    unsigned bal = __ballot_sync(0xffffffffu, hi == h && lo == l);
+    *mh = h;
+    *ml = l;
+    return __ffs(bal) - 1;
 }
 
 struct PlaceSmem {
     double deg[1024];
     int grp[1024], ord[1024], members[1024];
     int grp2[64], ord2[64], seeds[64], gsize[64];
-    double pv[2][32];
+    int ph[2][32];
+    unsigned pl[2][32];
     int pe[2][32];
     int wcnt[32];
     int pick;
@@ -51,14 +44,19 @@ struct PlaceSmem {
 
 // Algorithm 1 on n units and k groups.  MT[m * n + e] = M[e][m] (so that a step reads one
 // contiguous row); score is [k][n] scratch in global memory, each element touched by one thread.
-__device__ void alg1(int n, int k, const double *MT, double *score, const uint32_t *rnd, int *grp, int *ord,
-                     PlaceSmem &sm)
+// The scores of groups g < gs live in shared memory (sscore), the rest in global memory (score):
+// a global store does not allocate in L1, so a global score costs an L2 round trip per step.
+__device__ void alg1(int n, int k, const double *MT, double *score, double *sscore, int gs, const uint32_t *rnd,
+                     int *grp, int *ord, PlaceSmem &sm)
 {
     const int e = threadIdx.x, lane = e & 31, wid = e >> 5, nw = blockDim.x >> 5;
     double d = 0.0;
     if (e < n) {                                              // line 1: ascending j, j != e
-        for (int j = 0; j < n; ++j)
-            if (j != e) d += MT[(size_t)j * n + e];
+#pragma unroll 16
+        for (int j = 0; j < n; ++j) {
+            double x = MT[(size_t)j * n + e];
+            if (j != e) d += x;
+        }
         sm.deg[e] = d;
     }
     __syncthreads();
@@ -79,25 +77,29 @@ __device__ void alg1(int n, int k, const double *MT, double *score, const uint32
     }
     __syncthreads();
     if (e < n)
-        for (int g = 0; g < k; ++g) score[(size_t)g * n + e] = 0.0 + MT[(size_t)sm.seeds[g] * n + e];
+        for (int g = 0; g < k; ++g)
+            *(g < gs ? sscore + g * n + e : score + (size_t)g * n + e) = 0.0 + MT[(size_t)sm.seeds[g] * n + e];
     const int steps = n - k;
+    // The rank-1 update of group g's scores (line 13's effect on line 9) is next needed k steps later:
+    // for k >= 2 the row of MT is loaded in step s and added in step s + 1, which takes the L2 latency
+    // of that load off the step's dependent chain (same operands, same order: same bits).
+    double mval = 0.0;
+    int gpend = -1;
     for (int step = 0; step < steps; ++step) {                // line 8
         const int g = step % k, par = step & 1;               // line 14
-        Best b;
-        b.v = inU ? score[(size_t)g * n + e] : -1.0;
-        b.e = inU ? e : INT_MAX;
-        b = warp_best(b);                                     // lines 9-10
+        double v = inU ? *(g < gs ? sscore + g * n + e : score + (size_t)g * n + e) : 0.0;
+        int mh, wh;
+        unsigned ml, wl;
+        int src = warp_argmax(inU ? __double2hiint(v) : -1, (unsigned)__double2loint(v), &mh, &ml);   // lines 9-10
         if (lane == 0) {
-            sm.pv[par][wid] = b.v;
-            sm.pe[par][wid] = b.e;
+            sm.ph[par][wid] = mh;
+            sm.pl[par][wid] = ml;
+            sm.pe[par][wid] = (wid << 5) + src;
         }
         __syncthreads();
-        Best c;
-        c.v = lane < nw ? sm.pv[par][lane] : -1.0;
-        c.e = lane < nw ? sm.pe[par][lane] : INT_MAX;
-        c = warp_best(c);
-        int pick = c.e;
-        if (c.v == 0.0) {                                     // lines 11-12 (block-uniform branch)
+        int src2 = warp_argmax(lane < nw ? sm.ph[par][lane] : -1, lane < nw ? sm.pl[par][lane] : 0u, &wh, &wl);
+        int pick = sm.pe[par][src2];
+        if (wh == 0 && wl == 0u) {                            // lines 11-12 (block-uniform branch)
             uint32_t r = (rnd ? rnd[step] : 0u) % (uint32_t)(steps - step);
             unsigned bal = __ballot_sync(0xffffffffu, inU);
             if (lane == 0) sm.wcnt[wid] = __popc(bal);
@@ -114,7 +116,15 @@ __device__ void alg1(int n, int k, const double *MT, double *score, const uint32
             ord[e] = sm.gsize[g];
             sm.gsize[g] += 1;
         }
-        if (inU) score[(size_t)g * n + e] += MT[(size_t)pick * n + e];
+        if (e < n) {
+            if (gpend >= 0) *(gpend < gs ? sscore + gpend * n + e : score + (size_t)gpend * n + e) += mval;
+            mval = MT[(size_t)pick * n + e];
+            gpend = g;
+            if (k == 1) {
+                *(gs > 0 ? sscore + e : score + e) += mval;
+                gpend = -1;
+            }
+        }
     }
     __syncthreads();
 }
@@ -122,9 +132,10 @@ __device__ void alg1(int n, int k, const double *MT, double *score, const uint32
 __global__ void __launch_bounds__(1024, 1)
 place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coact, int E, int D, int N,
              const uint32_t *__restrict__ rnd, double *p_out, double *wsP, double *wsS, double *wsW,
-             int32_t *expert_group, int32_t *group_node, int32_t *expert_dev)
+             int32_t *expert_group, int32_t *group_node, int32_t *expert_dev, int gs1)
 {
     __shared__ PlaceSmem sm;
+    extern __shared__ double sscore[];
     const int l = blockIdx.x, tid = threadIdx.x;
     const int64_t *n = counts + (size_t)l * E;
     const int32_t *C = coact + (size_t)l * E * E;
@@ -144,7 +155,7 @@ place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coa
         pT[(size_t)j * E + i] = v;
     }
     __syncthreads();
-    alg1(E, D, pT, score, r1, sm.grp, sm.ord, sm);
+    alg1(E, D, pT, score, sscore, gs1, r1, sm.grp, sm.ord, sm);
 
     // stage 2 (R24): W[a][b] = sum over i in G[a] (ascending), j in G[b] (ascending) of p_ij
     const int m = E / D;
@@ -165,7 +176,7 @@ place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coa
         WT[(size_t)b * D + a] = s;
     }
     __syncthreads();
-    alg1(D, N, WT, score, r1 ? r1 + E : nullptr, sm.grp2, sm.ord2, sm);
+    alg1(D, N, WT, score, sscore, N, r1 ? r1 + E : nullptr, sm.grp2, sm.ord2, sm);
 
     if (tid < E) {
         int g = sm.grp[tid];
@@ -191,9 +202,20 @@ int launch_place(const int64_t *counts, const int32_t *coact, int32_t L, int32_t
     double *wsS = wsP + (size_t)L * E * E;
     double *wsW = wsS + (size_t)L * D * E;
     int threads = ((E > 64 ? E : 64) + 31) & ~31;
+    // shared-memory score rows: as many groups as fit in 200 KB beside the static 22 KB
+    int gs1 = (int)((size_t)204800 / ((size_t)E * sizeof(double)));
+    if (gs1 > D) gs1 = D;
+    size_t dyn = (size_t)gs1 * E * sizeof(double);
+    if (dyn < (size_t)N * D * sizeof(double)) dyn = (size_t)N * D * sizeof(double);
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 204800) != cudaSuccess)
+            return check_launch("place_kernel attribute");
+        attr_set = true;
+    }
     KernelTimerScope kt("coact_placement", st);
-    place_kernel<<<L, threads, 0, st>>>(counts, coact, E, D, N, rnd, p_out, wsP, wsS, wsW, expert_group,
-                                        group_node, expert_dev);
+    place_kernel<<<L, threads, dyn, st>>>(counts, coact, E, D, N, rnd, p_out, wsP, wsS, wsW, expert_group,
+                                          group_node, expert_dev, gs1);
     note_launch();
     return check_launch("place_kernel");
 }

@@ -63,6 +63,9 @@ def test_host_side_einval_without_gpu(lib):
     assert pl(128, 65, 1) == cap.EINVAL and pl(16, 4, 2) == cap.EINVAL                 # NULL arrays
     assert lib.cap_coact_placement(None, None, 0, 16, 4, 2, None, None, None, None, None, None, 0,
                                    None) == cap.EWORKSPACE
+    assert lib.cap_pairwise_objective(None, None, 1, 16, None, 2, None, 0.5, None, None, None, None, None) == cap.EINVAL
+    assert lib.cap_pairwise_objective(None, None, 1, 16, None, 2, C.byref(topo), 0.5, None, None, None, None,
+                                      None) == cap.EINVAL                                 # D = 0
     assert lib.cap_workspace_bytes(cap.CALL_COACT_PLACEMENT, 2, 0, 128, 1, 16, 0) >= 2 * 8 * (128 * 128 + 16 * 128 + 256)
 
 

@@ -116,3 +116,70 @@ def test_placement_kernel_time_all_layers():
         torch.cuda.synchronize()
         np.testing.assert_array_equal(host(got[2]), ref[2])
         print(f"cap_coact_placement {name}: L={L} E={cfg.E} D={cfg.D} N={cfg.N}: {a.elapsed_time(b) / 5 * 1e3:.1f} us per call")
+
+
+# ------------------------------------------------------------------ cap_pairwise_objective (Eq. 2-3, Eq. 5)
+OBJ_RTOL = 1e-10   # include/cap.h: summation order only; (E^2 / 2) ulp bound on non-negative terms
+
+
+def check_objective(cnt, C, maps, dn, cost_intra, cost_inter, lam, imb, tag=""):
+    D = dn.shape[0]
+    N = int(dn.max()) + 1
+    ref = O.pairwise_objective(cnt, C, maps, dn, cost_intra=cost_intra, cost_inter=cost_inter, lam=lam,
+                               imbalance=imb)
+    dnd = dev(dn)
+    topo = cap.topology(dnd, 0, cost_intra, cost_inter, 0, N=N)
+    got = cap.pairwise_objective(dev(cnt), dev(C), dev(maps), topo, lam=lam, imbalance=dev(imb))
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(host(got[0]), ref[0], err_msg=tag + "obj_count")
+    np.testing.assert_allclose(host(got[1]), ref[1], rtol=OBJ_RTOL, atol=0, err_msg=tag + "obj_prob")
+    if imb is not None:
+        np.testing.assert_allclose(host(got[2]), ref[2], rtol=OBJ_RTOL, atol=0, err_msg=tag + "combined")
+    return ref
+
+
+@pytest.mark.parametrize("name,layers,T,P", [("tiny", (0,), 4096, 4), ("qwen3", (0, 17), 16384, 64),
+                                             ("target", (0,), 65536, 256), ("dsv3", (0, 31), 8192, 128),
+                                             ("stress", (0,), 16384, 1024)])
+def test_objective_on_baseline_configs(name, layers, T, P):
+    cfg = W.CONFIGS[name]
+    _, _, idx, cnt, C = trace_stats(cfg, layers, T)
+    maps = np.stack([W.candidates(cfg, l, P) for l in layers])
+    rng = np.random.default_rng(3)
+    imb = 1.0 + rng.random((len(layers), P))
+    ref = check_objective(cnt, C, maps, W.dev_node(cfg), 1, cfg.cost_inter, 0.3, imb, tag=name + " ")
+    # the planted cluster-aligned candidate cuts less than the sequential one (not under group-limited
+    # routing, where the contiguous groups of the sequential map are themselves what the gate favours)
+    if cfg.clusters is not None and cfg.n_group == 1:
+        assert np.all(ref[0][:, 2] < ref[0][:, 0])
+
+
+@pytest.mark.parametrize("E,D,N,P", [(8, 4, 2, 2), (33, 11, 1, 9), (100, 10, 5, 17), (1024, 64, 8, 3), (1, 1, 1, 1)])
+def test_objective_ragged_shapes(E, D, N, P):
+    rng = np.random.default_rng(E + P)
+    L, k, T = 2, min(4, E), 300
+    idx = np.stack([[rng.choice(E, k, replace=False) for _ in range(T)] for _ in range(L)]).astype(np.int32)
+    cnt, C = O.coactivation(idx, E=E)
+    maps = rng.integers(0, D, (L, P, E)).astype(np.int32)
+    dn = (np.arange(D) // (D // N)).astype(np.int32)
+    check_objective(cnt, C, maps, dn, 2, 7, 0.75, None, tag=f"E{E} ")
+    check_objective(cnt, C, maps, dn, 1, 1, 0.0, rng.random((L, P)) + 1, tag=f"E{E} uniform ")
+
+
+def test_objective_kernel_time():
+    for name in ("target", "stress"):
+        cfg = W.CONFIGS[name]
+        _, _, _, cnt, C = trace_stats(cfg, (0,), 8192)
+        maps = W.candidates(cfg, 0)[None]
+        dnd = dev(W.dev_node(cfg))
+        topo = cap.topology(dnd, 0, 1, cfg.cost_inter, 0, N=cfg.N)
+        dc, dC, dm = dev(cnt), dev(C), dev(maps)
+        cap.pairwise_objective(dc, dC, dm, topo)
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(10):
+            cap.pairwise_objective(dc, dC, dm, topo)
+        b.record()
+        torch.cuda.synchronize()
+        print(f"cap_pairwise_objective {name}: E={cfg.E} P={cfg.P}: {a.elapsed_time(b) / 10 * 1e3:.1f} us per call")
