@@ -32,6 +32,7 @@ __device__ __forceinline__ int warp_argmax(int hi, unsigned lo, int *mh, unsigne
 }
 
 struct PlaceSmem {
+    long long cnt[1024];
     double deg[1024];
     int grp[1024], ord[1024], members[1024];
     int grp2[64], ord2[64], seeds[64], gsize[64];
@@ -46,7 +47,7 @@ struct PlaceSmem {
 // contiguous row); score is [k][n] scratch in global memory, each element touched by one thread.
 // The scores of groups g < gs live in shared memory (sscore), the rest in global memory (score):
 // a global store does not allocate in L1, so a global score costs an L2 round trip per step.
-__device__ void alg1(int n, int k, const double *MT, double *score, double *sscore, int gs, const uint32_t *rnd,
+__device__ __forceinline__ void alg1(int n, int k, const double *MT, double *score, double *sscore, int gs, const uint32_t *rnd,
                      int *grp, int *ord, PlaceSmem &sm)
 {
     const int e = threadIdx.x, lane = e & 31, wid = e >> 5, nw = blockDim.x >> 5;
@@ -77,17 +78,23 @@ __device__ void alg1(int n, int k, const double *MT, double *score, double *ssco
     }
     __syncthreads();
     if (e < n)
-        for (int g = 0; g < k; ++g)
-            *(g < gs ? sscore + g * n + e : score + (size_t)g * n + e) = 0.0 + MT[(size_t)sm.seeds[g] * n + e];
+        for (int g = 0; g < k; ++g) {
+            double x = 0.0 + MT[(size_t)sm.seeds[g] * n + e];
+            if (g < gs) sscore[g * n + e] = x;
+            else score[(size_t)g * n + e] = x;
+        }
     const int steps = n - k;
-    // The rank-1 update of group g's scores (line 13's effect on line 9) is next needed k steps later:
-    // for k >= 2 the row of MT is loaded in step s and added in step s + 1, which takes the L2 latency
-    // of that load off the step's dependent chain (same operands, same order: same bits).
-    double mval = 0.0;
-    int gpend = -1;
+    // The rank-1 update of group g's scores (line 13's effect on line 9) is next needed k steps later, so
+    // the row of MT loaded in step s is added in step s + depth (depth = 4 when k >= 5, 1 when k >= 2,
+    // 0 when k = 1): a step is ~300 cycles, an L2 row read ~800, and this takes the read off the step's
+    // dependent chain without changing any operand or the order of the additions to a score.
+    const int depth = k >= 5 ? 4 : (k >= 2 ? 1 : 0);
+    double m0 = 0.0, m1 = 0.0, m2 = 0.0, m3 = 0.0;
+    int g0 = -1, g1 = -1, g2 = -1, g3 = -1;                   // oldest first
     for (int step = 0; step < steps; ++step) {                // line 8
         const int g = step % k, par = step & 1;               // line 14
-        double v = inU ? *(g < gs ? sscore + g * n + e : score + (size_t)g * n + e) : 0.0;
+        double v = 0.0;
+        if (inU) v = g < gs ? sscore[g * n + e] : score[(size_t)g * n + e];
         int mh, wh;
         unsigned ml, wl;
         int src = warp_argmax(inU ? __double2hiint(v) : -1, (unsigned)__double2loint(v), &mh, &ml);   // lines 9-10
@@ -117,12 +124,24 @@ __device__ void alg1(int n, int k, const double *MT, double *score, double *ssco
             sm.gsize[g] += 1;
         }
         if (e < n) {
-            if (gpend >= 0) *(gpend < gs ? sscore + gpend * n + e : score + (size_t)gpend * n + e) += mval;
-            mval = MT[(size_t)pick * n + e];
-            gpend = g;
-            if (k == 1) {
-                *(gs > 0 ? sscore + e : score + e) += mval;
-                gpend = -1;
+            double mnew = MT[(size_t)pick * n + e];
+            double ma;
+            int ga;
+            if (depth == 4) {
+                ma = m0; ga = g0;
+                m0 = m1; g0 = g1;
+                m1 = m2; g1 = g2;
+                m2 = m3; g2 = g3;
+                m3 = mnew; g3 = g;
+            } else if (depth == 1) {
+                ma = m3; ga = g3;
+                m3 = mnew; g3 = g;
+            } else {
+                ma = mnew; ga = g;
+            }
+            if (ga >= 0) {
+                if (ga < gs) sscore[ga * n + e] += ma;
+                else score[(size_t)ga * n + e] += ma;
             }
         }
     }
@@ -146,10 +165,13 @@ place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coa
     const uint32_t *r1 = rnd ? rnd + (size_t)l * (E + D) : nullptr;
 
     // p_ij = C_ij / (n_i + n_j - C_ij): exact int -> double conversions, one IEEE divide (R3)
+    for (int e = tid; e < E; e += blockDim.x) sm.cnt[e] = n[e];
+    __syncthreads();
+#pragma unroll 4
     for (int q = tid; q < E * E; q += blockDim.x) {
         int i = q / E, j = q - i * E;
         long long c = C[q];
-        long long den = n[i] + n[j] - c;
+        long long den = sm.cnt[i] + sm.cnt[j] - c;
         double v = (i == j || den == 0) ? 0.0 : __ddiv_rn((double)c, (double)den);
         if (po) po[q] = v;
         pT[(size_t)j * E + i] = v;
@@ -201,15 +223,17 @@ int launch_place(const int64_t *counts, const int32_t *coact, int32_t L, int32_t
     double *wsP = (double *)(((uintptr_t)ws + 255) & ~(uintptr_t)255);
     double *wsS = wsP + (size_t)L * E * E;
     double *wsW = wsS + (size_t)L * D * E;
-    int threads = ((E > 64 ? E : 64) + 31) & ~31;
-    // shared-memory score rows: as many groups as fit in 200 KB beside the static 22 KB
-    int gs1 = (int)((size_t)204800 / ((size_t)E * sizeof(double)));
+    // at least 512 threads: the E^2 prologue (probabilities, degrees' operands) is latency-bound and wants
+    // the memory-level parallelism; threads beyond E only take part in the barriers of the greedy loop
+    int threads = ((E > 512 ? E : 512) + 31) & ~31;
+    // shared-memory score rows: as many groups as fit in 192 KB beside the static 30 KB
+    int gs1 = (int)((size_t)196608 / ((size_t)E * sizeof(double)));
     if (gs1 > D) gs1 = D;
     size_t dyn = (size_t)gs1 * E * sizeof(double);
     if (dyn < (size_t)N * D * sizeof(double)) dyn = (size_t)N * D * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 204800) != cudaSuccess)
+        if (cudaFuncSetAttribute(place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 196608) != cudaSuccess)
             return check_launch("place_kernel attribute");
         attr_set = true;
     }
