@@ -4,7 +4,7 @@
 // scalarisation with a caller-supplied imbalance.
 //
 // Work is P * E^2 / 2 pair evaluations over an E x E matrix that stays in L2 (1 MB of int32 at E = 512):
-// a block scores PC = 8 candidates per pass over the matrix (coalesced row-major reads, the (device,
+// a block scores PC (8, fewer for small P) candidates per pass over the matrix (coalesced row-major reads, the (device,
 // node) codes of its candidates in shared memory), so the matrix is read P / 8 times from L2 and once
 // from HBM.  Bound: fp64 / integer ALU (one divide per pair and block, 8 select-multiply-adds).
 #include "cap_internal.cuh"
@@ -12,9 +12,9 @@
 namespace cap {
 namespace {
 
-constexpr int PC = 8;          // candidates per block
-constexpr int OBJ_THREADS = 256;
+constexpr int OBJ_THREADS = 512;
 
+template <int PC>   // candidates per block
 __global__ void __launch_bounds__(OBJ_THREADS)
 objective_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coact, int E,
                  const int32_t *__restrict__ expert_dev, int P, int D, const int32_t *__restrict__ dev_node,
@@ -44,11 +44,12 @@ objective_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__
         ac[c] = 0;
         ap[c] = 0.0;
     }
+    // latency-bound L2 reads: the loads of four iterations are issued together
+#pragma unroll 4
     for (int q = tid; q < E * E; q += OBJ_THREADS) {
-        int i = q / E, j = q - i * E;
-        if (j <= i) continue;
         long long c = C[q];
-        if (c == 0) continue;                // p_ij = 0 as well
+        int i = q / E, j = q - i * E;
+        if (j <= i || c == 0) continue;      // upper triangle; c = 0 means p_ij = 0 as well
         long long den = cnt[i] + cnt[j] - c;
         double pij = den == 0 ? 0.0 : __ddiv_rn((double)c, (double)den);
 #pragma unroll
@@ -106,10 +107,19 @@ extern "C" int cap_pairwise_objective(const int64_t *counts, const int32_t *coac
     if (L == 0 || P == 0) return CAP_OK;
     cudaStream_t st = (cudaStream_t)stream;
     KernelTimerScope kt("objective", st);
-    dim3 grid((P + PC - 1) / PC, L);
-    objective_kernel<<<grid, OBJ_THREADS, 0, st>>>(counts, coact, E, expert_dev, P, topo->D, topo->dev_node,
-                                                   topo->cost_intra, topo->cost_inter, lambda, imbalance, obj_count,
-                                                   obj_prob, combined);
+    // 8 candidates per block amortise the pass over the matrix; fewer when that would leave SMs idle
+    const long long want = sm_count();
+    int pc = 8;
+    while (pc > 1 && (long long)((P + pc - 1) / pc) * L < want) pc >>= 1;
+#define CAP_OBJ_LAUNCH(PCV)                                                                                      \
+    objective_kernel<PCV><<<dim3((P + PCV - 1) / PCV, L), OBJ_THREADS, 0, st>>>(                                  \
+        counts, coact, E, expert_dev, P, topo->D, topo->dev_node, topo->cost_intra, topo->cost_inter, lambda,    \
+        imbalance, obj_count, obj_prob, combined)
+    if (pc == 8) CAP_OBJ_LAUNCH(8);
+    else if (pc == 4) CAP_OBJ_LAUNCH(4);
+    else if (pc == 2) CAP_OBJ_LAUNCH(2);
+    else CAP_OBJ_LAUNCH(1);
+#undef CAP_OBJ_LAUNCH
     note_launch();
     return check_launch("objective_kernel");
 }
