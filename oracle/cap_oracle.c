@@ -638,3 +638,41 @@ int capo_pairwise_objective(const int64_t *counts, const int32_t *coact, int32_t
     }
     return CAPO_OK;
 }
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-4  device-centric dispatch rows.  P:L58 (sec.
+ * II-C, Fig. 2): "each token is sent once to each device that hosts activated
+ * experts" -- one row per (token, destination device), not per (token,
+ * expert) as in S5 (R18).  Rows are grouped by device, ascending token inside
+ * a device: rows_token[row_offsets[d] + r] = the r-th token (ascending) that
+ * keeps at least one expert on d; row_offsets[D] = number of rows (= S3's
+ * dev_visits; row_offsets[d+1]-row_offsets[d] = recv_tokens[d]).  pair_row[i]
+ * (i = t*k+s, nullable) = the row that carries token t to the device of its
+ * slot s, -1 for a pruned pair: the pointer the local weighted aggregation of
+ * Fig. 2 needs.  Plain loops: devices outer, tokens inner.
+ * ------------------------------------------------------------------------- */
+int capo_dispatch_rows(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,
+                       const int32_t *expert_dev, int32_t D, int32_t *rows_token,
+                       int32_t *pair_row, int64_t *row_offsets)
+{
+    if (T < 0 || k < 1 || E < 1 || D < 1) return CAPO_EINVAL;
+    int64_t n = 0;
+    if (pair_row)
+        for (int64_t i = 0; i < T * k; ++i) pair_row[i] = -1;
+    for (int32_t d = 0; d < D; ++d) {
+        row_offsets[d] = n;
+        for (int64_t t = 0; t < T; ++t) {
+            int hit = 0;
+            for (int32_t s = 0; s < k; ++s) {
+                size_t i = (size_t)t * k + s;
+                if (kept && !kept[i]) continue;
+                if (expert_dev[idx[i]] != d) continue;
+                hit = 1;
+                if (pair_row) pair_row[i] = (int32_t)n;
+            }
+            if (hit) rows_token[n++] = (int32_t)t;
+        }
+    }
+    row_offsets[D] = n;
+    return CAPO_OK;
+}

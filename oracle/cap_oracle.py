@@ -208,3 +208,21 @@ def pairwise_objective(counts, coact, expert_dev, dev_node, *, cost_intra=1, cos
     if rc != 0:
         raise ValueError(f"capo_pairwise_objective -> {rc}")
     return oc, op, cb
+
+
+def dispatch_rows(idx, expert_dev, D, *, kept=None):
+    """NEXT-4: one row per (token, destination device).  idx [T,k]; expert_dev [E] ->
+    (rows_token [n_rows], row_offsets [D+1], pair_row [T*k])."""
+    idx = _c(idx, np.int32)
+    T, k = idx.shape
+    expert_dev = _c(expert_dev, np.int32)
+    E = expert_dev.shape[0]
+    kept = _c(kept, np.uint8)
+    rows = np.empty((T * k,), np.int32)
+    pair_row = np.empty((T * k,), np.int32)
+    offsets = np.empty((D + 1,), np.int64)
+    rc = lib().capo_dispatch_rows(_p(idx), _p(kept), C.c_int64(T), C.c_int32(k), C.c_int32(E),
+                                  _p(expert_dev), C.c_int32(D), _p(rows), _p(pair_row), _p(offsets))
+    if rc != 0:
+        raise ValueError(f"capo_dispatch_rows -> {rc}")
+    return rows[: int(offsets[D])], offsets, pair_row

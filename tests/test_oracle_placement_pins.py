@@ -251,3 +251,47 @@ def test_objective_prefers_cluster_aligned_placement(oracle):
     oc, op, _ = oracle.pairwise_objective(cnt, C, maps, W.dev_node(cfg), cost_intra=1, cost_inter=cfg.cost_inter)
     assert oc[0, 2] < oc[0, 0] and op[0, 2] < op[0, 0]
     assert oc[0, 3] < oc[0, 0] and op[0, 3] < op[0, 0]
+
+
+# ------------------------------------------------------------------ NEXT-4: device-centric dispatch rows
+def test_dispatch_rows_worked_example_by_hand(oracle, golden):
+    """Worked example under pi_A (e // 2), by hand from Fig. 2's rule (one copy per device):
+    d0 <- t0,t1,t2,t3; d1 <- t0 (expert 2), t2 (expert 3), t3 (expert 2); d2 <- t1 (4,5), t3 (4);
+    d3 <- t2 (6).  Row counts = recv_tokens [4,3,2,1] of the S3 golden values."""
+    g = golden["worked_example"]
+    idx = np.array(g["idx"], np.int32)
+    rows, off, pr = oracle.dispatch_rows(idx, np.array(g["pi_A"], np.int32), 4)
+    assert rows.tolist() == [0, 1, 2, 3, 0, 2, 3, 1, 3, 2]
+    assert off.tolist() == [0, 4, 7, 9, 10]
+    assert pr.tolist() == [0, 4, 0, 7, 7, 1, 2, 9, 5, 3, 6, 8]
+    assert np.diff(off).tolist() == g["eval_A"]["recv_tokens"]
+    kept = np.array(g["prune_A_p025"]["kept"], np.uint8)
+    rows, off, pr = oracle.dispatch_rows(idx, np.array(g["pi_A"], np.int32), 4, kept=kept)
+    # kept = [[1,0,1],[1,1,0],[1,1,0],[1,0,1]]: t0 -> d0; t1 -> d2; t2 -> d0, d3; t3 -> d0, d2
+    assert rows.tolist() == [0, 2, 3, 1, 3, 2] and off.tolist() == [0, 3, 3, 5, 6]
+    assert pr.tolist() == [0, -1, 0, 3, 3, -1, 1, 5, -1, 2, -1, 4]
+
+
+def test_dispatch_rows_vs_python_sets_and_s3(oracle):
+    rng = np.random.default_rng(21)
+    T, E, k, D = 500, 40, 6, 8
+    idx = np.stack([rng.choice(E, k, replace=False) for _ in range(T)]).astype(np.int32)
+    kept = (rng.random((T, k)) < 0.7).astype(np.uint8)
+    pi = rng.integers(0, D, E).astype(np.int32)
+    for m in (None, kept):
+        rows, off, pr = oracle.dispatch_rows(idx, pi, D, kept=m)
+        want = sorted({(int(pi[idx[t, s]]), t) for t in range(T) for s in range(k) if m is None or m[t, s]})
+        got = [(d, int(t)) for d in range(D) for t in rows[off[d]:off[d + 1]]]
+        assert got == want
+        ev = oracle.eval_placements(idx[None], pi[None, None], np.zeros(D, np.int32), kept=None if m is None else m[None])
+        assert np.diff(off).tolist() == ev.recv_tokens[0, 0].tolist() and off[D] == ev.dev_visits[0, 0]
+        for t in range(T):
+            for s in range(k):
+                i = t * k + s
+                if m is not None and not m[t, s]:
+                    assert pr[i] == -1
+                else:
+                    d = pi[idx[t, s]]
+                    assert off[d] <= pr[i] < off[d + 1] and rows[pr[i]] == t
+    rows, off, pr = oracle.dispatch_rows(idx[:0], pi, D)
+    assert rows.size == 0 and off.tolist() == [0] * (D + 1)
