@@ -49,6 +49,7 @@ extern "C" {
 #define CAP_CALL_DISPATCH_LAYOUT 4
 #define CAP_CALL_TRACE_FUSED 5
 #define CAP_CALL_COACT_PLACEMENT 6   /* T, k, P ignored */
+#define CAP_CALL_DISPATCH_ROWS 7     /* L, E, k, P ignored */
 
 /* Gate configuration (Eq. 1; scoring / group-limited routing / tie rule from
  * BASELINE.json, readings R1, R2, R14, R21). */
@@ -178,6 +179,22 @@ int cap_coact_placement(const int64_t *counts, const int32_t *coact, int32_t L, 
                         int32_t *group_node, int32_t *expert_dev, void *ws, size_t ws_bytes,
                         void *stream);
 
+/* Device-centric dispatch rows.  P:L58 (sec. II-C, Fig. 2): "each token is sent once
+ * to each device that hosts activated experts" and aggregated there -- one row per (token, destination
+ * device) instead of cap_dispatch_layout's one entry per (token, expert) pair (R18).
+ *   rows_token [capacity >= T * min(k, D)] int32: token ids grouped by device, ascending token inside a
+ *     device; rows_token[row_offsets[d] + r] = the r-th token that keeps at least one expert on device d.
+ *   row_offsets [D + 1] int64: row_offsets[D] = number of rows (= dev_visits of cap_eval_placements for
+ *     this map; row_offsets[d + 1] - row_offsets[d] = recv_tokens[d]).
+ *   pair_row [T * k] int32, nullable: for pair i = t * k + s the row that carries token t to the device of
+ *     its slot s (what the local weighted aggregation of Fig. 2 indexes), -1 for a pruned pair.
+ * topk_idx [T][k], kept [T][k] nullable (= all kept), expert_dev [E] as in cap_dispatch_layout; one layer
+ * per call.  T = 0 is valid (offsets zeroed).  Workspace: cap_workspace_bytes(CAP_CALL_DISPATCH_ROWS, 1, T,
+ * E, k, D, 0).  Out-of-range experts / devices are clamped (memory-safe, result undefined). */
+int cap_dispatch_rows(const int32_t *topk_idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,
+                      const int32_t *expert_dev, int32_t D, int32_t *rows_token, int32_t *pair_row,
+                      int64_t *row_offsets, void *ws, size_t ws_bytes, void *stream);
+
 /* Pairwise communication objective of P:L152-158 (Eq. 2-3) for P candidate placements, computed from
  * the co-activation statistics alone: C(pi) = sum_{i<j} w_ij d(pi(i), pi(j)) with
  * d = 0 on the same device, topo->cost_intra (the paper's 1) on the same node, topo->cost_inter (the
@@ -216,7 +233,7 @@ int64_t cap_launch_count(void);
 /* Profiling aid (not part of the data path; not thread-safe).  cap_kernel_timer_arm(tag, slot)
  * makes the next launch of the kernel tagged `tag` ("gate_topk", "coact", "eval", "eval_finalize",
  * "eval_table", "eval_decode", "masked_counts", "prune", "dispatch_hist", "dispatch_scan",
- * "dispatch_scatter", "trace_fused", "coact_placement", "objective")
+ * "dispatch_scatter", "trace_fused", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter")
  * record a CUDA event pair, owned by the library, around itself on its stream; up to 128 arms
  * may be pending, slot in [0,4096).  cap_kernel_timer_ms(slot) returns the elapsed device time
  * in milliseconds once that work has completed (the caller synchronises), or -1. */

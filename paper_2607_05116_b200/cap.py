@@ -13,16 +13,16 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcap_b200.so")
 
 (CALL_GATE_TOPK, CALL_COACTIVATION, CALL_EVAL_PLACEMENTS, CALL_PRUNE, CALL_DISPATCH_LAYOUT, CALL_TRACE_FUSED,
- CALL_COACT_PLACEMENT) = range(7)
+ CALL_COACT_PLACEMENT, CALL_DISPATCH_ROWS) = range(8)
 OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
-           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_workspace_bytes",
+           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
-               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective")
+               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter")
 
 
 class GateCfg(C.Structure):
@@ -80,6 +80,7 @@ def lib():
         L.cap_validate_placements.argtypes = [vp, i32, i32, i32, i32, vp]
         L.cap_pairwise_objective.argtypes = [vp, vp, i32, i32, vp, i32, C.POINTER(Topology), C.c_double, vp, vp, vp,
                                              vp, vp]
+        L.cap_dispatch_rows.argtypes = [vp, vp, i64, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
         L.cap_coact_placement.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.cap_profile_fused_kernel.argtypes = [C.POINTER(C.c_void_p), i32, i32, i32, i64, C.POINTER(GateCfg), vp, vp,
                                                vp, vp, vp, i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz,
@@ -255,6 +256,24 @@ def coact_placement(counts, coact, D, N, rnd=None, want_p=False, ws=None):
                                    _ptr(expert_dev), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_coact_placement")
     return expert_group, group_node, expert_dev, p
+
+
+def dispatch_rows(idx, kept, expert_dev, D, want_pair_row=True, ws=None):
+    """cap_dispatch_rows: one row per (token, destination device).  idx [T,k], kept [T,k] or None,
+    expert_dev [E] -> (rows_token [T*min(k,D)] (valid up to row_offsets[D]), row_offsets [D+1], pair_row)."""
+    T, k = idx.shape
+    E = expert_dev.numel()
+    dev = idx.device
+    rows = torch.empty((max(T * min(k, D), 1),), dtype=torch.int32, device=dev)
+    pair_row = torch.empty((T * k,), dtype=torch.int32, device=dev) if want_pair_row else None
+    offsets = torch.empty((D + 1,), dtype=torch.int64, device=dev)
+    if ws is None:
+        ws = workspace(CALL_DISPATCH_ROWS, 1, T, E, k, D, 0, device=dev)
+    rc = lib().cap_dispatch_rows(_ptr(idx, torch.int32), _ptr(kept, torch.uint8), T, k, E,
+                                 _ptr(expert_dev, torch.int32), D, _ptr(rows), _ptr(pair_row), _ptr(offsets),
+                                 _ptr(ws), ws.numel(), _stream())
+    _check(rc, "cap_dispatch_rows")
+    return rows, offsets, pair_row
 
 
 def pairwise_objective(counts, coact, expert_dev, topo, lam=0.5, imbalance=None):

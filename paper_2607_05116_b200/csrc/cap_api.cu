@@ -167,6 +167,9 @@ size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int3
     case CAP_CALL_DISPATCH_LAYOUT:
         if (D < 1) return 0;
         return dispatch_ws_bytes(T, k, D);
+    case CAP_CALL_DISPATCH_ROWS:
+        if (D < 1) return 0;
+        return dispatch_rows_ws_bytes(T, D);
     case CAP_CALL_COACT_PLACEMENT:
         if (D < 1) return 0;
         return place_ws_bytes(L, E, D);

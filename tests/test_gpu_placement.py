@@ -183,3 +183,55 @@ def test_objective_kernel_time():
         b.record()
         torch.cuda.synchronize()
         print(f"cap_pairwise_objective {name}: E={cfg.E} P={cfg.P}: {a.elapsed_time(b) / 10 * 1e3:.1f} us per call")
+
+
+# ------------------------------------------------------------------ cap_dispatch_rows (Fig. 2)
+def check_rows(idx, kept, pi, D, tag=""):
+    rows_r, off_r, pr_r = O.dispatch_rows(idx, pi, D, kept=kept)
+    rows, off, pr = cap.dispatch_rows(dev(idx), dev(kept), dev(pi), D)
+    torch.cuda.synchronize()
+    np.testing.assert_array_equal(host(off), off_r, err_msg=tag + "row_offsets")
+    np.testing.assert_array_equal(host(rows)[: len(rows_r)], rows_r, err_msg=tag + "rows_token")
+    np.testing.assert_array_equal(host(pr), pr_r, err_msg=tag + "pair_row")
+
+
+@pytest.mark.parametrize("name,T", [("tiny", 4096), ("qwen3", 16384), ("target", 65536), ("dsv3", 32768),
+                                    ("stress", 65536)])
+def test_dispatch_rows_on_baseline_configs(name, T):
+    cfg = W.CONFIGS[name]
+    x = W.logits(cfg.with_(T=T), 0)[None]
+    b = W.gate_bias(cfg, 0)
+    idx, w = O.gate_topk(x, None if b is None else b[None], **cfg.gate)
+    cand = W.candidates(cfg, 0)
+    for c in (0, 2 if cand.shape[0] > 2 else 1):
+        kept, _ = O.prune(idx, w, cand[None, c], W.dev_node(cfg), cfg.taus[-1], cost_inter=cfg.cost_inter)
+        check_rows(idx[0], None, cand[c], cfg.D, tag=f"{name} cand{c} ")
+        check_rows(idx[0], kept[0], cand[c], cfg.D, tag=f"{name} cand{c} pruned ")
+
+
+@pytest.mark.parametrize("T,E,k,D", [(0, 16, 2, 4), (1, 16, 2, 4), (255, 8, 8, 1), (257, 64, 16, 64), (5000, 1024, 16, 64),
+                                     (70001, 40, 3, 7), (1000, 33, 1, 5)])
+def test_dispatch_rows_ragged_and_edges(T, E, k, D):
+    rng = np.random.default_rng(T + E)
+    idx = (np.stack([rng.choice(E, k, replace=False) for _ in range(T)]) if T else np.zeros((0, k))).astype(np.int32)
+    pi = rng.integers(0, D, E).astype(np.int32)
+    check_rows(idx, None, pi, D, tag="all ")
+    check_rows(idx, (rng.random((T, k)) < 0.5).astype(np.uint8), pi, D, tag="half ")
+    check_rows(idx, np.zeros((T, k), np.uint8), pi, D, tag="none ")
+
+
+def test_dispatch_rows_kernel_time():
+    cfg = W.CONFIGS["target"]
+    x = W.logits(cfg, 0)[None]
+    idx, _ = O.gate_topk(x, None, **cfg.gate)
+    di, dp = dev(idx[0]), dev(W.candidates(cfg, 0)[0])
+    ws = cap.workspace(cap.CALL_DISPATCH_ROWS, 1, cfg.T, cfg.E, cfg.k, cfg.D, 0)
+    cap.dispatch_rows(di, None, dp, cfg.D, ws=ws)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(20):
+        cap.dispatch_rows(di, None, dp, cfg.D, ws=ws)
+    b.record()
+    torch.cuda.synchronize()
+    print(f"cap_dispatch_rows target: T={cfg.T} k={cfg.k} D={cfg.D}: {a.elapsed_time(b) / 20 * 1e3:.1f} us per call")
