@@ -379,6 +379,24 @@ def run_cap(args, cfg, W):
     torch.cuda.synchronize()
     us_place = ev6.elapsed_time(ev7) / 10 * 1e3
 
+    def time_us(fn, n=10):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(n):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n * 1e3
+
+    maps0 = d_sets[0][2]
+    us_obj = time_us(lambda: cap.pairwise_objective(pipe.fb.counts, pipe.fb.coact, maps0, pipe.topo))
+    ws_rows = cap.workspace(cap.CALL_DISPATCH_ROWS, 1, T, E, k, D, 0, device=dev)
+    pi0 = maps0[0, 0].contiguous()
+    us_rows = time_us(lambda: cap.dispatch_rows(pipe.fb.idx[0], pipe.kept[0], pi0, D, ws=ws_rows))
+
     if world > 1:
         tt = torch.tensor([ms, ms_e2e], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
@@ -420,7 +438,12 @@ def run_cap(args, cfg, W):
         out["next"] = {"coact_placement": {
             "us_per_call": us_place, "layers": L, "greedy_steps_per_layer": (E - D) + (D - cfg.N),
             "what": "cap_coact_placement (P:L106-144, L148, L162-164) on the step's counts / coact; latency-bound "
-                    "sequential greedy, one CTA per layer; not part of `value`"}}
+                    "sequential greedy, one CTA per layer; not part of `value`"},
+            "pairwise_objective": {"us_per_call": us_obj, "candidates": P, "what": "cap_pairwise_objective (Eq. 2-3) "
+                                   "on the step's counts / coact and its P candidate maps"},
+            "dispatch_rows": {"us_per_call": us_rows, "what": "cap_dispatch_rows (P:L58, Fig. 2) for layer 0 under "
+                              "candidate 0 with the step's pruning mask; three direct launches through the binding, "
+                              "output tensors allocated per call"}}
         if not args.no_cpu_baseline:
             out["cpu_baseline"] = time_oracle(cfg, W, args.cpu_seconds)
         print(json.dumps(out))

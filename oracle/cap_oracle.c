@@ -676,3 +676,77 @@ int capo_dispatch_rows(const int32_t *idx, const uint8_t *kept, int64_t T, int32
     row_offsets[D] = n;
     return CAPO_OK;
 }
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-2  the Adjustment Approach: "We start from
+ * the communication-oriented placement ... and iteratively refine it through
+ * expert swaps.  In each adjustment step, we swap a pair of experts between
+ * high-load and low-load devices to reduce load imbalance while preserving as
+ * much co-activation locality as possible."  The paper gives no selection
+ * rule: PARITY UNPINNED AGAINST THE PAPER; the rule below is reading R27 and
+ * the pins check it against its own stated properties and a hand example.
+ *   load L_d = sum of n_e over the experts on d (R6, load_pairs);
+ *   hot = device with the largest load, cold = with the smallest (ties -> lower id);
+ *   candidates: a on hot, b on cold with 0 < n_a - n_b < L_hot - L_cold (both
+ *     devices end strictly below L_hot: the imbalance cannot rise);
+ *   choose the candidate with the smallest locality loss
+ *     loss = aff(a, hot\a) + aff(b, cold\b) - aff(a, cold\b) - aff(b, hot\a),
+ *     aff(x, S) = sum_{v in S} C_xv (integer co-activation counts, exact),
+ *     ties -> lower a, then lower b;
+ *   no candidate -> stop (the remaining spectrum entries repeat the last map).
+ * expert_dev0 [L][E]; spectrum [L][S][E] = the map after each step; n_done [L];
+ * swaps [L][S][2] = (a, b) of each step, -1 after the stop.
+ * ------------------------------------------------------------------------- */
+int capo_adjust_spectrum(const int64_t *counts, const int32_t *coact, int32_t L, int32_t E,
+                         int32_t D, const int32_t *expert_dev0, int32_t S, int32_t *spectrum,
+                         int32_t *n_done, int32_t *swaps)
+{
+    if (L < 0 || E < 1 || D < 1 || S < 0) return CAPO_EINVAL;
+    int32_t *pi = (int32_t *)malloc(sizeof(int32_t) * (size_t)E);
+    int64_t *load = (int64_t *)malloc(sizeof(int64_t) * (size_t)D);
+    for (int32_t l = 0; l < L; ++l) {
+        const int64_t *n = counts + (size_t)l * E;
+        const int32_t *C = coact + (size_t)l * E * E;
+        memcpy(pi, expert_dev0 + (size_t)l * E, sizeof(int32_t) * (size_t)E);
+        int32_t done = S, stopped = 0;
+        for (int32_t s = 0; s < S; ++s) {
+            int32_t besta = -1, bestb = -1;
+            if (!stopped) {
+                for (int32_t d = 0; d < D; ++d) load[d] = 0;
+                for (int32_t e = 0; e < E; ++e) load[pi[e]] += n[e];
+                int32_t hot = 0, cold = 0;
+                for (int32_t d = 1; d < D; ++d) {
+                    if (load[d] > load[hot]) hot = d;
+                    if (load[d] < load[cold]) cold = d;
+                }
+                int64_t bestloss = 0;
+                for (int32_t a = 0; a < E; ++a) {
+                    if (pi[a] != hot) continue;
+                    for (int32_t b = 0; b < E; ++b) {
+                        if (pi[b] != cold || hot == cold) continue;
+                        int64_t delta = n[a] - n[b];
+                        if (delta <= 0 || delta >= load[hot] - load[cold]) continue;
+                        int64_t loss = 0;
+                        for (int32_t v = 0; v < E; ++v) {
+                            if (pi[v] == hot && v != a)
+                                loss += (int64_t)C[(size_t)a * E + v] - (int64_t)C[(size_t)b * E + v];
+                            if (pi[v] == cold && v != b)
+                                loss += (int64_t)C[(size_t)b * E + v] - (int64_t)C[(size_t)a * E + v];
+                        }
+                        if (besta < 0 || loss < bestloss) { besta = a; bestb = b; bestloss = loss; }
+                    }
+                }
+                if (besta < 0) { stopped = 1; done = s; }
+                else { pi[besta] = cold; pi[bestb] = hot; }
+            }
+            memcpy(spectrum + ((size_t)l * S + s) * E, pi, sizeof(int32_t) * (size_t)E);
+            if (swaps) {
+                swaps[((size_t)l * S + s) * 2] = besta;
+                swaps[((size_t)l * S + s) * 2 + 1] = bestb;
+            }
+        }
+        if (n_done) n_done[l] = done;
+    }
+    free(pi); free(load);
+    return CAPO_OK;
+}

@@ -226,3 +226,20 @@ def dispatch_rows(idx, expert_dev, D, *, kept=None):
     if rc != 0:
         raise ValueError(f"capo_dispatch_rows -> {rc}")
     return rows[: int(offsets[D])], offsets, pair_row
+
+
+def adjust_spectrum(counts, coact, expert_dev0, *, D, S):
+    """NEXT-2: S swap steps of the Adjustment Approach (reading R27).  expert_dev0 [L,E] ->
+    (spectrum [L,S,E], n_done [L], swaps [L,S,2])."""
+    counts = _c(counts, np.int64)
+    coact = _c(coact, np.int32)
+    expert_dev0 = _c(expert_dev0, np.int32)
+    L, E = expert_dev0.shape
+    spectrum = np.empty((L, S, E), np.int32)
+    n_done = np.empty((L,), np.int32)
+    swaps = np.empty((L, S, 2), np.int32)
+    rc = lib().capo_adjust_spectrum(_p(counts), _p(coact), C.c_int32(L), C.c_int32(E), C.c_int32(D),
+                                    _p(expert_dev0), C.c_int32(S), _p(spectrum), _p(n_done), _p(swaps))
+    if rc != 0:
+        raise ValueError(f"capo_adjust_spectrum -> {rc}")
+    return spectrum, n_done, swaps

@@ -295,3 +295,88 @@ def test_dispatch_rows_vs_python_sets_and_s3(oracle):
                     assert off[d] <= pr[i] < off[d + 1] and rows[pr[i]] == t
     rows, off, pr = oracle.dispatch_rows(idx[:0], pi, D)
     assert rows.size == 0 and off.tolist() == [0] * (D + 1)
+
+
+# ------------------------------------------------------------------ NEXT-2: adjustment spectrum (R27)
+def _sym(E, pairs):
+    Cm = np.zeros((E, E), np.int32)
+    for (i, j), v in pairs.items():
+        Cm[i, j] = Cm[j, i] = v
+    return Cm
+
+
+def test_adjust_hand_example(oracle):
+    """E=6, D=2, pi0 = [0,0,0,1,1,1], n = [9,5,4,1,2,3] (loads 18 / 6).  By hand (R27):
+    step 1: all nine pairs are candidates; losses: (2,3) = 2+2-0-0 = 4 is the smallest -> swap 2,3
+            (loads 15 / 9);
+    step 2: candidates (0,2) d=5, (1,2) d=1, (1,4) d=3, (1,5) d=2; losses 3, 3, 8, 8 -> tie -> (0,2)
+            (loads 10 / 14);
+    step 3: hot = 1; candidates (4,3) d=1, (5,3) d=2; losses 5, 5 -> (4,3) (loads 11 / 13);
+    step 4: hot = 1 {0,3,5}, cold = 0 {1,2,4}, gap 2: only (5,4) has 0 < d=1 < 2 -> swap (loads 12 / 12);
+    step 5: equal loads -> stop."""
+    n = np.array([[9, 5, 4, 1, 2, 3]], np.int64)
+    Cm = _sym(6, {(0, 1): 6, (0, 2): 1, (1, 2): 1, (3, 4): 1, (3, 5): 1, (4, 5): 4, (2, 3): 2})[None]
+    spec, done, sw = oracle.adjust_spectrum(n, Cm, np.array([[0, 0, 0, 1, 1, 1]], np.int32), D=2, S=6)
+    assert sw[0, :5].tolist() == [[2, 3], [0, 2], [4, 3], [5, 4], [-1, -1]]
+    assert spec[0, 0].tolist() == [0, 0, 1, 0, 1, 1]
+    assert spec[0, 1].tolist() == [1, 0, 0, 0, 1, 1]
+    assert spec[0, 2].tolist() == [1, 0, 0, 1, 0, 1]
+    assert spec[0, 3].tolist() == [1, 0, 0, 1, 1, 0]
+    assert spec[0, 4].tolist() == spec[0, 3].tolist() == spec[0, 5].tolist() and done[0] == 4
+
+
+def test_adjust_properties_and_python_replay(oracle):
+    """Random traces: every step swaps one expert of the then-hottest device with one of the
+    then-coldest, device sizes never change, the maximum load never rises, and a set-based Python
+    replay of R27 takes the same decisions."""
+    rng = np.random.default_rng(9)
+    E, k, T, D, S = 24, 4, 400, 4, 12
+    idx = np.stack([rng.choice(E, k, replace=False, p=np.arange(1, E + 1) / (E * (E + 1) / 2))
+                    for _ in range(T)]).astype(np.int32)[None]
+    cnt, C = oracle.coactivation(idx, E=E)
+    pi0 = (np.arange(E) // (E // D)).astype(np.int32)
+    spec, done, sw = oracle.adjust_spectrum(cnt, C, pi0[None], D=D, S=S)
+    n, Cm = cnt[0], C[0].astype(np.int64)
+    pi = pi0.copy()
+    prev_max = max(n[pi == d].sum() for d in range(D))
+    assert done[0] >= 2
+    for s in range(S):
+        load = [int(n[pi == d].sum()) for d in range(D)]
+        hot = max(range(D), key=lambda d: (load[d], -d))
+        cold = min(range(D), key=lambda d: (load[d], d))
+        best = None
+        for a in np.flatnonzero(pi == hot):
+            for b in np.flatnonzero(pi == cold):
+                dl = int(n[a] - n[b])
+                if hot == cold or not (0 < dl < load[hot] - load[cold]):
+                    continue
+                H = [v for v in np.flatnonzero(pi == hot) if v != a]
+                Cd = [v for v in np.flatnonzero(pi == cold) if v != b]
+                loss = int(Cm[a, H].sum() + Cm[b, Cd].sum() - Cm[a, Cd].sum() - Cm[b, H].sum())
+                if best is None or loss < best[0]:
+                    best = (loss, int(a), int(b))
+        if best is None:
+            assert done[0] == s and sw[0, s].tolist() == [-1, -1]
+            break
+        assert sw[0, s].tolist() == [best[1], best[2]]
+        pi[best[1]], pi[best[2]] = cold, hot
+        assert spec[0, s].tolist() == pi.tolist()
+        assert np.bincount(pi, minlength=D).tolist() == [E // D] * D
+        new_max = max(n[pi == d].sum() for d in range(D))
+        assert new_max <= prev_max
+        prev_max = new_max
+
+
+def test_adjust_trades_communication_for_balance(oracle):
+    """from the Algorithm 1 placement the spectrum moves toward lower imbalance at the
+    cost of more devices per token."""
+    cfg = W.CONFIGS["qwen3"].with_(T=8192)
+    idx, _ = oracle.gate_topk(W.logits(cfg, 0)[None], k=cfg.k)
+    cnt, C = oracle.coactivation(idx, E=cfg.E)
+    _, _, ed, _ = oracle.coact_placement(cnt, C, D=cfg.D, N=cfg.N)
+    spec, done, _ = oracle.adjust_spectrum(cnt, C, ed, D=cfg.D, S=6)
+    maps = np.concatenate([ed[:, None], spec], 1)
+    ev = oracle.eval_placements(idx, maps, W.dev_node(cfg))
+    assert done[0] == 6
+    assert np.all(np.diff(ev.imbalance[0]) <= 1e-12) and ev.imbalance[0, -1] < ev.imbalance[0, 0] - 0.02
+    assert ev.dev_visits[0, -1] >= ev.dev_visits[0, 0]
