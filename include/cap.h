@@ -179,6 +179,26 @@ int cap_coact_placement(const int64_t *counts, const int32_t *coact, int32_t L, 
                         int32_t *group_node, int32_t *expert_dev, void *ws, size_t ws_bytes,
                         void *stream);
 
+/* Adjustment Approach.  P:L194: "We start from the communication-oriented placement
+ * produced by the Placement Approach and iteratively refine it through expert swaps.  In each adjustment
+ * step, we swap a pair of experts between high-load and low-load devices to reduce load imbalance while
+ * preserving as much co-activation locality as possible."  The paper states no selection rule; this call
+ * implements reading R27 of DESIGN.md (parity unpinned against the paper, exact against the oracle):
+ * load L_d = sum of counts over the experts on d; hot / cold = the device with the largest / smallest load
+ * (ties to the lower id); candidates = (a on hot, b on cold) with 0 < n_a - n_b < L_hot - L_cold; the
+ * candidate with the smallest loss = aff(a, hot\a) + aff(b, cold\b) - aff(a, cold\b) - aff(b, hot\a),
+ * aff(x, S) = sum_{v in S} coact[x][v] (int64), is swapped (ties to the lower a, then the lower b); no
+ * candidate stops the layer.
+ *   expert_dev0 [L][E]: the starting maps (values clamped to [0, D)); S: number of steps;
+ *   spectrum [L][S][E]: the map after each step (after a stop the last map is repeated) -- directly usable
+ *     as the candidate array of cap_eval_placements / cap_pairwise_objective with P = S;
+ *   n_done [L] int32, nullable: steps performed before the stop (S if none);
+ *   swaps [L][S][2] int32, nullable: (a, b) of each step, (-1, -1) from the stop on.
+ * counts / coact as written by cap_coactivation.  No workspace.  S = 0 or L = 0: nothing is written. */
+int cap_adjust_spectrum(const int64_t *counts, const int32_t *coact, int32_t L, int32_t E, int32_t D,
+                        const int32_t *expert_dev0, int32_t S, int32_t *spectrum, int32_t *n_done,
+                        int32_t *swaps, void *stream);
+
 /* Device-centric dispatch rows.  P:L58 (sec. II-C, Fig. 2): "each token is sent once
  * to each device that hosts activated experts" and aggregated there -- one row per (token, destination
  * device) instead of cap_dispatch_layout's one entry per (token, expert) pair (R18).
@@ -233,7 +253,7 @@ int64_t cap_launch_count(void);
 /* Profiling aid (not part of the data path; not thread-safe).  cap_kernel_timer_arm(tag, slot)
  * makes the next launch of the kernel tagged `tag` ("gate_topk", "coact", "eval", "eval_finalize",
  * "eval_table", "eval_decode", "masked_counts", "prune", "dispatch_hist", "dispatch_scan",
- * "dispatch_scatter", "trace_fused", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter")
+ * "dispatch_scatter", "trace_fused", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
  * record a CUDA event pair, owned by the library, around itself on its stream; up to 128 arms
  * may be pending, slot in [0,4096).  cap_kernel_timer_ms(slot) returns the elapsed device time
  * in milliseconds once that work has completed (the caller synchronises), or -1. */

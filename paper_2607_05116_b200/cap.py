@@ -17,12 +17,12 @@ LIB_PATH = os.path.join(_HERE, "libcap_b200.so")
 OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
-           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_workspace_bytes",
+           "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_adjust_spectrum", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
-               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter")
+               "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
 
 
 class GateCfg(C.Structure):
@@ -80,6 +80,7 @@ def lib():
         L.cap_validate_placements.argtypes = [vp, i32, i32, i32, i32, vp]
         L.cap_pairwise_objective.argtypes = [vp, vp, i32, i32, vp, i32, C.POINTER(Topology), C.c_double, vp, vp, vp,
                                              vp, vp]
+        L.cap_adjust_spectrum.argtypes = [vp, vp, i32, i32, i32, vp, i32, vp, vp, vp, vp]
         L.cap_dispatch_rows.argtypes = [vp, vp, i64, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
         L.cap_coact_placement.argtypes = [vp, vp, i32, i32, i32, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         L.cap_profile_fused_kernel.argtypes = [C.POINTER(C.c_void_p), i32, i32, i32, i64, C.POINTER(GateCfg), vp, vp,
@@ -256,6 +257,21 @@ def coact_placement(counts, coact, D, N, rnd=None, want_p=False, ws=None):
                                    _ptr(expert_dev), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_coact_placement")
     return expert_group, group_node, expert_dev, p
+
+
+def adjust_spectrum(counts, coact, expert_dev0, D, S):
+    """cap_adjust_spectrum: S swap steps of the Adjustment Approach.  expert_dev0 [L,E] int32 ->
+    (spectrum [L,S,E], n_done [L], swaps [L,S,2])."""
+    L, E = expert_dev0.shape
+    dev = counts.device
+    spectrum = torch.empty((L, S, E), dtype=torch.int32, device=dev)
+    n_done = torch.empty((L,), dtype=torch.int32, device=dev)
+    swaps = torch.empty((L, S, 2), dtype=torch.int32, device=dev)
+    rc = lib().cap_adjust_spectrum(_ptr(counts, torch.int64), _ptr(coact, torch.int32), L, E, D,
+                                   _ptr(expert_dev0, torch.int32), S, _ptr(spectrum), _ptr(n_done), _ptr(swaps),
+                                   _stream())
+    _check(rc, "cap_adjust_spectrum")
+    return spectrum, n_done, swaps
 
 
 def dispatch_rows(idx, kept, expert_dev, D, want_pair_row=True, ws=None):

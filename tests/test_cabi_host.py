@@ -68,6 +68,8 @@ def test_host_side_einval_without_gpu(lib):
                                       None) == cap.EINVAL                                 # D = 0
     assert lib.cap_dispatch_rows(None, None, 4, 2, 16, None, 65, None, None, None, None, 0, None) == cap.EINVAL
     assert lib.cap_dispatch_rows(None, None, 4, 17, 16, None, 4, None, None, None, None, 0, None) == cap.EINVAL
+    assert lib.cap_adjust_spectrum(None, None, 1, 16, 65, None, 3, None, None, None, None) == cap.EINVAL
+    assert lib.cap_adjust_spectrum(None, None, 1, 16, 4, None, 3, None, None, None, None) == cap.EINVAL   # NULL arrays
     assert lib.cap_workspace_bytes(cap.CALL_DISPATCH_ROWS, 1, 65536, 128, 8, 16, 0) >= 256 * 16 * 4
     assert lib.cap_workspace_bytes(cap.CALL_COACT_PLACEMENT, 2, 0, 128, 1, 16, 0) >= 2 * 8 * (128 * 128 + 16 * 128 + 256)
 

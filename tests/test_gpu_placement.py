@@ -235,3 +235,55 @@ def test_dispatch_rows_kernel_time():
     b.record()
     torch.cuda.synchronize()
     print(f"cap_dispatch_rows target: T={cfg.T} k={cfg.k} D={cfg.D}: {a.elapsed_time(b) / 20 * 1e3:.1f} us per call")
+
+
+# ------------------------------------------------------------------ cap_adjust_spectrum (R27)
+def check_adjust(cnt, C, pi0, D, S, tag=""):
+    ref = O.adjust_spectrum(cnt, C, pi0, D=D, S=S)
+    got = cap.adjust_spectrum(dev(cnt), dev(C), dev(pi0), D, S)
+    torch.cuda.synchronize()
+    for name, g, r in zip(("spectrum", "n_done", "swaps"), got, ref):
+        np.testing.assert_array_equal(host(g), r, err_msg=tag + name)
+    return ref
+
+
+@pytest.mark.parametrize("name,layers,T,S", [("tiny", (0,), 4096, 7), ("qwen3", (0, 17, 47), 16384, 7),
+                                             ("target", (0,), 65536, 12), ("dsv3", (0, 31), 8192, 7),
+                                             ("stress", (0,), 16384, 7)])
+def test_adjust_on_baseline_configs(name, layers, T, S):
+    """The paper's pipeline: Algorithm 1's placement, then the swap spectrum (7 placements)."""
+    cfg = W.CONFIGS[name]
+    _, _, idx, cnt, C = trace_stats(cfg, layers, T)
+    _, _, ed, _ = O.coact_placement(cnt, C, D=cfg.D, N=cfg.N)
+    ref = check_adjust(cnt, C, ed, cfg.D, S, tag=name + " ")
+    seq = np.tile((np.arange(cfg.E) // (cfg.E // cfg.D)).astype(np.int32), (len(layers), 1))
+    check_adjust(cnt, C, seq, cfg.D, S, tag=name + " from sequential ")
+    assert np.all(ref[1] >= 1)
+
+
+@pytest.mark.parametrize("E,D,k,T,S", [(6, 2, 2, 20, 8), (24, 4, 4, 400, 40), (64, 64, 4, 100, 5), (33, 1, 3, 50, 3),
+                                       (1024, 64, 16, 300, 6), (100, 7, 5, 200, 10)])
+def test_adjust_shapes_stops_and_unbalanced_maps(E, D, k, T, S):
+    rng = np.random.default_rng(E + S)
+    L = 2
+    idx = np.stack([[rng.choice(E, k, replace=False) for _ in range(T)] for _ in range(L)]).astype(np.int32)
+    cnt, C = O.coactivation(idx, E=E)
+    pi0 = rng.integers(0, D, (L, E)).astype(np.int32)          # arbitrary (unbalanced) maps
+    check_adjust(cnt, C, pi0, D, S, tag=f"E{E} D{D} ")
+
+
+def test_adjust_kernel_time():
+    cfg = W.CONFIGS["qwen3"]
+    _, _, _, cnt, C = trace_stats(cfg, (0,), 8192)
+    L = 48
+    _, _, ed, _ = O.coact_placement(cnt, C, D=cfg.D, N=cfg.N)
+    dc, dC, de = dev(np.repeat(cnt, L, 0)), dev(np.repeat(C, L, 0)), dev(np.repeat(ed, L, 0))
+    cap.adjust_spectrum(dc, dC, de, cfg.D, 7)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(5):
+        cap.adjust_spectrum(dc, dC, de, cfg.D, 7)
+    b.record()
+    torch.cuda.synchronize()
+    print(f"cap_adjust_spectrum qwen3: L={L} E={cfg.E} D={cfg.D} S=7: {a.elapsed_time(b) / 5 * 1e3:.1f} us per call")
