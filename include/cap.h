@@ -164,7 +164,9 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
  * best score takes the r-th smallest unassigned expert, r = rnd[step] mod |U|); P:L162-164 applies
  * it again to the device groups with strength W[a][b] = sum_{i in G[a]} sum_{j in G[b]} p_ij
  * (ascending i outer, ascending j inner, R24) to form N node groups.
- *   counts [L][E] int64, coact [L][E][E] int32: as written by cap_coactivation / cap_trace_fused.
+ *   counts [L][E] int64, coact [L][E][E] int32: as written by cap_coactivation / cap_trace_fused; coact
+ *     must be symmetric, as those calls write it (the kernel reads rows where the definition reads
+ *     columns); a non-symmetric matrix gives an undefined but memory-safe result.
  *   rnd [L][E + D] uint32, nullable (= zeros): stage 1 growth step s reads rnd[s], stage 2 step s
  *     reads rnd[E + s]; only consumed on the zero-score branch (line 12 of the listing).
  *   p_out [L][E][E] fp64, nullable: the probabilities.

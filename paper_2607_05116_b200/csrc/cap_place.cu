@@ -43,13 +43,21 @@ struct PlaceSmem {
     int pick;
 };
 
+// File-scope shared state: every access below is then a direct shared-memory access.  With the struct and
+// the score rows passed as pointers the compiler formed generic addresses, which costs a read of the CTA's
+// cluster rank (S2R SR_CgaCtaId) inside every greedy step.
+__shared__ PlaceSmem sm;
+extern __shared__ double sscore[];
+
 // Algorithm 1 on n units and k groups.  MT[m * n + e] = M[e][m] (so that a step reads one
 // contiguous row); score is [k][n] scratch in global memory, each element touched by one thread.
 // The scores of groups g < gs live in shared memory (sscore), the rest in global memory (score):
 // a global store does not allocate in L1, so a global score costs an L2 round trip per step.
-__device__ __forceinline__ void alg1(int n, int k, const double *MT, double *score, double *sscore, int gs, const uint32_t *rnd,
-                     int *grp, int *ord, PlaceSmem &sm)
+template <bool STAGE2>
+__device__ __forceinline__ void alg1(int n, int k, const double *MT, double *score, int gs, const uint32_t *rnd)
 {
+    int *const grp = STAGE2 ? sm.grp2 : sm.grp;
+    int *const ord = STAGE2 ? sm.ord2 : sm.ord;
     const int e = threadIdx.x, lane = e & 31, wid = e >> 5, nw = blockDim.x >> 5;
     double d = 0.0;
     if (e < n) {                                              // line 1: ascending j, j != e
@@ -153,8 +161,6 @@ place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coa
              const uint32_t *__restrict__ rnd, double *p_out, double *wsP, double *wsS, double *wsW,
              int32_t *expert_group, int32_t *group_node, int32_t *expert_dev, int gs1)
 {
-    __shared__ PlaceSmem sm;
-    extern __shared__ double sscore[];
     const int l = blockIdx.x, tid = threadIdx.x;
     const int64_t *n = counts + (size_t)l * E;
     const int32_t *C = coact + (size_t)l * E * E;
@@ -174,10 +180,10 @@ place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coa
         long long den = sm.cnt[i] + sm.cnt[j] - c;
         double v = (i == j || den == 0) ? 0.0 : __ddiv_rn((double)c, (double)den);
         if (po) po[q] = v;
-        pT[(size_t)j * E + i] = v;
+        pT[q] = v;                           // coact is symmetric (cap.h), so p is its own transpose
     }
     __syncthreads();
-    alg1(E, D, pT, score, sscore, gs1, r1, sm.grp, sm.ord, sm);
+    alg1<false>(E, D, pT, score, gs1, r1);
 
     // stage 2 (R24): W[a][b] = sum over i in G[a] (ascending), j in G[b] (ascending) of p_ij
     const int m = E / D;
@@ -193,12 +199,13 @@ place_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__ coa
         if (a != b)
             for (int x = 0; x < m; ++x) {
                 int i = sm.members[a * m + x];
+#pragma unroll 8
                 for (int y = 0; y < m; ++y) s += pT[(size_t)sm.members[b * m + y] * E + i];
             }
         WT[(size_t)b * D + a] = s;
     }
     __syncthreads();
-    alg1(D, N, WT, score, sscore, N, r1 ? r1 + E : nullptr, sm.grp2, sm.ord2, sm);
+    alg1<true>(D, N, WT, score, N, r1 ? r1 + E : nullptr);
 
     if (tid < E) {
         int g = sm.grp[tid];
