@@ -58,7 +58,7 @@ __device__ __forceinline__ void alg1(int n, int k, const double *MT, double *sco
 {
     int *const grp = STAGE2 ? sm.grp2 : sm.grp;
     int *const ord = STAGE2 ? sm.ord2 : sm.ord;
-    const int e = threadIdx.x, lane = e & 31, wid = e >> 5, nw = blockDim.x >> 5;
+    const int e = threadIdx.x, lane = e & 31, wid = e >> 5;
     double d = 0.0;
     if (e < n) {                                              // line 1: ascending j, j != e
 #pragma unroll 16
@@ -99,8 +99,12 @@ __device__ __forceinline__ void alg1(int n, int k, const double *MT, double *sco
     const int depth = k >= 5 ? 4 : (k >= 2 ? 1 : 0);
     double m0 = 0.0, m1 = 0.0, m2 = 0.0, m3 = 0.0;
     int g0 = -1, g1 = -1, g2 = -1, g3 = -1;                   // oldest first
-    for (int step = 0; step < steps; ++step) {                // line 8
-        const int g = step % k, par = step & 1;               // line 14
+    // only the warps that own units take part in the greedy loop (named barrier 1 over nwa warps); the
+    // others wait at the __syncthreads() after it
+    const int nwa = (n + 31) >> 5;
+    int g = 0;
+    for (int step = 0; wid < nwa && step < steps; ++step, g = (g + 1 == k) ? 0 : g + 1) {   // lines 8, 14
+        const int par = step & 1;
         double v = 0.0;
         if (inU) v = g < gs ? sscore[g * n + e] : score[(size_t)g * n + e];
         int mh, wh;
@@ -111,18 +115,18 @@ __device__ __forceinline__ void alg1(int n, int k, const double *MT, double *sco
             sm.pl[par][wid] = ml;
             sm.pe[par][wid] = (wid << 5) + src;
         }
-        __syncthreads();
-        int src2 = warp_argmax(lane < nw ? sm.ph[par][lane] : -1, lane < nw ? sm.pl[par][lane] : 0u, &wh, &wl);
+        asm volatile("bar.sync 1, %0;" ::"r"(nwa * 32) : "memory");
+        int src2 = warp_argmax(lane < nwa ? sm.ph[par][lane] : -1, lane < nwa ? sm.pl[par][lane] : 0u, &wh, &wl);
         int pick = sm.pe[par][src2];
         if (wh == 0 && wl == 0u) {                            // lines 11-12 (block-uniform branch)
             uint32_t r = (rnd ? rnd[step] : 0u) % (uint32_t)(steps - step);
             unsigned bal = __ballot_sync(0xffffffffu, inU);
             if (lane == 0) sm.wcnt[wid] = __popc(bal);
-            __syncthreads();
+            asm volatile("bar.sync 1, %0;" ::"r"(nwa * 32) : "memory");
             int pre = __popc(bal & ((1u << lane) - 1u));
             for (int w = 0; w < wid; ++w) pre += sm.wcnt[w];
             if (inU && pre == (int)r) sm.pick = e;
-            __syncthreads();
+            asm volatile("bar.sync 1, %0;" ::"r"(nwa * 32) : "memory");
             pick = sm.pick;
         }
         if (e == pick) {                                      // line 13
