@@ -44,12 +44,24 @@ objective_kernel(const int64_t *__restrict__ counts, const int32_t *__restrict__
         ac[c] = 0;
         ap[c] = 0.0;
     }
-    // latency-bound L2 reads: the loads of four iterations are issued together
+    // Upper triangle only, folded so that every folded row has E - 1 entries: folded row r holds row r's
+    // E - 1 - r entries (j > r) followed by row E - 1 - r's r entries; contiguous runs, so the reads stay
+    // coalesced.  Latency-bound L2 reads: the loads of four iterations are issued together.
+    const int W1 = E - 1, R = (E + 1) >> 1;
 #pragma unroll 4
-    for (int q = tid; q < E * E; q += OBJ_THREADS) {
-        long long c = C[q];
-        int i = q / E, j = q - i * E;
-        if (j <= i || c == 0) continue;      // upper triangle; c = 0 means p_ij = 0 as well
+    for (int q = tid; q < R * W1; q += OBJ_THREADS) {
+        int r = q / W1, cc = q - r * W1;
+        int i, j;
+        if (cc < W1 - r) {
+            i = r;
+            j = r + 1 + cc;
+        } else {
+            i = W1 - r;
+            j = i + 1 + (cc - (W1 - r));
+        }
+        bool ok = cc < W1 - r || 2 * r != W1;   // odd E: the middle row is its own partner, count it once
+        long long c = ok ? C[(size_t)i * E + j] : 0;
+        if (c == 0) continue;                // c = 0 means p_ij = 0 as well
         long long den = cnt[i] + cnt[j] - c;
         double pij = den == 0 ? 0.0 : __ddiv_rn((double)c, (double)den);
 #pragma unroll
