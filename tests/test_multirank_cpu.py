@@ -37,8 +37,17 @@ def _worker(rank, world, port, q):
               ev.remote_node, ev.cost, ev.bytes, ev.load_pairs, ev.recv_tokens)]
     for t in parts:
         dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    # the consumers of the merged statistics (Algorithm 1 placement, adjustment spectrum) are
+    # deterministic: every rank derives the same placement from the all-reduced counts / coact
+    g, gn, ed, _ = O.coact_placement(parts[0].numpy(), parts[1].numpy().astype(np.int32), D=cfg.D, N=cfg.N)
+    spec, _, _ = O.adjust_spectrum(parts[0].numpy(), parts[1].numpy().astype(np.int32), ed, D=cfg.D, S=3)
+    mine = torch.from_numpy(np.concatenate([ed.ravel(), spec.ravel()]).astype(np.int64))
+    lo_t, hi_t = mine.clone(), mine.clone()
+    dist.all_reduce(lo_t, op=dist.ReduceOp.MIN)
+    dist.all_reduce(hi_t, op=dist.ReduceOp.MAX)
+    assert torch.equal(lo_t, hi_t)
     if rank == 0:
-        q.put([t.numpy() for t in parts])
+        q.put([t.numpy() for t in parts] + [mine.numpy()])
     dist.barrier()
     dist.destroy_process_group()
 
@@ -64,5 +73,9 @@ def test_two_rank_shards_sum_to_whole():
     for p in procs:
         p.join(timeout=60)
         assert p.exitcode == 0
+    _, _, ed, _ = O.coact_placement(counts, coact, D=cfg.D, N=cfg.N)
+    spec, _, _ = O.adjust_spectrum(counts, coact, ed, D=cfg.D, S=3)
+    ref.append(np.concatenate([ed.ravel(), spec.ravel()]))
+    assert len(got) == len(ref)
     for g, r in zip(got, ref):
         assert np.array_equal(g, np.asarray(r).astype(np.int64))
