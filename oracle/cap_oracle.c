@@ -5,7 +5,7 @@
  * per-token routing-trace pipeline (arXiv 2607.05116, "Communication-Aware
  * Placement and Pruning for Efficient Mixture-of-Experts Inference"), written
  * from the paper (P:Lnnn = /root/reference/PAPER.md line nnn) and from the
- * readings listed in DESIGN.md section 3 (R1..R21).  It shares no code, header,
+ * readings listed in DESIGN.md section 3 (R1..R27).  It shares no code, header,
  * table or helper with the CUDA path under paper_2607_05116_b200/csrc/ and
  * neither imports the other.  Only tests/, __graft_entry__.smoke() and the
  * cpu_baseline / --impl reference legs of bench.py may call it.
@@ -14,11 +14,21 @@
  * -ffp-contract=off matters: every fp32 step below is one IEEE operation, the
  * only fused operations are the explicit fmaf() calls in expS.
  *
- * Pins (tests/test_oracle_pins.py): every function here is pinned by something
- * other than itself -- closed forms, brute force, library routines, the
- * paper's Table III "Default" value.  No function is "parity unpinned"; the one
- * reading that cannot be pinned against the paper (which load definition the
- * paper's Table IV uses, R6) is handled by exporting both quantities.
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_placement_pins.py): every
+ * function here is pinned by something other than itself -- closed forms,
+ * brute force, library routines, hand-worked examples, the paper's Table III
+ * "Default" value.  PARITY UNPINNED: capo_adjust_spectrum only -- P:L194 states
+ * the goal of an adjustment step but no selection rule, so the rule is reading
+ * R27 of DESIGN.md; it is pinned against R27's own hand example and properties,
+ * not against the paper.  The one other reading that cannot be pinned against
+ * the paper (which load definition Table IV uses, R6) is handled by exporting
+ * both quantities.
+ *
+ * Functions: the five stages S1..S5 (capo_gate_topk, capo_coactivation,
+ * capo_eval_placements, capo_prune, capo_dispatch_layout) and the consumers of
+ * S2 in SURVEY.md 8(f): capo_coact_placement (p_ij + Algorithm 1),
+ * capo_adjust_spectrum, capo_pairwise_objective (Eq. 2-3, Eq. 5),
+ * capo_dispatch_rows (Fig. 2's one copy per device).
  *
  * All arrays are HOST pointers, row-major, layouts as in include/cap.h.
  */
