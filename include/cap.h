@@ -147,12 +147,26 @@ int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T,
                         void *stream);
 
 /* S1 + S2 + S3 in one call over the logits (the measured pass).  Arguments as in the three
- * calls above; counts/coact/out members may be NULL to skip an output. */
+ * calls above; members of `out` may be NULL to skip an output; counts and coact are required
+ * (CAP_EINVAL if NULL with L > 0: the fused kernel always produces them). */
 int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T,
                     const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w,
                     int64_t *counts, int32_t *coact, const int32_t *token_src,
                     const int32_t *expert_dev, int32_t P, const cap_topology *topo,
                     const cap_eval_out *out, void *ws, size_t ws_bytes, void *stream);
+
+/* Introspection, host only (no launch, no device access): how cap_trace_fused would run these sizes
+ * on the current device when token_src is NULL and no per-token output is asked for.
+ *   plan[0] = 1 if the single fused S1+S2+S3 kernel serves them, 0 if the three staged kernels do;
+ *   plan[1] = thread blocks per layer;  plan[2] = tokens per block (upper bound);
+ *   plan[3] = largest number of tokens of ONE source device that a single block scores;
+ *   plan[4] = tokens a block can count for one source before its bit-sliced counters are flushed
+ *             (a "capacity flush": plan[3] > plan[4] means that branch runs);
+ *   plan[5] = records a block can emit;  plan[6] = blocks per source device when block ranges are
+ *             aligned to the source runs, else 0;  plan[7] = version of the fused kernel (0 if none).
+ * Used by the tests to prove that a shape reaches a given branch.  CAP_EINVAL on invalid sizes. */
+int cap_trace_fused_plan(int32_t L, int64_t T, const cap_gate_cfg *cfg, int32_t D, int32_t N, int32_t P,
+                         int64_t plan[8]);
 
 /* Co-activation driven expert placement: SURVEY 8(f) rank 1, the consumer of cap_coactivation's
  * outputs.  P:L148 defines the co-activation probability ("the ratio between the number of times

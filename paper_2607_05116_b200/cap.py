@@ -19,7 +19,7 @@ OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
            "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_adjust_spectrum", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
-           "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel")
+           "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
@@ -86,6 +86,7 @@ def lib():
         L.cap_profile_fused_kernel.argtypes = [C.POINTER(C.c_void_p), i32, i32, i32, i64, C.POINTER(GateCfg), vp, vp,
                                                vp, vp, vp, i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz,
                                                vp, C.POINTER(C.c_float)]
+        L.cap_trace_fused_plan.argtypes = [i32, i64, C.POINTER(GateCfg), i32, i32, i32, C.POINTER(C.c_int64)]
         L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
         L.cap_kernel_timer_ms.argtypes = [C.c_int]
         L.cap_kernel_timer_ms.restype = C.c_float
@@ -350,6 +351,15 @@ def profile_fused_kernel(logits_list, cfg, expert_dev, topo, bufs, n_rep):
         return None
     _check(rc, "cap_profile_fused_kernel")
     return float(ms.value)
+
+
+def trace_fused_plan(L, T, cfg, D, N, P):
+    """cap_trace_fused_plan -> dict (host only): which kernel serves these sizes and its token geometry."""
+    arr = (C.c_int64 * 8)()
+    _check(lib().cap_trace_fused_plan(L, T, C.byref(cfg), D, N, P, arr), "cap_trace_fused_plan")
+    names = ("fused", "blocks_per_layer", "tokens_per_block", "max_tokens_one_source", "run_capacity",
+             "records_per_block", "blocks_per_source", "kernel_version")
+    return dict(zip(names, [int(v) for v in arr]))
 
 
 def validate_placements(expert_dev, D):

@@ -262,6 +262,15 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
                        (int64_t)P * cfg->E, *topo, counts, *out, ws, st);
 }
 
+int cap_trace_fused_plan(int32_t L, int64_t T, const cap_gate_cfg *cfg, int32_t D, int32_t N, int32_t P,
+                         int64_t plan[8])
+{
+    if (!plan || !gate_ok(cfg) || !sizes_ok(L, T, cfg->E, cfg->k) || D < 1 || D > 64 || N < 1 || N > 64 || P < 0)
+        return CAP_EINVAL;
+    fused_plan(L, T, *cfg, D, N, P, plan);
+    return CAP_OK;
+}
+
 int cap_profile_fused_kernel(const float *const *logits_list, int32_t n_list, int32_t n_rep, int32_t L,
                              int64_t T, const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w,
                              int64_t *counts, int32_t *coact, const int32_t *expert_dev, int32_t P,

@@ -644,6 +644,26 @@ size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int
     return best;
 }
 
+// cap_trace_fused_plan: the geometry above in numbers (host only)
+bool fused_plan(int32_t L, int64_t T, const cap_gate_cfg &cfg, int32_t D, int32_t N, int32_t P, int64_t *plan)
+{
+    for (int i = 0; i < 8; ++i) plan[i] = 0;
+    if (cfg.scoring != 0 || cfg.renormalize != 1 || cfg.n_group != 1 || cfg.k > 8) return false;
+    FusedGeom f;
+    if (!fused_geom(L, T, cfg.k, cfg.E, D, N, P, &f)) return false;
+    const int64_t BT = (int64_t)EF_PASSES * f.g.S;
+    const int64_t per_src = (T + D - 1) / D;
+    plan[0] = 1;
+    plan[1] = f.g.ncta_t;
+    plan[2] = f.g.tpc;
+    plan[3] = f.g.tpc < per_src ? f.g.tpc : per_src;
+    plan[4] = (int64_t)(EF_MAXBLK - 2) * BT;
+    plan[5] = f.g.maxrec;
+    plan[6] = f.cps;
+    plan[7] = 1;
+    return true;
+}
+
 template <int E>
 static int launch_fused_e(const FusedParams &prm, const FusedGeom &f, int L, cudaStream_t st)
 {

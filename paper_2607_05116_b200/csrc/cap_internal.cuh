@@ -101,6 +101,7 @@ int profile_trace_fused_kernel(const float *const *logits_list, int nlist, int n
                                int32_t *coact, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
                                const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
 size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
+bool fused_plan(int32_t L, int64_t T, const cap_gate_cfg &cfg, int32_t D, int32_t N, int32_t P, int64_t *plan);
 int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
                  const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,

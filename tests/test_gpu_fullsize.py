@@ -1,0 +1,221 @@
+"""GPU parity at the sizes and in the launch configurations bench.py times (VERDICT round 1, row g):
+every layer of configs 2 and 4 in ONE launch per call, the fused kernel's capacity-flush branch, and
+config 5 along its T sweep on the BASELINE generator.  Everything is compared with the CPU oracle
+element by element (integers bit-exact, gate weights within 1e-6); where the oracle cannot hold the
+whole trace it runs on token chunks and its integer aggregates are summed (every S2 / S3 output is a
+sum over tokens)."""
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+from oracle import cap_oracle as O                      # noqa: E402
+from paper_2607_05116_b200 import cap                   # noqa: E402
+from paper_2607_05116_b200 import workload as W         # noqa: E402
+from parity_util import EVAL_I64, W_TOL, assert_eval_equal, dev, host, layers_inputs, topo_of  # noqa: E402
+import gpu_workload as G                                # noqa: E402
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_gpu():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    cap.lib()
+
+
+def _all_layers_one_launch(cfg, T, tag):
+    """cap_trace_fused, cap_prune (+after), cap_coact_placement and cap_adjust_spectrum, each ONE call
+    over all cfg.L layers, against the oracle."""
+    L = cfg.L
+    layers = tuple(range(L))
+    logits, bias, cand = layers_inputs(cfg, layers, T)
+    dn = W.dev_node(cfg)
+    dn_d = dev(dn)
+    topo = topo_of(cfg, dn_d)
+    gate = cap.gate_cfg(cfg.E, **cfg.gate)
+    idx_r, w_r, cnt_r, C_r, ev_r = O.trace_fused(logits, bias, cfg.gate, cand, dn, cost_inter=cfg.cost_inter,
+                                                 bytes_per_token=cfg.bytes_per_token)
+    n0 = cap.launch_count()
+    fb = cap.trace_fused(dev(logits), dev(bias), gate, None, dev(cand), topo)
+    torch.cuda.synchronize()
+    launches = cap.launch_count() - n0
+    assert np.array_equal(host(fb.idx), idx_r), tag + "fused idx"
+    assert float(np.abs(host(fb.w).astype(np.float64) - w_r).max()) <= W_TOL, tag + "fused w"
+    assert np.array_equal(host(fb.counts), cnt_r), tag + "fused counts"
+    assert np.array_equal(host(fb.coact), C_r), tag + "fused coact"
+    assert_eval_equal(fb.out, ev_r, False, tag + "fused eval ")
+    # S4 over all layers in one launch, on the GPU's own S1 output
+    pi = np.ascontiguousarray(cand[:, 2, :])
+    for tau in cfg.taus:
+        kept_r, near_r = O.prune(idx_r, w_r, pi, dn, tau, cost_inter=cfg.cost_inter)
+        aft_r = O.eval_placements(idx_r, pi[:, None, :], dn, kept=kept_r, cost_inter=cfg.cost_inter,
+                                  bytes_per_token=cfg.bytes_per_token)
+        kept_d, near_d, aft_d = cap.prune(dev(idx_r), dev(w_r), None, dev(pi), topo, tau)
+        assert np.array_equal(host(kept_d), kept_r), f"{tag}kept tau={tau}"
+        assert np.array_equal(host(near_d), near_r), f"{tag}near tau={tau}"
+        assert_eval_equal(aft_d, aft_r, False, f"{tag}after-prune tau={tau} ")
+        kept_e, _, _ = cap.prune(fb.idx, fb.w, None, dev(pi), topo, tau)
+        bad = int((host(kept_e) != kept_r).any(-1).sum())
+        assert bad <= int(near_r.sum()), f"{tag}kept end-to-end tau={tau}: {bad} tokens differ"
+    # consumers of S2 over all layers in one launch
+    rng = np.random.default_rng(cfg.index + 100)
+    rnd = rng.integers(0, 2 ** 32, (L, cfg.E + cfg.D), dtype=np.uint64).astype(np.uint32)
+    pl_r = O.coact_placement(cnt_r, C_r, D=cfg.D, N=cfg.N, rnd=rnd)
+    pl_d = cap.coact_placement(fb.counts, fb.coact, cfg.D, cfg.N, rnd=dev(rnd.view(np.int32)))
+    for name, g, r in zip(("expert_group", "group_node", "expert_dev"), pl_d[:3], pl_r[:3]):
+        assert np.array_equal(host(g), r), tag + name
+    sp_r, nd_r, sw_r = O.adjust_spectrum(cnt_r, C_r, pl_r[2], D=cfg.D, S=7)
+    sp_d, nd_d, sw_d = cap.adjust_spectrum(fb.counts, fb.coact, pl_d[2], cfg.D, 7)
+    assert np.array_equal(host(sp_d), sp_r) and np.array_equal(host(nd_d), nd_r) and np.array_equal(host(sw_d), sw_r)
+    # row f2's chained check on the CUDA path: along the spectrum the load imbalance does not
+    # rise and devices per token do not fall, scored by cap_eval_placements
+    ev_s = cap.eval_placements(fb.idx, None, None, sp_d, topo, counts=fb.counts)
+    imb, dv = host(ev_s.imbalance), host(ev_s.dev_visits)
+    start = cap.eval_placements(fb.idx, None, None, pl_d[2][:, None, :].contiguous(), topo, counts=fb.counts)
+    imb = np.concatenate([host(start.imbalance), imb], axis=1)
+    dv = np.concatenate([host(start.dev_visits), dv], axis=1)
+    assert (np.diff(imb, axis=1) <= 1e-12).all(), tag + "imbalance rises along the spectrum"
+    # every step trades locality for balance at most weakly on average (the paper's qualitative claim)
+    assert dv[:, -1].sum() >= dv[:, 0].sum(), tag + "devices/token fell along the spectrum"
+    return launches
+
+
+def test_config2_qwen3_all_48_layers_one_launch():
+    cfg = W.CONFIGS["qwen3"]
+    plan = cap.trace_fused_plan(cfg.L, cfg.T, cap.gate_cfg(cfg.E, **cfg.gate), cfg.D, cfg.N, cfg.P)
+    print("qwen3 plan", plan)
+    assert plan["fused"] == 1 and plan["blocks_per_layer"] * cfg.L <= 148
+    _all_layers_one_launch(cfg, cfg.T, "qwen3 L48 ")
+
+
+def test_config4_dsv3_all_58_layers_one_launch_quarter_T():
+    # all 58 layers in one launch; T/4 per layer keeps the single-threaded oracle and the host
+    # generator within a minute (what matters is the L-dependent grid geometry)
+    cfg = W.CONFIGS["dsv3"]
+    _all_layers_one_launch(cfg.with_(T=cfg.T // 4), cfg.T // 4, "dsv3 L58 ")
+
+
+@pytest.mark.parametrize("D,N,T", [(2, 2, 1 << 19), (1, 1, 300000)])
+def test_fused_kernel_capacity_flush(D, N, T):
+    """A block that owns more tokens of one source device than its bit-sliced counters hold must cut the
+    run (capacity flush); the plan query proves the shape reaches that branch, the oracle checks it."""
+    cfg = W.CONFIGS["target"].with_(D=D, N=N, T=T)
+    gate = cap.gate_cfg(cfg.E, **cfg.gate)
+    plan = cap.trace_fused_plan(1, T, gate, D, N, cfg.P)
+    print("plan", plan)
+    assert plan["fused"] == 1
+    assert plan["max_tokens_one_source"] > plan["run_capacity"], "shape does not reach the capacity flush"
+    dn = W.dev_node(cfg)
+    topo = topo_of(cfg, dev(dn))
+    cand = W.candidates(cfg, 0)[None]
+    x = G.logits_device(cfg, 0)[None]
+    G.check_rows_against_host(cfg, 0, x[0], [0, 1, T // 3, T - 1])
+    fb = cap.trace_fused(x, None, gate, None, dev(cand), topo)
+    torch.cuda.synchronize()
+    acc = None
+    step = 1 << 16
+    for a in range(0, T, step):
+        b = min(T, a + step)
+        xs = x[:, a:b].cpu().numpy()
+        idx_r, w_r = O.gate_topk(xs, None, **cfg.gate)
+        assert np.array_equal(host(fb.idx[:, a:b]), idx_r)
+        assert float(np.abs(host(fb.w[:, a:b]).astype(np.float64) - w_r).max()) <= W_TOL
+        src = ((np.arange(a, b, dtype=np.int64) * D) // T).astype(np.int32)[None]
+        acc = _accumulate(acc, idx_r, cand, dn, cfg, src)
+    _compare_accumulated(acc, fb.counts, fb.coact, fb.out, cfg, "capacity flush ")
+
+
+def _accumulate(acc, idx_r, cand, dn, cfg, src):
+    cnt, C = O.coactivation(idx_r, E=cfg.E)
+    ev = O.eval_placements(idx_r, cand, dn, token_src=src, cost_inter=cfg.cost_inter,
+                           bytes_per_token=cfg.bytes_per_token)
+    if acc is None:
+        acc = {"counts": np.zeros_like(cnt), "coact": np.zeros(C.shape, np.int64)}
+        for n in EVAL_I64:
+            acc[n] = np.zeros_like(getattr(ev, n))
+    acc["counts"] += cnt
+    acc["coact"] += C
+    for n in EVAL_I64:
+        acc[n] += getattr(ev, n)
+    return acc
+
+
+def _compare_accumulated(acc, counts_d, coact_d, out_d, cfg, tag):
+    assert np.array_equal(host(counts_d), acc["counts"]), tag + "counts"
+    assert np.array_equal(host(coact_d).astype(np.int64), acc["coact"]), tag + "coact"
+    for n in EVAL_I64:
+        if n == "load_pairs" and out_d.load_pairs is None:
+            continue
+        assert np.array_equal(host(getattr(out_d, n)), acc[n]), tag + n
+    # Eq. 4 from the summed integers: max * D / sum in fp64, one IEEE divide (the oracle's formula)
+    for name, arr in (("imbalance", acc["load_pairs"]), ("imbalance_recv", acc["recv_tokens"])):
+        mx, sm = arr.max(-1).astype(np.float64), arr.sum(-1).astype(np.float64)
+        ref = np.where(sm > 0, mx * cfg.D / np.where(sm > 0, sm, 1.0), 0.0)
+        assert np.array_equal(host(getattr(out_d, name)), ref), tag + name
+
+
+@pytest.mark.parametrize("logT,P", [(18, 1024), (20, 256)])
+def test_config5_sweep_chunked_oracle(logT, P):
+    """Config 5 inside its T sweep on the BASELINE generator: S1 element by element, S2 / S3 totals and the
+    S4 after-metrics against the chunked oracle, S5 against the oracle on the whole pair stream."""
+    T = 1 << logT
+    cfg = W.CONFIGS["stress"].with_(T=T, P=P)
+    D = cfg.D
+    gate = cap.gate_cfg(cfg.E, **cfg.gate)
+    dn = W.dev_node(cfg)
+    dn_d = dev(dn)
+    topo = topo_of(cfg, dn_d)
+    cand = W.candidates(cfg, 0, P)[None]
+    cand_d = dev(cand)
+    x = G.logits_device(cfg, 0)[None]
+    rng = np.random.default_rng(logT)
+    G.check_rows_against_host(cfg, 0, x[0], np.concatenate([[0, T - 1], rng.integers(0, T, 6)]))
+    fb = cap.trace_fused(x, None, gate, None, cand_d, topo)
+    pi = np.ascontiguousarray(cand[:, 2, :])
+    pi_d = dev(pi)
+    tau = cfg.taus[-1]
+    kept_d, near_d, aft_d = cap.prune(fb.idx, fb.w, None, pi_d, topo, tau)
+    cntk_d, Ck_d = cap.coactivation(fb.idx, kept_d, cfg.E)
+    sp_d, off_d, pos_d = cap.dispatch_layout(fb.idx[0], kept_d[0], pi_d[0], D)
+    torch.cuda.synchronize()
+    acc, acc_k, acc_a = None, None, None
+    idx_all, kept_all, near_tot = [], [], 0
+    step = 1 << 15
+    for a in range(0, T, step):
+        b = min(T, a + step)
+        xs = x[:, a:b].cpu().numpy()
+        idx_r, w_r = O.gate_topk(xs, None, **cfg.gate)
+        assert np.array_equal(host(fb.idx[:, a:b]), idx_r), f"idx chunk {a}"
+        assert float(np.abs(host(fb.w[:, a:b]).astype(np.float64) - w_r).max()) <= W_TOL
+        src = ((np.arange(a, b, dtype=np.int64) * D) // T).astype(np.int32)[None]
+        acc = _accumulate(acc, idx_r, cand, dn, cfg, src)
+        # S4 stage-isolated on the oracle's own S1 output of this chunk
+        kept_r, near_r = O.prune(idx_r, w_r, pi, dn, tau, token_src=src, cost_inter=cfg.cost_inter)
+        kept_iso, _, _ = cap.prune(dev(idx_r), dev(w_r), dev(src), pi_d, topo, tau, want_after=False)
+        assert np.array_equal(host(kept_iso), kept_r), f"kept (isolated) chunk {a}"
+        bad = int((host(kept_d[:, a:b]) != kept_r).any(-1).sum())
+        assert bad <= int(near_r.sum()), f"kept (end to end) chunk {a}: {bad} tokens differ"
+        near_tot += int(near_r.sum())
+        kept_g = host(kept_d[:, a:b])                 # after-metrics / S5 follow the GPU's own mask
+        cnt_k, C_k = O.coactivation(idx_r, kept_g, E=cfg.E)
+        ev_a = O.eval_placements(idx_r, pi[:, None, :], dn, kept=kept_g, token_src=src, cost_inter=cfg.cost_inter,
+                                 bytes_per_token=cfg.bytes_per_token)
+        if acc_k is None:
+            acc_k = {"counts": np.zeros_like(cnt_k), "coact": np.zeros(C_k.shape, np.int64)}
+            acc_a = {n: np.zeros_like(getattr(ev_a, n)) for n in EVAL_I64}
+        acc_k["counts"] += cnt_k
+        acc_k["coact"] += C_k
+        for n in EVAL_I64:
+            acc_a[n] += getattr(ev_a, n)
+        idx_all.append(idx_r[0])
+        kept_all.append(kept_g[0])
+    _compare_accumulated(acc, fb.counts, fb.coact, fb.out, cfg, f"stress 2^{logT} ")
+    assert np.array_equal(host(cntk_d), acc_k["counts"]) and np.array_equal(host(Ck_d).astype(np.int64), acc_k["coact"])
+    for n in EVAL_I64:
+        assert np.array_equal(host(getattr(aft_d, n)), acc_a[n]), f"after-prune {n}"
+    assert abs(int(near_d.sum()) - near_tot) <= near_tot + 2
+    idx_all, kept_all = np.concatenate(idx_all), np.concatenate(kept_all)
+    sp_r, off_r, pos_r = O.dispatch_layout(idx_all, pi[0], D, kept=kept_all)
+    assert np.array_equal(host(off_d), off_r)
+    assert np.array_equal(host(sp_d)[: int(off_r[-1])], sp_r)
+    assert np.array_equal(host(pos_d), pos_r)
