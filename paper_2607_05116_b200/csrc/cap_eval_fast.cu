@@ -94,7 +94,17 @@ size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D,
         if (b > best) best = b;
     }
     const size_t fb = fused_ws_bytes(L, T, k, E, D, P);
-    return fb > best ? fb : best;
+    if (fb > best) best = fb;
+    const size_t f2 = fused2_ws_bytes(L, T, k, E, D, P) + 256;
+    return f2 > best ? f2 : best;
+}
+
+// start of the region behind the generic accumulators that the fast paths carve (one of them runs per call)
+void *eval_fast_region(void *ws, int32_t L, int32_t E, int32_t D, int32_t P)
+{
+    EvalWs base = eval_ws_carve(ws, L, E, D, P);
+    uintptr_t a = reinterpret_cast<uintptr_t>(base.ldirect + (size_t)L * 64);
+    return reinterpret_cast<void *>((a + 255) & ~(uintptr_t)255);
 }
 
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,

@@ -101,6 +101,15 @@ int profile_trace_fused_kernel(const float *const *logits_list, int nlist, int n
                                int32_t *coact, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
                                const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
 size_t fused_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
+// single-launch fused kernel (cap_fused2.cu): *used = false when the configuration does not fit it;
+// ws_f2 = the fast-path region of the evaluation workspace (eval_fast_region)
+int launch_trace_fused2(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
+                        int32_t *idx, float *w, int64_t *counts, int32_t *coact, const int32_t *token_src,
+                        const int32_t *expert_dev, int32_t P, const cap_topology &topo, const cap_eval_out &out,
+                        void *ws_f2, cudaStream_t st, bool *used);
+size_t fused2_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
+bool fused2_plan(int32_t L, int64_t T, const cap_gate_cfg &cfg, int32_t D, int32_t N, int32_t P, int64_t *plan);
+void *eval_fast_region(void *ws, int32_t L, int32_t E, int32_t D, int32_t P);
 bool fused_plan(int32_t L, int64_t T, const cap_gate_cfg &cfg, int32_t D, int32_t N, int32_t P, int64_t *plan);
 int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L,
                  int64_t T, int32_t k, int32_t E, const int32_t *expert_dev,
