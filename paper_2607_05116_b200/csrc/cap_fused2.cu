@@ -541,6 +541,7 @@ __device__ __forceinline__ void f2_flush(const F2Params &q, const F2Planes8 &in,
 #undef F2_FETCH_SHFL
         ++np;
     }
+    F2_TR(9);
     // (2) the warps of a class: tree through shared memory (both classes keep the same barrier count)
     const int xbase = cls ? (q.nwd / 2) * 32 * F2_NPL : 0;
     for (int half = 4; half >= 1; half >>= 1) {
@@ -558,6 +559,7 @@ __device__ __forceinline__ void f2_flush(const F2Params &q, const F2Planes8 &in,
         if (act) ++np;
         f2_bar(1, ns3);
     }
+    F2_TR(10);
     // (3) warp 0 of each class leaves the run's planes as [plane][word] (device words, then node words)
     uint32_t *fin = reinterpret_cast<uint32_t *>(xch);
     const int nwords = (q.Cd + q.Cn) * 4;
@@ -567,6 +569,7 @@ __device__ __forceinline__ void f2_flush(const F2Params &q, const F2Planes8 &in,
         for (int p = 0; p < F2_NPL; ++p) *reinterpret_cast<uint4 *>(fin + (size_t)p * nwords + wb) = pl[p];
     }
     f2_bar(1, ns3);
+    F2_TR(11);
     // (4) every S3 thread decodes counters: counter i = bit (i & 31) of word i >> 5
     {
         uint32_t *rec = q.recs + rec_slot * (size_t)q.ncnt;
@@ -579,6 +582,7 @@ __device__ __forceinline__ void f2_flush(const F2Params &q, const F2Planes8 &in,
         }
         if (t3 == 0) q.rec_src[rec_slot] = src;
     }
+    F2_TR(12);
     f2_bar(1, ns3);
 }
 
@@ -972,7 +976,13 @@ static int pow2_ceil(int v)
 static bool f2_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P, F2Geom *g)
 {
 #define F2_FAIL(why) do { if (getenv("CAP_DEBUG")) fprintf(stderr, "f2_geom: %s\n", why); return false; } while (0)
-    if (getenv("CAP_NO_FUSED2")) F2_FAIL("disabled");
+    // Opt-in (CAP_FUSED2=1): on B200 this single-launch variant is slower than the four-kernel path of
+    // cap_fused.cu at every BASELINE size (config 3: 55.5 vs 49.0 us per call, config 2: 388 vs 179 us; see
+    // DESIGN.md 6.4 for the timeline that explains it), so the library does not select it by default.
+    {
+        const char *env = getenv("CAP_FUSED2");
+        if (!env || env[0] != '1') F2_FAIL("not enabled");
+    }
     if (E != 64 && E != 128 && E != 256) F2_FAIL("E");
     if (k > 8 || L < 1 || T < 1 || P < 1 || D < 1 || D > 64 || N < 1 || N > 8) F2_FAIL("sizes");
     g->WD = D <= 8 ? 8 : D <= 16 ? 16 : D <= 32 ? 32 : 64;

@@ -251,6 +251,32 @@ def test_fused_kernel_serves_these_shapes(shape):
     assert cap.kernel_timer_ms(7) > 0.0
 
 
+@pytest.mark.parametrize("shape", [_FAST_SHAPES[0], _FAST_SHAPES[5], _FAST_SHAPES[6], _FAST_SHAPES[11], _FAST_SHAPES[12],
+                                   dict(base="target", T=20000, D=4, N=2, P=100)],
+                         ids=["E128", "k3", "E64", "L3", "T70000", "multi-source"])
+def test_single_launch_variant_optin(shape, monkeypatch):
+    """cap_fused2.cu, the single cooperative-launch variant of cap_trace_fused (opt-in: CAP_FUSED2=1; slower than
+    the default path on B200), stays bit-exact against the oracle."""
+    monkeypatch.setenv("CAP_FUSED2", "1")
+    kw = dict(shape)
+    cfg = W.CONFIGS[kw.pop("base")].with_(**kw)
+    plan = cap.trace_fused_plan(cfg.L, cfg.T, cap.gate_cfg(cfg.E, **cfg.gate), cfg.D, cfg.N, cfg.P)
+    assert plan["kernel_version"] == 2, plan
+    from parity_util import layers_inputs
+    layers = tuple(range(cfg.L))
+    logits, bias, cand = layers_inputs(cfg, layers, cfg.T)
+    dn = W.dev_node(cfg)
+    topo = topo_of(cfg, dev(dn))
+    idx_r, w_r, cnt_r, C_r, ev_r = O.trace_fused(logits, bias, cfg.gate, cand, dn, cost_inter=cfg.cost_inter,
+                                                 bytes_per_token=cfg.bytes_per_token)
+    fb = cap.trace_fused(dev(logits), dev(bias), cap.gate_cfg(cfg.E, **cfg.gate), None, dev(cand), topo)
+    torch.cuda.synchronize()
+    assert np.array_equal(host(fb.idx), idx_r)
+    assert float(np.abs(host(fb.w).astype(np.float64) - w_r).max()) <= 1e-6
+    assert np.array_equal(host(fb.counts), cnt_r) and np.array_equal(host(fb.coact), C_r)
+    assert_eval_equal(fb.out, ev_r, False, "fused2 ")
+
+
 def test_host_pipeline_double_buffered_matches_single():
     """The end-to-end call with two staging sets (copies on side streams, as bench.py's e2e leg uses it)
     returns, step by step, exactly what the plain device pipeline computes on the same inputs."""
