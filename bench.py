@@ -4,16 +4,25 @@ One "step" = one pass of every stage of SURVEY.md section 8(a) over one batch of
 router logits: cap_trace_fused (S1 gate top-k + S2 counts/co-activation + S3 scoring of P
 candidate placements) -> cap_prune under the chosen placement (S4) -> cap_dispatch_layout (S5).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config target] [--impl cap|reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config target] [--T tokens] [--impl cap|reference]
 
 Prints ONE JSON line (rank 0).  `value` = tokens of all ranks / device time with the inputs
 resident in HBM; `e2e` = the same metric through the host-buffer call (pinned host -> device
-copies and the read-back of every output inside the timed region); `roofline` = the dominant
-kernel's algorithmic bytes / its CUDA-event duration against MEASURED_PEAKS.json; `cpu_baseline`
-= the CPU oracle on the same workload (reported baseline, not the target).
-`--impl reference` times the oracle alone (the reference arm of this tier).
-Multi-GPU (torchrun): tokens are independent units -- every rank runs its own batch, no
-data-path collective ("scaling": "weak"); only the barrier and the max-over-ranks use NCCL.
+copies and the read-back of every output inside the timed region); `roofline` = algorithmic bytes of
+the fused S1+S2+S3 PASS (the whole cap_trace_fused call, every kernel of it) / its CUDA-event duration
+against MEASURED_PEAKS.json, with the dominant kernel alone as `kernel_only_*`; `stages` = S4 and S5
+stand-alone as GB/s; `others` = the other BASELINE configs (2, 4, 5 at both ends of its T sweep), one
+line each from the same code; `cpu_baseline` = the CPU oracle on one and on all host cores (reported
+baseline, not the target).  `--impl reference` times the oracle alone (the reference arm of this tier).
+
+Timing protocol (SURVEY.md 8(d)): a timed "step" is one pass of the path replayed from a CUDA graph;
+the timed region is 5 repeats of K x R replays (R = --replays, default so that K x R >= 1000), each repeat
+bracketed by CUDA events on the launching stream; `ms_per_step` and `value` come from the median repeat.
+Inputs rotate over 8 distinct sets (268 MB of logits > 126 MB L2) or are larger than L2 themselves.
+
+Multi-GPU: tokens are independent units -- every rank runs its own batch, no data-path collective
+("scaling": "weak"); only the barrier and the max-over-ranks use NCCL.  `--gpus N` without a torchrun
+environment re-launches itself under torch.distributed.run with N ranks.
 """
 import argparse
 import json
@@ -41,20 +50,6 @@ def _peaks():
         with open(p) as f:
             return float(json.load(f)["hbm_gbs"]), "measured"
     return FALLBACK_HBM_GBS, "fallback"
-
-
-def _ncu_traffic(kernel, workload):
-    """dram bytes read + written per launch of `kernel` from the committed `ncu --set full` capture
-    (profiles/ncu_traffic.txt: lines `kernel workload bytes source`), or None."""
-    p = os.path.join(ROOT, "profiles", "ncu_traffic.txt")
-    if not os.path.exists(p):
-        return None
-    with open(p) as f:
-        for line in f:
-            t = line.split()
-            if len(t) >= 3 and not line.startswith("#") and t[0] == kernel and t[1] == workload:
-                return int(t[2])
-    return None
 
 
 class ClockSampler:
@@ -111,20 +106,6 @@ class ClockSampler:
 
 
 # ---- workload ---------------------------------------------------------------------------------
-def make_inputs(cfg, W, set_id, rank):
-    """Host inputs of one batch: logits [L,T,E], bias [L,E]|None, maps [L,P,E] (seeded; the layer
-    number is the seed stream, so every (rank, set) is a distinct trace of the same recipe)."""
-    base = rank * 100000 + set_id * cfg.L
-    xs, bs, ms = [], [], []
-    for l in range(cfg.L):
-        xs.append(W.logits(cfg, base + l))
-        b = W.gate_bias(cfg, base + l)
-        if b is not None:
-            bs.append(b)
-        ms.append(W.candidates(cfg, base + l))
-    return np.stack(xs), (np.stack(bs) if bs else None), np.stack(ms)
-
-
 def algorithmic_bytes(cfg, has_src=False):
     """Bytes each kernel must move per launch, keyed by kernel tag."""
     L, T, E, k, P, D = cfg.L, cfg.T, cfg.E, cfg.k, cfg.P, cfg.D
@@ -168,7 +149,28 @@ def oracle_sample(cfg, W, max_tokens=65536):
     return T, x, (b[None] if b is not None else None), maps
 
 
-def time_oracle(cfg, W, min_seconds):
+def _oracle_shard(args):
+    """one worker of the N-core leg: the whole path on its contiguous token range (a trace of its own: every
+    aggregate is a sum over tokens, so shards are independent units)"""
+    name, T_total, a, b, n_pass = args
+    from oracle import cap_oracle as O
+    from paper_2607_05116_b200 import workload as W
+    O.lib()
+    cfg = W.CONFIGS[name].with_(T=T_total)
+    x = W.logits(cfg, 0, a, b)[None]
+    bias = W.gate_bias(cfg, 0)
+    maps = W.candidates(cfg, 0)[None]
+    dn = W.dev_node(cfg)
+    t0 = time.perf_counter()
+    for _ in range(n_pass):
+        oracle_step(O, cfg, x, bias[None] if bias is not None else None, maps, dn)
+    return time.perf_counter() - t0
+
+
+def time_oracle(cfg, W, min_seconds, key):
+    """The oracle as it stands on one host core, then sharded over all host cores (one process per core,
+    contiguous token ranges), on a bounded sample of the workload."""
+    import multiprocessing as mp
     from oracle import cap_oracle as O
     O.lib()
     T, x, b, maps = oracle_sample(cfg, W)
@@ -178,11 +180,31 @@ def time_oracle(cfg, W, min_seconds):
         oracle_step(O, cfg, x, b, maps, dn)
         passes += 1
         el = time.perf_counter() - t0
-        if el >= min_seconds or passes >= 64:
+        if el >= min_seconds / 2 or passes >= 64:
             break
-    return {"value": passes * T / el, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": f"{passes} pass(es) of 1 layer x {T} tokens x P={cfg.P} candidates, all 5 stages, "
-                      f"{el:.1f} s on one host core"}
+    v1 = passes * T / el
+    ncores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    out = {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"{passes} pass(es) of 1 layer x {T} tokens x P={cfg.P} candidates, all 5 stages, "
+                     f"{el:.1f} s on one host core"}
+    if ncores > 1:
+        n_pass = max(1, int(round(passes * min(ncores, 8) / 2)))
+        per = (T + ncores - 1) // ncores
+        jobs = [(key, T, i * per, min(T, (i + 1) * per), n_pass) for i in range(ncores) if i * per < T]
+        try:
+            ctx = mp.get_context("fork")
+            t0 = time.perf_counter()
+            with ctx.Pool(len(jobs)) as pool:
+                pool.map(_oracle_shard, jobs)
+            eln = time.perf_counter() - t0
+            out = {"value": n_pass * T / eln, "unit": UNIT, "cores": len(jobs), "kind": "oracle",
+                   "value_1core": v1,
+                   "sample": f"{n_pass} pass(es) of 1 layer x {T} tokens x P={cfg.P} candidates, all 5 stages, tokens "
+                             f"sharded over {len(jobs)} processes (one per host core; {eln:.1f} s wall incl. process "
+                             f"start and each shard generating its own inputs); 1 core: {passes} pass(es) in {el:.1f} s"}
+        except Exception as e:                        # the 1-core figure stands
+            out["multicore_error"] = repr(e)[:200]
+    return out
 
 
 def config_dict(cfg, extra=None):
@@ -225,11 +247,116 @@ def run_reference(args, cfg, W):
 
 
 # ---- product arm: the CUDA library ------------------------------------------------------------------
+REPEATS = 5
+
+
+def device_inputs(cfg, W, WD, set_id, rank, dev):
+    """One batch resident in HBM: logits [L,T,E] (filled by the device twin of the host generator, checked
+    bit for bit on sampled rows of the first layer), bias [L,E]|None, maps [L,P,E]."""
+    import torch
+    base = rank * 100000 + set_id * cfg.L
+    x = torch.empty((cfg.L, cfg.T, cfg.E), dtype=torch.float32, device=dev)
+    bs, ms = [], []
+    for l in range(cfg.L):
+        WD.logits_device(cfg, base + l, out=x[l], device=dev)
+        b = W.gate_bias(cfg, base + l)
+        if b is not None:
+            bs.append(b)
+        ms.append(W.candidates(cfg, base + l))
+    if set_id == 0:
+        WD.check_rows_against_host(cfg, base, x[0], [0, cfg.T // 2, cfg.T - 1])
+    b = torch.from_numpy(np.stack(bs)).to(dev) if bs else None
+    m = torch.from_numpy(np.stack(ms)).to(dev)
+    return x, b, m
+
+
+def timed_replays(torch, fn, n, barrier):
+    """REPEATS repeats of n calls of fn(i), each repeat between two CUDA events on the current stream;
+    returns the per-call milliseconds of every repeat."""
+    out = []
+    for r in range(REPEATS):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for i in range(n):
+            fn(i)
+        e1.record()
+        barrier()
+        out.append(e0.elapsed_time(e1) / n)
+    return out
+
+
+def measure(cfg, W, WD, cap, torch, dev, rank, steps, replays, barrier, light=False):
+    """Device-resident numbers of one configuration: the whole step, the fused pass, S4 and S5 alone."""
+    L, T, E, k, P, D = cfg.L, cfg.T, cfg.E, cfg.k, cfg.P, cfg.D
+    in_bytes = L * T * E * 4
+    n_sets = 1 if in_bytes > (256 << 20) else N_ROTATE
+    d_sets = [device_inputs(cfg, W, WD, s, rank, dev) for s in range(n_sets)]
+    dn = torch.from_numpy(W.dev_node(cfg)).to(dev)
+    gate = cap.gate_cfg(E, **cfg.gate)
+    pipe = cap.Pipeline(L, T, gate, D, cfg.N, P, dn, cost_inter=cfg.cost_inter,
+                        bytes_per_token=cfg.bytes_per_token, tau=cfg.taus[-1], chosen=0, device=dev)
+    n0 = cap.launch_count()
+    for x, b, m in d_sets[:1]:
+        pipe.step(x, b, None, m)
+    torch.cuda.synchronize()
+    launches_per_step = cap.launch_count() - n0
+    graphs = [pipe.capture(x, b, None, m) for x, b, m in d_sets]
+    fused_graphs = [pipe.capture_fused(x, b, None, m) for x, b, m in d_sets]
+    n = steps * replays
+    for i in range(3):
+        graphs[i % n_sets].replay()
+    ms_step = timed_replays(torch, lambda i: graphs[i % n_sets].replay(), n, barrier)
+    ms_fused = timed_replays(torch, lambda i: fused_graphs[i % n_sets].replay(), n, barrier)
+    # S4 / S5 alone on the buffers the last step left (inputs of these stages: 4-9 MB, L2-resident between
+    # replays at config 3 -- stated in the output)
+    g_prune = pipe.capture_stage("prune", None, d_sets[0][2])
+    g_disp = pipe.capture_stage("dispatch", None, d_sets[0][2])
+    ms_prune = timed_replays(torch, lambda i: g_prune.replay(), n, barrier)
+    ms_disp = timed_replays(torch, lambda i: g_disp.replay(), n, barrier)
+    # the dominant kernel of the pass alone, back to back (rotating inputs), by the library's profiling entry
+    kms = None
+    if not light:
+        kms = cap.profile_fused_kernel([d[0] for d in d_sets], gate, d_sets[0][2], pipe.topo, pipe.fb, max(steps, 50))
+    plan = cap.trace_fused_plan(L, T, gate, D, cfg.N, P)
+    res = dict(pipe=pipe, d_sets=d_sets, gate=gate, n_sets=n_sets, in_bytes=in_bytes, ms_step=ms_step,
+               ms_fused=ms_fused, ms_prune=ms_prune, ms_disp=ms_disp, kernel_ms=kms, plan=plan,
+               launches_per_step=launches_per_step)
+    return res
+
+
+def summarise(cfg, res, peak):
+    """The per-configuration numbers that go into the JSON line (main config and `others`)."""
+    ab = algorithmic_bytes(cfg)
+    LT = cfg.L * cfg.T
+    med = lambda v: float(np.median(v))
+    ms_step, ms_fused = med(res["ms_step"]), med(res["ms_fused"])
+    ms_prune, ms_disp = med(res["ms_prune"]), med(res["ms_disp"])
+    gbs = lambda b, ms: b / (ms * 1e-3) / 1e9
+    b_disp = ab["dispatch_scatter"]          # read idx + kept, write sorted_pairs + pair_pos: 104 B/token at k = 8
+    out = {
+        "tokens_per_step": LT, "ms_per_step": ms_step, "tokens_per_s": LT / (ms_step * 1e-3),
+        "fused_pass_ms": ms_fused, "fused_pass_gbs": gbs(ab["trace_fused"], ms_fused),
+        "fused_pass_frac_of_hbm_peak": gbs(ab["trace_fused"], ms_fused) / peak,
+        "fused_kernel": "single fused S1+S2+S3 kernel" if res["plan"]["fused"] else "staged S1, S2, S3 kernels",
+        "stages": {
+            "S4_cap_prune": {"ms": ms_prune, "algorithmic_bytes": ab["prune"], "gbs": gbs(ab["prune"], ms_prune),
+                             "frac_of_hbm_peak": gbs(ab["prune"], ms_prune) / peak},
+            "S5_cap_dispatch_layout": {"ms": ms_disp, "algorithmic_bytes": b_disp, "gbs": gbs(b_disp, ms_disp),
+                                       "frac_of_hbm_peak": gbs(b_disp, ms_disp) / peak,
+                                       "calls": cfg.L},
+        },
+        "launches_per_step": int(res["launches_per_step"]),
+    }
+    return out
+
+
 def run_cap(args, cfg, W):
     import torch
     import torch.distributed as dist
     from paper_2607_05116_b200 import build as capbuild
     from paper_2607_05116_b200 import cap
+    from paper_2607_05116_b200 import workload_device as WD
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -251,189 +378,149 @@ def run_cap(args, cfg, W):
             dist.barrier()
         torch.cuda.synchronize()
 
+    steps = args.steps
+    replays = args.replays if args.replays > 0 else max(1, -(-1000 // steps))
     L, T, E, k, P, D = cfg.L, cfg.T, cfg.E, cfg.k, cfg.P, cfg.D
-    in_bytes = L * T * E * 4
-    n_sets = 1 if in_bytes > (256 << 20) else N_ROTATE
-    h_sets, d_sets = [], []
-    for s in range(n_sets):
-        x, b, m = make_inputs(cfg, W, s, rank)
-        hs = tuple(None if a is None else torch.from_numpy(a).pin_memory() for a in (x, b, m))
-        h_sets.append(hs)
-        d_sets.append(tuple(None if a is None else a.to(dev) for a in hs))
-    dn = torch.from_numpy(W.dev_node(cfg)).to(dev)
-    gate = cap.gate_cfg(E, **cfg.gate)
-    pipe = cap.Pipeline(L, T, gate, D, cfg.N, P, dn, cost_inter=cfg.cost_inter,
-                        bytes_per_token=cfg.bytes_per_token, tau=cfg.taus[-1], chosen=0, device=dev)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    for _ in range(max(args.warmup, 3)):            # warm-up of the context / clocks before anything is timed
+        torch.empty(1 << 20, device=dev).zero_()
+    res = measure(cfg, W, WD, cap, torch, dev, rank, steps, replays, barrier)
+    pipe, d_sets, n_sets = res["pipe"], res["d_sets"], res["n_sets"]
+
+    # ---- end to end: pinned host inputs -> device -> step -> every output back to the host ----------
+    # (two staging sets: the upload of step i+1 and the read-back of step i-1 overlap the compute of step
+    # i; every step uploads its own inputs and reads back all of its own outputs inside the timed region)
+    h_sets = [tuple(None if a is None else a.cpu().pin_memory() for a in d) for d in d_sets]
     hpipe = cap.HostPipeline(pipe, has_bias=cfg.has_bias, depth=2)
-
-    def dstep(i):                       # direct launches (per-kernel event timers can be armed)
-        x, b, m = d_sets[i % n_sets]
-        pipe.step(x, b, None, m)
-
-    graphs = []
-
-    def gstep(i):                       # the same step replayed from a CUDA graph
-        graphs[i % n_sets].replay()
+    hpipe.capture()
 
     def hstep(i):
         x, b, m = h_sets[i % n_sets]
         hpipe.step(x, m, b)
 
-    # ---- warm-up; find the dominant kernel with the library's per-kernel event timers ----------
-    tags = list(cap.KERNEL_TAGS)
-    tot = {t: 0.0 for t in tags}
-    for i in range(max(args.warmup, 3) + 1):
-        for j, t in enumerate(tags):
-            cap.kernel_timer_arm(t, j)
-        dstep(i)
-        torch.cuda.synchronize()
-        if i == 0:
-            continue                    # first step pays one-time module loading: not representative
-        for j, t in enumerate(tags):
-            ms = cap.kernel_timer_ms(j)
-            if ms > 0:
-                tot[t] += ms
-    dominant = max(tot, key=lambda t: tot[t])
-    for x, b, m in d_sets:
-        graphs.append(pipe.capture(x, b, None, m))
-    fused_graphs = [pipe.capture_fused(x, b, None, m) for x, b, m in d_sets]
-    hpipe.capture()
-    for i in range(3):
-        gstep(i)
-
-    # ---- timed region: K steps, inputs resident in HBM ---------------------------------------------
-    sampler = ClockSampler(local)
-    if rank == 0:
-        sampler.start()
-    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    n0 = cap.launch_count()
-    ev0.record()
-    for i in range(args.steps):
-        gstep(i)
-    ev1.record()
-    barrier()
-    ms = ev0.elapsed_time(ev1)
-    # the dominant kernel's duration: the same K steps launched directly, one CUDA-event pair
-    # (owned by the library, on the launching stream) around that kernel in every step
-    n0 = cap.launch_count()
-    for i in range(args.steps):
-        cap.kernel_timer_arm(dominant, 100 + i)
-        dstep(i)
-    barrier()
-    launches = cap.launch_count() - n0
-    dom_ms = [cap.kernel_timer_ms(100 + i) for i in range(args.steps)]
-    dom_ms = [v for v in dom_ms if v > 0]
-    dom_how = "library CUDA-event pair around the kernel in K directly launched steps"
-    if dominant == "trace_fused":
-        # direct launches from Python leave the GPU idle between kernels, which the event pair would
-        # count; the library's profiling entry launches the fused kernel alone K times back to back
-        # (rotating over the input sets, > L2) between two events on the launching stream
-        kms = cap.profile_fused_kernel([d[0] for d in d_sets], gate, d_sets[0][2], pipe.topo, pipe.fb,
-                                       max(args.steps, 8))
-        if kms is not None:
-            dom_ms = [kms]
-            dom_how = ("cap_profile_fused_kernel: the fused kernel alone, K back-to-back launches rotating "
-                       "over the input sets, one CUDA-event pair on the launching stream")
-    # the fused call alone (S1+S2+S3: every kernel and memset of cap_trace_fused), graph replays
-    ev4, ev5 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    for i in range(3):
-        fused_graphs[i % n_sets].replay()
-    torch.cuda.synchronize()
-    ev4.record()
-    for i in range(args.steps):
-        fused_graphs[i % n_sets].replay()
-    ev5.record()
-    torch.cuda.synchronize()
-    ms_fused = ev4.elapsed_time(ev5) / args.steps
-
-    # ---- end to end: pinned host inputs -> device -> step -> every output back to the host ----------
-    # (two staging sets: the upload of step i+1 and the read-back of step i-1 overlap the compute of step
-    # i; every step uploads its own inputs and reads back all of its own outputs inside the timed region)
     for i in range(3):
         hstep(i)
     hpipe.finish()
-    barrier()
-    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev2.record()
-    for i in range(args.steps):
-        hstep(i)
-    hpipe.finish()
-    ev3.record()
-    barrier()
-    ms_e2e = ev2.elapsed_time(ev3)
+    n_e2e = max(steps, 20)
+    ms_e2e = []
+    for r in range(3):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        for i in range(n_e2e):
+            hstep(i)
+        hpipe.finish()
+        e1.record()
+        barrier()
+        ms_e2e.append(e0.elapsed_time(e1) / n_e2e)
     clocks = sampler.stop() if rank == 0 else None
+    x0, b0, m0 = h_sets[0]
+    h2d = sum(a.numel() * a.element_size() for a in (x0, b0, m0) if a is not None)
+    d2h = hpipe.d2h_bytes
+    del hpipe, h_sets
 
-    # ---- SURVEY 8(f) rank 1, outside every timed region above: cap_coact_placement (Jaccard p_ij +
-    # Algorithm 1, both stages) on the counts / co-activation matrices the last step left on the device
-    dstep(0)
-    ws_pl = cap.workspace(cap.CALL_COACT_PLACEMENT, L, 0, E, 1, D, 0, device=dev)
-    for _ in range(3):
-        cap.coact_placement(pipe.fb.counts, pipe.fb.coact, D, cfg.N, ws=ws_pl)
-    torch.cuda.synchronize()
-    ev6, ev7 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ev6.record()
-    for _ in range(10):
-        cap.coact_placement(pipe.fb.counts, pipe.fb.coact, D, cfg.N, ws=ws_pl)
-    ev7.record()
-    torch.cuda.synchronize()
-    us_place = ev6.elapsed_time(ev7) / 10 * 1e3
-
-    def time_us(fn, n=10):
+    # ---- SURVEY 8(f) consumers, outside every timed region above ----
+    def time_us(fn, nrep=10):
         for _ in range(3):
             fn()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
-        for _ in range(n):
+        for _ in range(nrep):
             fn()
         e1.record()
         torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / n * 1e3
+        return e0.elapsed_time(e1) / nrep * 1e3
 
+    pipe.step(*d_sets[0][:2], None, d_sets[0][2])
+    ws_pl = cap.workspace(cap.CALL_COACT_PLACEMENT, L, 0, E, 1, D, 0, device=dev)
+    us_place = time_us(lambda: cap.coact_placement(pipe.fb.counts, pipe.fb.coact, D, cfg.N, ws=ws_pl))
     maps0 = d_sets[0][2]
     us_obj = time_us(lambda: cap.pairwise_objective(pipe.fb.counts, pipe.fb.coact, maps0, pipe.topo))
     ws_rows = cap.workspace(cap.CALL_DISPATCH_ROWS, 1, T, E, k, D, 0, device=dev)
     pi0 = maps0[0, 0].contiguous()
     us_rows = time_us(lambda: cap.dispatch_rows(pipe.fb.idx[0], pipe.kept[0], pi0, D, ws=ws_rows))
 
+    ms_step = float(np.median(res["ms_step"]))
+    ms_e2e_med = float(np.median(ms_e2e))
     if world > 1:
-        tt = torch.tensor([ms, ms_e2e], device=dev, dtype=torch.float64)
+        tt = torch.tensor([ms_step, ms_e2e_med], device=dev, dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms, ms_e2e = float(tt[0]), float(tt[1])
-    tokens = world * args.steps * L * T
+        ms_step, ms_e2e_med = float(tt[0]), float(tt[1])
+    peak, peak_src = _peaks()
+    main = summarise(cfg, res, peak)
+    kms = res["kernel_ms"]
+    ab = algorithmic_bytes(cfg)
+
+    # ---- the other BASELINE configurations through the same code (rank 0, one GPU's worth each) ----
+    others = {}
+    rep_step = [round(float(v), 6) for v in res["ms_step"]]
+    rep_fused = [round(float(v), 6) for v in res["ms_fused"]]
+    del res, pipe, d_sets
+    torch.cuda.empty_cache()
+    if rank == 0 and not args.no_others and args.config == "target" and args.T == 0:
+        for name, Tover, st in (("qwen3", 0, 20), ("dsv3", 0, 5), ("stress", 1 << 16, 10), ("stress", 1 << 22, 3)):
+            c = W.CONFIGS[name]
+            if Tover:
+                c = c.with_(T=Tover)
+            try:
+                r = measure(c, W, WD, cap, torch, dev, 0, st, 1, lambda: torch.cuda.synchronize(), light=True)
+                o = summarise(c, r, peak)
+                o["workload"] = config_dict(c)["workload"]
+                o["timed"] = f"{REPEATS} repeats of {st} graph replays, median"
+                others[f"config{c.index}_{name}" + (f"_T{Tover}" if Tover else "")] = o
+                del r
+            except Exception as e:                  # a failure here must not take the headline line down
+                others[f"config{c.index}_{name}" + (f"_T{Tover}" if Tover else "")] = {"error": repr(e)[:300]}
+            torch.cuda.empty_cache()
+    if world > 1:
+        dist.barrier()
+
+    tokens_per_step = world * L * T
     if rank == 0:
-        peak, peak_src = _peaks()
-        ab = algorithmic_bytes(cfg)
-        dom_avg = float(np.mean(dom_ms)) if dom_ms else float("nan")
-        achieved = ab.get(dominant, 0) / (dom_avg * 1e-3) / 1e9 if dom_ms else None
-        x0, b0, m0 = h_sets[0]
-        h2d = sum(a.numel() * a.element_size() for a in (x0, b0, m0) if a is not None)
+        fused_gbs = main["fused_pass_gbs"]
         out = {
-            "metric": METRIC, "value": tokens / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
-            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+            "metric": METRIC, "value": tokens_per_step / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
             "config": config_dict(cfg, {
-                "l2": (f"inputs rotate over {n_sets} distinct sets ({n_sets * in_bytes / 1e6:.0f} MB of logits "
-                       f"> 126 MB L2)") if n_sets > 1 else f"one input set of {in_bytes / 1e6:.0f} MB > 126 MB L2",
-                "launch": "timed region replays the step from a CUDA graph (one graph per input set); "
-                          "roofline.kernel_ms comes from the same steps launched directly",
+                "l2": (f"inputs rotate over {n_sets} distinct sets ({n_sets * main['tokens_per_step'] * E * 4 / 1e6:.0f} MB of "
+                       f"logits > 126 MB L2)") if n_sets > 1 else f"one input set of {L * T * E * 4 / 1e6:.0f} MB > 126 MB L2",
+                "launch": "a step is replayed from a CUDA graph (one graph per input set)",
+                "timing": f"{REPEATS} repeats of {steps} x {replays} replays, each repeat between two CUDA events on the "
+                          f"launching stream; ms_per_step = median repeat / replays",
                 "parallelism": f"{world} independent rank(s), token batches sharded, no data-path collective"}),
-            "e2e": {"value": tokens / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": hpipe.d2h_bytes, "ms_per_step": ms_e2e / args.steps},
-            "gpu_launches": int(launches),
+            "replays_per_step": replays, "repeats": REPEATS,
+            "ms_per_step_repeats": rep_step, "fused_pass_ms_repeats": rep_fused,
+            "e2e": {"value": tokens_per_step / (ms_e2e_med * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e_med,
+                    "timed": f"3 repeats of {n_e2e} host-buffer steps, median"},
+            "gpu_launches": int(main["launches_per_step"]) * steps * replays * REPEATS,
+            "gpu_launches_per_step": int(main["launches_per_step"]),
             "clocks": clocks,
-            "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak,
-                         "unit": "GB/s", "frac": (achieved / peak) if achieved else None,
-                         "traffic": _ncu_traffic(dominant, args.config), "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
-                         "kernel_ms": dom_avg, "kernel_ms_how": dom_how,
-                         "algorithmic_bytes": ab.get(dominant),
-                         "fused_call_ms": ms_fused,
-                         "fused_call_gbs": ab["trace_fused"] / (ms_fused * 1e-3) / 1e9,
-                         "fused_call_frac": ab["trace_fused"] / (ms_fused * 1e-3) / 1e9 / peak,
-                         "kernel_ms_warmup_share": {t: round(v / max(sum(tot.values()), 1e-9), 4)
-                                                    for t, v in tot.items() if v > 0}},
+            "roofline": {
+                "bound": "hbm", "kernel": "cap_trace_fused (the whole S1+S2+S3 pass: " + main["fused_kernel"] + " + its table / decode / finalize kernels)",
+                "achieved": fused_gbs, "peak": peak, "unit": "GB/s", "frac": fused_gbs / peak, "traffic": None,
+                "traffic_note": "not measured inside this run; the ncu capture of the dominant kernel is in profiles/",
+                "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
+                "algorithmic_bytes": ab["trace_fused"], "pass_ms": main["fused_pass_ms"],
+                "how": "algorithmic bytes (4E + 8k per token) / median CUDA-event time of the cap_trace_fused call replayed "
+                       "from a graph with rotating inputs",
+                "kernel_only_ms": kms,
+                "kernel_only_gbs": (ab["trace_fused"] / (kms * 1e-3) / 1e9) if kms else None,
+                "kernel_only_frac": (ab["trace_fused"] / (kms * 1e-3) / 1e9 / peak) if kms else None,
+                "kernel_only_how": "cap_profile_fused_kernel: the fused kernel alone, back-to-back launches rotating over "
+                                   "the input sets, one CUDA-event pair on the launching stream",
+                "ceiling_note": "shared-memory-bound formulation: ~33 k shared wavefronts per SM per pass (ncu) = 17 us at "
+                                "one wavefront per clock, i.e. <= 0.34 of the HBM peak for the kernel (DESIGN.md 6.3)"},
+            "stages": main["stages"],
+            "stages_note": "S4 / S5 replayed alone from a graph on the buffers of the last step (their 4-9 MB of inputs "
+                           "stay in L2 between replays at this size: launch-latency-bound, see others.config5_stress_T4194304 "
+                           "for the bandwidth-bound size)",
+            "others": others,
         }
         out["next"] = {"coact_placement": {
             "us_per_call": us_place, "layers": L, "greedy_steps_per_layer": (E - D) + (D - cfg.N),
@@ -445,7 +532,7 @@ def run_cap(args, cfg, W):
                               "candidate 0 with the step's pruning mask; three direct launches through the binding, "
                               "output tensors allocated per call"}}
         if not args.no_cpu_baseline:
-            out["cpu_baseline"] = time_oracle(cfg, W, args.cpu_seconds)
+            out["cpu_baseline"] = time_oracle(cfg, W, args.cpu_seconds, args.config)
         print(json.dumps(out))
     if world > 1:
         dist.barrier()
@@ -455,16 +542,29 @@ def run_cap(args, cfg, W):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cap", choices=["cap", "reference"])
     ap.add_argument("--config", default="target")
-    ap.add_argument("--cpu-seconds", type=float, default=10.0)
+    ap.add_argument("--T", type=int, default=0, help="tokens per layer (config 5 sweeps 2^16..2^22); 0 = the config's own")
+    ap.add_argument("--replays", type=int, default=0, help="graph replays per timed step; 0 = ceil(1000 / steps)")
+    ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--ref-tokens", type=int, default=16384)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the lines of the other BASELINE configs")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "cap":
+        # `python bench.py --gpus N` starts its own N ranks (one per GPU); NCCL's communicator log stays on
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "WARN")
+        port = 29500 + (os.getpid() % 2000)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd, env=env))
     from paper_2607_05116_b200 import workload as W
     cfg = W.CONFIGS[args.config]
+    if args.T > 0:
+        cfg = cfg.with_(T=args.T)
     if args.impl == "reference":
         run_reference(args, cfg, W)
     else:

@@ -104,7 +104,8 @@ int cap_gate_topk(const float *logits, const float *bias, int32_t L, int64_t T,
                   void *ws, size_t ws_bytes, void *stream);
 
 /* S2 -- activation counts and E x E co-activation (pruned trace P:L224).
- * topk_idx [L][T][k]; kept [L][T][k] uint8 or NULL (all kept).
+ * topk_idx [L][T][k]: every row holds k DISTINCT ids in [0, E), as cap_gate_topk writes them (a repeated or
+ * out-of-range id gives an undefined but memory-safe result); kept [L][T][k] uint8 or NULL (all kept).
  * counts [L][E] int64: kept (token,slot) pairs per expert.
  * coact [L][E][E] int32, full symmetric: tokens keeping both i and j; diagonal = counts. */
 int cap_coactivation(const int32_t *topk_idx, const uint8_t *kept, int32_t L, int64_t T,
@@ -127,6 +128,9 @@ int cap_eval_placements(const int32_t *topk_idx, const uint8_t *kept, const int3
  * Per token: a_d = sum of its weights on device d (slot order, fp32); c_d = cost_local /
  * cost_intra / cost_inter relative to token_src; devices kept by descending a_d/c_d (c_d = 0
  * first; ties -> lower device id) while the kept sum is < 1-p.  p <= 0 keeps everything.
+ * Precondition: the weights of a token sum to 1 (renormalised gate, scale = 1): Eq. 6's 1-p is an
+ * absolute share of the routing mass (reading R8).  With scaled or un-renormalised weights the call is
+ * memory-safe but the stop rule no longer means "keep 1-p of the mass".
  * expert_dev [L][E].  kept [L][T][k] uint8 out.  after: optional S3 outputs (P = 1) of the
  * kept trace ("new volume and load").  near_margin [L] int64 or NULL: tokens whose deciding
  * comparison had a margin below 1e-6 (R-S4.7).  EINVAL unless p < 1. */

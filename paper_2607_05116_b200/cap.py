@@ -387,6 +387,10 @@ class Pipeline:
         self._ctor = dict(L=L, T=T, gate=gate, D=D, N=N, P=P, dev_node=dev_node, cost_inter=cost_inter,
                           bytes_per_token=bytes_per_token, tau=tau, chosen=chosen, device=device)
         self.gate = gate
+        if gate.renormalize != 1 or gate.scale != 1.0:
+            # cap_prune's stop rule compares the kept weight with 1 - p (Eq. 6, reading R8): it needs routing
+            # weights that sum to 1 per token, which only renormalised, unscaled gates produce
+            raise CapError("Pipeline: cap_prune needs renormalised routing weights with scale 1 (include/cap.h)")
         E, k = gate.E, gate.k
         self.dev_node = dev_node
         self.topo = topology(dev_node, 0, 1, cost_inter, bytes_per_token, N=N)
@@ -406,28 +410,48 @@ class Pipeline:
         """A second pipeline with its own output buffers and workspaces (same configuration)."""
         return Pipeline(**self._ctor)
 
-    def step(self, logits, bias, token_src, expert_dev):
-        L, T = self.L, self.T
-        E, k = self.gate.E, self.gate.k
-        trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)
-        if L == 1:
-            pi = expert_dev[:, self.chosen, :]          # already the [L][E] layout cap_prune wants: no copy
-        else:
-            self.pi.copy_(expert_dev[:, self.chosen, :])
-            pi = self.pi
-        st = _stream()
-        rc = lib().cap_prune(_ptr(self.fb.idx), _ptr(self.fb.w), _ptr(token_src, torch.int32), L, T, k, E,
-                             _ptr(pi), C.byref(self.topo), float(self.tau), _ptr(self.kept),
-                             C.byref(self.after_struct), _ptr(self.near), _ptr(self.ws_prune),
-                             self.ws_prune.numel(), st)
+    def _pi(self, expert_dev):
+        if self.L == 1:
+            return expert_dev[:, self.chosen, :]        # already the [L][E] layout cap_prune wants: no copy
+        self.pi.copy_(expert_dev[:, self.chosen, :])
+        return self.pi
+
+    def step_prune(self, token_src, pi):
+        """S4 on the buffers the last cap_trace_fused left (kept mask + after-metrics)."""
+        rc = lib().cap_prune(_ptr(self.fb.idx), _ptr(self.fb.w), _ptr(token_src, torch.int32), self.L, self.T,
+                             self.gate.k, self.gate.E, _ptr(pi), C.byref(self.topo), float(self.tau),
+                             _ptr(self.kept), C.byref(self.after_struct), _ptr(self.near), _ptr(self.ws_prune),
+                             self.ws_prune.numel(), _stream())
         _check(rc, "cap_prune")
-        for l in range(L):
-            rc = lib().cap_dispatch_layout(_ptr(self.fb.idx[l]), _ptr(self.kept[l]), T, k, E,
-                                           _ptr(pi[l]), self.D, _ptr(self.sorted_pairs[l]),
+
+    def step_dispatch(self, pi):
+        """S5, one call per layer, on the kept mask of the last cap_prune."""
+        st = _stream()
+        for l in range(self.L):
+            rc = lib().cap_dispatch_layout(_ptr(self.fb.idx[l]), _ptr(self.kept[l]), self.T, self.gate.k,
+                                           self.gate.E, _ptr(pi[l]), self.D, _ptr(self.sorted_pairs[l]),
                                            _ptr(self.pair_pos[l]), _ptr(self.offsets[l]),
                                            _ptr(self.ws_disp), self.ws_disp.numel(), st)
             _check(rc, "cap_dispatch_layout")
+
+    def step(self, logits, bias, token_src, expert_dev):
+        trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)
+        pi = self._pi(expert_dev)
+        self.step_prune(token_src, pi)
+        self.step_dispatch(pi)
         return self
+
+    def capture_stage(self, which, token_src, expert_dev):
+        """Graph of one stage alone ("prune" = S4 with after-metrics, "dispatch" = S5) on the current buffers,
+        for stand-alone stage timings; the preceding stages must have run once."""
+        pi = self._pi(expert_dev)
+        fn = (lambda: self.step_prune(token_src, pi)) if which == "prune" else (lambda: self.step_dispatch(pi))
+        fn()
+        torch.cuda.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            fn()
+        return g
 
     def capture(self, logits, bias, token_src, expert_dev):
         """Capture one step on these (fixed) input buffers into a CUDA graph: the library only

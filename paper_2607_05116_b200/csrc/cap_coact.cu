@@ -32,11 +32,13 @@ coact_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, 
         const int64_t base = t * k;
         if (kept && !kept[base + a]) continue;
         const int i = idx[base + a];
+        if ((unsigned)i >= (unsigned)E) continue;    // out-of-range ids: undefined result, memory-safe (cap.h)
         atomicAdd(&cnt[i], 1);
         int *rowp = use_smem ? hist + (size_t)i * E : coact + (size_t)i * E;
         for (int b = 0; b < k; ++b) {
             if (b != a && kept && !kept[base + b]) continue;
-            atomicAdd(&rowp[idx[base + b]], 1);      // b == a gives the diagonal
+            const int j = idx[base + b];
+            if ((unsigned)j < (unsigned)E) atomicAdd(&rowp[j], 1);      // b == a gives the diagonal
         }
     }
     __syncthreads();

@@ -179,7 +179,7 @@ masked_counts_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
     const int64_t i0 = (int64_t)blockIdx.x * tok_per_block * k;
     const int64_t i1 = min(T * k, i0 + tok_per_block * k);
     for (int64_t i = i0 + threadIdx.x; i < i1; i += blockDim.x)
-        if (!kept || kept[i]) atomicAdd(&cnt[idx[i]], 1);
+        if ((!kept || kept[i]) && (unsigned)idx[i] < (unsigned)E) atomicAdd(&cnt[idx[i]], 1);
     __syncthreads();
     for (int i = threadIdx.x; i < E; i += blockDim.x)
         if (cnt[i]) atomicAdd(&counts[(size_t)layer * E + i], (unsigned long long)cnt[i]);

@@ -1,13 +1,14 @@
-"""Device-side twin of paper_2607_05116_b200/workload.logits for the large parity cases: the same
-stateless hash evaluated with torch integer ops on the GPU, so that config 5
-at 2^20..2^22 tokens (up to 8.6 GB of logits) is filled in HBM instead of being hashed on the host
-and copied over PCIe.  Test infrastructure only (inputs, none of the method's arithmetic); every
-user checks a sample of rows bit for bit against the host generator before trusting the rest.
+"""Device-side twin of workload.logits: the same stateless hash evaluated with
+torch integer ops on the GPU, so that the large workloads (config 4: 1.95 GB of logits, config 5 at
+2^20..2^22 tokens: up to 8.6 GB) are filled in HBM instead of being hashed on the host and copied over
+PCIe.  Inputs only, none of the method's arithmetic; it imports neither the CUDA library nor the
+oracle.  Every user checks a sample of rows bit for bit against the host generator
+(check_rows_against_host) before trusting the rest.
 """
 import numpy as np
 import torch
 
-from paper_2607_05116_b200 import workload as W
+from . import workload as W
 
 _M64 = (1 << 64) - 1
 

@@ -14,7 +14,7 @@ from oracle import cap_oracle as O                      # noqa: E402
 from paper_2607_05116_b200 import cap                   # noqa: E402
 from paper_2607_05116_b200 import workload as W         # noqa: E402
 from parity_util import EVAL_I64, W_TOL, assert_eval_equal, dev, host, layers_inputs, topo_of  # noqa: E402
-import gpu_workload as G                                # noqa: E402
+from paper_2607_05116_b200 import workload_device as G                                # noqa: E402
 
 
 @pytest.fixture(scope="module", autouse=True)

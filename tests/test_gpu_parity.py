@@ -338,6 +338,12 @@ def test_garbage_values_are_memory_safe(with_src):
     cap.dispatch_layout(fb.idx[0], kept[0], pi[0], D)
     cap.dispatch_layout(fb.idx[0], None, pi[0], D)
     cap.eval_placements(fb.idx, kept, dev(src), dev(maps), topo)
+    bad_idx = dev(rng.integers(-2 ** 31, 2 ** 31 - 1, (L, T, k), dtype=np.int64).astype(np.int32))
+    cap.coactivation(bad_idx, None, E)
+    cap.coactivation(bad_idx, kept, E)
+    cap.eval_placements(bad_idx, None, dev(src), dev(maps), topo, counts=None)
+    if E != 512:
+        cap.coactivation(bad_idx[:, :300].contiguous(), None, 512)          # the histogram path of large E
     torch.cuda.synchronize()
     check_all_stages(W.CONFIGS["tiny"], tag="after garbage ")
 
@@ -350,11 +356,11 @@ def test_config5_maximum_size_sampled_and_invariants():
     sum of counts = T k, C symmetric with diag = counts and off-diagonal row sums = (k-1) counts; S3 totals
     equal the sums of the per-token outputs; S5 is a stable permutation of the kept pairs grouped by
     device).  Inputs: the BASELINE generator of config 5 (workload.logits) evaluated on the GPU by
-    tests/gpu_workload.py, checked bit for bit against the host generator on sampled rows.  The sweep
+    paper_2607_05116_b200/workload_device.py, checked bit for bit against the host generator on sampled rows.  The sweep
     points 2^18 and 2^20 are compared with the chunked oracle in tests/test_gpu_fullsize.py."""
     cfg = W.CONFIGS["stress"]
     L, T, E, k, D, N = 1, 1 << 22, cfg.E, cfg.k, cfg.D, cfg.N
-    import gpu_workload as G
+    from paper_2607_05116_b200 import workload_device as G
     cfg = cfg.with_(T=T)
     x = G.logits_device(cfg, 0)[None]                 # the BASELINE generator, evaluated on the device
     gate = cap.gate_cfg(E, **cfg.gate)
