@@ -150,6 +150,23 @@ int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T,
                         int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes,
                         void *stream);
 
+/* S5 without a workspace, for callers that cannot allocate (CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc).  Same result, bit for bit, as cap_dispatch_layout; the scratch is a static device
+ * array of CAP_STATIC_SCRATCH_BYTES (4 MiB) inside the library, held by every GPU that loads it until exit.
+ * Limit: cap_workspace_bytes(CAP_CALL_DISPATCH_LAYOUT, 1, T, E, k, D, 0) <= CAP_STATIC_SCRATCH_BYTES, i.e.
+ * ceil128(ceil(T k / 256)) * D <= 524 256 -- e.g. T k <= 8.3 M pairs at D = 16, 2.0 M at D = 64; larger
+ * sizes return CAP_EWORKSPACE (nothing is launched).  Calls no cudaMalloc / cudaFree; the array's device
+ * address is resolved once per device (cudaGetSymbolAddress) on the first call made with that device
+ * current -- make that call outside a stream capture.  All calls on a device share the array: it needs no
+ * clearing between calls (each call writes what it reads), but calls that overlap on the GPU race on it --
+ * order them on one stream or with an event.  Arguments as in cap_dispatch_layout. */
+#define CAP_STATIC_SCRATCH_BYTES (4 * 1024 * 1024)
+int cap_dispatch_layout_static(const int32_t *topk_idx, const uint8_t *kept, int64_t T, int32_t k,
+                               int32_t E, const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs,
+                               int32_t *pair_pos, int64_t *offsets, void *stream);
+/* CAP_STATIC_SCRATCH_BYTES as the loaded library was built. */
+size_t cap_static_scratch_bytes(void);
+
 /* S1 + S2 + S3 in one call over the logits (the measured pass).  Arguments as in the three
  * calls above; members of `out` may be NULL to skip an output; counts and coact are required
  * (CAP_EINVAL if NULL with L > 0: the fused kernel always produces them). */

@@ -19,7 +19,8 @@ OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
            "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_adjust_spectrum", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
-           "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan")
+           "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan",
+           "cap_dispatch_layout_static", "cap_static_scratch_bytes")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
@@ -87,6 +88,8 @@ def lib():
                                                vp, vp, vp, i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz,
                                                vp, C.POINTER(C.c_float)]
         L.cap_trace_fused_plan.argtypes = [i32, i64, C.POINTER(GateCfg), i32, i32, i32, C.POINTER(C.c_int64)]
+        L.cap_dispatch_layout_static.argtypes = [vp, vp, i64, i32, i32, vp, i32, vp, vp, vp, vp]
+        L.cap_static_scratch_bytes.restype = C.c_size_t
         L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
         L.cap_kernel_timer_ms.argtypes = [C.c_int]
         L.cap_kernel_timer_ms.restype = C.c_float
@@ -238,6 +241,23 @@ def dispatch_layout(idx, kept, expert_dev, D, want_pos=True, ws=None):
                                    _ptr(expert_dev, torch.int32), D, _ptr(sorted_pairs),
                                    _ptr(pair_pos), _ptr(offsets), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_dispatch_layout")
+    return sorted_pairs, offsets, pair_pos
+
+
+def dispatch_layout_static(idx, kept, expert_dev, D, sorted_pairs, offsets, pair_pos=None):
+    """cap_dispatch_layout_static: S5 into CALLER-provided outputs with the library's static scratch (no
+    workspace, nothing allocated here or in the library).  sorted_pairs [T*k] int32, offsets [D+1] int64,
+    pair_pos [T*k] int32 or None.  Raises CapError(CAP_EWORKSPACE) beyond the static limit."""
+    T, k = idx.shape
+    E = expert_dev.shape[0]
+    rc = lib().cap_dispatch_layout_static(_ptr(idx, torch.int32), _ptr(kept, torch.uint8), T, k, E,
+                                          _ptr(expert_dev, torch.int32), D, _ptr(sorted_pairs, torch.int32),
+                                          _ptr(pair_pos, torch.int32), _ptr(offsets, torch.int64), _stream())
+    if rc == EWORKSPACE:
+        need = int(lib().cap_workspace_bytes(CALL_DISPATCH_LAYOUT, 1, T, E, k, D, 0))
+        raise CapError(f"cap_dispatch_layout_static -> CAP_EWORKSPACE: T={T} k={k} D={D} needs {need} bytes of scratch, "
+                       f"the static array holds {int(lib().cap_static_scratch_bytes())}; use cap_dispatch_layout")
+    _check(rc, "cap_dispatch_layout_static")
     return sorted_pairs, offsets, pair_pos
 
 
