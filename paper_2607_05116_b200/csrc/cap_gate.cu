@@ -237,6 +237,8 @@ int launch_gate_topk(const float *logits, const float *bias, int32_t L, int64_t 
     bool fast = false;
     CAP_TRY(launch_gate_fast(logits, bias, L, T, cfg, idx, w, st, &fast));
     if (fast) return CAP_OK;
+    CAP_TRY(launch_gate_sig(logits, bias, L, T, cfg, idx, w, st, &fast));
+    if (fast) return CAP_OK;
     GateParams prm;
     prm.logits = logits;
     prm.bias = bias;

@@ -10,7 +10,9 @@
 namespace cap {
 
 constexpr int GF_NP = 2;                       // producer warps
-constexpr int GF_NC = 14;                      // consumer warps
+constexpr int GF_NC = 12;                      // consumer warps; stages = a multiple of GF_NC (one consumer warp per stage:
+                                               // with 14 warps on the 12 stages of E = 256 a warp's first tile could be the
+                                               // SECOND use of a stage, whose parity wait passes before the first use landed)
 constexpr int GF_THREADS = 32 * (GF_NC + GF_NP);
 constexpr int GF_MAXST = 32;
 constexpr int GF_TILE = 16;                    // tokens per tile (one warp, two lanes per token)
@@ -107,6 +109,7 @@ static int launch_e(GateFastParams prm, cudaStream_t st)
     constexpr int STAGEB = GF_TILE * (E * 4);
     int nst = (200 * 1024) / STAGEB;
     if (nst > GF_MAXST) nst = GF_MAXST;
+    nst = (nst / GF_NC) * GF_NC;
     prm.nst = nst;
     static bool attr_set = false;
     if (!attr_set) {

@@ -80,6 +80,53 @@ def test_gate_group_limited(E, n_group, topk_group, k, group_score):
     check_gate(x, None, dict(scoring=0, **g))
 
 
+@pytest.mark.parametrize("E", [64, 128, 256])
+@pytest.mark.parametrize("grouped,group_score", [(False, 0), (True, 0), (True, 1)])
+def test_gate_sigmoid_fast_path(E, grouped, group_score):
+    """The two-lanes-per-token sigmoid kernel (cap_gate_sig.cu: cheap sigmoid inside payload keys + exact redo of
+    uncertified tokens) must give the oracle's result on exactly the inputs that stress its certification:
+    heavy exact ties, all-equal rows, -0/+0, saturated sigmoids (scores tied at 1.0 / near 0), near-ties one ulp
+    apart, biases that reorder experts.  T is a multiple of 16, so the fast path serves these calls."""
+    rng = np.random.default_rng(E * 3 + group_score + 7 * grouped)
+    T = 1024
+    ng = E // 32
+    x = rng.normal(0, 1.5, (3, T, E)).astype(np.float32)
+    x[1] = np.round(x[1] * 2) / 2                                   # heavy exact ties
+    x[2, :256] = x[2, :256] * 12.0                                   # saturated: many scores at 1.0 or ~0
+    x[2, 256:512] = -8.0 + 0.01 * x[2, 256:512]                      # every score far below 0.25
+    base = rng.normal(0, 1, (256, 1)).astype(np.float32)
+    near = np.nextafter(np.broadcast_to(base, (256, E)).astype(np.float32), np.float32(np.inf))
+    x[2, 512:768] = np.where(rng.random((256, E)) < 0.5, near, np.broadcast_to(base, (256, E)))   # one ulp apart
+    x[0, :5] = 0.25
+    x[0, 5, :3] = -0.0
+    x[0, 5, 3:] = 0.0
+    bias = rng.uniform(-0.05, 0.05, (3, E)).astype(np.float32)
+    bias[1] = np.round(bias[1] * 64) / 64                            # biases that create exact score ties
+    for k in (1, 3, 8):
+        for tg in ((1, ng) if grouped else (1,)):
+            if grouped and k > tg * 32:
+                continue
+            g = dict(k=k, scoring=1, n_group=ng if grouped else 1, topk_group=tg if grouped else 1,
+                     group_score=group_score)
+            if grouped and ng == 8:
+                g4 = dict(g, topk_group=4)
+                check_gate(x, bias, g4, tag=f"sigfast E{E} {g4} ")
+            check_gate(x, bias, g, tag=f"sigfast E{E} {g} ")
+            check_gate(x, None, dict(g, scale=2.5), tag=f"sigfast/nobias E{E} {g} ")
+
+
+@pytest.mark.parametrize("scoring", [0, 1])
+def test_gate_ring_wraps_many_times_E256(scoring):
+    """E = 256 gives the TMA ring of the standalone gate kernels only 12 stages: 70 000 tokens make every block
+    wrap it more than twice (regression: stages consumed by changing warps desynchronised the ring)."""
+    cfg = W.CONFIGS["dsv3"].with_(T=70000 - 70000 % 16)
+    x = W.logits(cfg, 0)[None]
+    if scoring == 0:
+        check_gate(x, None, dict(k=8), tag="E256 softmax wrap ")
+    else:
+        check_gate(x, W.gate_bias(cfg, 0)[None], cfg.gate, tag="E256 sigmoid wrap ")
+
+
 def test_gate_empty_and_single():
     cfg = cap.gate_cfg(128, 8)
     idx, w = cap.gate_topk(torch.empty((1, 0, 128), device="cuda"), None, cfg)
