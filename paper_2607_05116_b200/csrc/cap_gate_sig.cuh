@@ -29,10 +29,10 @@ __device__ __forceinline__ float gs_cheap_sigmoid(float x)
     return __fdividef(1.0f, 1.0f + __expf(-x));     // ex2.approx + rcp.approx
 }
 
-// key of the cheap score at position pos of the lane's half row (compile-time after unrolling)
-__device__ __forceinline__ float gs_key(float x, float b, int pos)
+// key of the cheap score: low byte <- byte j of the payload word (positions of four consecutive experts)
+__device__ __forceinline__ float gs_key_rt(float x, float b, uint32_t pay, int j)
 {
-    return gate_key(__fadd_rn(gs_cheap_sigmoid(x), b), pos);
+    return __uint_as_float(__byte_perm(__float_as_uint(__fadd_rn(gs_cheap_sigmoid(x), b)), pay, 0x3214u + (uint32_t)j));
 }
 
 // Exact selection of one token by the WHOLE warp (all lanes call it with the same row): lane l holds
@@ -115,9 +115,14 @@ __device__ __forceinline__ void gate_select_sig_pair(const float *row, const flo
     float lst[G][8], l9[G];
 #pragma unroll
     for (int g = 0; g < G; ++g) {
+        // The four 8-expert sub-blocks of a group are a ROLLED loop (runtime payload word): fully unrolled, the
+        // selection is ~6 000 instructions (96 KB), which 12 warps at different positions cannot keep in the
+        // 32 KB instruction cache -- ncu showed 57 % of the stall samples as no_inst.
         float r[8];
-        float r9 = sent;
 #pragma unroll
+        for (int i = 0; i < 8; ++i) r[i] = sent;
+        float r9 = sent;
+#pragma unroll 1
         for (int sb = 0; sb < 4; ++sb) {
             const uint32_t off = (uint32_t)(g * 128 + sb * 32);
             float4 va, vb, ba = make_float4(0.f, 0.f, 0.f, 0.f), bb = ba;
@@ -130,19 +135,16 @@ __device__ __forceinline__ void gate_select_sig_pair(const float *row, const flo
                 ba = __ldg(reinterpret_cast<const float4 *>(bp + (off ^ ((uint32_t)t7 << 4))));
                 bb = __ldg(reinterpret_cast<const float4 *>(bp + ((off + 16u) ^ ((uint32_t)t7 << 4))));
             }
-            const int p0 = g * 32 + sb * 8;
+            // payload words: bytes = positions p0..p0+3 and p0+4..p0+7 of the lane's half row
+            const uint32_t payA = 0x03020100u + 0x01010101u * (uint32_t)(g * 32 + sb * 8);
+            const uint32_t payB = payA + 0x04040404u;
             float q[8];
-            q[0] = gs_key(va.x, ba.x, p0 + 0); q[1] = gs_key(va.y, ba.y, p0 + 1);
-            q[2] = gs_key(va.z, ba.z, p0 + 2); q[3] = gs_key(va.w, ba.w, p0 + 3);
-            q[4] = gs_key(vb.x, bb.x, p0 + 4); q[5] = gs_key(vb.y, bb.y, p0 + 5);
-            q[6] = gs_key(vb.z, bb.z, p0 + 6); q[7] = gs_key(vb.w, bb.w, p0 + 7);
+            q[0] = gs_key_rt(va.x, ba.x, payA, 0); q[1] = gs_key_rt(va.y, ba.y, payA, 1);
+            q[2] = gs_key_rt(va.z, ba.z, payA, 2); q[3] = gs_key_rt(va.w, ba.w, payA, 3);
+            q[4] = gs_key_rt(vb.x, bb.x, payB, 0); q[5] = gs_key_rt(vb.y, bb.y, payB, 1);
+            q[6] = gs_key_rt(vb.z, bb.z, payB, 2); q[7] = gs_key_rt(vb.w, bb.w, payB, 3);
             sort8_desc(q);
-            if (sb == 0) {
-#pragma unroll
-                for (int i = 0; i < 8; ++i) r[i] = q[i];
-            } else {
-                merge8_desc(r, q, r9);
-            }
+            merge8_desc(r, q, r9);          // the first merge meets the fillers
         }
 #pragma unroll
         for (int i = 0; i < 8; ++i) lst[g][i] = r[i];
