@@ -57,6 +57,18 @@ __device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity
     while (!mbar_try_wait(bar, parity)) __nanosleep(ns);
 }
 
+// release / acquire accesses to a shared-memory word (monotonic progress counters next to the mbarriers)
+__device__ __forceinline__ void st_release_shared(uint32_t *p, uint32_t v)
+{
+    asm volatile("st.release.cta.shared::cta.u32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t ld_acquire_shared(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.acquire.cta.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+
 // TMA bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned) global -> shared,
 // completing `bytes` of transaction count on `bar`.
 __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)

@@ -14,10 +14,7 @@
 namespace cap {
 
 constexpr int GS_NP = 2;                       // producer warps
-constexpr int GS_NC = 12;                      // consumer warps; the ring has a multiple of GS_NC stages, so that a stage
-                                               // is always consumed by the SAME warp (tile j -> warp j % NC, stage j % nst):
-                                               // a warp that waited on a later phase of a barrier it never saw complete
-                                               // would read `try_wait.parity` of a phase two behind as "done"
+constexpr int GS_NC = 12;                      // consumer warps (24 measured slower: the 12 stages of E = 256 cannot feed them)
 constexpr int GS_THREADS = 32 * (GS_NC + GS_NP);
 constexpr int GS_MAXST = 32;
 constexpr int GS_TILE = 16;                    // tokens per tile (one warp, two lanes per token)
@@ -38,6 +35,11 @@ __global__ void __launch_bounds__(GS_THREADS) gate_sig_kernel(GateSigParams q)
 {
     extern __shared__ __align__(1024) unsigned char gs_sm[];
     __shared__ uint64_t full_bar[GS_MAXST], empty_bar[GS_MAXST];
+    // use number of every stage, set by the producer before it refills the stage.  There are more consumer warps
+    // than stages, so consecutive uses of a stage belong to different warps, and a warp may reach use u of a
+    // stage whose barrier is still two phases behind -- where `try_wait.parity` would report "done".  A consumer
+    // therefore first waits until the stage is in ITS use, then on the barrier's parity.
+    __shared__ uint32_t stage_use[GS_MAXST];
     constexpr int ROWB = E * 4;
     constexpr int STAGEB = GS_TILE * ROWB;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -46,6 +48,7 @@ __global__ void __launch_bounds__(GS_THREADS) gate_sig_kernel(GateSigParams q)
         for (int s = 0; s < nst; ++s) {
             mbar_init(&full_bar[s], 1);
             mbar_init(&empty_bar[s], 1);
+            stage_use[s] = 0xffffffffu;
         }
         mbar_fence_init();
     }
@@ -63,6 +66,7 @@ __global__ void __launch_bounds__(GS_THREADS) gate_sig_kernel(GateSigParams q)
                 if (j >= nst) mbar_wait(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1));
                 const int64_t tok0 = (tile0 + j) * GS_TILE;
                 const int rows = (int)min((int64_t)GS_TILE, q.LT - tok0);
+                st_release_shared(&stage_use[st], (uint32_t)(j / nst));
                 mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
                 bulk_g2s(gs_sm + (size_t)st * STAGEB, q.logits + tok0 * E, (uint32_t)rows * E * 4, &full_bar[st]);
             }
@@ -73,7 +77,9 @@ __global__ void __launch_bounds__(GS_THREADS) gate_sig_kernel(GateSigParams q)
         const int h = lane >> 4, tl = lane & 15;
         for (int64_t j = c; j < nt; j += GS_NC) {
             const int st = (int)(j % nst);
-            mbar_wait(&full_bar[st], (uint32_t)((j / nst) & 1));
+            const uint32_t use = (uint32_t)(j / nst);
+            while (ld_acquire_shared(&stage_use[st]) != use) __nanosleep(32);
+            mbar_wait(&full_bar[st], use & 1u);
             const int64_t tok0 = (tile0 + j) * GS_TILE;
             const int64_t tok = tok0 + tl;
             const bool valid = tok < q.LT;
@@ -113,7 +119,6 @@ static int launch_sig_e(GateSigParams prm, cudaStream_t st)
     constexpr int STAGEB = GS_TILE * (E * 4);
     int nst = (200 * 1024) / STAGEB;
     if (nst > GS_MAXST) nst = GS_MAXST;
-    nst = (nst / GS_NC) * GS_NC;                 // 12 stages at E = 256, 24 at E = 128 / 64
     prm.nst = nst;
     // set on every launch: the attribute is per device and cheap (cap.h: calls are re-entrant)
     cudaFuncSetAttribute(gate_sig_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);

@@ -24,9 +24,15 @@ constexpr float GS_EPS = 2.0e-6f;       // |cheap score - reference score|, boun
 constexpr float GS_THRG = 1.4e-4f;      // group scores (sums of two keys): 2 * (2 * (GS_EPS + 256 ulp(1.0)) + rounding)
 constexpr uint32_t GS_SENT = 0xff000000u;   // list filler (-1.7e38): stays finite under the payload arithmetic
 
+// 1 / (1 + 2^(-x log2 e)) on the special-function unit: FMUL, MUFU.EX2, FADD, MUFU.RCP.  The raw .ftz
+// instructions, not __expf / __fdividef: without fast-math those carry denormal-range fix-ups (14 instructions
+// per expert instead of 4).  Saturation is right by construction: 2^(+big) = inf -> 1/inf = 0, 2^(-big) = 0 -> 1.
 __device__ __forceinline__ float gs_cheap_sigmoid(float x)
 {
-    return __fdividef(1.0f, 1.0f + __expf(-x));     // ex2.approx + rcp.approx
+    float e, r;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(__fmul_rn(x, -1.4426950408889634f)));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(__fadd_rn(1.0f, e)));
+    return r;
 }
 
 // key of the cheap score: low byte <- byte j of the payload word (positions of four consecutive experts)
