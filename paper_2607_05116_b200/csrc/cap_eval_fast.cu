@@ -348,17 +348,24 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
     }
 }
 
-// ---- decode: add all records of one record word in the bit-sliced domain, extract once -------------
+// ---- decode + finalize: add all records of one record word in the bit-sliced domain, extract the integers
+// once and turn them straight into the caller's outputs (Eq. 3 costs, Eq. 4 imbalance).  A block
+// owns one record word, i.e. a few whole candidates: a device word carries the received tokens per device and the
+// local / same-node sums of its candidates (both 32-bit halves of a 64-bit field are done by the block of the even
+// word), a node word the node sums -- no accumulator array, no atomics, no separate finalize launch.  load_pairs is
+// gathered from counts x map at the start of the block, while the record loads are in flight.
 struct DecodeParams {
     const int32_t *rec_src;
     const uint32_t *rec_planes;
     const int32_t *dev_node;
-    unsigned long long *acc;    // [L][P][ACC_N]
-    unsigned long long *recv;   // [L][P][D]
-    int32_t P, D, N, WD, WN, Pc, PC, DW, W, NPR, nslots, na;
+    const int32_t *expert_dev;  // [L][P][E]
+    const long long *counts;    // [L][E]
+    cap_eval_out out;
+    long long bytes_per_token;
+    int32_t P, D, N, E, WD, WN, Pc, PC, DW, W, NPR, nslots, na;
+    int32_t cost_local, cost_intra, cost_inter;
 };
 
-// acc (na planes) += x (planes 0..EF_NPL-1 of a[], masked), ripple carry
 #define CAP_DEC_ADD(ACC, MASK)                                        \
     do {                                                              \
         uint32_t cy = 0u;                                             \
@@ -404,11 +411,17 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
     __shared__ unsigned long long nodeset[8];
     __shared__ unsigned char s_dn[64];
     __shared__ uint32_t s_part[DEC_WARPS - 1][3][NA];
+    __shared__ unsigned long long s_lp[4][64];          // load_pairs of the block's candidates (<= 4 per device word)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int w = blockIdx.x, pc = blockIdx.y, layer = blockIdx.z;
+    const int w0 = blockIdx.x, pc = blockIdx.y, layer = blockIdx.z;
+    const bool devword = w0 < q.DW;
+    const int fw = devword ? q.WD : q.WN;                 // field width of this word
+    const int nwords = (devword && q.WD == 64) ? 2 : 1;   // both halves of a 64-bit device field
     pdl_launch_dependents();
     pdl_wait();
+    if (devword && q.WD == 64 && (w0 & 1)) return;        // done by the block of the even word
     if (threadIdx.x < 64) s_dn[threadIdx.x] = (int)threadIdx.x < q.D ? (unsigned char)q.dev_node[threadIdx.x] : 0;
+    for (int i = threadIdx.x; i < 4 * 64; i += blockDim.x) (&s_lp[0][0])[i] = 0ull;
     __syncthreads();
     if (threadIdx.x < 8) {
         const int n = threadIdx.x;              // from the shared copy: one round of global loads, not D
@@ -417,117 +430,169 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
             if (s_dn[d] == n) m |= 1ull << d;
         nodeset[n] = m;
     }
+    // candidates of this block: device word -> 32 / WD of them (one for WD >= 32); their load_pairs
+    const int ncand = devword ? (q.WD >= 32 ? 1 : 32 / q.WD) : 0;
+    const int pl0 = devword ? (q.WD == 64 ? (w0 >> 1) : w0 * 32 / q.WD) : 0;
+    if (devword && (q.out.load_pairs || q.out.imbalance)) {
+        const long long *cnt = q.counts + (size_t)layer * q.E;
+        for (int c = 0; c < ncand; ++c) {
+            const int p = pc * q.Pc + pl0 + c;
+            if (pl0 + c >= q.Pc || p >= q.P) continue;
+            const int32_t *pi = q.expert_dev + ((size_t)layer * q.P + p) * q.E;
+            for (int e = threadIdx.x; e < q.E; e += blockDim.x) {
+                const int d = pi[e];
+                const long long v = __ldcg(cnt + e);
+                if ((unsigned)d < (unsigned)q.D && v) atomicAdd(&s_lp[c][d], (unsigned long long)v);
+            }
+        }
+    }
     __syncthreads();
-    const bool devword = w < q.DW;
-    uint32_t tot[NA], loc[NA], sam[NA];
-#pragma unroll
-    for (int p = 0; p < NA; ++p) tot[p] = loc[p] = sam[p] = 0u;
+    // running per-candidate results over the words of this block (meaningful on the field's leader lane)
+    unsigned long long a_gt = 0ull, a_gl = 0ull, a_gs = 0ull;
+    long long mx = 0, sm = 0, mxr = 0, smr = 0;
     const size_t sbase = ((size_t)layer * q.PC + pc) * q.nslots;
-    constexpr int DEC_SL = 2;     // record slots a thread has in flight
-    for (int s0 = threadIdx.x; s0 < q.nslots; s0 += 32 * DEC_WARPS * DEC_SL) {
-        int srcs[DEC_SL];
+    for (int wi = 0; wi < nwords; ++wi) {
+        const int w = w0 + wi;
+        uint32_t tot[NA], loc[NA], sam[NA];
 #pragma unroll
-        for (int j = 0; j < DEC_SL; ++j) {
-            const int s = s0 + j * 32 * DEC_WARPS;
-            srcs[j] = s < q.nslots ? q.rec_src[sbase + s] : -1;
-        }
-        uint32_t av[DEC_SL][EF_NPL];
+        for (int p = 0; p < NA; ++p) tot[p] = loc[p] = sam[p] = 0u;
+        constexpr int DEC_SL = 2;     // record slots a thread has in flight
+        for (int s0 = threadIdx.x; s0 < q.nslots; s0 += 32 * DEC_WARPS * DEC_SL) {
+            int srcs[DEC_SL];
 #pragma unroll
-        for (int j = 0; j < DEC_SL; ++j) {
-            const int s = s0 + j * 32 * DEC_WARPS;
-            // one 64-byte run per (slot, word); not conditional on srcs[j]: the loads go out together with the
-            // header loads (unused slots hold stale planes, skipped below)
-            const uint4 *pp = reinterpret_cast<const uint4 *>(q.rec_planes + ((sbase + s) * (size_t)q.W + w) * EF_RECW);
-            uint32_t t16[EF_RECW];
+            for (int j = 0; j < DEC_SL; ++j) {
+                const int s = s0 + j * 32 * DEC_WARPS;
+                srcs[j] = s < q.nslots ? q.rec_src[sbase + s] : -1;
+            }
+            uint32_t av[DEC_SL][EF_NPL];
 #pragma unroll
-            for (int i = 0; i < EF_RECW / 4; ++i) {
-                const uint4 x = s < q.nslots ? pp[i] : make_uint4(0u, 0u, 0u, 0u);
-                t16[4 * i] = x.x;
-                t16[4 * i + 1] = x.y;
-                t16[4 * i + 2] = x.z;
-                t16[4 * i + 3] = x.w;
+            for (int j = 0; j < DEC_SL; ++j) {
+                const int s = s0 + j * 32 * DEC_WARPS;
+                // one 64-byte run per (slot, word); not conditional on srcs[j]: the loads go out together with the
+                // header loads (unused slots hold stale planes, skipped below)
+                const uint4 *pp = reinterpret_cast<const uint4 *>(q.rec_planes + ((sbase + s) * (size_t)q.W + w) * EF_RECW);
+                uint32_t t16[EF_RECW];
+#pragma unroll
+                for (int i = 0; i < EF_RECW / 4; ++i) {
+                    const uint4 x = s < q.nslots ? pp[i] : make_uint4(0u, 0u, 0u, 0u);
+                    t16[4 * i] = x.x;
+                    t16[4 * i + 1] = x.y;
+                    t16[4 * i + 2] = x.z;
+                    t16[4 * i + 3] = x.w;
+                }
+#pragma unroll
+                for (int p = 0; p < EF_NPL; ++p) av[j][p] = t16[p];
             }
 #pragma unroll
-            for (int p = 0; p < EF_NPL; ++p) av[j][p] = t16[p];
+            for (int j = 0; j < DEC_SL; ++j) {
+                if (srcs[j] < 0) continue;
+                const int src = srcs[j] & 63;
+                const int node = s_dn[src] & 7;
+                uint32_t mloc, msam;
+                if (devword) {
+                    mloc = ef_devmask_word(q.WD, w, 1ull << src);
+                    msam = ef_devmask_word(q.WD, w, nodeset[node]);
+                } else {
+                    mloc = ef_nodemask_word(q.WN, node);
+                    msam = 0u;
+                }
+                const uint32_t(&a)[EF_NPL] = av[j];
+                CAP_DEC_ADD(tot, 0xffffffffu);
+                CAP_DEC_ADD(loc, mloc);
+                CAP_DEC_ADD(sam, msam);
+            }
         }
 #pragma unroll
-        for (int j = 0; j < DEC_SL; ++j) {
-            if (srcs[j] < 0) continue;
-            const int src = srcs[j];
-            const int node = s_dn[src];
-            uint32_t mloc, msam;
+        for (int off = 16; off > 0; off >>= 1) {
+            CAP_DEC_BFLY(tot, off);
+            CAP_DEC_BFLY(loc, off);
+            CAP_DEC_BFLY(sam, off);
+        }
+        // every lane of a warp now holds the warp's sums; warps 1.. hand theirs to warp 0
+        __syncthreads();                 // s_part of the previous word has been read
+        if (warp > 0 && lane < 3) {
+#pragma unroll
+            for (int p = 0; p < NA; ++p) {
+                const uint32_t v = lane == 0 ? tot[p] : lane == 1 ? loc[p] : sam[p];
+                s_part[warp - 1][lane][p] = v;
+            }
+        }
+        __syncthreads();
+        if (warp == 0) {
+            for (int o = 0; o < DEC_WARPS - 1; ++o) {
+                uint32_t a[NA];
+#pragma unroll
+                for (int p = 0; p < NA; ++p) a[p] = s_part[o][0][p];
+                CAP_DEC_ADD32(tot);
+#pragma unroll
+                for (int p = 0; p < NA; ++p) a[p] = s_part[o][1][p];
+                CAP_DEC_ADD32(loc);
+#pragma unroll
+                for (int p = 0; p < NA; ++p) a[p] = s_part[o][2][p];
+                CAP_DEC_ADD32(sam);
+            }
+            unsigned long long vt = 0ull, vl = 0ull, vs = 0ull;
+#pragma unroll
+            for (int p = 0; p < NA; ++p) {
+                vt |= (unsigned long long)((tot[p] >> lane) & 1u) << p;
+                vl |= (unsigned long long)((loc[p] >> lane) & 1u) << p;
+                vs |= (unsigned long long)((sam[p] >> lane) & 1u) << p;
+            }
+            // lane = bit position of the word = (candidate, device or node) of this chunk
+            const int bitpos = (devword ? w : w - q.DW) * 32 + lane;
+            const int pl = bitpos / fw, f = bitpos - pl * fw;
+            const int p = pc * q.Pc + pl;
+            const bool pvalid = pl < q.Pc && p < q.P;
+            const size_t o = (size_t)layer * q.P + p;
+            const int gw = fw < 32 ? fw : 32;
+            unsigned long long gt = vt, gl = vl, gs = vs;
+            long long l = 0, r = 0;
             if (devword) {
-                mloc = ef_devmask_word(q.WD, w, 1ull << src);
-                msam = ef_devmask_word(q.WD, w, nodeset[node]);
-            } else {
-                mloc = ef_nodemask_word(q.WN, node);
-                msam = 0u;
+                const int c = pl - pl0;
+                if (pvalid && f < q.D) {
+                    l = (long long)s_lp[c & 3][f];
+                    r = (long long)vt;
+                    if (q.out.load_pairs) q.out.load_pairs[o * q.D + f] = l;
+                    if (q.out.recv_tokens) q.out.recv_tokens[o * q.D + f] = r;
+                }
             }
-            const uint32_t(&a)[EF_NPL] = av[j];
-            CAP_DEC_ADD(tot, 0xffffffffu);
-            CAP_DEC_ADD(loc, mloc);
-            CAP_DEC_ADD(sam, msam);
-        }
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        CAP_DEC_BFLY(tot, off);
-        CAP_DEC_BFLY(loc, off);
-        CAP_DEC_BFLY(sam, off);
-    }
-    // every lane of a warp now holds the warp's sums; warps 1.. hand theirs to warp 0
-    if (warp > 0 && lane < 3) {
-#pragma unroll
-        for (int p = 0; p < NA; ++p) {
-            const uint32_t v = lane == 0 ? tot[p] : lane == 1 ? loc[p] : sam[p];
-            s_part[warp - 1][lane][p] = v;
-        }
-    }
-    __syncthreads();
-    if (warp > 0) return;
-    for (int o = 0; o < DEC_WARPS - 1; ++o) {
-        uint32_t a[NA];
-#pragma unroll
-        for (int p = 0; p < NA; ++p) a[p] = s_part[o][0][p];
-        CAP_DEC_ADD32(tot);
-#pragma unroll
-        for (int p = 0; p < NA; ++p) a[p] = s_part[o][1][p];
-        CAP_DEC_ADD32(loc);
-#pragma unroll
-        for (int p = 0; p < NA; ++p) a[p] = s_part[o][2][p];
-        CAP_DEC_ADD32(sam);
-    }
-    unsigned long long vt = 0ull, vl = 0ull, vs = 0ull;
-#pragma unroll
-    for (int p = 0; p < NA; ++p) {
-        {
-            vt |= (unsigned long long)((tot[p] >> lane) & 1u) << p;
-            vl |= (unsigned long long)((loc[p] >> lane) & 1u) << p;
-            vs |= (unsigned long long)((sam[p] >> lane) & 1u) << p;
-        }
-    }
-    const int fw = devword ? q.WD : q.WN;                 // field width of this word
-    const int bitpos = (devword ? w : w - q.DW) * 32 + lane;
-    const int pl = bitpos / fw, f = bitpos - pl * fw;
-    const int p = pc * q.Pc + pl;
-    const bool pvalid = pl < q.Pc && p < q.P;
-    if (devword && pvalid && f < q.D) q.recv[((size_t)layer * q.P + p) * q.D + f] = vt;
-    const int gw = fw < 32 ? fw : 32;
-    unsigned long long gt = vt, gl = vl, gs = vs;
-    for (int off = 1; off < gw; off <<= 1) {
-        gt += __shfl_xor_sync(0xffffffffu, gt, off);
-        gl += __shfl_xor_sync(0xffffffffu, gl, off);
-        gs += __shfl_xor_sync(0xffffffffu, gs, off);
-    }
-    if ((lane & (gw - 1)) == 0 && pvalid) {
-        unsigned long long *ac = q.acc + ((size_t)layer * q.P + p) * ACC_N;
-        if (devword) {
-            if (gt) atomicAdd(&ac[ACC_DEV], gt);
-            if (gl) atomicAdd(&ac[ACC_LOCAL], gl);
-            if (gs) atomicAdd(&ac[ACC_SAMENODE], gs);
-        } else {
-            if (gt) atomicAdd(&ac[ACC_NODE], gt);
-            if (gt - gl) atomicAdd(&ac[ACC_RNODE], gt - gl);
+            long long wmx = l, wsm = l, wmxr = r, wsmr = r;
+            for (int off = 1; off < gw; off <<= 1) {
+                gt += __shfl_xor_sync(0xffffffffu, gt, off);
+                gl += __shfl_xor_sync(0xffffffffu, gl, off);
+                gs += __shfl_xor_sync(0xffffffffu, gs, off);
+                wmx = max(wmx, __shfl_xor_sync(0xffffffffu, wmx, off));
+                wmxr = max(wmxr, __shfl_xor_sync(0xffffffffu, wmxr, off));
+                wsm += __shfl_xor_sync(0xffffffffu, wsm, off);
+                wsmr += __shfl_xor_sync(0xffffffffu, wsmr, off);
+            }
+            a_gt += gt;
+            a_gl += gl;
+            a_gs += gs;
+            mx = max(mx, wmx);
+            mxr = max(mxr, wmxr);
+            sm += wsm;
+            smr += wsmr;
+            if (wi == nwords - 1 && (lane & (gw - 1)) == 0 && pvalid) {
+                if (devword) {
+                    const long long dv = (long long)a_gt, lc = (long long)a_gl, same = (long long)a_gs;
+                    const long long rdev = dv - lc, intra = same - lc, inter = dv - same;
+                    if (q.out.dev_visits) q.out.dev_visits[o] = dv;
+                    if (q.out.remote_dev) q.out.remote_dev[o] = rdev;
+                    if (q.out.remote_intra) q.out.remote_intra[o] = intra;
+                    if (q.out.remote_inter) q.out.remote_inter[o] = inter;
+                    if (q.out.cost)
+                        q.out.cost[o] = (long long)q.cost_local * lc + (long long)q.cost_intra * intra +
+                                        (long long)q.cost_inter * inter;
+                    if (q.out.bytes) q.out.bytes[o] = rdev * q.bytes_per_token;
+                    if (q.out.imbalance) q.out.imbalance[o] = sm ? __ddiv_rn((double)(mx * q.D), (double)sm) : 0.0;
+                    if (q.out.imbalance_recv)
+                        q.out.imbalance_recv[o] = smr ? __ddiv_rn((double)(mxr * q.D), (double)smr) : 0.0;
+                } else {
+                    if (q.out.node_visits) q.out.node_visits[o] = (long long)a_gt;
+                    if (q.out.remote_node) q.out.remote_node[o] = (long long)(a_gt - a_gl);
+                }
+            }
         }
     }
 }
@@ -582,17 +647,24 @@ int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *
     return check_launch("eval_table_kernel");
 }
 
-// adds all records (g.ncta_t * g.maxrec slots per layer and chunk) into acc / recv of the generic workspace
-int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int32_t L, int64_t T, int32_t E,
-                     int32_t P, const cap_topology &topo, cudaStream_t st)
+// adds all records (g.ncta_t * g.maxrec slots per layer and chunk) and writes the caller's outputs (out: device
+// pointers, members may be NULL; counts: [L][E] kept pairs per expert, complete before this launch)
+int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, int32_t L, int64_t T, int32_t E, int32_t P,
+                     const cap_topology &topo, const int32_t *expert_dev, const int64_t *counts,
+                     const cap_eval_out &out, cudaStream_t st)
 {
-    EvalWs base = eval_ws_carve(ws, L, E, topo.D, P);
     DecodeParams dq;
     dq.rec_src = fw.rec_src;
     dq.rec_planes = fw.rec_planes;
     dq.dev_node = topo.dev_node;
-    dq.acc = base.acc;
-    dq.recv = base.recv;
+    dq.expert_dev = expert_dev;
+    dq.counts = reinterpret_cast<const long long *>(counts);
+    dq.out = out;
+    dq.bytes_per_token = topo.bytes_per_token;
+    dq.cost_local = topo.cost_local;
+    dq.cost_intra = topo.cost_intra;
+    dq.cost_inter = topo.cost_inter;
+    dq.E = E;
     dq.P = P;
     dq.D = topo.D;
     dq.N = topo.N;
@@ -623,7 +695,7 @@ int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int3
 
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                      int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
-                     void *ws, cudaStream_t st, bool *used)
+                     const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used)
 {
     *used = false;
     EvalFastGeom g;
@@ -666,7 +738,7 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     default: rc = launch_kp<16>(prm, g, L, st); break;
     }
     CAP_TRY(rc);
-    CAP_TRY(ef_launch_decode(g, fw, ws, L, T, E, P, topo, st));
+    CAP_TRY(ef_launch_decode(g, fw, L, T, E, P, topo, expert_dev, counts, out, st));
     *used = true;
     return CAP_OK;
 }

@@ -64,8 +64,9 @@ struct EfFill {
 };
 int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *expert_dev, const int32_t *dev_node,
                     int32_t L, int32_t E, int32_t P, int32_t D, cudaStream_t st, const EfFill *fills, int nfill);
-int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, void *ws, int32_t L, int64_t T, int32_t E,
-                     int32_t P, const cap_topology &topo, cudaStream_t st);
+int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, int32_t L, int64_t T, int32_t E, int32_t P,
+                     const cap_topology &topo, const int32_t *expert_dev, const int64_t *counts,
+                     const cap_eval_out &out, cudaStream_t st);
 
 // ---- device helpers ------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t lop_xor3(uint32_t a, uint32_t b, uint32_t c)

@@ -694,14 +694,12 @@ static int fused_core(const float *const *logits_list, int nlist, int nrep, floa
     const int E = cfg.E;
     EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, f.g);
     // every buffer the pass accumulates into is cleared by the table kernel itself (no memset nodes)
-    EvalWs base = eval_ws_carve(ws, L, E, topo.D, P);
-    const EfFill fills[4] = {
+    const EfFill fills[3] = {
         {counts, sizeof(int64_t) * (size_t)L * E, 0u},
         {coact, sizeof(int32_t) * (size_t)L * E * E, 0u},
         {fw.rec_src, f.g.rec_slots * 4, 0xffffffffu},
-        {base.acc, sizeof(unsigned long long) * ((size_t)L * P * ACC_N + (size_t)L * P * topo.D), 0u},
     };
-    CAP_TRY(ef_launch_table(f.g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st, fills, 4));
+    CAP_TRY(ef_launch_table(f.g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st, fills, 3));
     FusedParams prm;
     prm.logits = logits_list[0];
     prm.idx = idx;
@@ -754,8 +752,7 @@ static int fused_core(const float *const *logits_list, int nlist, int nrep, floa
         *used = true;
         return CAP_OK;        // accumulators hold nrep passes: profiling only, outputs are not finalised
     }
-    CAP_TRY(ef_launch_decode(f.g, fw, ws, L, T, E, P, topo, st));
-    CAP_TRY(launch_eval_finalize(L, E, P, expert_dev, topo, counts, out, ws, st));
+    CAP_TRY(ef_launch_decode(f.g, fw, L, T, E, P, topo, expert_dev, counts, out, st));
     *used = true;
     return CAP_OK;
 }

@@ -119,9 +119,10 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
                  const cap_topology &topo, float p, uint8_t *kept, int64_t *near_margin,
                  const cap_eval_out *after, void *ws, cudaStream_t st);
 // S3 fast path (cap_eval_fast.cu): *used = false when the sizes do not fit it
+// (decodes and finishes the outputs itself: no launch_eval_finalize after it)
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                      int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
-                     void *ws, cudaStream_t st, bool *used);
+                     const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
 size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D);
 size_t place_ws_bytes(int32_t L, int32_t E, int32_t D);   // cap_place.cu
