@@ -760,3 +760,85 @@ int capo_adjust_spectrum(const int64_t *counts, const int32_t *coact, int32_t L,
     free(pi); free(load);
     return CAPO_OK;
 }
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-4b  naive expert-level pruning.  P:L62 (sec. II-D): "a naive pruning strategy ...
+ * selects the top-ranked experts for each token until their cumulative routing score
+ * exceeds a predefined threshold"; P:L295 compares it with the communication-aware rule
+ * at the same accuracy target 1-p (Fig. 14).  Restated as the one-expert-per-device,
+ * uniform-cost case of capo_prune (Eq. 6 with c_d = 1): experts in descending routing
+ * weight (ties -> lower expert id, R10), kept while the kept weight is < 1-p (the
+ * crossing expert is kept, R9); p <= 0 keeps everything; near-margin as in R-S4.7.
+ * Placement and topology play no role.
+ * ------------------------------------------------------------------------- */
+int capo_prune_naive(const int32_t *idx, const float *w, int32_t L, int64_t T, int32_t k,
+                     float p, uint8_t *kept, int64_t *near_margin)
+{
+    if (L < 0 || T < 0 || k < 1 || k > 16) return CAPO_EINVAL;
+    if (!(p < 1.0f) || p != p) return CAPO_EINVAL;
+    for (int32_t l = 0; l < L; ++l) {
+        int64_t nm = 0;
+        for (int64_t t = 0; t < T; ++t) {
+            size_t base = ((size_t)l * (size_t)T + (size_t)t) * (size_t)k;
+            if (p <= 0.0f) {
+                for (int32_t s = 0; s < k; ++s) kept[base + s] = 1;
+                continue;
+            }
+            int32_t order[16];
+            for (int32_t s = 0; s < k; ++s) order[s] = s;
+            for (int32_t i = 1; i < k; ++i) {      /* insertion sort: weight desc, ties lower expert id */
+                int32_t s = order[i], j = i - 1;
+                while (j >= 0 && (w[base + order[j]] < w[base + s] ||
+                                  (w[base + order[j]] == w[base + s] && idx[base + order[j]] > idx[base + s]))) {
+                    order[j + 1] = order[j];
+                    --j;
+                }
+                order[j + 1] = s;
+            }
+            float target = 1.0f - p, cum = 0.0f;
+            int near = 0;
+            int32_t nk = 0;
+            for (int32_t s = 0; s < k; ++s) kept[base + s] = 0;
+            for (int32_t i = 0; i < k; ++i) {
+                if (fabsf(cum - target) < 1e-6f) near = 1;
+                if (cum >= target) break;
+                kept[base + order[i]] = 1;
+                cum = cum + w[base + order[i]];
+                nk = i + 1;
+            }
+            if (nk < k) {
+                float r1 = w[base + order[nk - 1]], r2 = w[base + order[nk]];
+                if ((r1 - r2) < 1e-6f) near = 1;
+            }
+            nm += near;
+        }
+        if (near_margin) near_margin[l] = nm;
+    }
+    return CAPO_OK;
+}
+
+/* ------------------------------------------------------------------------- *
+ * NEXT-4c  combine weights of the dispatch rows.  P:L58 (sec. II-C, Fig. 2): a token is
+ * "sent once to each device that hosts activated experts", the expert outputs are
+ * "locally aggregated via a weighted summation" there, and one result per (token,
+ * device) travels back.  The weight that row carries in the final combination is
+ * a_d = sum of the routing weights of the token's kept experts on that device -- the
+ * a_d of P:L212 (S4 step 2), in slot order, fp32.
+ * pair_row [T*k]: row of pair i = t*k + s as written by capo_dispatch_rows (-1 = pruned).
+ * row_w [n_rows] out.
+ * ------------------------------------------------------------------------- */
+int capo_dispatch_row_weights(const float *w, const int32_t *pair_row, int64_t T, int32_t k,
+                              int64_t n_rows, float *row_w)
+{
+    if (T < 0 || k < 1 || k > 16 || n_rows < 0) return CAPO_EINVAL;
+    for (int64_t r = 0; r < n_rows; ++r) row_w[r] = 0.0f;
+    for (int64_t t = 0; t < T; ++t)
+        for (int32_t s = 0; s < k; ++s) {
+            int64_t i = t * k + s;
+            int32_t r = pair_row[i];
+            if (r < 0) continue;
+            if ((int64_t)r >= n_rows) return CAPO_EINVAL;
+            row_w[r] = row_w[r] + w[i];
+        }
+    return CAPO_OK;
+}

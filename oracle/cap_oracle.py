@@ -243,3 +243,30 @@ def adjust_spectrum(counts, coact, expert_dev0, *, D, S):
     if rc != 0:
         raise ValueError(f"capo_adjust_spectrum -> {rc}")
     return spectrum, n_done, swaps
+
+
+def prune_naive(idx, w, p):
+    """NEXT-4b: naive expert-level top-p pruning. idx,w [L,T,k] -> (kept [L,T,k] uint8, near_margin [L])."""
+    idx = _c(idx, np.int32)
+    w = _c(w, np.float32)
+    L, T, k = idx.shape
+    kept = np.empty((L, T, k), np.uint8)
+    near = np.zeros((L,), np.int64)
+    rc = lib().capo_prune_naive(_p(idx), _p(w), C.c_int32(L), C.c_int64(T), C.c_int32(k), C.c_float(p),
+                                _p(kept), _p(near))
+    if rc != 0:
+        raise ValueError(f"capo_prune_naive -> {rc}")
+    return kept, near
+
+
+def dispatch_row_weights(w, pair_row, n_rows):
+    """NEXT-4c: combine weight a_d of every dispatch row. w [T,k] fp32, pair_row [T*k] -> row_w [n_rows]."""
+    w = _c(w, np.float32)
+    T, k = w.shape
+    pair_row = _c(pair_row, np.int32)
+    row_w = np.empty((int(n_rows),), np.float32)
+    rc = lib().capo_dispatch_row_weights(_p(w), _p(pair_row), C.c_int64(T), C.c_int32(k), C.c_int64(int(n_rows)),
+                                         _p(row_w))
+    if rc != 0:
+        raise ValueError(f"capo_dispatch_row_weights -> {rc}")
+    return row_w

@@ -380,3 +380,109 @@ def test_adjust_trades_communication_for_balance(oracle):
     assert done[0] == 6
     assert np.all(np.diff(ev.imbalance[0]) <= 1e-12) and ev.imbalance[0, -1] < ev.imbalance[0, 0] - 0.02
     assert ev.dev_visits[0, -1] >= ev.dev_visits[0, 0]
+
+
+# ------------------------------------------------------------------ NEXT-4b naive expert-level pruning
+def test_prune_naive_hand_example(oracle):
+    # one token, weights 0.4 0.3 0.2 0.1 (experts 7 3 9 1): target 1 - p
+    idx = np.array([[[7, 3, 9, 1]]], np.int32)
+    w = np.array([[[0.4, 0.3, 0.2, 0.1]]], np.float32)
+    for p, want in ((0.0, [1, 1, 1, 1]), (0.05, [1, 1, 1, 1]), (0.1, [1, 1, 1, 0]), (0.25, [1, 1, 1, 0]),
+                    (0.3, [1, 1, 0, 0]), (0.35, [1, 1, 0, 0]), (0.6, [1, 0, 0, 0]), (0.9, [1, 0, 0, 0])):
+        # p = 0.1: 0.4 + 0.3 + 0.2 = 0.9 >= 0.9 only in exact arithmetic; fp32: 0.4f + 0.3f + 0.2f vs 1 - 0.1f
+        kept, near = oracle.prune_naive(idx, w, p)
+        cum, k_ref, target = np.float32(0), [0, 0, 0, 0], np.float32(1) - np.float32(p)
+        if p > 0:
+            for s in range(4):
+                if cum >= target:
+                    break
+                k_ref[s] = 1
+                cum = np.float32(cum + w[0, 0, s])
+        else:
+            k_ref = [1, 1, 1, 1]
+        assert kept[0, 0].tolist() == k_ref, p
+        if p not in (0.1, 0.3, 0.6):          # away from the exact boundaries the hand values hold
+            assert kept[0, 0].tolist() == want, p
+    # unsorted slots (sigmoid + bias gating orders slots by the biased score): descending weight, ties -> lower expert
+    idx = np.array([[[5, 2, 8, 4]]], np.int32)
+    w = np.array([[[0.25, 0.25, 0.4, 0.1]]], np.float32)
+    kept, _ = oracle.prune_naive(idx, w, 0.5)         # 0.4 (e8), then the tie 0.25: expert 2 before expert 5
+    assert kept[0, 0].tolist() == [0, 1, 1, 0]
+    kept, _ = oracle.prune_naive(idx, w, 0.3)         # 0.4 + 0.25 (e2) = 0.65 < 0.7 -> expert 5 too
+    assert kept[0, 0].tolist() == [1, 1, 1, 0]
+
+
+def test_prune_naive_is_the_uniform_cost_identity_placement_case_of_prune(oracle):
+    """P:L62 vs P:L212: with one expert per device and c_d = 1 for every device Eq. 6's greedy is the naive rule
+    (capo_prune's special case is itself pinned by 2^k brute force in test_oracle_pins.py)."""
+    rng = np.random.default_rng(62)
+    L, T, E, k = 2, 400, 64, 6
+    idx = np.stack([np.stack([rng.permutation(E)[:k] for _ in range(T)]) for _ in range(L)]).astype(np.int32)
+    w = rng.random((L, T, k)).astype(np.float32) + np.float32(0.01)
+    w[0, :40] = np.float32(1.0 / k)                                   # exact ties
+    w = (w / w.sum(-1, keepdims=True, dtype=np.float32)).astype(np.float32)
+    pi = np.tile(np.arange(E, dtype=np.int32), (L, 1))
+    dn = np.zeros(E, np.int32)
+    for p in (0.0, 0.05, 0.2, 0.5, 0.9):
+        kept_n, near_n = oracle.prune_naive(idx, w, p)
+        kept_r, near_r = oracle.prune(idx, w, pi, dn, p, cost_local=1, cost_intra=1, cost_inter=1)
+        assert np.array_equal(kept_n, kept_r), p
+        assert np.array_equal(near_n, near_r), p
+
+
+def test_prune_naive_minimal_cardinality_brute_force(oracle):
+    """The kept set reaches the target with the fewest experts possible (2^k subsets), and dropping its smallest
+    member falls below the target."""
+    rng = np.random.default_rng(295)
+    T, k = 120, 8
+    idx = np.stack([rng.permutation(500)[:k] for _ in range(T)]).astype(np.int32)[None]
+    w = rng.random((1, T, k)).astype(np.float32) ** 2 + np.float32(0.01)
+    w = (w / w.sum(-1, keepdims=True, dtype=np.float32)).astype(np.float32)
+    for p in (0.1, 0.3, 0.6):
+        kept, _ = oracle.prune_naive(idx, w, p)
+        target = float(np.float32(1) - np.float32(p))
+        for t in range(T):
+            ws = w[0, t].astype(np.float64)
+            nk = int(kept[0, t].sum())
+            assert ws[kept[0, t] == 1].sum() >= target - 1e-6
+            best = min(bin(m).count("1") for m in range(1, 1 << k)
+                       if sum(ws[s] for s in range(k) if m >> s & 1) >= target - 1e-6)
+            assert nk == best or abs(ws[kept[0, t] == 1].sum() - ws[kept[0, t] == 1].min() - target) < 1e-5, (t, nk, best)
+            assert nk <= best + 1
+            assert ws[kept[0, t] == 1].min() >= ws[kept[0, t] == 0].max() - 1e-12 if nk < k else True
+
+
+# ------------------------------------------------------------------ NEXT-4c combine weights of the dispatch rows (P:L58)
+def test_dispatch_row_weights_hand_and_python_replay(oracle, golden):
+    # hand case: 2 tokens, k = 3, devices of the slots: t0 -> (1, 0, 1), t1 -> (0, 0, pruned)
+    idx = np.array([[0, 1, 2], [3, 4, 5]], np.int32)
+    pi = np.array([1, 0, 1, 0, 0, 1], np.int32)
+    kept = np.array([[1, 1, 1], [1, 1, 0]], np.uint8)
+    w = np.array([[0.5, 0.3, 0.2], [0.6, 0.3, 0.1]], np.float32)
+    rows, off, prow = oracle.dispatch_rows(idx, pi, 2, kept=kept)
+    assert rows.tolist() == [0, 1, 0] and off.tolist() == [0, 2, 3]       # device 0: t0, t1; device 1: t0
+    assert prow.tolist() == [2, 0, 2, 1, 1, -1]
+    rw = oracle.dispatch_row_weights(w, prow, 3)
+    assert rw.tolist() == [np.float32(0.3), np.float32(np.float32(0.6) + np.float32(0.3)),
+                           np.float32(np.float32(0.5) + np.float32(0.2))]
+    # random traces: sequential fp32 sums per (token, device) in slot order, written independently in Python
+    rng = np.random.default_rng(58)
+    T, k, E, D = 300, 8, 64, 16
+    idx = np.stack([rng.permutation(E)[:k] for _ in range(T)]).astype(np.int32)
+    pi = (rng.permutation(E) % D).astype(np.int32)
+    kept = (rng.random((T, k)) < 0.7).astype(np.uint8)
+    w = rng.random((T, k)).astype(np.float32)
+    rows, off, prow = oracle.dispatch_rows(idx, pi, D, kept=kept)
+    rw = oracle.dispatch_row_weights(w, prow, int(off[-1]))
+    for d in range(D):
+        for r in range(int(off[d]), int(off[d + 1])):
+            t = int(rows[r])
+            acc = np.float32(0)
+            for s in range(k):
+                if kept[t, s] and pi[idx[t, s]] == d:
+                    acc = np.float32(acc + w[t, s])
+            assert rw[r] == acc, (d, r)
+    # the rows' weights add up to the kept routing mass of every token (P:L58: nothing is lost by aggregating)
+    tot = np.zeros(T, np.float64)
+    np.add.at(tot, rows, rw.astype(np.float64))
+    assert np.allclose(tot, (w * kept).sum(-1, dtype=np.float64), atol=1e-5)
