@@ -252,6 +252,26 @@ int cap_dispatch_rows(const int32_t *topk_idx, const uint8_t *kept, int64_t T, i
                       const int32_t *expert_dev, int32_t D, int32_t *rows_token, int32_t *pair_row,
                       int64_t *row_offsets, void *ws, size_t ws_bytes, void *stream);
 
+/* Combine weights of the dispatch rows.  P:L58: the outputs of a token's experts on one
+ * device are "locally aggregated via a weighted summation" and one result per (token, device) row returns; the
+ * weight of that row is a_d of P:L212 -- the fp32 sum, in slot order, of the routing weights of the token's kept
+ * experts on the device.
+ *   topk_w [T][k] fp32; pair_row [T*k] int32 as written by cap_dispatch_rows (-1 = pruned pair);
+ *   n_rows = row_offsets[D] of that call (the caller reads it back, or passes the capacity T * min(k, D));
+ *   row_w [n_rows] fp32 out: row_w[pair_row[i]] = sum over the pairs of that row.  Rows >= n_rows are skipped.
+ * Bit-exact against the oracle (single IEEE adds in a fixed order).  No workspace. */
+int cap_dispatch_row_weights(const float *topk_w, const int32_t *pair_row, int64_t T, int32_t k, int64_t n_rows,
+                             float *row_w, void *stream);
+
+/* Naive expert-level pruning (the baseline of Fig. 14 / P:L295): per token the experts
+ * in descending routing weight (ties -> lower expert id) are kept while the kept weight is < 1 - p (the crossing
+ * expert is kept; p <= 0 keeps everything) -- cap_prune's rule with one expert per device and c_d = 1, so that the
+ * two can be compared at the same accuracy target.  No placement, no topology.
+ *   topk_idx, topk_w [L][T][k]; kept [L][T][k] uint8 out; near_margin [L] int64 or NULL (as in cap_prune).
+ * Same precondition as cap_prune: a token's weights sum to 1.  EINVAL unless p < 1.  No workspace. */
+int cap_prune_naive(const int32_t *topk_idx, const float *topk_w, int32_t L, int64_t T, int32_t k, float p,
+                    uint8_t *kept, int64_t *near_margin, void *stream);
+
 /* Pairwise communication objective of P:L152-158 (Eq. 2-3) for P candidate placements, computed from
  * the co-activation statistics alone: C(pi) = sum_{i<j} w_ij d(pi(i), pi(j)) with
  * d = 0 on the same device, topo->cost_intra (the paper's 1) on the same node, topo->cost_inter (the

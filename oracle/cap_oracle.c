@@ -28,7 +28,9 @@
  * capo_eval_placements, capo_prune, capo_dispatch_layout) and the consumers of
  * S2 in SURVEY.md 8(f): capo_coact_placement (p_ij + Algorithm 1),
  * capo_adjust_spectrum, capo_pairwise_objective (Eq. 2-3, Eq. 5),
- * capo_dispatch_rows (Fig. 2's one copy per device).
+ * capo_dispatch_rows (Fig. 2's one copy per device), capo_dispatch_row_weights
+ * (the combine weight a_d of each row) and capo_prune_naive (the naive
+ * expert-level baseline of P:L62 / Fig. 14).
  *
  * All arrays are HOST pointers, row-major, layouts as in include/cap.h.
  */

@@ -20,7 +20,7 @@ EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prun
            "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_adjust_spectrum", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan",
-           "cap_dispatch_layout_static", "cap_static_scratch_bytes")
+           "cap_dispatch_layout_static", "cap_static_scratch_bytes", "cap_prune_naive", "cap_dispatch_row_weights")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
@@ -90,6 +90,8 @@ def lib():
         L.cap_trace_fused_plan.argtypes = [i32, i64, C.POINTER(GateCfg), i32, i32, i32, C.POINTER(C.c_int64)]
         L.cap_dispatch_layout_static.argtypes = [vp, vp, i64, i32, i32, vp, i32, vp, vp, vp, vp]
         L.cap_static_scratch_bytes.restype = C.c_size_t
+        L.cap_prune_naive.argtypes = [vp, vp, i32, i64, i32, f32, vp, vp, vp]
+        L.cap_dispatch_row_weights.argtypes = [vp, vp, i64, i32, i64, vp, vp]
         L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
         L.cap_kernel_timer_ms.argtypes = [C.c_int]
         L.cap_kernel_timer_ms.restype = C.c_float
@@ -311,6 +313,30 @@ def dispatch_rows(idx, kept, expert_dev, D, want_pair_row=True, ws=None):
                                  _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_dispatch_rows")
     return rows, offsets, pair_row
+
+
+def prune_naive(idx, w, p, kept=None, near_margin=None):
+    """cap_prune_naive: naive expert-level top-p pruning. idx, w [L,T,k] -> (kept [L,T,k] uint8, near [L])."""
+    L, T, k = idx.shape
+    if kept is None:
+        kept = torch.empty((L, T, k), dtype=torch.uint8, device=idx.device)
+    if near_margin is None:
+        near_margin = torch.empty((L,), dtype=torch.int64, device=idx.device)
+    rc = lib().cap_prune_naive(_ptr(idx, torch.int32), _ptr(w, torch.float32), L, T, k, float(p), _ptr(kept),
+                               _ptr(near_margin), _stream())
+    _check(rc, "cap_prune_naive")
+    return kept, near_margin
+
+
+def dispatch_row_weights(w, pair_row, n_rows, row_w=None):
+    """cap_dispatch_row_weights: combine weight a_d of every dispatch row. w [T,k], pair_row [T*k]."""
+    T, k = w.shape
+    if row_w is None:
+        row_w = torch.empty((max(int(n_rows), 1),), dtype=torch.float32, device=w.device)
+    rc = lib().cap_dispatch_row_weights(_ptr(w, torch.float32), _ptr(pair_row, torch.int32), T, k, int(n_rows),
+                                        _ptr(row_w), _stream())
+    _check(rc, "cap_dispatch_row_weights")
+    return row_w[: int(n_rows)]
 
 
 def pairwise_objective(counts, coact, expert_dev, topo, lam=0.5, imbalance=None):

@@ -287,3 +287,59 @@ def test_adjust_kernel_time():
     b.record()
     torch.cuda.synchronize()
     print(f"cap_adjust_spectrum qwen3: L={L} E={cfg.E} D={cfg.D} S=7: {a.elapsed_time(b) / 5 * 1e3:.1f} us per call")
+
+
+# ------------------------------------------------------------------ rest of SURVEY 8(f) rank 4
+@pytest.mark.parametrize("name,T", [("tiny", 4096), ("target", 65536), ("dsv3", 8192), ("stress", 16384)])
+def test_prune_naive_and_row_weights_on_baseline_configs(name, T):
+    """cap_prune_naive and cap_dispatch_row_weights bit-exact against the oracle, chained on the CUDA
+    path: gate -> naive pruning -> dispatch rows under the sequential placement -> combine weights."""
+    cfg = W.CONFIGS[name]
+    xs, bias, idx_r, _, _ = trace_stats(cfg, (0, 1) if cfg.L > 1 else (0,), T)
+    _, w_r = O.gate_topk(xs, bias, **cfg.gate)
+    gi, gw = cap.gate_topk(dev(xs), dev(bias), cap.gate_cfg(cfg.E, **cfg.gate))
+    for p in (0.0, 0.05, 0.3, 0.7):
+        kept_r, near_r = O.prune_naive(idx_r, w_r, p)
+        kept_d, near_d = cap.prune_naive(dev(idx_r), dev(w_r), p)
+        np.testing.assert_array_equal(host(kept_d), kept_r, err_msg=f"{name} p={p} kept")
+        np.testing.assert_array_equal(host(near_d), near_r, err_msg=f"{name} p={p} near")
+        kept_e, _ = cap.prune_naive(gi, gw, p)                       # end to end on the GPU's own S1 output
+        assert int((host(kept_e) != kept_r).any(-1).sum()) <= int(near_r.sum())
+    # exact ties and unsorted weights
+    rng = np.random.default_rng(cfg.index)
+    w_t = np.round(rng.random(w_r.shape).astype(np.float32) * 8) / 8 + np.float32(0.125)
+    w_t = (w_t / w_t.sum(-1, keepdims=True, dtype=np.float32)).astype(np.float32)
+    kept_r, near_r = O.prune_naive(idx_r, w_t, 0.25)
+    kept_d, near_d = cap.prune_naive(dev(idx_r), dev(w_t), 0.25)
+    np.testing.assert_array_equal(host(kept_d), kept_r)
+    np.testing.assert_array_equal(host(near_d), near_r)
+    # combine weights of the rows of layer 0 under the sequential placement, pruned trace
+    pi = W.candidates(cfg, 0)[0]
+    kept0, _ = O.prune_naive(idx_r[:1], w_r[:1], 0.3)
+    rows_r, off_r, prow_r = O.dispatch_rows(idx_r[0], pi, cfg.D, kept=kept0[0])
+    rw_r = O.dispatch_row_weights(w_r[0], prow_r, int(off_r[-1]))
+    rows_d, off_d, prow_d = cap.dispatch_rows(dev(idx_r[0]), dev(kept0[0]), dev(pi), cfg.D)
+    n_rows = int(off_d[-1])
+    rw_d = cap.dispatch_row_weights(dev(w_r[0]), prow_d, n_rows)
+    np.testing.assert_array_equal(host(prow_d), prow_r)
+    np.testing.assert_array_equal(host(rw_d).view(np.int32), rw_r.view(np.int32), err_msg="row weights (bits)")
+
+
+def test_prune_naive_edges():
+    idx = torch.zeros((1, 0, 4), dtype=torch.int32, device="cuda")
+    w = torch.zeros((1, 0, 4), dtype=torch.float32, device="cuda")
+    kept, near = cap.prune_naive(idx, w, 0.1)
+    assert kept.shape == (1, 0, 4) and int(near[0]) == 0
+    with pytest.raises(cap.CapError, match="EINVAL"):
+        cap.prune_naive(idx, w, 1.0)
+    rng = np.random.default_rng(1)
+    for k in (1, 9, 16):
+        T = 1000
+        idx_h = np.stack([rng.permutation(1024)[:k] for _ in range(T)]).astype(np.int32)[None]
+        w_h = rng.random((1, T, k)).astype(np.float32) + np.float32(0.01)
+        w_h = (w_h / w_h.sum(-1, keepdims=True, dtype=np.float32)).astype(np.float32)
+        for p in (0.1, 0.5):
+            kept_r, near_r = O.prune_naive(idx_h, w_h, p)
+            kept_d, near_d = cap.prune_naive(dev(idx_h), dev(w_h), p)
+            np.testing.assert_array_equal(host(kept_d), kept_r)
+            np.testing.assert_array_equal(host(near_d), near_r)
