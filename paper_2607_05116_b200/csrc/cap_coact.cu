@@ -69,11 +69,8 @@ int launch_coactivation(const int32_t *idx, const uint8_t *kept, int32_t L, int6
     const size_t smem_full = sizeof(int) * ((size_t)E * E + E);
     const int use_smem = smem_full <= 160 * 1024;
     const size_t smem = use_smem ? smem_full : sizeof(int) * (size_t)E;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(coact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 164 * 1024);
-        attr_set = true;
-    }
+    // per device and cheap: set on every launch (a per-process flag would leave a second GPU without the opt-in)
+    cudaFuncSetAttribute(coact_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 164 * 1024);
     // enough blocks per layer to fill the machine, but each block's flush costs E*E atomics
     int64_t want = (2 * (int64_t)sm_count() + L - 1) / L;
     if (want < 1) want = 1;

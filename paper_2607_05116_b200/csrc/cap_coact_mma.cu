@@ -190,12 +190,9 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
 template <int EP, int KMAX>
 static int launch_ep(const CoactMmaParams &prm, int L, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(coact_mma_kernel<EP, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             2 * EP * CM_TK);
-        attr_set = true;
-    }
+    // per device and cheap: set on every launch (a per-process flag would leave a second GPU without the opt-in)
+    cudaFuncSetAttribute(coact_mma_kernel<EP, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    2 * EP * CM_TK);
     const int64_t nblk = (prm.T + prm.tpc - 1) / prm.tpc;
     {
         KernelTimerScope ts("coact", st);

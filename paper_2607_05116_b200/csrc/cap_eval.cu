@@ -285,11 +285,8 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
         while (PC > 32 && eval_smem_bytes(E, D, PC, want_tok) > 200 * 1024) PC >>= 1;
         if (P < PC) PC = ((P + 31) / 32) * 32;
         const size_t smem = eval_smem_bytes(E, D, PC, want_tok);
-        static bool attr_set = false;
-        if (!attr_set) {
-            cudaFuncSetAttribute(eval_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-            attr_set = true;
-        }
+        // per device and cheap: set on every launch (a per-process flag would leave a second GPU without the opt-in)
+        cudaFuncSetAttribute(eval_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
         const int pchunks = (P + PC - 1) / PC;
         int64_t want = (2 * (int64_t)sm_count() + (int64_t)pchunks * L - 1) / ((int64_t)pchunks * L);
         if (want < 1) want = 1;

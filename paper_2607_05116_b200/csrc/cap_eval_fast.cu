@@ -23,9 +23,9 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     g->KP = (k + 3) & ~3;
     const int unit = 128 / g->WD;                 // candidates per 16-byte column of the device section
     const int Pfull = ((P + unit - 1) / unit) * unit;
-    // largest chunk whose table fits: (E + 1) rows of RS * 16 bytes
-    int Pc = Pfull;
-    for (;;) {
+    // largest chunk whose table fits: (E + 1) rows of RS * 16 bytes; the chunk shrinks in single-column steps and
+    // the chunks are then equalised
+    auto fits = [&](int Pc, bool commit) {
         const int dcol = Pc * g->WD / 128;
         const int ncol = (Pc * g->WN + 127) / 128;
         const int R = dcol + ncol;
@@ -36,7 +36,8 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
         const size_t offs = (size_t)2 * EF_PASSES * S * g->KP * 4;
         const size_t xch = (size_t)(S / 2) * R * EF_NPL * 16;
         const size_t smem = tbl + offs + xch + 128;
-        if (smem <= smem_budget && R * 1 <= 320) {
+        if (smem > smem_budget || R > 320) return false;
+        if (commit) {
             g->Pc = Pc;
             g->DW = dcol * 4;
             g->NW = ncol * 4;
@@ -46,10 +47,19 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
             g->S = S;
             g->logS = ceil_log2(S);
             g->smem = smem;
-            break;
         }
+        return true;
+    };
+    int Pc = Pfull;
+    while (!fits(Pc, false)) {
         if (Pc <= unit) return false;
-        Pc = ((Pc / 2 + unit - 1) / unit) * unit;
+        Pc -= unit;
+    }
+    {
+        const int chunks = (Pfull + Pc - 1) / Pc;
+        int eq = (((Pfull + chunks - 1) / chunks + unit - 1) / unit) * unit;
+        if (eq > Pc || !fits(eq, false)) eq = Pc;
+        fits(eq, true);
     }
     g->PC = (P + g->Pc - 1) / g->Pc;
     // enough threads to own every (sub-slot, column) pair and to prefetch a block's index entries
@@ -63,8 +73,25 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     g->nthreads = ((need + 31) / 32) * 32;
     if (g->nthreads > EF_MAXTHREADS) return false;
     const int64_t blk = (int64_t)EF_PASSES * g->S;
-    int64_t want = ((int64_t)target_ctas + (int64_t)g->PC * L - 1) / ((int64_t)g->PC * L);
-    if (want < 1) want = 1;
+    // Blocks along the token axis per (layer, chunk).  All blocks do the same work, so the kernel lasts
+    // ceil(blocks / SMs) block-times of 1 / want of a unit each: pick the `want` that minimises
+    // ceil(units * want / SMs) / want (ncu on config 5: 32 units x 5 = 160 blocks on 148 SMs was 1.08 waves, i.e.
+    // two block-times with 12 blocks alone in the second; 32 x 9 = 288 blocks is 1.95 waves of blocks half the size),
+    // among block sizes that still amortise the table copy (>= 16 scoring blocks of tokens each).
+    const int64_t units = (int64_t)g->PC * L;
+    int64_t want = 1;
+    {
+        const int64_t max_want = (T / (16 * blk)) > 1 ? (T / (16 * blk)) : 1;
+        double best = 1e30;
+        for (int64_t wnt = 1; wnt <= 64 && wnt <= max_want; ++wnt) {
+            const int64_t waves = (units * wnt + target_ctas - 1) / target_ctas;
+            const double cost = (double)waves / (double)wnt * (1.0 + 0.01 * (double)wnt);   // mild pull toward fewer blocks
+            if (cost < best - 1e-12) {
+                best = cost;
+                want = wnt;
+            }
+        }
+    }
     int64_t tpc = (T + want - 1) / want;
     tpc = ((tpc + blk - 1) / blk) * blk;
     g->tpc = tpc;

@@ -668,11 +668,8 @@ bool fused_plan(int32_t L, int64_t T, const cap_gate_cfg &cfg, int32_t D, int32_
 template <int E>
 static int launch_fused_e(const FusedParams &prm, const FusedGeom &f, int L, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(trace_fused_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
-        attr_set = true;
-    }
+    // per device and cheap: set on every launch (a per-process flag would leave a second GPU without the opt-in)
+    cudaFuncSetAttribute(trace_fused_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
     {
         KernelTimerScope ts("trace_fused", st);
         launch_pdl(trace_fused_kernel<E>, dim3((unsigned)f.g.ncta_t, (unsigned)L), dim3(f.nthreads), f.smem, st, prm);

@@ -111,11 +111,8 @@ static int launch_e(GateFastParams prm, cudaStream_t st)
     if (nst > GF_MAXST) nst = GF_MAXST;
     nst = (nst / GF_NC) * GF_NC;
     prm.nst = nst;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(gate_fast_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
-        attr_set = true;
-    }
+    // per device and cheap: set on every launch (a per-process flag would leave a second GPU without the opt-in)
+    cudaFuncSetAttribute(gate_fast_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
     const int64_t ntiles = (prm.LT + GF_TILE - 1) / GF_TILE;
     int64_t grid = sm_count();
     if (grid > ntiles) grid = ntiles;

@@ -242,12 +242,9 @@ int launch_place(const int64_t *counts, const int32_t *coact, int32_t L, int32_t
     if (gs1 > D) gs1 = D;
     size_t dyn = (size_t)gs1 * E * sizeof(double);
     if (dyn < (size_t)N * D * sizeof(double)) dyn = (size_t)N * D * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 196608) != cudaSuccess)
-            return check_launch("place_kernel attribute");
-        attr_set = true;
-    }
+    // per device and cheap: set on every launch (a per-process flag would leave a second GPU without the opt-in)
+    if (cudaFuncSetAttribute(place_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 196608) != cudaSuccess)
+        return check_launch("place_kernel attribute");
     KernelTimerScope kt("coact_placement", st);
     place_kernel<<<L, threads, dyn, st>>>(counts, coact, E, D, N, rnd, p_out, wsP, wsS, wsW, expert_group,
                                           group_node, expert_dev, gs1);
