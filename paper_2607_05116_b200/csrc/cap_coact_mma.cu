@@ -218,8 +218,9 @@ int launch_coact_mma(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     prm.E = E;
     prm.EP = E <= 128 ? 128 : 256;
     prm.pack64 = (E % 2 == 0) && (reinterpret_cast<uintptr_t>(coact) & 7u) == 0;
-    int64_t want = ((int64_t)sm_count() + L - 1) / L;
-    if (want < 1) want = 1;
+    // one block per SM is resident at EP = 256 (all 512 TMEM columns); every block ends with E^2 reductions into
+    // the matrix, so a block should own at least ~1 000 tokens
+    int64_t want = balanced_blocks_per_unit(L, sm_count(), T / 1024 > 1 ? T / 1024 : 1);
     int64_t tpc = (T + want - 1) / want;
     tpc = ((tpc + CM_TK - 1) / CM_TK) * CM_TK;
     prm.tpc = tpc;

@@ -109,7 +109,7 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     return true;
 }
 
-static size_t ef_budget() { return 200 * 1024; }
+static size_t ef_budget() { return 224 * 1024; }    // of the 227 KB a block may opt into (no static shared memory here)
 
 size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P)
 {
@@ -630,7 +630,7 @@ static int launch_kp(const EvalFastParams &prm, const EvalFastGeom &g, int L, cu
 {
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(eval_fast_kernel<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 210 * 1024);
+        cudaFuncSetAttribute(eval_fast_kernel<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
         attr_set = true;
     }
     dim3 grid((unsigned)g.ncta_t, (unsigned)g.PC, (unsigned)L);

@@ -53,6 +53,27 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+// Blocks per unit (layer, candidate chunk) of a grid whose blocks all do the same work on `slots` concurrently
+// resident blocks: the kernel lasts ceil(units * w / slots) block-times of 1 / w of a unit each, so minimise
+// ceil(units * w / slots) / w (58 layers x 3 = 174 blocks on 148 SMs is two block-times; x 5 = 290 is two block-times
+// of blocks 3/5 the size).  A small per-block term keeps the count low where it does not matter.
+inline int64_t balanced_blocks_per_unit(int64_t units, int64_t slots, int64_t max_w)
+{
+    if (units < 1) units = 1;
+    if (max_w > slots) max_w = slots;
+    int64_t best_w = 1;
+    double best = 1e300;
+    for (int64_t w = 1; w <= max_w; ++w) {
+        const int64_t waves = (units * w + slots - 1) / slots;
+        const double cost = (double)waves / (double)w * (1.0 + 0.002 * (double)w);
+        if (cost < best - 1e-12) {
+            best = cost;
+            best_w = w;
+        }
+    }
+    return best_w;
+}
+
 #define CAP_TRY(expr)                      \
     do {                                   \
         int _rc = (expr);                  \
