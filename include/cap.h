@@ -150,6 +150,15 @@ int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T,
                         int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes,
                         void *stream);
 
+/* S5 for L layers in one call (three launches for all layers instead of three per layer: at the BASELINE sizes a
+ * layer's sort is launch-latency-bound).  Per layer exactly cap_dispatch_layout: topk_idx / kept [L][T][k],
+ * expert_dev [L][E] (one chosen placement per layer), sorted_pairs / pair_pos [L][T*k] (layer l's first
+ * offsets[l][D] entries valid), offsets [L][D+1].  Workspace: cap_workspace_bytes(CAP_CALL_DISPATCH_LAYOUT, L, T,
+ * E, k, D, 0) (for L = 1 that is cap_dispatch_layout's size). */
+int cap_dispatch_layout_batched(const int32_t *topk_idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
+                                int32_t E, const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs,
+                                int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes, void *stream);
+
 /* S5 without a workspace, for callers that cannot allocate (CUDA graph capture, serving loops, harnesses
  * that forbid cudaMalloc).  Same result, bit for bit, as cap_dispatch_layout; the scratch is a static device
  * array of CAP_STATIC_SCRATCH_BYTES (4 MiB) inside the library, held by every GPU that loads it until exit.

@@ -20,7 +20,7 @@ EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prun
            "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_adjust_spectrum", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan",
-           "cap_dispatch_layout_static", "cap_static_scratch_bytes", "cap_prune_naive", "cap_dispatch_row_weights")
+           "cap_dispatch_layout_static", "cap_static_scratch_bytes", "cap_prune_naive", "cap_dispatch_row_weights", "cap_dispatch_layout_batched")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
@@ -92,6 +92,7 @@ def lib():
         L.cap_static_scratch_bytes.restype = C.c_size_t
         L.cap_prune_naive.argtypes = [vp, vp, i32, i64, i32, f32, vp, vp, vp]
         L.cap_dispatch_row_weights.argtypes = [vp, vp, i64, i32, i64, vp, vp]
+        L.cap_dispatch_layout_batched.argtypes = [vp, vp, i32, i64, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
         L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
         L.cap_kernel_timer_ms.argtypes = [C.c_int]
         L.cap_kernel_timer_ms.restype = C.c_float
@@ -243,6 +244,26 @@ def dispatch_layout(idx, kept, expert_dev, D, want_pos=True, ws=None):
                                    _ptr(expert_dev, torch.int32), D, _ptr(sorted_pairs),
                                    _ptr(pair_pos), _ptr(offsets), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_dispatch_layout")
+    return sorted_pairs, offsets, pair_pos
+
+
+def dispatch_layout_batched(idx, kept, expert_dev, D, want_pos=True, ws=None, out=None):
+    """cap_dispatch_layout_batched: S5 for all layers in one call.  idx [L,T,k], kept [L,T,k]|None, expert_dev [L,E]
+    -> (sorted_pairs [L,T*k], offsets [L,D+1], pair_pos [L,T*k]|None)."""
+    L, T, k = idx.shape
+    E = expert_dev.shape[-1]
+    if out is None:
+        sorted_pairs = torch.empty((L, T * k), dtype=torch.int32, device=idx.device)
+        pair_pos = torch.empty((L, T * k), dtype=torch.int32, device=idx.device) if want_pos else None
+        offsets = torch.empty((L, D + 1), dtype=torch.int64, device=idx.device)
+    else:
+        sorted_pairs, offsets, pair_pos = out
+    if ws is None:
+        ws = workspace(CALL_DISPATCH_LAYOUT, L, T, E, k, D, 0, idx.device)
+    rc = lib().cap_dispatch_layout_batched(_ptr(idx, torch.int32), _ptr(kept, torch.uint8), L, T, k, E,
+                                           _ptr(expert_dev, torch.int32), D, _ptr(sorted_pairs), _ptr(pair_pos),
+                                           _ptr(offsets), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "cap_dispatch_layout_batched")
     return sorted_pairs, offsets, pair_pos
 
 
@@ -449,7 +470,7 @@ class Pipeline:
         self.sorted_pairs = torch.empty((L, T * k), dtype=torch.int32, device=device)
         self.pair_pos = torch.empty((L, T * k), dtype=torch.int32, device=device)
         self.offsets = torch.empty((L, D + 1), dtype=torch.int64, device=device)
-        self.ws_disp = workspace(CALL_DISPATCH_LAYOUT, 1, T, E, k, D, 0, device)
+        self.ws_disp = workspace(CALL_DISPATCH_LAYOUT, L, T, E, k, D, 0, device)
         self.pi = torch.empty((L, E), dtype=torch.int32, device=device)
 
     def clone(self):
@@ -471,14 +492,9 @@ class Pipeline:
         _check(rc, "cap_prune")
 
     def step_dispatch(self, pi):
-        """S5, one call per layer, on the kept mask of the last cap_prune."""
-        st = _stream()
-        for l in range(self.L):
-            rc = lib().cap_dispatch_layout(_ptr(self.fb.idx[l]), _ptr(self.kept[l]), self.T, self.gate.k,
-                                           self.gate.E, _ptr(pi[l]), self.D, _ptr(self.sorted_pairs[l]),
-                                           _ptr(self.pair_pos[l]), _ptr(self.offsets[l]),
-                                           _ptr(self.ws_disp), self.ws_disp.numel(), st)
-            _check(rc, "cap_dispatch_layout")
+        """S5 for every layer on the kept mask of the last cap_prune: one batched call (three launches)."""
+        dispatch_layout_batched(self.fb.idx, self.kept, pi if pi.is_contiguous() else pi.contiguous(), self.D,
+                                ws=self.ws_disp, out=(self.sorted_pairs, self.offsets, self.pair_pos))
 
     def step(self, logits, bias, token_src, expert_dev):
         trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)

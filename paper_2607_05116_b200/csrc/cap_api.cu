@@ -168,7 +168,7 @@ size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int3
         return eval_ws_bytes(L, T, E, k, D, 1);
     case CAP_CALL_DISPATCH_LAYOUT:
         if (D < 1) return 0;
-        return dispatch_ws_bytes(T, k, D);
+        return L > 1 ? dispatch_ws_bytes_batched(L, T, k, D) : dispatch_ws_bytes(T, k, D);   // L > 1: the batched call
     case CAP_CALL_DISPATCH_ROWS:
         if (D < 1) return 0;
         return dispatch_rows_ws_bytes(T, D);
@@ -236,6 +236,18 @@ int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T,
     if (T > 0 && (!ws || ws_bytes < dispatch_ws_bytes(T, k, D))) return CAP_EWORKSPACE;
     return launch_dispatch(topk_idx, kept, T, k, E, expert_dev, D, sorted_pairs, pair_pos, offsets, ws,
                            (cudaStream_t)stream);
+}
+
+int cap_dispatch_layout_batched(const int32_t *topk_idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
+                                int32_t E, const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs,
+                                int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes, void *stream)
+{
+    if (!sizes_ok(L, T, E, k) || D < 1 || D > 64) return CAP_EINVAL;
+    if (L > 0 && (!offsets || !expert_dev)) return CAP_EINVAL;
+    if ((int64_t)L * T > 0 && (!topk_idx || !sorted_pairs)) return CAP_EINVAL;
+    if ((int64_t)L * T > 0 && (!ws || ws_bytes < dispatch_ws_bytes_batched(L, T, k, D))) return CAP_EWORKSPACE;
+    return launch_dispatch_batched(topk_idx, kept, L, T, k, E, expert_dev, D, sorted_pairs, pair_pos, offsets, ws,
+                                   (cudaStream_t)stream);
 }
 
 int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T,

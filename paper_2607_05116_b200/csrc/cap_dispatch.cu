@@ -27,6 +27,21 @@ size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D)
     return (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
 }
 
+// all layers of cap_dispatch_layout_batched: [L][hist | base]
+size_t dispatch_ws_bytes_batched(int32_t L, int64_t T, int32_t k, int32_t D)
+{
+    const int64_t n = T * k;
+    return (size_t)(L < 1 ? 1 : L) * (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
+}
+
+// layer strides of the batched call (blockIdx.y = layer; all zero-cost for a single layer)
+struct DsBatch {
+    int64_t pair_stride;    // T k: idx / kept / sorted_pairs / pair_pos
+    int64_t ws_stride;      // 2 stride D ints: hist and base of one layer
+    int32_t map_stride;     // E
+    int32_t off_stride;     // D + 1
+};
+
 // expert of pair i, -1 if the pair is pruned or past the end (both loads are issued unconditionally and
 // before the placement map is staged: one memory round trip instead of three)
 __device__ __forceinline__ int pair_expert(const int32_t *idx, const uint8_t *kept, int64_t i, int64_t n)
@@ -49,12 +64,16 @@ __device__ __forceinline__ int expert_key(int e, const int *s_map, int E, int D)
 __global__ void __launch_bounds__(DS_THREADS)
 dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, int64_t n,
                      int E, int D, const int32_t *__restrict__ expert_dev, int *__restrict__ hist,
-                     int64_t stride)
+                     int64_t stride, DsBatch lb)
 {
     extern __shared__ int sm[];
     int *s_map = sm;                               // [E]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *cnt = sm + E + warp * DS_MAXD;            // [D] private to the warp
+    idx += blockIdx.y * lb.pair_stride;
+    if (kept) kept += blockIdx.y * lb.pair_stride;
+    expert_dev += blockIdx.y * lb.map_stride;
+    hist += blockIdx.y * lb.ws_stride;
     pdl_launch_dependents();
     pdl_wait();
     const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
@@ -83,10 +102,13 @@ dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
 // per lane), eight chunks in flight: the loop is bound by L2 latency, not by arithmetic.
 __global__ void __launch_bounds__(1024)
 dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, long long *__restrict__ offsets,
-                     int D, int64_t stride)
+                     int D, int64_t stride, DsBatch lb)
 {
     __shared__ long long tot[DS_MAXD];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    hist += blockIdx.y * lb.ws_stride;
+    base += blockIdx.y * lb.ws_stride;
+    offsets += blockIdx.y * lb.off_stride;
     const int64_t nch = stride / 128;
     pdl_launch_dependents();
     pdl_wait();
@@ -130,12 +152,20 @@ __global__ void __launch_bounds__(DS_THREADS)
 dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, int64_t n,
                         int E, int D, const int32_t *__restrict__ expert_dev,
                         const int *__restrict__ base, const long long *__restrict__ offsets,
-                        int32_t *__restrict__ sorted_pairs, int32_t *__restrict__ pair_pos, int64_t stride)
+                        int32_t *__restrict__ sorted_pairs, int32_t *__restrict__ pair_pos, int64_t stride,
+                        DsBatch lb)
 {
     extern __shared__ int sm[];
     int *s_map = sm;                               // [E]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *running = sm + E + warp * DS_MAXD;        // [D] next free position per device, private to the warp
+    idx += blockIdx.y * lb.pair_stride;
+    if (kept) kept += blockIdx.y * lb.pair_stride;
+    expert_dev += blockIdx.y * lb.map_stride;
+    base += blockIdx.y * lb.ws_stride;
+    offsets += blockIdx.y * lb.off_stride;
+    sorted_pairs += blockIdx.y * lb.pair_stride;
+    if (pair_pos) pair_pos += blockIdx.y * lb.pair_stride;
     const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
     pdl_launch_dependents();
     pdl_wait();
@@ -168,13 +198,16 @@ dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restri
     }
 }
 
-int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,
-                    const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
-                    int64_t *offsets, void *ws, cudaStream_t st)
+// L layers in three launches (blockIdx.y = layer): idx / kept [L][T][k], expert_dev [L][E], sorted_pairs / pair_pos
+// [L][T k], offsets [L][D + 1]; ws holds hist and base of every layer.
+int launch_dispatch_batched(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k, int32_t E,
+                            const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
+                            int64_t *offsets, void *ws, cudaStream_t st)
 {
+    if (L == 0) return CAP_OK;
     const int64_t n = T * k;
     if (n == 0) {
-        if (cudaMemsetAsync(offsets, 0, sizeof(int64_t) * (size_t)(D + 1), st) != cudaSuccess)
+        if (cudaMemsetAsync(offsets, 0, sizeof(int64_t) * (size_t)L * (size_t)(D + 1), st) != cudaSuccess)
             return check_launch("memset offsets");
         return CAP_OK;
     }
@@ -183,27 +216,39 @@ int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t 
     const size_t smem = sizeof(int) * (size_t)(E + DS_NW * DS_MAXD);
     int *hist = reinterpret_cast<int *>((reinterpret_cast<uintptr_t>(ws) + 255) & ~(uintptr_t)255);
     int *base = hist + stride * D;
+    DsBatch lb;
+    lb.pair_stride = n;
+    lb.ws_stride = 2 * stride * D;
+    lb.map_stride = E;
+    lb.off_stride = D + 1;
     {
     KernelTimerScope ts("dispatch_hist", st);
-    launch_pdl(dispatch_hist_kernel, dim3((unsigned)nbh), dim3(DS_THREADS), smem, st, idx, kept, n, E, D, expert_dev, hist,
-               stride);
+    launch_pdl(dispatch_hist_kernel, dim3((unsigned)nbh, (unsigned)L), dim3(DS_THREADS), smem, st, idx, kept, n, E, D,
+               expert_dev, hist, stride, lb);
     }
     note_launch();
     CAP_TRY(check_launch("dispatch_hist_kernel"));
     {
     KernelTimerScope ts("dispatch_scan", st);
-    launch_pdl(dispatch_scan_kernel, dim3(1), dim3(D <= 16 ? 512 : 1024), 0, st, hist, base,
-               reinterpret_cast<long long *>(offsets), D, stride);
+    launch_pdl(dispatch_scan_kernel, dim3(1, (unsigned)L), dim3(D <= 16 ? 512 : 1024), 0, st, hist, base,
+               reinterpret_cast<long long *>(offsets), D, stride, lb);
     }
     note_launch();
     CAP_TRY(check_launch("dispatch_scan_kernel"));
     {
     KernelTimerScope ts("dispatch_scatter", st);
-    launch_pdl(dispatch_scatter_kernel, dim3((unsigned)nb), dim3(DS_THREADS), smem, st, idx, kept, n, E, D, expert_dev,
-               base, reinterpret_cast<const long long *>(offsets), sorted_pairs, pair_pos, stride);
+    launch_pdl(dispatch_scatter_kernel, dim3((unsigned)nb, (unsigned)L), dim3(DS_THREADS), smem, st, idx, kept, n, E, D,
+               expert_dev, base, reinterpret_cast<const long long *>(offsets), sorted_pairs, pair_pos, stride, lb);
     }
     note_launch();
     return check_launch("dispatch_scatter_kernel");
+}
+
+int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,
+                    const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
+                    int64_t *offsets, void *ws, cudaStream_t st)
+{
+    return launch_dispatch_batched(idx, kept, 1, T, k, E, expert_dev, D, sorted_pairs, pair_pos, offsets, ws, st);
 }
 
 }  // namespace cap

@@ -146,6 +146,10 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
                      const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
 size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D);
+size_t dispatch_ws_bytes_batched(int32_t L, int64_t T, int32_t k, int32_t D);
+int launch_dispatch_batched(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k, int32_t E,
+                            const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
+                            int64_t *offsets, void *ws, cudaStream_t st);
 size_t place_ws_bytes(int32_t L, int32_t E, int32_t D);   // cap_place.cu
 size_t dispatch_rows_ws_bytes(int64_t T, int32_t D);        // cap_dispatch_rows.cu
 int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,

@@ -222,6 +222,30 @@ def test_dispatch_edge_cases(T, k, E, D):
     assert host(off_d).tolist() == [0] * (D + 1)
 
 
+@pytest.mark.parametrize("L,T,k,E,D", [(3, 4097, 8, 128, 16), (2, 1, 1, 4, 2), (5, 30000, 10, 512, 64), (4, 2048, 3, 16, 3)])
+def test_dispatch_batched_matches_per_layer_oracle(L, T, k, E, D):
+    """cap_dispatch_layout_batched = cap_dispatch_layout per layer (own placement, own mask), in three launches."""
+    rng = np.random.default_rng(L * 1000 + T)
+    idx = _trace(rng, L, T, E, k)
+    pi = rng.integers(0, D, (L, E)).astype(np.int32)
+    pi[:, 0] = D - 1
+    kept = (rng.random((L, T, k)) < 0.5).astype(np.uint8)
+    kept[L - 1] = 0                                                   # one layer with every pair pruned
+    for m in (None, kept):
+        n0 = cap.launch_count()
+        sp_d, off_d, pos_d = cap.dispatch_layout_batched(dev(idx), dev(m), dev(pi), D)
+        torch.cuda.synchronize()
+        assert cap.launch_count() - n0 == 3
+        for l in range(L):
+            sp_r, off_r, pos_r = O.dispatch_layout(idx[l], pi[l], D, kept=None if m is None else m[l])
+            n = int(off_r[-1])
+            assert np.array_equal(host(off_d[l]), off_r), (l, "offsets")
+            assert np.array_equal(host(sp_d[l])[:n], sp_r), (l, "sorted_pairs")
+            assert np.array_equal(host(pos_d[l]), pos_r), (l, "pair_pos")
+    sp_d, off_d, _ = cap.dispatch_layout_batched(dev(idx[:, :0]), None, dev(pi), D)      # T = 0
+    assert host(off_d).tolist() == [[0] * (D + 1)] * L
+
+
 def test_error_codes():
     x = torch.zeros((1, 4, 16), device="cuda")
     b = torch.zeros((1, 16), device="cuda")
