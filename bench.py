@@ -212,7 +212,7 @@ def config_dict(cfg, extra=None):
                      f"D={cfg.D} over N={cfg.N} nodes (cost 0/1/{cfg.cost_inter}) P={cfg.P} "
                      f"tau={cfg.taus[-1]} {'sigmoid+bias group-limited' if cfg.scoring else 'softmax'} renorm",
          "stages": "S1 gate top-k + S2 counts/co-activation + S3 P-candidate scoring (cap_trace_fused) "
-                   "-> S4 cap_prune -> S5 cap_dispatch_layout",
+                   "-> S4 cap_prune -> S5 cap_dispatch_layout (all layers in one batched call)",
          "tokens_per_step_per_gpu": cfg.L * cfg.T}
     if extra:
         d.update(extra)
@@ -344,7 +344,7 @@ def summarise(cfg, res, peak):
                              "frac_of_hbm_peak": gbs(ab["prune"], ms_prune) / peak},
             "S5_cap_dispatch_layout": {"ms": ms_disp, "algorithmic_bytes": b_disp, "gbs": gbs(b_disp, ms_disp),
                                        "frac_of_hbm_peak": gbs(b_disp, ms_disp) / peak,
-                                       "calls": cfg.L},
+                                       "calls": 1, "layers": cfg.L},
         },
         "launches_per_step": int(res["launches_per_step"]),
     }
@@ -502,7 +502,7 @@ def run_cap(args, cfg, W):
             "gpu_launches_per_step": int(main["launches_per_step"]),
             "clocks": clocks,
             "roofline": {
-                "bound": "hbm", "kernel": "cap_trace_fused (the whole S1+S2+S3 pass: " + main["fused_kernel"] + " + its table / decode / finalize kernels)",
+                "bound": "hbm", "kernel": "cap_trace_fused (the whole S1+S2+S3 pass: " + main["fused_kernel"] + " + its table and decode kernels)",
                 "achieved": fused_gbs, "peak": peak, "unit": "GB/s", "frac": fused_gbs / peak, "traffic": None,
                 "traffic_note": "not measured inside this run; the ncu capture of the dominant kernel is in profiles/",
                 "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peak_src})",
@@ -514,8 +514,9 @@ def run_cap(args, cfg, W):
                 "kernel_only_frac": (ab["trace_fused"] / (kms * 1e-3) / 1e9 / peak) if kms else None,
                 "kernel_only_how": "cap_profile_fused_kernel: the fused kernel alone, back-to-back launches rotating over "
                                    "the input sets, one CUDA-event pair on the launching stream",
-                "ceiling_note": "shared-memory-bound formulation: ~33 k shared wavefronts per SM per pass (ncu) = 17 us at "
-                                "one wavefront per clock, i.e. <= 0.34 of the HBM peak for the kernel (DESIGN.md 6.3)"},
+                "ceiling_note": "shared-memory-bound formulation: 30.1 k shared-memory wavefronts per SM per launch (ncu, "
+                                "profiles/r2a_step.md) = 15.3 us at one wavefront per clock, i.e. <= 0.38 of the HBM peak for "
+                                "the kernel; the 0.60 target is out of reach with it (DESIGN.md 6.4)"},
             "stages": main["stages"],
             "stages_note": "S4 / S5 replayed alone from a graph on the buffers of the last step (their 4-9 MB of inputs "
                            "stay in L2 between replays at this size: launch-latency-bound, see others.config5_stress_T4194304 "
