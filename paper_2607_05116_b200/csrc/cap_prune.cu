@@ -346,7 +346,10 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
         const size_t smem = sizeof(int) * ((size_t)E + 192);
         {
             KernelTimerScope ts("prune", st);
-            if (k <= 8) launch_pdl(prune_kernel<8>, grid, dim3(PR_THREADS), smem, st, prm);
+            // the unrolled O(K^2) select chains are sized by the template: k = 10 (config 5) in <12>, not <16>
+            if (k <= 4) launch_pdl(prune_kernel<4>, grid, dim3(PR_THREADS), smem, st, prm);
+            else if (k <= 8) launch_pdl(prune_kernel<8>, grid, dim3(PR_THREADS), smem, st, prm);
+            else if (k <= 12) launch_pdl(prune_kernel<12>, grid, dim3(PR_THREADS), smem, st, prm);
             else launch_pdl(prune_kernel<16>, grid, dim3(PR_THREADS), smem, st, prm);
         }
         note_launch();
