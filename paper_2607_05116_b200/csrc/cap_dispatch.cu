@@ -24,20 +24,20 @@ static int64_t ds_stride(int64_t n)
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D)
 {
     const int64_t n = T * k;
-    return (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
+    return (size_t)(2 * ds_stride(n) * D + 64) * sizeof(int) + 256;
 }
 
-// all layers of cap_dispatch_layout_batched: [L][hist | base]
+// all layers of cap_dispatch_layout_batched: [L][hist | base | 64 device totals]
 size_t dispatch_ws_bytes_batched(int32_t L, int64_t T, int32_t k, int32_t D)
 {
     const int64_t n = T * k;
-    return (size_t)(L < 1 ? 1 : L) * (size_t)(2 * ds_stride(n) * D) * sizeof(int) + 256;
+    return (size_t)(L < 1 ? 1 : L) * (size_t)(2 * ds_stride(n) * D + 64) * sizeof(int) + 256;
 }
 
 // layer strides of the batched call (blockIdx.y = layer; all zero-cost for a single layer)
 struct DsBatch {
     int64_t pair_stride;    // T k: idx / kept / sorted_pairs / pair_pos
-    int64_t ws_stride;      // 2 stride D ints: hist and base of one layer
+    int64_t ws_stride;      // 2 stride D + 64 ints: hist, base and the device totals of one layer
     int32_t map_stride;     // E
     int32_t off_stride;     // D + 1
 };
@@ -98,64 +98,78 @@ dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
     for (int d = lane; d < D; d += 32) hist[(int64_t)d * stride + sub] = cnt[d];
 }
 
-// One block, warp w scans devices w, w + nwarps, ... in coalesced chunks of 128 sub-chunks (one int4
-// per lane), eight chunks in flight: the loop is bound by L2 latency, not by arithmetic.
-__global__ void __launch_bounds__(1024)
-dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, long long *__restrict__ offsets,
-                     int D, int64_t stride, DsBatch lb)
+// One block per device row: warp w owns a contiguous span of the row's 128-entry chunks.  Pass 1 adds the span up,
+// the span totals are scanned across the warps, pass 2 writes the exclusive prefixes (one int4 per lane, eight
+// chunks in flight) starting from the span's base.  The row total goes to devtot[d]; the scatter kernel turns the
+// D totals into the device offsets.  (Round 1 scanned all rows in ONE block: 893 of S5's 1 455 us at 2^22 tokens.)
+__global__ void __launch_bounds__(512)
+dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, int D, int64_t stride, DsBatch lb)
 {
-    __shared__ long long tot[DS_MAXD];
+    __shared__ int s_span[16];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
-    hist += blockIdx.y * lb.ws_stride;
-    base += blockIdx.y * lb.ws_stride;
-    offsets += blockIdx.y * lb.off_stride;
+    const int d = blockIdx.x;
+    hist += blockIdx.y * lb.ws_stride + (int64_t)d * stride;
+    base += blockIdx.y * lb.ws_stride + (int64_t)d * stride;
+    int *devtot = const_cast<int *>(hist) - (int64_t)d * stride + 2 * stride * D;     // behind hist and base of the layer
     const int64_t nch = stride / 128;
+    const int64_t cpw = (nch + nw - 1) / nw;
+    const int64_t c_lo = min(nch, (int64_t)warp * cpw), c_hi = min(nch, c_lo + cpw);
     pdl_launch_dependents();
     pdl_wait();
-    for (int d = warp; d < D; d += nw) {
-        const int4 *h = reinterpret_cast<const int4 *>(hist + (int64_t)d * stride) + lane;
-        int4 *bs = reinterpret_cast<int4 *>(base + (int64_t)d * stride) + lane;
-        int run = 0;                               // pairs of device d before the current chunk
-        for (int64_t c0 = 0; c0 < nch; c0 += 8) {
-            int4 v[8];
+    const int4 *h = reinterpret_cast<const int4 *>(hist) + lane;
+    int4 *bs = reinterpret_cast<int4 *>(base) + lane;
+    int acc = 0;
+    for (int64_t c0 = c_lo; c0 < c_hi; c0 += 8) {
+        int4 v[8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) v[j] = c0 + j < nch ? h[(c0 + j) * 32] : make_int4(0, 0, 0, 0);
+        for (int j = 0; j < 8; ++j) v[j] = c0 + j < c_hi ? h[(c0 + j) * 32] : make_int4(0, 0, 0, 0);
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const int sum = (v[j].x + v[j].y) + (v[j].z + v[j].w);
-                int inc = sum;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int y = __shfl_up_sync(0xffffffffu, inc, o);
-                    if (lane >= o) inc += y;
-                }
-                int4 o;
-                o.x = run + inc - sum;             // exclusive, within device d
-                o.y = o.x + v[j].x;
-                o.z = o.y + v[j].y;
-                o.w = o.z + v[j].z;
-                if (c0 + j < nch) bs[(c0 + j) * 32] = o;
-                run += __shfl_sync(0xffffffffu, inc, 31);
-            }
-        }
-        if (lane == 0) tot[d] = run;
+        for (int j = 0; j < 8; ++j) acc += (v[j].x + v[j].y) + (v[j].z + v[j].w);
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) s_span[warp] = acc;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        long long acc = 0;
-        for (int d = 0; d < D; ++d) { offsets[d] = acc; acc += tot[d]; }
-        offsets[D] = acc;
+    int run = 0, total = 0;                        // pairs of device d before this warp's span / in the row
+    for (int w2 = 0; w2 < nw; ++w2) {
+        const int v = s_span[w2];
+        run += w2 < warp ? v : 0;
+        total += v;
+    }
+    if (threadIdx.x == 0) devtot[d] = total;
+    for (int64_t c0 = c_lo; c0 < c_hi; c0 += 8) {
+        int4 v[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) v[j] = c0 + j < c_hi ? h[(c0 + j) * 32] : make_int4(0, 0, 0, 0);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int sum = (v[j].x + v[j].y) + (v[j].z + v[j].w);
+            int inc = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, inc, o);
+                if (lane >= o) inc += y;
+            }
+            int4 o;
+            o.x = run + inc - sum;             // exclusive, within device d
+            o.y = o.x + v[j].x;
+            o.z = o.y + v[j].y;
+            o.w = o.z + v[j].z;
+            if (c0 + j < c_hi) bs[(c0 + j) * 32] = o;
+            run += __shfl_sync(0xffffffffu, inc, 31);
+        }
     }
 }
 
 __global__ void __launch_bounds__(DS_THREADS)
 dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, int64_t n,
                         int E, int D, const int32_t *__restrict__ expert_dev,
-                        const int *__restrict__ base, const long long *__restrict__ offsets,
+                        const int *__restrict__ base, long long *__restrict__ offsets,
                         int32_t *__restrict__ sorted_pairs, int32_t *__restrict__ pair_pos, int64_t stride,
                         DsBatch lb)
 {
     extern __shared__ int sm[];
+    __shared__ int s_off[65];                      // exclusive prefix of the device totals (T k < 2^31)
     int *s_map = sm;                               // [E]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *running = sm + E + warp * DS_MAXD;        // [D] next free position per device, private to the warp
@@ -174,9 +188,27 @@ dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restri
 #pragma unroll
     for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_expert(idx, kept, i0 + r * 32 + lane, n);
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
-    if (i0 < n)
-        for (int d = lane; d < D; d += 32) running[d] = (int)offsets[d] + base[(int64_t)d * stride + sub];
+    if (warp == 0) {
+        // device offsets from the row totals the scan kernel left behind hist and base
+        const int *devtot = base + 2 * stride * D - stride * D;
+        int v0 = lane < D ? devtot[lane] : 0, v1 = lane + 32 < D ? devtot[lane + 32] : 0;
+        int i0s = v0, i1s = v1;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y0 = __shfl_up_sync(0xffffffffu, i0s, o), y1 = __shfl_up_sync(0xffffffffu, i1s, o);
+            if (lane >= o) { i0s += y0; i1s += y1; }
+        }
+        const int t0 = __shfl_sync(0xffffffffu, i0s, 31);
+        s_off[lane] = i0s - v0;
+        s_off[lane + 32] = t0 + i1s - v1;
+        if (lane == 31) s_off[64] = t0 + i1s;
+    }
     __syncthreads();
+    if (blockIdx.x == 0 && (int)threadIdx.x <= D)
+        offsets[threadIdx.x] = (long long)((int)threadIdx.x < D ? s_off[threadIdx.x] : s_off[D < 64 ? D : 64]);
+    if (i0 < n)
+        for (int d = lane; d < D; d += 32) running[d] = s_off[d] + base[(int64_t)d * stride + sub];
+    __syncwarp();
     if (i0 >= n) return;
 #pragma unroll
     for (int r = 0; r < DS_SUB / 32; ++r) key[r] = expert_key(key[r], s_map, E, D);
@@ -218,7 +250,7 @@ int launch_dispatch_batched(const int32_t *idx, const uint8_t *kept, int32_t L, 
     int *base = hist + stride * D;
     DsBatch lb;
     lb.pair_stride = n;
-    lb.ws_stride = 2 * stride * D;
+    lb.ws_stride = 2 * stride * D + 64;
     lb.map_stride = E;
     lb.off_stride = D + 1;
     {
@@ -230,15 +262,15 @@ int launch_dispatch_batched(const int32_t *idx, const uint8_t *kept, int32_t L, 
     CAP_TRY(check_launch("dispatch_hist_kernel"));
     {
     KernelTimerScope ts("dispatch_scan", st);
-    launch_pdl(dispatch_scan_kernel, dim3(1, (unsigned)L), dim3(D <= 16 ? 512 : 1024), 0, st, hist, base,
-               reinterpret_cast<long long *>(offsets), D, stride, lb);
+    launch_pdl(dispatch_scan_kernel, dim3((unsigned)D, (unsigned)L), dim3(stride >= 128 * 16 ? 512 : 128), 0, st, hist, base,
+               D, stride, lb);
     }
     note_launch();
     CAP_TRY(check_launch("dispatch_scan_kernel"));
     {
     KernelTimerScope ts("dispatch_scatter", st);
     launch_pdl(dispatch_scatter_kernel, dim3((unsigned)nb, (unsigned)L), dim3(DS_THREADS), smem, st, idx, kept, n, E, D,
-               expert_dev, base, reinterpret_cast<const long long *>(offsets), sorted_pairs, pair_pos, stride, lb);
+               expert_dev, base, reinterpret_cast<long long *>(offsets), sorted_pairs, pair_pos, stride, lb);
     }
     note_launch();
     return check_launch("dispatch_scatter_kernel");
