@@ -240,7 +240,10 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
     proxy_fence_async();
     tc_fence_before();
     pdl_launch_dependents();
-    pdl_wait();                       // everything above touched shared memory / TMEM only
+    // No grid-dependency wait here: the predecessor (eval_table_kernel) produces the code table and clears the
+    // accumulators, which this kernel consumes late -- the table when S3 starts, the cleared outputs at the flush
+    // and the drain.  The logits stream and the selection depend on nothing it writes, so they start while it
+    // still runs; pdl_wait() sits at the three consumers below.
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = s_tmem;
@@ -249,15 +252,22 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
     if (warp == 0) {
         // ================= producer =================
         if (lane == 0 && nt > 0) {
-            mbar_expect_tx(&tbl_bar, (uint32_t)(E + 1) * rowb);
-            bulk_g2s(tbl, q.table + (size_t)layer * (E + 1) * q.RS * 4, (uint32_t)(E + 1) * rowb, &tbl_bar);
-            for (int j = 0; j < nt; ++j) {
+            auto issue = [&](int j) {
                 const int st = j % nst;
-                if (j >= nst) mbar_wait_relaxed(&empty_bar[st], (uint32_t)(((j / nst) - 1) & 1), 256);
                 const int64_t tok0 = t0 + (int64_t)j * FU_TILE;
                 const int rows = (int)min((int64_t)FU_TILE, t1 - tok0);
                 mbar_expect_tx(&full_bar[st], (uint32_t)rows * E * 4);
                 bulk_g2s(ring + (size_t)st * TILE_BYTES, logits + tok0 * E, (uint32_t)rows * E * 4, &full_bar[st]);
+            };
+            const int npre = nt < nst ? nt : nst;
+            for (int j = 0; j < npre; ++j) issue(j);          // the first ring needs no free-stage wait
+            // the logits are on their way: now the code table, the first thing the predecessor produced
+            pdl_wait();
+            mbar_expect_tx(&tbl_bar, (uint32_t)(E + 1) * rowb);
+            bulk_g2s(tbl, q.table + (size_t)layer * (E + 1) * q.RS * 4, (uint32_t)(E + 1) * rowb, &tbl_bar);
+            for (int j = npre; j < nt; ++j) {
+                mbar_wait_relaxed(&empty_bar[j % nst], (uint32_t)(((j / nst) - 1) & 1), 256);
+                issue(j);
             }
         }
         FU_TR(2, FU_NOW());
@@ -393,6 +403,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
         FU_TR(7, tr_wc);
         // ---- drain the co-activation accumulator: S1 warps 0..3, one TMEM lane quadrant each ----
         if (c < 4 && nm > 0) {
+            pdl_wait();                 // counts / coact were cleared by the predecessor
             mbar_wait_relaxed(&acc_done, 0u, 128);
             FU_TR(3, FU_NOW());
             tc_fence_after();
@@ -469,6 +480,7 @@ __global__ void __launch_bounds__(FU_MAXTHREADS, 1) trace_fused_kernel(FusedPara
         bool have_run = false;
 
         auto flush = [&]() {
+            pdl_wait();                 // the record headers were reset by the predecessor
             // add the S sub-slots in the bit-sliced domain (tree through shared memory), write the record
             for (int lvl = 0; lvl < q.logS; ++lvl) {
                 const int half = S >> (lvl + 1);
@@ -672,7 +684,7 @@ static int launch_fused_e(const FusedParams &prm, const FusedGeom &f, int L, cud
     cudaFuncSetAttribute(trace_fused_kernel<E>, cudaFuncAttributeMaxDynamicSharedMemorySize, 225 * 1024);
     {
         KernelTimerScope ts("trace_fused", st);
-        launch_pdl(trace_fused_kernel<E>, dim3((unsigned)f.g.ncta_t, (unsigned)L), dim3(f.nthreads), f.smem, st, prm);
+        launch_pdl_edge(trace_fused_kernel<E>, dim3((unsigned)f.g.ncta_t, (unsigned)L), dim3(f.nthreads), f.smem, st, prm);
     }
     note_launch();
     return check_launch("trace_fused_kernel");

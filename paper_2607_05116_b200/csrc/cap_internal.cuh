@@ -74,6 +74,26 @@ inline int64_t balanced_blocks_per_unit(int64_t units, int64_t slots, int64_t ma
     return best_w;
 }
 
+// The same launch with the programmatic edge kept INSIDE a stream capture as well.  Only for a kernel whose early
+// part is independent of its predecessor's output and that calls pdl_wait() exactly where it first consumes it
+// (trace_fused_kernel after eval_table_kernel): there the overlap pays; on the chains of short kernels it did not.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl_edge(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                                   Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 #define CAP_TRY(expr)                      \
     do {                                   \
         int _rc = (expr);                  \
