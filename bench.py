@@ -318,9 +318,16 @@ def measure(cfg, W, WD, cap, torch, dev, rank, steps, replays, barrier, light=Fa
     kms = None
     if not light:
         kms = cap.profile_fused_kernel([d[0] for d in d_sets], gate, d_sets[0][2], pipe.topo, pipe.fb, max(steps, 50))
+    # the general reading R5 (explicit, non-contiguous token sources): staged S1 / S2 kernels + the generic S3 kernel
+    ms_src = None
+    if not light:
+        src = torch.from_numpy(np.stack([W.token_src_random(cfg, l) for l in range(L)])).to(dev)
+        g_src = [pipe.capture_fused(x, b, src, m) for x, b, m in d_sets]
+        ms_src = timed_replays(torch, lambda i: g_src[i % n_sets].replay(), max(10, n // 20), barrier)
+        del g_src
     plan = cap.trace_fused_plan(L, T, gate, D, cfg.N, P)
     res = dict(pipe=pipe, d_sets=d_sets, gate=gate, n_sets=n_sets, in_bytes=in_bytes, ms_step=ms_step,
-               ms_fused=ms_fused, ms_prune=ms_prune, ms_disp=ms_disp, kernel_ms=kms, plan=plan,
+               ms_fused=ms_fused, ms_prune=ms_prune, ms_disp=ms_disp, kernel_ms=kms, plan=plan, ms_src=ms_src,
                launches_per_step=launches_per_step)
     return res
 
@@ -348,6 +355,12 @@ def summarise(cfg, res, peak):
         },
         "launches_per_step": int(res["launches_per_step"]),
     }
+    if res.get("ms_src"):
+        ms = med(res["ms_src"])
+        out["explicit_token_src_pass"] = {
+            "ms": ms, "gbs": gbs(ab["trace_fused"], ms), "frac_of_hbm_peak": gbs(ab["trace_fused"], ms) / peak,
+            "what": "cap_trace_fused with an explicit random token_src (reading R5): staged gate + co-activation "
+                    "kernels, tokens grouped by source with the S5 counting sort, then the bit-sliced S3 kernel over the runs"}
     return out
 
 
@@ -518,6 +531,7 @@ def run_cap(args, cfg, W):
                                 "profiles/r2a_step.md) = 15.3 us at one wavefront per clock, i.e. <= 0.38 of the HBM peak for "
                                 "the kernel; the 0.60 target is out of reach with it (DESIGN.md 6.4)"},
             "stages": main["stages"],
+            "explicit_token_src_pass": main.get("explicit_token_src_pass"),
             "stages_note": "S4 / S5 replayed alone from a graph on the buffers of the last step (their 4-9 MB of inputs "
                            "stay in L2 between replays at this size: launch-latency-bound, see others.config5_stress_T4194304 "
                            "for the bandwidth-bound size)",

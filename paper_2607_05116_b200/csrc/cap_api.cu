@@ -2,6 +2,8 @@
 // carving and kernel launches.  No allocation, no synchronisation (cap_validate_placements
 // excepted), no global state beyond the launch counter and the per-thread last CUDA error.
 #include <atomic>
+#include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 #include "cap_internal.cuh"
@@ -13,10 +15,11 @@ static thread_local int tl_last_err = 0;
 
 void note_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
-int check_launch(const char *)
+int check_launch(const char *what)
 {
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) {
+        if (getenv("CAP_DEBUG")) fprintf(stderr, "cap: %s: %s\n", what ? what : "?", cudaGetErrorString(e));
         tl_last_err = (int)e;
         return CAP_ECUDA;
     }

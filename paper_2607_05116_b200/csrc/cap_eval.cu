@@ -276,9 +276,10 @@ int launch_eval(const int32_t *idx, const uint8_t *kept, const int32_t *token_sr
             CAP_TRY(check_launch("masked_counts_kernel"));
         }
         bool fast = false;
-        if (!token_src && !want_tok) {
+        if (!want_tok) {
             CAP_TRY(launch_eval_fast(idx, kept, L, T, k, E, expert_dev, P, topo,
-                                     counts ? counts : reinterpret_cast<const int64_t *>(w.mcounts), out, ws, st, &fast));
+                                     counts ? counts : reinterpret_cast<const int64_t *>(w.mcounts), out, ws, st, &fast,
+                                     token_src));
             if (fast) return CAP_OK;         // the decode kernel of the fast path writes the outputs itself
         }
         int PC = 256;

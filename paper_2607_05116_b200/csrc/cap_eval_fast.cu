@@ -2,6 +2,9 @@
 // Tables II-IV).  Used when the token sources are the default contiguous blocks (token_src NULL,
 // reading R5) and no per-token output is wanted; otherwise the generic kernel of cap_eval.cu runs.
 // Method and data layout: cap_eval_fast.cuh and DESIGN.md section 6.
+#include <cstdio>
+#include <cstdlib>
+
 #include "cap_eval_fast.cuh"
 
 namespace cap {
@@ -15,7 +18,7 @@ static int ceil_log2(long long v)
 }
 
 bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P,
-                    int target_ctas, size_t smem_budget, EvalFastGeom *g)
+                    int target_ctas, size_t smem_budget, EvalFastGeom *g, bool explicit_src)
 {
     if (L < 1 || T < 1 || P < 1 || D < 1 || D > 64 || N < 1 || N > 8 || k < 1 || k > 16) return false;
     g->WD = D <= 8 ? 8 : D <= 16 ? 16 : D <= 32 ? 32 : 64;
@@ -83,7 +86,8 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     {
         const int64_t max_want = (T / (16 * blk)) > 1 ? (T / (16 * blk)) : 1;
         double best = 1e30;
-        for (int64_t wnt = 1; wnt <= 64 && wnt <= max_want; ++wnt) {
+        const int64_t cap_want = 64 > (target_ctas + units - 1) / units ? 64 : (target_ctas + units - 1) / units;
+        for (int64_t wnt = 1; wnt <= cap_want && wnt <= max_want; ++wnt) {
             const int64_t waves = (units * wnt + target_ctas - 1) / target_ctas;
             const double cost = (double)waves / (double)wnt * (1.0 + 0.01 * (double)wnt);   // mild pull toward fewer blocks
             if (cost < best - 1e-12) {
@@ -99,7 +103,8 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     if (g->ncta_t > 65535) return false;
     const int64_t cap_run = (int64_t)EF_MAXBLK * blk;
     // runs split at capacity and at source boundaries
-    const int64_t srcb = ((tpc - 1) * D) / T + 1;      // source boundaries inside a block's range
+    // source boundaries inside a block's range (an explicit token_src can put all of them into one block)
+    const int64_t srcb = explicit_src ? D - 1 : ((tpc - 1) * D) / T + 1;
     g->maxrec = (int)((tpc + cap_run - 1) / cap_run + (srcb < D - 1 ? srcb : D - 1));
     if (g->maxrec < 1) g->maxrec = 1;
     g->NPR = EF_BT + g->logS;
@@ -120,6 +125,13 @@ size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D,
         const size_t b = g.rec_slots * 4 + 256 + g.rec_words * 4 + 256 + g.table_words * 4 + 256;
         if (b > best) best = b;
     }
+    for (int N = 2; N <= 8; N *= 2) {      // explicit token_src: more record slots, the permutation and the sort
+        EvalFastGeom g;
+        if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), ef_budget(), &g, true)) continue;
+        const size_t b = g.rec_slots * 4 + 256 + g.rec_words * 4 + 256 + g.table_words * 4 + 256 + (size_t)L * T * 4 + 256 +
+                         (size_t)L * (D + 1) * 8 + 256 + (size_t)L * 64 * 4 + 256 + dispatch_ws_bytes_batched(L, T, 1, D) + 256;
+        if (b > best) best = b;
+    }
     const size_t fb = fused_ws_bytes(L, T, k, E, D, P);
     if (fb > best) best = fb;
     const size_t f2 = fused2_ws_bytes(L, T, k, E, D, P) + 256;
@@ -135,7 +147,7 @@ void *eval_fast_region(void *ws, int32_t L, int32_t E, int32_t D, int32_t P)
 }
 
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
-                              const EvalFastGeom &g)
+                              const EvalFastGeom &g, int64_t T)
 {
     // the fast-path region follows the generic region (acc, recv, mcounts)
     EvalWs base = eval_ws_carve(ws, L, E, D, P);
@@ -149,7 +161,27 @@ EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t
     a += g.rec_words * 4;
     a = (a + 255) & ~(uintptr_t)255;
     w.table = reinterpret_cast<uint32_t *>(a);
+    a += g.table_words * 4;
+    a = (a + 255) & ~(uintptr_t)255;
+    w.perm = reinterpret_cast<int32_t *>(a);
+    a += (size_t)L * T * 4;
+    a = (a + 255) & ~(uintptr_t)255;
+    w.srcoff = reinterpret_cast<long long *>(a);
+    a += (size_t)L * (D + 1) * 8;
+    a = (a + 255) & ~(uintptr_t)255;
+    w.ident = reinterpret_cast<int32_t *>(a);
+    a += (size_t)L * 64 * 4;
+    a = (a + 255) & ~(uintptr_t)255;
+    w.sort_ws = reinterpret_cast<void *>(a);
     return w;
+}
+
+// identity maps [L][64] for the sort of the tokens by source device (entries >= D are never a valid key)
+__global__ void eval_iota_kernel(int32_t *p)
+{
+    pdl_launch_dependents();
+    pdl_wait();
+    if (threadIdx.x < 64) p[blockIdx.x * 64 + threadIdx.x] = (int)threadIdx.x;
 }
 
 // ---- main kernel ---------------------------------------------------------------------------------------
@@ -161,6 +193,10 @@ struct EvalFastParams {
     int32_t *rec_src;
     uint32_t *rec_planes;
     const uint32_t *table;       // [L][PC][E + 1][RS * 4]
+    // explicit token sources (reading R5): token ids grouped by source device by a stable counting sort, and the
+    // start of every source's range in that order; NULL = contiguous blocks floor(t D / T), no indirection
+    const int32_t *perm;         // [L][T]
+    const long long *srcoff;     // [L][D + 1]
     int64_t T, tpc;
     int32_t k, E, P, D;
     int32_t WD, WN, Pc, PC, DW, NW, R, RS, S, logS, ncta_t, maxrec, NPR;
@@ -276,17 +312,33 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
     const uint32_t zero_row = (uint32_t)E * rowb;
     const int nent = EF_PASSES * S * KP;          // index entries per block of tokens
     const int64_t T = q.T;
+    __shared__ long long s_srcoff[65];
+    const int32_t *perm = q.perm ? q.perm + (size_t)layer * q.T : nullptr;
+    if (perm) {
+        if (tid <= D) s_srcoff[tid] = q.srcoff[(size_t)layer * (D + 1) + tid];
+        __syncthreads();
+    }
+    const int64_t Tend = perm ? min(T, (int64_t)s_srcoff[D]) : T;     // tokens with an out-of-range source are left out
     const int64_t t0 = (int64_t)blockIdx.x * q.tpc;
-    const int64_t t1 = min(T, t0 + q.tpc);
+    const int64_t t1 = min(Tend, t0 + q.tpc);
     const size_t slot0 = (((size_t)layer * q.PC + pc) * q.ncta_t + blockIdx.x) * q.maxrec;
     const int blk_tokens = EF_PASSES * S;
 
     int nrec = 0;
+    int psrc = 0;                                   // sources only grow along the sorted order
     int64_t t = t0;
     while (t < t1) {
         // ---- one run: tokens [t, rend) share the source device and fit the thread counters ----
-        const int src = (int)((t * D) / T);
-        const int64_t bnd = ((int64_t)(src + 1) * T + D - 1) / D;
+        int src;
+        int64_t bnd;
+        if (perm) {
+            while (psrc < D - 1 && (int64_t)s_srcoff[psrc + 1] <= t) ++psrc;
+            src = psrc;
+            bnd = (int64_t)s_srcoff[src + 1];
+        } else {
+            src = (int)((t * D) / T);
+            bnd = ((int64_t)(src + 1) * T + D - 1) / D;
+        }
         int64_t rend = min(t1, bnd);
         rend = min(rend, t + (int64_t)EF_MAXBLK * blk_tokens);
         uint4 pl[EF_NPL];
@@ -304,7 +356,7 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
                     const int slot = i / KP, s = i - slot * KP;
                     const int64_t tok = base + slot;
                     if (tok < rend && s < k) {
-                        const int64_t a = tok * k + s;
+                        const int64_t a = (perm ? (int64_t)perm[tok] : tok) * k + s;
                         const int e = idx[a];
                         if ((!kept || kept[a]) && (unsigned)e < (unsigned)E) o = (uint32_t)e * rowb;
                     }
@@ -628,11 +680,10 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
 template <int KP>
 static int launch_kp(const EvalFastParams &prm, const EvalFastGeom &g, int L, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(eval_fast_kernel<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        attr_set = true;
-    }
+    // per device and cheap: set on every launch, to what this launch needs (the kernel also has 520 B of static
+    // shared memory, so the full 227 KB would not be a legal dynamic size)
+    if (cudaFuncSetAttribute(eval_fast_kernel<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem) != cudaSuccess)
+        return check_launch("eval_fast_kernel attribute");
     dim3 grid((unsigned)g.ncta_t, (unsigned)g.PC, (unsigned)L);
     {
         KernelTimerScope ts("eval", st);
@@ -722,12 +773,22 @@ int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, int32_t L, int
 
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                      int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
-                     const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used)
+                     const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used,
+                     const int32_t *token_src)
 {
     *used = false;
     EvalFastGeom g;
-    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g)) return CAP_OK;
-    EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g);
+    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g, token_src != nullptr)) return CAP_OK;
+    EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g, T);
+    if (token_src) {
+        // explicit sources (reading R5): group the token ids by source device with the stable counting sort of S5
+        // (pairs = tokens, k = 1, "expert" = the source, identity map); runs of one source follow from its offsets
+        launch_pdl(eval_iota_kernel, dim3((unsigned)L), dim3(64), 0, st, fw.ident);
+        note_launch();
+        CAP_TRY(check_launch("eval_iota_kernel"));
+        CAP_TRY(launch_dispatch_batched(token_src, nullptr, L, T, 1, 64, fw.ident, topo.D, fw.perm, nullptr,
+                                        reinterpret_cast<int64_t *>(fw.srcoff), fw.sort_ws, st));
+    }
     const EfFill fill = {fw.rec_src, g.rec_slots * 4, 0xffffffffu};
     CAP_TRY(ef_launch_table(g, fw, expert_dev, topo.dev_node, L, E, P, topo.D, st, &fill, 1));
     EvalFastParams prm = {};
@@ -738,6 +799,8 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     prm.rec_src = fw.rec_src;
     prm.rec_planes = fw.rec_planes;
     prm.table = fw.table;
+    prm.perm = token_src ? fw.perm : nullptr;
+    prm.srcoff = token_src ? fw.srcoff : nullptr;
     prm.T = T;
     prm.tpc = g.tpc;
     prm.k = k;

@@ -44,17 +44,23 @@ struct EvalFastGeom {
 };
 
 // false when the fast path does not apply to these sizes (the generic kernel is used instead)
+// explicit_src: the tokens come grouped by an arbitrary token_src (any number of source boundaries per block)
 bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P,
-                    int target_ctas, size_t smem_budget, EvalFastGeom *g);
+                    int target_ctas, size_t smem_budget, EvalFastGeom *g, bool explicit_src = false);
 size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 
 struct EvalFastWs {
     int32_t *rec_src;       // [L][PC][ncta_t][maxrec], -1 = unused
     uint32_t *rec_planes;   // [L][PC][ncta_t][maxrec][W][EF_RECW] (word-major: the decode reads 64-byte runs)
     uint32_t *table;        // [L][PC][E + 1][RS * 4] one-hot code table
+    // explicit token_src only: tokens sorted by source device
+    int32_t *perm;          // [L][T]
+    long long *srcoff;      // [L][D + 1]
+    int32_t *ident;         // [L][64] identity maps of the sort
+    void *sort_ws;          // workspace of the batched counting sort (k = 1)
 };
 EvalFastWs eval_fast_ws_carve(void *ws, int32_t L, int32_t E, int32_t D, int32_t P,
-                              const EvalFastGeom &g);
+                              const EvalFastGeom &g, int64_t T = 0);
 
 // a buffer the table kernel fills with a 32-bit value on the side (bytes must be a multiple of 4)
 struct EfFill {

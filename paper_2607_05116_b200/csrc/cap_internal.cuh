@@ -163,7 +163,8 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
 // (decodes and finishes the outputs itself: no launch_eval_finalize after it)
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                      int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
-                     const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used);
+                     const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used,
+                     const int32_t *token_src = nullptr);
 size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D);
 size_t dispatch_ws_bytes_batched(int32_t L, int64_t T, int32_t k, int32_t D);

@@ -322,6 +322,31 @@ def test_fused_kernel_serves_these_shapes(shape):
     assert cap.kernel_timer_ms(7) > 0.0
 
 
+@pytest.mark.parametrize("skew", ["uniform", "one-source", "two-sources"])
+def test_bitsliced_eval_serves_explicit_token_src(skew):
+    """An explicit token_src (reading R5) keeps the bit-sliced S3 kernel: tokens are grouped by source with the S5
+    counting sort and the kernel walks the runs ('eval_decode' only fires behind that kernel).  Skewed sources
+    (every token from one device; two devices, the others empty) against the oracle."""
+    cfg = W.CONFIGS["target"].with_(T=9001, P=70)
+    rng = np.random.default_rng(11)
+    L, T, E, k, D = 2, cfg.T, cfg.E, cfg.k, cfg.D
+    idx = _trace(rng, L, T, E, k)
+    kept = (rng.random((L, T, k)) < 0.7).astype(np.uint8)
+    cand = np.stack([W.candidates(cfg, l) for l in range(L)])
+    src = {"uniform": rng.integers(0, D, (L, T)), "one-source": np.full((L, T), D - 1),
+           "two-sources": rng.choice([3, D - 2], (L, T))}[skew].astype(np.int32)
+    dn = W.dev_node(cfg)
+    topo = topo_of(cfg, dev(dn))
+    for m in (None, kept):
+        ref = O.eval_placements(idx, cand, dn, kept=m, token_src=src, cost_inter=cfg.cost_inter,
+                                bytes_per_token=cfg.bytes_per_token)
+        cap.kernel_timer_arm("eval_decode", 6)
+        got = cap.eval_placements(dev(idx), dev(m), dev(src), dev(cand), topo)
+        torch.cuda.synchronize()
+        assert cap.kernel_timer_ms(6) > 0.0
+        assert_eval_equal(got, ref, False, f"{skew} ")
+
+
 @pytest.mark.parametrize("shape", [_FAST_SHAPES[0], _FAST_SHAPES[5], _FAST_SHAPES[6], _FAST_SHAPES[11], _FAST_SHAPES[12],
                                    dict(base="target", T=20000, D=4, N=2, P=100)],
                          ids=["E128", "k3", "E64", "L3", "T70000", "multi-source"])
