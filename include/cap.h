@@ -198,6 +198,32 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
 int cap_trace_fused_plan(int32_t L, int64_t T, const cap_gate_cfg *cfg, int32_t D, int32_t N, int32_t P,
                          int64_t plan[8]);
 
+/* cap_trace_fused in two halves, for callers that overlap the end of S3 with the stages that follow
+ * (S4 / S5 read topk_idx / topk_w, never the S3 outputs).  The candidate scoring (P:L64-66, P:L178,
+ * P:L263) ends with a short launch that adds the per-block records up and writes `out`; _begin runs
+ * everything before that launch and hands the launch back, _finish issues it on a stream of the
+ * caller's choice:
+ *     cap_trace_fused_begin(..., &pend, s);      topk_idx / topk_w / counts / coact final in order of s
+ *     <event: s2 after s>   cap_trace_fused_finish(&pend, s2);    `out` final in order of s2
+ *     cap_prune(..., s); cap_dispatch_layout(..., s);  <event: s after s2>
+ * Arguments of _begin are those of cap_trace_fused (same checks, same results bit for bit).  `pend` is
+ * plain host data owned by the caller (kind = 0: nothing owed -- the shape took a path that finishes
+ * `out` itself --, _finish is then a no-op).  Between the halves `ws`, `counts`, `expert_dev`,
+ * `topo->dev_node` and the `out` arrays must stay untouched; the ordering of s2 against s (and of the next
+ * call that reuses `ws` against s2) is the caller's: the library adds no event.  A pending launch that is
+ * never finished leaves `out` unwritten and leaks nothing. */
+typedef struct cap_pending {
+    int32_t kind;               /* 0 none, 1 decode launch of the bit-sliced S3 path */
+    int32_t reserved;
+    unsigned char blob[496];    /* launch parameters; opaque */
+} cap_pending;
+int cap_trace_fused_begin(const float *logits, const float *bias, int32_t L, int64_t T,
+                          const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w, int64_t *counts,
+                          int32_t *coact, const int32_t *token_src, const int32_t *expert_dev, int32_t P,
+                          const cap_topology *topo, const cap_eval_out *out, void *ws, size_t ws_bytes,
+                          cap_pending *pend, void *stream);
+int cap_trace_fused_finish(const cap_pending *pend, void *stream);
+
 /* Co-activation driven expert placement: SURVEY 8(f) rank 1, the consumer of cap_coactivation's
  * outputs.  P:L148 defines the co-activation probability ("the ratio between the number of times
  * they are selected together and the total number of times either of them is selected"; reading R3:

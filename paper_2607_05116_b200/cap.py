@@ -20,7 +20,8 @@ EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prun
            "cap_dispatch_layout", "cap_trace_fused", "cap_coact_placement", "cap_pairwise_objective", "cap_dispatch_rows", "cap_adjust_spectrum", "cap_workspace_bytes",
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan",
-           "cap_dispatch_layout_static", "cap_static_scratch_bytes", "cap_prune_naive", "cap_dispatch_row_weights", "cap_dispatch_layout_batched")
+           "cap_dispatch_layout_static", "cap_static_scratch_bytes", "cap_prune_naive", "cap_dispatch_row_weights", "cap_dispatch_layout_batched",
+           "cap_trace_fused_begin", "cap_trace_fused_finish")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
@@ -402,6 +403,36 @@ def trace_fused(logits, bias, cfg, token_src, expert_dev, topo, bufs=None, per_t
     return bufs
 
 
+class Pending(C.Structure):
+    """cap_pending (include/cap.h): the launch cap_trace_fused_begin hands back."""
+    _fields_ = [("kind", C.c_int32), ("reserved", C.c_int32), ("blob", C.c_ubyte * 496)]
+
+
+def trace_fused_begin(logits, bias, cfg, token_src, expert_dev, topo, bufs=None, per_token=False, pend=None):
+    """cap_trace_fused up to the last launch of S3 (current stream); returns (bufs, pend).  bufs.idx / w / counts /
+    coact are final in stream order, bufs.out only after trace_fused_finish(pend)."""
+    L, T, E = logits.shape
+    P = expert_dev.shape[1]
+    if bufs is None:
+        bufs = FusedBuffers(L, T, E, cfg.k, topo.D, P, logits.device, per_token)
+    if pend is None:
+        pend = Pending()
+    rc = lib().cap_trace_fused_begin(_ptr(logits, torch.float32), _ptr(bias, torch.float32), L, T,
+                                     C.byref(cfg), _ptr(bufs.idx), _ptr(bufs.w), _ptr(bufs.counts),
+                                     _ptr(bufs.coact), _ptr(token_src, torch.int32),
+                                     _ptr(expert_dev, torch.int32), P, C.byref(topo),
+                                     C.byref(bufs.out_struct), _ptr(bufs.ws), bufs.ws.numel(), C.byref(pend),
+                                     _stream())
+    _check(rc, "cap_trace_fused_begin")
+    return bufs, pend
+
+
+def trace_fused_finish(pend):
+    """Issue the launch trace_fused_begin handed back, on the CURRENT stream (the caller orders it after the
+    stream _begin ran on)."""
+    _check(lib().cap_trace_fused_finish(C.byref(pend), _stream()), "cap_trace_fused_finish")
+
+
 def profile_fused_kernel(logits_list, cfg, expert_dev, topo, bufs, n_rep):
     """Average device time (ms) of the fused S1+S2+S3 kernel alone over n_rep back-to-back launches
     rotating over logits_list; returns None if the configuration is not served by the fused kernel."""
@@ -472,6 +503,8 @@ class Pipeline:
         self.offsets = torch.empty((L, D + 1), dtype=torch.int64, device=device)
         self.ws_disp = workspace(CALL_DISPATCH_LAYOUT, L, T, E, k, D, 0, device)
         self.pi = torch.empty((L, E), dtype=torch.int32, device=device)
+        self.side = torch.cuda.Stream(device=device)       # the S3 decode runs here, beside S4 / S5 (step)
+        self.pend = Pending()
 
     def clone(self):
         """A second pipeline with its own output buffers and workspaces (same configuration)."""
@@ -497,6 +530,25 @@ class Pipeline:
                                 ws=self.ws_disp, out=(self.sorted_pairs, self.offsets, self.pair_pos))
 
     def step(self, logits, bias, token_src, expert_dev):
+        """One pass S1..S5.  S4 and S5 read the routing trace, not the S3 outputs, so the last launch of S3 (the
+        decode of the per-block records into fb.out) runs on a side stream beside them: fork after the scoring
+        kernel, join at the end of the step (inside a CUDA graph: two parallel branches)."""
+        main = torch.cuda.current_stream()
+        _, pend = trace_fused_begin(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb,
+                                    pend=self.pend)
+        if pend.kind:
+            self.side.wait_stream(main)
+            with torch.cuda.stream(self.side):
+                trace_fused_finish(pend)
+        pi = self._pi(expert_dev)
+        self.step_prune(token_src, pi)
+        self.step_dispatch(pi)
+        if pend.kind:
+            main.wait_stream(self.side)
+        return self
+
+    def step_serial(self, logits, bias, token_src, expert_dev):
+        """The same pass with every launch on the current stream (one dependent chain)."""
         trace_fused(logits, bias, self.gate, token_src, expert_dev, self.topo, self.fb)
         pi = self._pi(expert_dev)
         self.step_prune(token_src, pi)

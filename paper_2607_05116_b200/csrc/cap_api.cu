@@ -279,6 +279,30 @@ int cap_trace_fused(const float *logits, const float *bias, int32_t L, int64_t T
                        (int64_t)P * cfg->E, *topo, counts, *out, ws, st);
 }
 
+int cap_trace_fused_begin(const float *logits, const float *bias, int32_t L, int64_t T,
+                          const cap_gate_cfg *cfg, int32_t *topk_idx, float *topk_w, int64_t *counts,
+                          int32_t *coact, const int32_t *token_src, const int32_t *expert_dev, int32_t P,
+                          const cap_topology *topo, const cap_eval_out *out, void *ws, size_t ws_bytes,
+                          cap_pending *pend, void *stream)
+{
+    if (!pend) return CAP_EINVAL;
+    memset(pend, 0, sizeof(*pend));
+    ef_decode_park(true);
+    const int rc = cap_trace_fused(logits, bias, L, T, cfg, topk_idx, topk_w, counts, coact, token_src, expert_dev, P,
+                                   topo, out, ws, ws_bytes, stream);
+    if (rc == CAP_OK && ef_decode_take(pend->blob, sizeof(pend->blob))) pend->kind = 1;
+    ef_decode_park(false);
+    return rc;
+}
+
+int cap_trace_fused_finish(const cap_pending *pend, void *stream)
+{
+    if (!pend) return CAP_EINVAL;
+    if (pend->kind == 0) return CAP_OK;
+    if (pend->kind != 1) return CAP_EINVAL;
+    return ef_decode_launch_parked(pend->blob, (cudaStream_t)stream);
+}
+
 int cap_trace_fused_plan(int32_t L, int64_t T, const cap_gate_cfg *cfg, int32_t D, int32_t N, int32_t P,
                          int64_t plan[8])
 {

@@ -4,6 +4,7 @@
 // Method and data layout: cap_eval_fast.cuh and DESIGN.md section 6.
 #include <cstdio>
 #include <cstdlib>
+#include <cstring>
 
 #include "cap_eval_fast.cuh"
 
@@ -725,6 +726,31 @@ int ef_launch_table(const EvalFastGeom &g, const EvalFastWs &fw, const int32_t *
     return check_launch("eval_table_kernel");
 }
 
+static int decode_launch(const DecodeParams &dq, dim3 dgrid, cudaStream_t st)
+{
+    const int na = dq.na;
+    {
+        KernelTimerScope ts("eval_decode", st);
+        if (na <= 12) launch_pdl(eval_decode_kernel<12>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 16) launch_pdl(eval_decode_kernel<16>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 20) launch_pdl(eval_decode_kernel<20>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 24) launch_pdl(eval_decode_kernel<24>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else if (na <= 28) launch_pdl(eval_decode_kernel<28>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        else launch_pdl(eval_decode_kernel<32>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+    }
+    note_launch();
+    return check_launch("eval_decode_kernel");
+}
+
+// A decode launch parked on this host thread (cap_trace_fused_begin arms it, ef_launch_decode fills it,
+// cap_trace_fused_begin takes it): plain data, copied into the caller's cap_pending.
+struct ParkedDecode {
+    DecodeParams dq;
+    uint32_t gx, gy, gz;
+};
+static thread_local bool t_park_armed = false, t_park_full = false;
+static thread_local ParkedDecode t_park;
+
 // adds all records (g.ncta_t * g.maxrec slots per layer and chunk) and writes the caller's outputs (out: device
 // pointers, members may be NULL; counts: [L][E] kept pairs per expert, complete before this launch)
 int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, int32_t L, int64_t T, int32_t E, int32_t P,
@@ -757,18 +783,40 @@ int ef_launch_decode(const EvalFastGeom &g, const EvalFastWs &fw, int32_t L, int
     int na = 1;
     while (na < 32 && (1ll << na) <= T) ++na;
     dq.na = na;
-    {
-        KernelTimerScope ts("eval_decode", st);
-        const dim3 dgrid((unsigned)g.W, (unsigned)g.PC, (unsigned)L);
-        if (na <= 12) launch_pdl(eval_decode_kernel<12>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 16) launch_pdl(eval_decode_kernel<16>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 20) launch_pdl(eval_decode_kernel<20>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 24) launch_pdl(eval_decode_kernel<24>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 28) launch_pdl(eval_decode_kernel<28>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else launch_pdl(eval_decode_kernel<32>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+    const dim3 dgrid((unsigned)g.W, (unsigned)g.PC, (unsigned)L);
+    if (t_park_armed) {
+        // cap_trace_fused_begin: the launch is handed back to the caller, who issues it with cap_trace_fused_finish
+        t_park.dq = dq;
+        t_park.gx = dgrid.x;
+        t_park.gy = dgrid.y;
+        t_park.gz = dgrid.z;
+        t_park_full = true;
+        return CAP_OK;
     }
-    note_launch();
-    return check_launch("eval_decode_kernel");
+    return decode_launch(dq, dgrid, st);
+}
+
+void ef_decode_park(bool on)
+{
+    t_park_armed = on;
+    t_park_full = false;
+}
+
+bool ef_decode_take(void *blob, size_t cap)
+{
+    static_assert(sizeof(ParkedDecode) <= 496, "cap_pending.blob (include/cap.h) is too small for a parked decode launch");
+    if (!t_park_full || cap < sizeof(ParkedDecode)) return false;
+    memcpy(blob, &t_park, sizeof(ParkedDecode));
+    t_park_full = false;
+    return true;
+}
+
+int ef_decode_launch_parked(const void *blob, cudaStream_t st)
+{
+    ParkedDecode pd;
+    memcpy(&pd, blob, sizeof(ParkedDecode));
+    if (pd.gx == 0 || pd.gy == 0 || pd.gz == 0 || pd.gy > 65535u || pd.gz > 65535u) return CAP_EINVAL;
+    return decode_launch(pd.dq, dim3(pd.gx, pd.gy, pd.gz), st);
 }
 
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,

@@ -161,6 +161,11 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
                  const cap_eval_out *after, void *ws, cudaStream_t st);
 // S3 fast path (cap_eval_fast.cu): *used = false when the sizes do not fit it
 // (decodes and finishes the outputs itself: no launch_eval_finalize after it)
+// deferred decode of the bit-sliced S3 path (cap_trace_fused_begin / _finish; cap_eval_fast.cu): while parking is on
+// for this host thread, the decode launch is stored instead of issued
+void ef_decode_park(bool on);
+bool ef_decode_take(void *blob, size_t cap);
+int ef_decode_launch_parked(const void *blob, cudaStream_t st);
 int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k,
                      int32_t E, const int32_t *expert_dev, int32_t P, const cap_topology &topo,
                      const int64_t *counts, const cap_eval_out &out, void *ws, cudaStream_t st, bool *used,

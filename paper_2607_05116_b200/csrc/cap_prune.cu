@@ -15,6 +15,7 @@
 
 #include "cap_eval_final.cuh"
 #include "cap_internal.cuh"
+#include "cap_prune_core.cuh"
 
 namespace cap {
 
@@ -39,20 +40,21 @@ struct PruneParams {
 };
 
 constexpr int PR_THREADS = 128;
+constexpr int PR_WARPS = PR_THREADS / 32;
 
 template <int KMAX>
 __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
 {
-    extern __shared__ int s_map[];     // [E] expert -> device, [64] device -> node, [64] recv, [64] pairs per device
+    extern __shared__ int s_map[];     // [E] expert -> device, [64] device -> node
     __shared__ unsigned long long s_nodemask[64];
     __shared__ unsigned long long s_acc[ACC_N];
     __shared__ unsigned long long s_lp[64];
+    __shared__ unsigned int s_cnt[PR_WARPS][64];   // per warp and device: tokens received << 16 | kept pairs
     __shared__ int s_last;
     const int layer = blockIdx.y;
     const int E = prm.E, D = prm.D, k = prm.k;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *s_dn = s_map + E;
-    int *s_recv = s_dn + 64;
-    int *s_ld = s_recv + 64;
     const bool want_eval = prm.acc != nullptr;
     pdl_launch_dependents();
     pdl_wait();
@@ -70,17 +72,15 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = prm.expert_dev[(size_t)layer * E + i];
     if (threadIdx.x < 64) {
         s_dn[threadIdx.x] = (int)threadIdx.x < D ? prm.dev_node[threadIdx.x] : 0;
-        s_recv[threadIdx.x] = 0;
-        s_ld[threadIdx.x] = 0;
+        s_nodemask[threadIdx.x] = 0ull;
     }
+    for (int i = threadIdx.x; i < PR_WARPS * 64; i += blockDim.x) (&s_cnt[0][0])[i] = 0u;
     if (threadIdx.x < ACC_N) s_acc[threadIdx.x] = 0ull;
     __syncthreads();
-    if (threadIdx.x < 64) {
-        // devices of node threadIdx.x (from the shared copy: one round of global loads, not D)
-        unsigned long long m = 0ull;
-        for (int d = 0; d < D; ++d)
-            if (s_dn[d] == (int)threadIdx.x) m |= 1ull << d;
-        s_nodemask[threadIdx.x] = (int)threadIdx.x < prm.N ? m : 0ull;
+    // devices of every node: one shared-memory OR per device (from the staged copy)
+    if ((int)threadIdx.x < D) {
+        const int n = s_dn[threadIdx.x];
+        if ((unsigned)n < (unsigned)prm.N) atomicOr(&s_nodemask[n], 1ull << threadIdx.x);
     }
     __syncthreads();
 
@@ -88,10 +88,6 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
     const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int near = 0;
     unsigned a_dev = 0, a_loc = 0, a_same = 0, a_node = 0, a_rnode = 0;
-    unsigned long long km = 0ull;      // kept device set of this thread's token (after-metrics)
-    int dkey[KMAX];                    // device of every kept slot, -1 otherwise
-#pragma unroll
-    for (int s = 0; s < KMAX; ++s) dkey[s] = -1;
     if (t < T) {
         const int64_t base = ((int64_t)layer * T + t) * k;
         int e[KMAX], d[KMAX];
@@ -113,90 +109,24 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
 #pragma unroll
         for (int s = 0; s < KMAX; ++s) {
             const int ee = (unsigned)e[s] < (unsigned)E ? e[s] : 0;
-            d[s] = s < k ? (s_map[ee] & 63) : -1 - s;      // absent slots: distinct negative ids
-            e[s] = ee;
+            d[s] = s_map[ee] & 63;
         }
         // source device of the token (reading A5): explicit, or contiguous blocks floor(t D / T); the 32-bit
         // quotient is exact whenever T D < 2^32 (one short division instead of a 64-bit one)
-        const int tok_src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63)
-                            : prm.small ? (int)(((unsigned)t * (unsigned)D) / (unsigned)T) : (int)((t * D) / T);
+        const int src = prm.token_src ? (prm.token_src[(int64_t)layer * T + t] & 63)
+                        : prm.small ? (int)(((unsigned)t * (unsigned)D) / (unsigned)T) : (int)((t * D) / T);
         unsigned long long keepmask = 0ull;
+        PruneRuns<KMAX> runs;
         if (prm.p <= 0.0f) {
 #pragma unroll
             for (int s = 0; s < KMAX; ++s)
                 if (s < k) keepmask |= 1ull << d[s];
+            if (want_eval) prune_runs_only<KMAX>(d, k, runs);
         } else {
-            const int src = tok_src;
-            const int srcn = s_dn[src];
-            // 1. per-device weight at the device's first slot, added in slot order
-            bool rep[KMAX];
-            float a[KMAX];
-#pragma unroll
-            for (int s = 0; s < KMAX; ++s) {
-                rep[s] = s < k;
-                a[s] = wv[s];
-            }
-#pragma unroll
-            for (int s = 1; s < KMAX; ++s) {
-#pragma unroll
-                for (int j = 0; j < s; ++j) {          // selects, not branches: the warp's tokens diverge everywhere
-                    const bool hit = (s < k) & rep[j] & (d[j] == d[s]);
-                    a[j] = hit ? __fadd_rn(a[j], wv[s]) : a[j];
-                    rep[s] = rep[s] & !hit;
-                }
-            }
-            // 2. cost ratio of every represented device
-            float ratio[KMAX];
-            int m = 0;
-#pragma unroll
-            for (int s = 0; s < KMAX; ++s) {
-                const int dd = d[s] & 63;
-                const int c = (dd == src) ? prm.cost_local : (s_dn[dd] == srcn) ? prm.cost_intra : prm.cost_inter;
-                ratio[s] = (c == 0) ? CUDART_INF_F : __fdiv_rn(a[s], (float)c);
-                m += rep[s] ? 1 : 0;
-            }
-            // 3. rank: devices with a larger ratio, or an equal ratio and a lower id, come first
-            int rank[KMAX];
-#pragma unroll
-            for (int s = 0; s < KMAX; ++s) rank[s] = 0;
-#pragma unroll
-            for (int s = 1; s < KMAX; ++s) {
-#pragma unroll
-                for (int j = 0; j < s; ++j) {          // each pair once: exactly one of two represented devices comes first
-                    const bool jfirst = (ratio[j] > ratio[s]) | ((ratio[j] == ratio[s]) & (d[j] < d[s]));
-                    rank[s] += (int)(rep[j] & jfirst);
-                    rank[j] += (int)(rep[s] & !jfirst);
-                }
-            }
-            // 4. greedy in rank order
-            const float target = __fsub_rn(1.0f, prm.p);
-            float cum = 0.0f, r_last = 0.0f, r_cut = 0.0f;
-            bool stopped = false;
-#pragma unroll
-            for (int r = 0; r < KMAX; ++r) {
-                float Ar = 0.0f, Rr = 0.0f;
-                int dr = 0;
-#pragma unroll
-                for (int s = 0; s < KMAX; ++s) {
-                    const bool sel = rep[s] & (rank[s] == r);
-                    Ar = sel ? a[s] : Ar;
-                    Rr = sel ? ratio[s] : Rr;
-                    dr = sel ? d[s] : dr;
-                }
-                const bool act = (r < m) & !stopped;
-                const bool reached = cum >= target;
-                near |= (int)(act & (fabsf(__fsub_rn(cum, target)) < 1e-6f));
-                const bool stop_now = act & reached, keep_now = act & !reached;
-                r_cut = stop_now ? Rr : r_cut;
-                keepmask |= keep_now ? (1ull << dr) : 0ull;
-                cum = keep_now ? __fadd_rn(cum, Ar) : cum;
-                r_last = keep_now ? Rr : r_last;
-                stopped = stopped | stop_now;
-            }
-            if (stopped && r_last != CUDART_INF_F && r_cut != CUDART_INF_F && __fsub_rn(r_last, r_cut) < 1e-6f)
-                near = 1;
+            keepmask = prune_token<KMAX>(d, wv, k, src, s_dn, prm.cost_local, prm.cost_intra, prm.cost_inter, prm.p,
+                                         near, runs);
         }
-        // 5. kept mask per slot
+        // kept mask per slot
         if (KMAX == 8 && k == 8 && prm.vec) {
             unsigned lo = 0, hi = 0;
 #pragma unroll
@@ -212,17 +142,17 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
         }
         // evaluation of the kept trace under this placement (P = 1)
         if (want_eval) {
-            const int src = tok_src;
             const int srcn = s_dn[src];
             unsigned long long nodebits = 0ull;
 #pragma unroll
-            for (int s = 0; s < KMAX; ++s) {
-                if (s < k && ((keepmask >> d[s]) & 1ull)) {
-                    nodebits |= 1ull << s_dn[d[s]];
-                    dkey[s] = d[s];
+            for (int i = 0; i < KMAX; ++i) {
+                const uint32_t r = runs.run[i];
+                const int dd = (int)(r & 63u);
+                if (r != 0u && ((keepmask >> dd) & 1ull)) {
+                    nodebits |= 1ull << s_dn[dd];
+                    atomicAdd(&s_cnt[warp][dd], 0x10000u | ((r >> 8) & 0xffu));   // one token, run-length pairs
                 }
             }
-            km = keepmask;
             a_dev = __popcll(keepmask);
             a_loc = (unsigned)((keepmask >> src) & 1ull);
             a_same = __popcll(keepmask & s_nodemask[srcn]);
@@ -234,27 +164,9 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
     }
     if (prm.near_margin) {
         const unsigned b = __ballot_sync(0xffffffffu, near != 0);
-        if ((threadIdx.x & 31) == 0 && b) atomicAdd(&prm.near_margin[(size_t)layer * prm.near_stride], (unsigned long long)__popc(b));
+        if (lane == 0 && b) atomicAdd(&prm.near_margin[(size_t)layer * prm.near_stride], (unsigned long long)__popc(b));
     }
     if (want_eval) {
-        const int lane = threadIdx.x & 31;
-        // kept pairs per device: equal keys of a slot are counted once per warp (match), no per-pair atomics
-#pragma unroll
-        for (int s = 0; s < KMAX; ++s) {
-            const unsigned grp = __match_any_sync(0xffffffffu, dkey[s]);
-            if (dkey[s] >= 0 && (grp & ((1u << lane) - 1u)) == 0u) atomicAdd(&s_ld[dkey[s]], __popc(grp));
-        }
-        // tokens received per device: one ballot per device, lane d keeps the count of devices d, d + 32
-        int r0 = 0, r1 = 0;
-        for (int dd = 0; dd < D; ++dd) {
-            const int c = __popc(__ballot_sync(0xffffffffu, (km >> dd) & 1ull));
-            if (lane == (dd & 31)) {
-                if (dd < 32) r0 = c;
-                else r1 = c;
-            }
-        }
-        if (r0) atomicAdd(&s_recv[lane], r0);
-        if (r1) atomicAdd(&s_recv[lane + 32], r1);
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) {
             a_dev += __shfl_xor_sync(0xffffffffu, a_dev, off);
@@ -263,7 +175,7 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             a_node += __shfl_xor_sync(0xffffffffu, a_node, off);
             a_rnode += __shfl_xor_sync(0xffffffffu, a_rnode, off);
         }
-        if ((threadIdx.x & 31) == 0) {
+        if (lane == 0) {
             atomicAdd(&s_acc[ACC_DEV], (unsigned long long)a_dev);
             atomicAdd(&s_acc[ACC_LOCAL], (unsigned long long)a_loc);
             atomicAdd(&s_acc[ACC_SAMENODE], (unsigned long long)a_same);
@@ -273,10 +185,18 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
         __syncthreads();
         if (threadIdx.x < ACC_N && s_acc[threadIdx.x])
             atomicAdd(&prm.acc[(size_t)layer * ACC_N + threadIdx.x], s_acc[threadIdx.x]);
-        if ((int)threadIdx.x < D && s_recv[threadIdx.x])
-            atomicAdd(&prm.recv[(size_t)layer * D + threadIdx.x], (unsigned long long)s_recv[threadIdx.x]);
-        if (threadIdx.x < 64 && s_ld[threadIdx.x])
-            atomicAdd(&prm.ldirect[(size_t)layer * 64 + threadIdx.x], (unsigned long long)s_ld[threadIdx.x]);
+        if (threadIdx.x < 64) {
+            // the block's tokens received / kept pairs per device
+            unsigned rc = 0, pr = 0;
+#pragma unroll
+            for (int w2 = 0; w2 < PR_WARPS; ++w2) {
+                const unsigned v = s_cnt[w2][threadIdx.x];
+                rc += v >> 16;
+                pr += v & 0xffffu;
+            }
+            if ((int)threadIdx.x < D && rc) atomicAdd(&prm.recv[(size_t)layer * D + threadIdx.x], (unsigned long long)rc);
+            if (pr) atomicAdd(&prm.ldirect[(size_t)layer * 64 + threadIdx.x], (unsigned long long)pr);
+        }
         // last block of the layer: all sums are in L2, finish the outputs
         __threadfence();
         __syncthreads();
@@ -343,7 +263,7 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
         prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
                   (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
         dim3 grid((unsigned)((T + PR_THREADS - 1) / PR_THREADS), (unsigned)L);
-        const size_t smem = sizeof(int) * ((size_t)E + 192);
+        const size_t smem = sizeof(int) * ((size_t)E + 64);
         {
             KernelTimerScope ts("prune", st);
             // the unrolled O(K^2) select chains are sized by the template: k = 10 (config 5) in <12>, not <16>

@@ -373,6 +373,70 @@ def test_single_launch_variant_optin(shape, monkeypatch):
     assert_eval_equal(fb.out, ev_r, False, "fused2 ")
 
 
+@pytest.mark.parametrize("base,kw", [("target", dict(T=4099, P=40)), ("qwen3", dict(T=1500, L=3)),
+                                     ("dsv3", dict(T=1024, L=2, P=16)), ("tiny", dict())],
+                         ids=["fused", "fused-L3", "staged-sigmoid", "tiny"])
+def test_trace_fused_begin_finish_and_forked_step(base, kw):
+    """cap_trace_fused_begin / _finish (include/cap.h): the two halves give the results of the single call, and
+    Pipeline.step -- which runs the second half on a side stream beside S4 / S5 -- gives those of the serial
+    chain, launched directly and replayed from a CUDA graph (fork / join inside the capture)."""
+    cfg = W.CONFIGS[base].with_(**kw)
+    from parity_util import layers_inputs
+    layers = tuple(range(cfg.L))
+    logits, bias, cand = layers_inputs(cfg, layers, cfg.T)
+    dn = W.dev_node(cfg)
+    dn_d = dev(dn)
+    topo = topo_of(cfg, dn_d)
+    gate = cap.gate_cfg(cfg.E, **cfg.gate)
+    x_d, b_d, c_d = dev(logits), dev(bias), dev(cand)
+    idx_r, w_r, cnt_r, C_r, ev_r = O.trace_fused(logits, bias, cfg.gate, cand, dn, cost_inter=cfg.cost_inter,
+                                                 bytes_per_token=cfg.bytes_per_token)
+    n0 = cap.launch_count()
+    fb, pend = cap.trace_fused_begin(x_d, b_d, gate, None, c_d, topo)
+    n1 = cap.launch_count()
+    cap.trace_fused_finish(pend)                       # same stream: ordered behind the first half
+    torch.cuda.synchronize()
+    assert cap.launch_count() - n1 == (1 if pend.kind else 0)
+    assert pend.kind == 1                               # all four shapes reach the bit-sliced S3 path
+    _, p0 = cap.trace_fused_begin(x_d, b_d, gate, None, c_d, topo, per_token=True)
+    assert p0.kind == 0                                 # per-token outputs: generic S3 kernel, nothing owed
+    cap.trace_fused_finish(p0)
+    assert np.array_equal(host(fb.idx), idx_r) and np.array_equal(host(fb.counts), cnt_r)
+    assert np.array_equal(host(fb.coact), C_r)
+    assert_eval_equal(fb.out, ev_r, False, "begin/finish ")
+    n2 = cap.launch_count()
+    cap.trace_fused(x_d, b_d, gate, None, c_d, topo)   # the plain call still launches the decode itself
+    assert cap.launch_count() - n2 == (n1 - n0) + (1 if pend.kind else 0)
+
+    mk = lambda: cap.Pipeline(cfg.L, cfg.T, gate, cfg.D, cfg.N, cfg.P, dn_d, cost_inter=cfg.cost_inter,
+                              bytes_per_token=cfg.bytes_per_token, tau=cfg.taus[-1], chosen=0, device="cuda")
+    ser, forked, graphed = mk(), mk(), mk()
+    ser.step_serial(x_d, b_d, None, c_d)
+    forked.step(x_d, b_d, None, c_d)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        graphed.step(x_d, b_d, None, c_d)              # warm-up outside the capture
+    torch.cuda.current_stream().wait_stream(s)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        graphed.step(x_d, b_d, None, c_d)
+    for t in graphed.result_tensors():
+        t.zero_()
+    g.replay()
+    g.replay()
+    torch.cuda.synchronize()
+    assert_eval_equal(forked.fb.out, ev_r, False, "forked ")
+    assert_eval_equal(graphed.fb.out, ev_r, False, "graphed ")
+    for a, b, c in zip(ser.result_tensors(), forked.result_tensors(), graphed.result_tensors()):
+        if a.shape == ser.sorted_pairs.shape and a.dtype == torch.int32 and a is not ser.pair_pos:
+            for l in range(cfg.L):
+                n = int(ser.offsets[l, -1])
+                assert torch.equal(a[l, :n], b[l, :n]) and torch.equal(a[l, :n], c[l, :n])
+        else:
+            assert torch.equal(a, b) and torch.equal(a, c)
+
+
 def test_host_pipeline_double_buffered_matches_single():
     """The end-to-end call with two staging sets (copies on side streams, as bench.py's e2e leg uses it)
     returns, step by step, exactly what the plain device pipeline computes on the same inputs."""
