@@ -314,6 +314,8 @@ def measure(cfg, W, WD, cap, torch, dev, rank, steps, replays, barrier, light=Fa
     g_disp = pipe.capture_stage("dispatch", None, d_sets[0][2])
     ms_prune = timed_replays(torch, lambda i: g_prune.replay(), n, barrier)
     ms_disp = timed_replays(torch, lambda i: g_disp.replay(), n, barrier)
+    g_pd = pipe.capture_stage("prune_dispatch", None, d_sets[0][2])
+    ms_pd = timed_replays(torch, lambda i: g_pd.replay(), n, barrier)
     # the dominant kernel of the pass alone, back to back (rotating inputs), by the library's profiling entry
     kms = None
     if not light:
@@ -327,7 +329,7 @@ def measure(cfg, W, WD, cap, torch, dev, rank, steps, replays, barrier, light=Fa
         del g_src
     plan = cap.trace_fused_plan(L, T, gate, D, cfg.N, P)
     res = dict(pipe=pipe, d_sets=d_sets, gate=gate, n_sets=n_sets, in_bytes=in_bytes, ms_step=ms_step,
-               ms_fused=ms_fused, ms_prune=ms_prune, ms_disp=ms_disp, kernel_ms=kms, plan=plan, ms_src=ms_src,
+               ms_fused=ms_fused, ms_prune=ms_prune, ms_disp=ms_disp, ms_pd=ms_pd, kernel_ms=kms, plan=plan, ms_src=ms_src,
                launches_per_step=launches_per_step)
     return res
 
@@ -352,6 +354,11 @@ def summarise(cfg, res, peak):
             "S5_cap_dispatch_layout": {"ms": ms_disp, "algorithmic_bytes": b_disp, "gbs": gbs(b_disp, ms_disp),
                                        "frac_of_hbm_peak": gbs(b_disp, ms_disp) / peak,
                                        "calls": 1, "layers": cfg.L},
+            "S4S5_cap_prune_dispatch": {"ms": med(res["ms_pd"]), "algorithmic_bytes": ab["prune"] + b_disp,
+                                        "gbs": gbs(ab["prune"] + b_disp, med(res["ms_pd"])),
+                                        "frac_of_hbm_peak": gbs(ab["prune"] + b_disp, med(res["ms_pd"])) / peak,
+                                        "what": "the fused S4 + S5 call the step uses (three launches); the two rows "
+                                                "above are the stand-alone calls"},
         },
         "launches_per_step": int(res["launches_per_step"]),
     }

@@ -50,6 +50,7 @@ extern "C" {
 #define CAP_CALL_TRACE_FUSED 5
 #define CAP_CALL_COACT_PLACEMENT 6   /* T, k, P ignored */
 #define CAP_CALL_DISPATCH_ROWS 7     /* L, E, k, P ignored */
+#define CAP_CALL_PRUNE_DISPATCH 8    /* P ignored */
 
 /* Gate configuration (Eq. 1; scoring / group-limited routing / tie rule from
  * BASELINE.json, readings R1, R2, R14, R21). */
@@ -149,6 +150,21 @@ int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T,
                         int32_t E, const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs,
                         int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes,
                         void *stream);
+
+/* S4 followed by S5 under the same placement, in three launches instead of the six nodes of cap_prune +
+ * cap_dispatch_layout_batched (at the BASELINE sizes both stages are launch-latency-bound).  Results are exactly
+ * those of cap_prune(..., kept, after, near_margin, ...) followed by cap_dispatch_layout_batched(topk_idx, kept,
+ * ..., expert_dev, D, sorted_pairs, pair_pos, offsets, ...): the pruning kernel (Eq. 6) also counts
+ * the kept pairs per device of every 32 tokens, which is the histogram the stable counting sort starts
+ * from; the sort's scan and scatter launches carry one extra block each that adds up / writes the after-metrics,
+ * so no accumulator is zeroed and no separate histogram or finalize launch is needed.
+ *   Arguments as in the two calls (expert_dev [L][E]: the chosen placement per layer; after, near_margin, pair_pos
+ *   nullable).  Workspace: cap_workspace_bytes(CAP_CALL_PRUNE_DISPATCH, L, T, E, k, D, 0). */
+int cap_prune_dispatch(const int32_t *topk_idx, const float *topk_w, const int32_t *token_src, int32_t L,
+                       int64_t T, int32_t k, int32_t E, const int32_t *expert_dev, const cap_topology *topo,
+                       float p, uint8_t *kept, const cap_eval_out *after, int64_t *near_margin,
+                       int32_t *sorted_pairs, int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes,
+                       void *stream);
 
 /* S5 for L layers in one call (three launches for all layers instead of three per layer: at the BASELINE sizes a
  * layer's sort is launch-latency-bound).  Per layer exactly cap_dispatch_layout: topk_idx / kept [L][T][k],

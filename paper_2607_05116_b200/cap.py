@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcap_b200.so")
 
 (CALL_GATE_TOPK, CALL_COACTIVATION, CALL_EVAL_PLACEMENTS, CALL_PRUNE, CALL_DISPATCH_LAYOUT, CALL_TRACE_FUSED,
- CALL_COACT_PLACEMENT, CALL_DISPATCH_ROWS) = range(8)
+ CALL_COACT_PLACEMENT, CALL_DISPATCH_ROWS, CALL_PRUNE_DISPATCH) = range(9)
 OK, EINVAL, EWORKSPACE, ECUDA = 0, -1, -2, -3
 
 EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prune",
@@ -21,7 +21,7 @@ EXPORTS = ("cap_gate_topk", "cap_coactivation", "cap_eval_placements", "cap_prun
            "cap_validate_placements", "cap_last_cuda_error", "cap_launch_count", "cap_version",
            "cap_kernel_timer_arm", "cap_kernel_timer_ms", "cap_profile_fused_kernel", "cap_trace_fused_plan",
            "cap_dispatch_layout_static", "cap_static_scratch_bytes", "cap_prune_naive", "cap_dispatch_row_weights", "cap_dispatch_layout_batched",
-           "cap_trace_fused_begin", "cap_trace_fused_finish")
+           "cap_trace_fused_begin", "cap_trace_fused_finish", "cap_prune_dispatch")
 
 KERNEL_TAGS = ("trace_fused", "gate_topk", "coact", "masked_counts", "eval_table", "eval", "eval_decode", "eval_finalize", "prune",
                "dispatch_hist", "dispatch_scan", "dispatch_scatter", "coact_placement", "objective", "rows_hist", "rows_scan", "rows_scatter", "adjust")
@@ -94,6 +94,11 @@ def lib():
         L.cap_prune_naive.argtypes = [vp, vp, i32, i64, i32, f32, vp, vp, vp]
         L.cap_dispatch_row_weights.argtypes = [vp, vp, i64, i32, i64, vp, vp]
         L.cap_dispatch_layout_batched.argtypes = [vp, vp, i32, i64, i32, i32, vp, i32, vp, vp, vp, vp, sz, vp]
+        L.cap_prune_dispatch.argtypes = [vp, vp, vp, i32, i64, i32, i32, vp, C.POINTER(Topology), f32, vp,
+                                         C.POINTER(EvalOut), vp, vp, vp, vp, vp, sz, vp]
+        L.cap_trace_fused_begin.argtypes = [vp, vp, i32, i64, C.POINTER(GateCfg), vp, vp, vp, vp, vp, vp,
+                                            i32, C.POINTER(Topology), C.POINTER(EvalOut), vp, sz, C.POINTER(Pending), vp]
+        L.cap_trace_fused_finish.argtypes = [C.POINTER(Pending), vp]
         L.cap_kernel_timer_arm.argtypes = [C.c_char_p, C.c_int]
         L.cap_kernel_timer_ms.argtypes = [C.c_int]
         L.cap_kernel_timer_ms.restype = C.c_float
@@ -266,6 +271,32 @@ def dispatch_layout_batched(idx, kept, expert_dev, D, want_pos=True, ws=None, ou
                                            _ptr(offsets), _ptr(ws), ws.numel(), _stream())
     _check(rc, "cap_dispatch_layout_batched")
     return sorted_pairs, offsets, pair_pos
+
+
+def prune_dispatch(idx, w, token_src, expert_dev, topo, p, want_after=True, want_pos=True, ws=None, bufs=None):
+    """cap_prune_dispatch: S4 + S5 under expert_dev [L,E] in three launches.  Returns (kept, near_margin, after,
+    sorted_pairs, offsets, pair_pos) -- what prune() followed by dispatch_layout_batched() returns."""
+    L, T, k = idx.shape
+    E = expert_dev.shape[-1]
+    D = topo.D
+    if bufs is None:
+        kept = torch.empty((L, T, k), dtype=torch.uint8, device=idx.device)
+        near = torch.empty((L,), dtype=torch.int64, device=idx.device)
+        after = alloc_eval_out(L, 1, D, T, False, idx.device) if want_after else None
+        sorted_pairs = torch.empty((L, T * k), dtype=torch.int32, device=idx.device)
+        pair_pos = torch.empty((L, T * k), dtype=torch.int32, device=idx.device) if want_pos else None
+        offsets = torch.empty((L, D + 1), dtype=torch.int64, device=idx.device)
+    else:
+        kept, near, after, sorted_pairs, offsets, pair_pos = bufs
+    if ws is None:
+        ws = workspace(CALL_PRUNE_DISPATCH, L, T, E, k, D, 0, idx.device)
+    s = _eval_struct(after) if after is not None else None
+    rc = lib().cap_prune_dispatch(_ptr(idx, torch.int32), _ptr(w, torch.float32), _ptr(token_src, torch.int32), L, T,
+                                  k, E, _ptr(expert_dev, torch.int32), C.byref(topo), float(p), _ptr(kept),
+                                  C.byref(s) if s is not None else None, _ptr(near), _ptr(sorted_pairs),
+                                  _ptr(pair_pos), _ptr(offsets), _ptr(ws), ws.numel(), _stream())
+    _check(rc, "cap_prune_dispatch")
+    return kept, near, after, sorted_pairs, offsets, pair_pos
 
 
 def dispatch_layout_static(idx, kept, expert_dev, D, sorted_pairs, offsets, pair_pos=None):
@@ -502,6 +533,7 @@ class Pipeline:
         self.pair_pos = torch.empty((L, T * k), dtype=torch.int32, device=device)
         self.offsets = torch.empty((L, D + 1), dtype=torch.int64, device=device)
         self.ws_disp = workspace(CALL_DISPATCH_LAYOUT, L, T, E, k, D, 0, device)
+        self.ws_pd = workspace(CALL_PRUNE_DISPATCH, L, T, E, k, D, 0, device)
         self.pi = torch.empty((L, E), dtype=torch.int32, device=device)
         self.side = torch.cuda.Stream(device=device)       # the S3 decode runs here, beside S4 / S5 (step)
         self.pend = Pending()
@@ -524,6 +556,15 @@ class Pipeline:
                              self.ws_prune.numel(), _stream())
         _check(rc, "cap_prune")
 
+    def step_prune_dispatch(self, token_src, pi):
+        """S4 + S5 as one call (cap_prune_dispatch: three launches) on the buffers of the last cap_trace_fused."""
+        rc = lib().cap_prune_dispatch(_ptr(self.fb.idx), _ptr(self.fb.w), _ptr(token_src, torch.int32), self.L,
+                                      self.T, self.gate.k, self.gate.E, _ptr(pi), C.byref(self.topo),
+                                      float(self.tau), _ptr(self.kept), C.byref(self.after_struct), _ptr(self.near),
+                                      _ptr(self.sorted_pairs), _ptr(self.pair_pos), _ptr(self.offsets),
+                                      _ptr(self.ws_pd), self.ws_pd.numel(), _stream())
+        _check(rc, "cap_prune_dispatch")
+
     def step_dispatch(self, pi):
         """S5 for every layer on the kept mask of the last cap_prune: one batched call (three launches)."""
         dispatch_layout_batched(self.fb.idx, self.kept, pi if pi.is_contiguous() else pi.contiguous(), self.D,
@@ -540,9 +581,7 @@ class Pipeline:
             self.side.wait_stream(main)
             with torch.cuda.stream(self.side):
                 trace_fused_finish(pend)
-        pi = self._pi(expert_dev)
-        self.step_prune(token_src, pi)
-        self.step_dispatch(pi)
+        self.step_prune_dispatch(token_src, self._pi(expert_dev))
         if pend.kind:
             main.wait_stream(self.side)
         return self
@@ -556,10 +595,12 @@ class Pipeline:
         return self
 
     def capture_stage(self, which, token_src, expert_dev):
-        """Graph of one stage alone ("prune" = S4 with after-metrics, "dispatch" = S5) on the current buffers,
+        """Graph of one stage alone ("prune" = S4 with after-metrics, "dispatch" = S5, "prune_dispatch" = the
+        fused S4 + S5 call the step uses) on the current buffers,
         for stand-alone stage timings; the preceding stages must have run once."""
         pi = self._pi(expert_dev)
-        fn = (lambda: self.step_prune(token_src, pi)) if which == "prune" else (lambda: self.step_dispatch(pi))
+        fn = {"prune": lambda: self.step_prune(token_src, pi), "dispatch": lambda: self.step_dispatch(pi),
+              "prune_dispatch": lambda: self.step_prune_dispatch(token_src, pi)}[which]
         fn()
         torch.cuda.synchronize()
         g = torch.cuda.CUDAGraph()

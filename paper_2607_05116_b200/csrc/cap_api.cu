@@ -175,6 +175,9 @@ size_t cap_workspace_bytes(int which_call, int32_t L, int64_t T, int32_t E, int3
     case CAP_CALL_DISPATCH_ROWS:
         if (D < 1) return 0;
         return dispatch_rows_ws_bytes(T, D);
+    case CAP_CALL_PRUNE_DISPATCH:
+        if (D < 1) return 0;
+        return prune_dispatch_ws_bytes(L, T, k, E, D);
     case CAP_CALL_COACT_PLACEMENT:
         if (D < 1) return 0;
         return place_ws_bytes(L, E, D);
@@ -228,6 +231,21 @@ int cap_prune(const int32_t *topk_idx, const float *topk_w, const int32_t *token
     if (after && (!ws || ws_bytes < eval_ws_bytes(L, T, E, k, topo->D, 1))) return CAP_EWORKSPACE;
     return launch_prune(topk_idx, topk_w, token_src, L, T, k, E, expert_dev, *topo, p, kept, near_margin, after,
                         ws, (cudaStream_t)stream);
+}
+
+int cap_prune_dispatch(const int32_t *topk_idx, const float *topk_w, const int32_t *token_src, int32_t L,
+                       int64_t T, int32_t k, int32_t E, const int32_t *expert_dev, const cap_topology *topo,
+                       float p, uint8_t *kept, const cap_eval_out *after, int64_t *near_margin,
+                       int32_t *sorted_pairs, int32_t *pair_pos, int64_t *offsets, void *ws, size_t ws_bytes,
+                       void *stream)
+{
+    if (!sizes_ok(L, T, E, k) || !topo_ok(topo)) return CAP_EINVAL;
+    if (!(p < 1.0f)) return CAP_EINVAL;   // also rejects NaN
+    if (L > 0 && (!expert_dev || !offsets)) return CAP_EINVAL;
+    if ((int64_t)L * T > 0 && (!topk_idx || !topk_w || !kept || !sorted_pairs)) return CAP_EINVAL;
+    if (L > 0 && (!ws || ws_bytes < prune_dispatch_ws_bytes(L, T, k, E, topo->D))) return CAP_EWORKSPACE;
+    return launch_prune_dispatch(topk_idx, topk_w, token_src, L, T, k, E, expert_dev, *topo, p, kept, near_margin,
+                                 after, sorted_pairs, pair_pos, offsets, ws, (cudaStream_t)stream);
 }
 
 int cap_dispatch_layout(const int32_t *topk_idx, const uint8_t *kept, int64_t T, int32_t k,

@@ -5,6 +5,7 @@
 // ordered scan over (device, sub-chunk) fixes every sub-chunk's base per device -- this is what makes
 // the sort stable across warps and blocks without global cursors; (3) every warp scatters its
 // sub-chunk in pair order, ranking equal keys inside a 32-pair round with match/popc.
+#include "cap_eval_final.cuh"
 #include "cap_internal.cuh"
 
 namespace cap {
@@ -15,11 +16,8 @@ constexpr int DS_NW = DS_THREADS / 32;
 constexpr int DS_MAXD = 64;
 
 // sub-chunks of n pairs, padded so that every lane of the scan owns whole 16-byte vectors
-static int64_t ds_stride(int64_t n)
-{
-    const int64_t nsub = (n + DS_SUB - 1) / DS_SUB;
-    return ((nsub + 127) / 128) * 128;
-}
+int64_t dispatch_stride_subs(int64_t nsub) { return ((nsub + 127) / 128) * 128; }
+static int64_t ds_stride(int64_t n) { return dispatch_stride_subs((n + DS_SUB - 1) / DS_SUB); }
 
 size_t dispatch_ws_bytes(int64_t T, int32_t k, int32_t D)
 {
@@ -102,12 +100,37 @@ dispatch_hist_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict_
 // the span totals are scanned across the warps, pass 2 writes the exclusive prefixes (one int4 per lane, eight
 // chunks in flight) starting from the span's base.  The row total goes to devtot[d]; the scatter kernel turns the
 // D totals into the device offsets.  (Round 1 scanned all rows in ONE block: 893 of S5's 1 455 us at 2^22 tokens.)
+// cap_prune_dispatch: block D of every layer adds up the per-block partial sums the S4 kernel left (PD_PART 32-bit
+// columns per block: the evaluation accumulators, then the tokens received per device) into the 64-bit sums the
+// finalize step reads.  Plain stores: nothing has to be zeroed beforehand.
 __global__ void __launch_bounds__(512)
-dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, int D, int64_t stride, DsBatch lb)
+dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, int D, int64_t stride, DsBatch lb, DsReduce rd)
 {
     __shared__ int s_span[16];
+    __shared__ unsigned long long s_red[7][PD_PART];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
     const int d = blockIdx.x;
+    if (d >= D) {
+        // reduce block j = d - D: S4 blocks [j per_rb, (j + 1) per_rb)
+        pdl_launch_dependents();
+        pdl_wait();
+        const int j = d - D;
+        const int ng = (int)blockDim.x / PD_PART;          // 7 groups of 72 threads in a 512-thread block, else 1
+        const int g = (int)threadIdx.x / PD_PART, col = (int)threadIdx.x % PD_PART;
+        const uint32_t *pp = rd.part + (size_t)blockIdx.y * rd.nblk * PD_PART;
+        const int64_t b_lo = (int64_t)j * rd.per_rb, b_hi = min(rd.nblk, b_lo + rd.per_rb);
+        unsigned long long sum = 0ull;
+        if (g < ng)
+            for (int64_t b = b_lo + g; b < b_hi; b += ng) sum += pp[b * PD_PART + col];
+        if (g < ng) s_red[g][col] = sum;
+        __syncthreads();
+        if ((int)threadIdx.x < PD_PART) {
+            unsigned long long tot = 0ull;
+            for (int g2 = 0; g2 < ng; ++g2) tot += s_red[g2][threadIdx.x];
+            rd.red[((size_t)blockIdx.y * rd.nrb + j) * PD_PART + threadIdx.x] = tot;
+        }
+        return;
+    }
     hist += blockIdx.y * lb.ws_stride + (int64_t)d * stride;
     base += blockIdx.y * lb.ws_stride + (int64_t)d * stride;
     int *devtot = const_cast<int *>(hist) - (int64_t)d * stride + 2 * stride * D;     // behind hist and base of the layer
@@ -161,15 +184,21 @@ dispatch_scan_kernel(const int *__restrict__ hist, int *__restrict__ base, int D
     }
 }
 
+// RMAX >= rounds: a warp's sub-chunk is `rounds` rounds of 32 consecutive pairs (8 for the stand-alone call; k for
+// cap_prune_dispatch, whose S4 kernel counted 32 tokens per warp).  fin_block >= 0: that block of every layer does
+// not scatter; it finishes the after-metrics of cap_prune_dispatch from the sums the scan kernel left (fin) and
+// from the pairs per device (= the row totals of the scan).
+template <int RMAX>
 __global__ void __launch_bounds__(DS_THREADS)
 dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, int64_t n,
                         int E, int D, const int32_t *__restrict__ expert_dev,
                         const int *__restrict__ base, long long *__restrict__ offsets,
                         int32_t *__restrict__ sorted_pairs, int32_t *__restrict__ pair_pos, int64_t stride,
-                        DsBatch lb)
+                        DsBatch lb, int rounds, int fin_block, FinalParams fin, DsReduce rd)
 {
     extern __shared__ int sm[];
     __shared__ int s_off[65];                      // exclusive prefix of the device totals (T k < 2^31)
+    __shared__ unsigned long long s_lp[64];
     int *s_map = sm;                               // [E]
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *running = sm + E + warp * DS_MAXD;        // [D] next free position per device, private to the warp
@@ -183,10 +212,27 @@ dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restri
     const int64_t sub = (int64_t)blockIdx.x * DS_NW + warp;
     pdl_launch_dependents();
     pdl_wait();
-    const int64_t i0 = sub * DS_SUB;
-    int key[DS_SUB / 32];
+    if ((int)blockIdx.x == fin_block) {
+        if ((int)threadIdx.x < PD_PART) {
+            unsigned long long tot = 0ull;
+            for (int j = 0; j < rd.nrb; ++j) tot += rd.red[((size_t)blockIdx.y * rd.nrb + j) * PD_PART + threadIdx.x];
+            if (threadIdx.x < ACC_N) rd.acc[(size_t)blockIdx.y * ACC_N + threadIdx.x] = tot;
+            else if ((int)threadIdx.x - ACC_N < D) rd.recv[(size_t)blockIdx.y * D + threadIdx.x - ACC_N] = tot;
+        }
+        __threadfence();
+        __syncthreads();
+        if (warp == 0) {
+            const int *devtot = base + 2 * stride * D - stride * D;
+            s_lp[lane] = lane < D ? (unsigned long long)devtot[lane] : 0ull;
+            s_lp[lane + 32] = lane + 32 < D ? (unsigned long long)devtot[lane + 32] : 0ull;
+            eval_finalize_one(fin, (int)blockIdx.y, lane, s_lp, true);
+        }
+        return;
+    }
+    const int64_t i0 = sub * 32 * rounds;
+    int key[RMAX];
 #pragma unroll
-    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = pair_expert(idx, kept, i0 + r * 32 + lane, n);
+    for (int r = 0; r < RMAX; ++r) key[r] = r < rounds ? pair_expert(idx, kept, i0 + r * 32 + lane, n) : -1;
     for (int i = threadIdx.x; i < E; i += blockDim.x) s_map[i] = expert_dev[i];
     if (warp == 0) {
         // device offsets from the row totals the scan kernel left behind hist and base
@@ -211,23 +257,69 @@ dispatch_scatter_kernel(const int32_t *__restrict__ idx, const uint8_t *__restri
     __syncwarp();
     if (i0 >= n) return;
 #pragma unroll
-    for (int r = 0; r < DS_SUB / 32; ++r) key[r] = expert_key(key[r], s_map, E, D);
+    for (int r = 0; r < RMAX; ++r) key[r] = expert_key(key[r], s_map, E, D);
 #pragma unroll
-    for (int r = 0; r < DS_SUB / 32; ++r) {
-        const int64_t i = i0 + r * 32 + lane;
-        const int d = key[r];
-        const unsigned grp = __match_any_sync(0xffffffffu, d);
-        const int rank = __popc(grp & ((1u << lane) - 1u));
-        int pos = -1;
-        if (d >= 0) {
-            pos = running[d] + rank;
-            sorted_pairs[pos] = (int32_t)i;
+    for (int r = 0; r < RMAX; ++r) {
+        if (r < rounds) {
+            const int64_t i = i0 + r * 32 + lane;
+            const int d = key[r];
+            const unsigned grp = __match_any_sync(0xffffffffu, d);
+            const int rank = __popc(grp & ((1u << lane) - 1u));
+            int pos = -1;
+            if (d >= 0) {
+                pos = running[d] + rank;
+                sorted_pairs[pos] = (int32_t)i;
+            }
+            if (pair_pos && i < n) pair_pos[i] = pos;
+            __syncwarp();
+            if (d >= 0 && rank == 0) running[d] += __popc(grp);
+            __syncwarp();
         }
-        if (pair_pos && i < n) pair_pos[i] = pos;
-        __syncwarp();
-        if (d >= 0 && rank == 0) running[d] += __popc(grp);
-        __syncwarp();
     }
+}
+
+// scan + scatter over a histogram that is already in place (hist rows of `stride` sub-chunks of 32 * rounds pairs).
+// rd / fin: the extra blocks of cap_prune_dispatch (rd.part == NULL: none).
+int launch_dispatch_tail(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t n, int32_t E,
+                         const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
+                         int64_t *offsets, int *hist, int64_t stride, int rounds, const DsReduce &rd,
+                         const FinalParams *fin, cudaStream_t st)
+{
+    const int64_t nsub = (n + 32 * rounds - 1) / (32 * rounds);
+    const int64_t nb = (nsub + DS_NW - 1) / DS_NW;
+    const size_t smem = sizeof(int) * (size_t)(E + DS_NW * DS_MAXD);
+    int *base = hist + stride * D;
+    DsBatch lb;
+    lb.pair_stride = n;
+    lb.ws_stride = 2 * stride * D + 64;
+    lb.map_stride = E;
+    lb.off_stride = D + 1;
+    const bool extra = rd.part != nullptr;
+    {
+    KernelTimerScope ts("dispatch_scan", st);
+    launch_pdl(dispatch_scan_kernel, dim3((unsigned)(D + (extra ? rd.nrb : 0)), (unsigned)L), dim3(stride >= 128 * 16 ? 512 : 128), 0, st,
+               (const int *)hist, base, D, stride, lb, rd);
+    }
+    note_launch();
+    CAP_TRY(check_launch("dispatch_scan_kernel"));
+    FinalParams f0 = {};
+    const FinalParams &f = fin ? *fin : f0;
+    const int fin_block = fin ? (int)nb : -1;
+    const dim3 grid((unsigned)(nb + (fin ? 1 : 0)), (unsigned)L);
+    {
+    KernelTimerScope ts("dispatch_scatter", st);
+#define CAP_SCATTER(R)                                                                                              \
+    launch_pdl(dispatch_scatter_kernel<R>, grid, dim3(DS_THREADS), smem, st, idx, kept, n, E, D, expert_dev,          \
+               (const int *)base, reinterpret_cast<long long *>(offsets), sorted_pairs, pair_pos, stride, lb, rounds, \
+               fin_block, f, rd)
+    if (rounds <= 4) CAP_SCATTER(4);
+    else if (rounds <= 8) CAP_SCATTER(8);
+    else if (rounds <= 12) CAP_SCATTER(12);
+    else CAP_SCATTER(16);
+#undef CAP_SCATTER
+    }
+    note_launch();
+    return check_launch("dispatch_scatter_kernel");
 }
 
 // L layers in three launches (blockIdx.y = layer): idx / kept [L][T][k], expert_dev [L][E], sorted_pairs / pair_pos
@@ -243,11 +335,10 @@ int launch_dispatch_batched(const int32_t *idx, const uint8_t *kept, int32_t L, 
             return check_launch("memset offsets");
         return CAP_OK;
     }
-    const int64_t nsub = (n + DS_SUB - 1) / DS_SUB, stride = ds_stride(n);
-    const int64_t nb = (nsub + DS_NW - 1) / DS_NW, nbh = stride / DS_NW;
+    const int64_t stride = ds_stride(n);
+    const int64_t nbh = stride / DS_NW;
     const size_t smem = sizeof(int) * (size_t)(E + DS_NW * DS_MAXD);
     int *hist = reinterpret_cast<int *>((reinterpret_cast<uintptr_t>(ws) + 255) & ~(uintptr_t)255);
-    int *base = hist + stride * D;
     DsBatch lb;
     lb.pair_stride = n;
     lb.ws_stride = 2 * stride * D + 64;
@@ -260,20 +351,9 @@ int launch_dispatch_batched(const int32_t *idx, const uint8_t *kept, int32_t L, 
     }
     note_launch();
     CAP_TRY(check_launch("dispatch_hist_kernel"));
-    {
-    KernelTimerScope ts("dispatch_scan", st);
-    launch_pdl(dispatch_scan_kernel, dim3((unsigned)D, (unsigned)L), dim3(stride >= 128 * 16 ? 512 : 128), 0, st, hist, base,
-               D, stride, lb);
-    }
-    note_launch();
-    CAP_TRY(check_launch("dispatch_scan_kernel"));
-    {
-    KernelTimerScope ts("dispatch_scatter", st);
-    launch_pdl(dispatch_scatter_kernel, dim3((unsigned)nb, (unsigned)L), dim3(DS_THREADS), smem, st, idx, kept, n, E, D,
-               expert_dev, base, reinterpret_cast<long long *>(offsets), sorted_pairs, pair_pos, stride, lb);
-    }
-    note_launch();
-    return check_launch("dispatch_scatter_kernel");
+    DsReduce rd = {};
+    return launch_dispatch_tail(idx, kept, L, n, E, expert_dev, D, sorted_pairs, pair_pos, offsets, hist, stride,
+                                DS_SUB / 32, rd, nullptr, st);
 }
 
 int launch_dispatch(const int32_t *idx, const uint8_t *kept, int64_t T, int32_t k, int32_t E,

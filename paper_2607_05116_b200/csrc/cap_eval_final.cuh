@@ -24,7 +24,9 @@ FinalParams make_final_params(int32_t L, int32_t E, int32_t P, const int32_t *ex
 // One warp finishes (layer, candidate) o: lanes stride over the experts (coalesced map and count
 // reads), per-device sums in lp (shared memory, 64 entries of this warp), then over the devices.
 // Reads go to L2 (__ldcg): the sums may have been produced by other blocks of the same launch.
-__device__ __forceinline__ void eval_finalize_one(const FinalParams &f, int o, int lane, unsigned long long *lp)
+// lp_ready: lp[0..63] already holds the pairs per device (the caller counted them itself).
+__device__ __forceinline__ void eval_finalize_one(const FinalParams &f, int o, int lane, unsigned long long *lp,
+                                                  bool lp_ready = false)
 {
     const int layer = o / f.P;
     // every global load of this candidate goes out first (independent: one L2 round trip for all of them)
@@ -32,7 +34,9 @@ __device__ __forceinline__ void eval_finalize_one(const FinalParams &f, int o, i
     const long long r1 = lane + 32 < f.D ? (long long)__ldcg(f.recv + (size_t)o * f.D + lane + 32) : 0ll;
     const unsigned long long *a = f.acc + (size_t)o * ACC_N;
     const unsigned long long av = lane < ACC_N ? __ldcg(a + lane) : 0ull;
-    if (f.load_direct) {
+    if (lp_ready) {
+        __syncwarp();
+    } else if (f.load_direct) {
         lp[lane] = __ldcg(f.load_direct + (size_t)o * 64 + lane);
         lp[lane + 32] = __ldcg(f.load_direct + (size_t)o * 64 + lane + 32);
     } else {

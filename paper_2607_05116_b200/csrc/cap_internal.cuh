@@ -161,6 +161,30 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
                  const cap_eval_out *after, void *ws, cudaStream_t st);
 // S3 fast path (cap_eval_fast.cu): *used = false when the sizes do not fit it
 // (decodes and finishes the outputs itself: no launch_eval_finalize after it)
+// cap_prune_dispatch (S4 + S5 in three launches): the S4 kernel leaves, per block, PD_PART 32-bit partial sums
+// (ACC_N evaluation accumulators, then tokens received per device) and, per warp of 32 tokens, the kept pairs per
+// device in the histogram rows of S5; the S5 scan / scatter kernels carry one extra block each that adds the
+// partials up and writes the after-metrics.
+constexpr int PD_PART = ACC_N + 64;
+constexpr int PD_MAXRB = 64;
+struct DsReduce {
+    const uint32_t *part;            // [L][nblk][PD_PART] or NULL
+    unsigned long long *red;         // [L][nrb][PD_PART]: sums of nrb slices of the blocks (scan kernel -> scatter kernel)
+    unsigned long long *acc, *recv;  // [L][ACC_N], [L][D]: the totals (written and read by the finishing block)
+    int64_t nblk;
+    int32_t nrb, per_rb;             // reduce blocks per layer, S4 blocks per reduce block
+};
+struct FinalParams;
+int64_t dispatch_stride_subs(int64_t nsub);
+int launch_dispatch_tail(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t n, int32_t E,
+                         const int32_t *expert_dev, int32_t D, int32_t *sorted_pairs, int32_t *pair_pos,
+                         int64_t *offsets, int *hist, int64_t stride, int rounds, const DsReduce &rd,
+                         const FinalParams *fin, cudaStream_t st);
+size_t prune_dispatch_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D);
+int launch_prune_dispatch(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L, int64_t T,
+                          int32_t k, int32_t E, const int32_t *expert_dev, const cap_topology &topo, float p,
+                          uint8_t *kept, int64_t *near_margin, const cap_eval_out *after, int32_t *sorted_pairs,
+                          int32_t *pair_pos, int64_t *offsets, void *ws, cudaStream_t st);
 // deferred decode of the bit-sliced S3 path (cap_trace_fused_begin / _finish; cap_eval_fast.cu): while parking is on
 // for this host thread, the decode launch is stored instead of issued
 void ef_decode_park(bool on);

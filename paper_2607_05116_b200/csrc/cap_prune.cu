@@ -37,6 +37,11 @@ struct PruneParams {
     int64_t T;
     int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec, small;
     float p;
+    // cap_prune_dispatch: kept pairs per device of every warp's 32 tokens -> histogram rows of S5, the block's sums
+    // -> part (plain stores; no accumulator has to be zeroed, no ticket)
+    int *hist;                    // [L][...] rows of hist_stride sub-chunks, layers hist_layer apart; or NULL
+    int64_t hist_stride, hist_layer;
+    uint32_t *part;               // [L][gridDim.x][PD_PART]
 };
 
 constexpr int PR_THREADS = 128;
@@ -55,7 +60,8 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
     const int E = prm.E, D = prm.D, k = prm.k;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *s_dn = s_map + E;
-    const bool want_eval = prm.acc != nullptr;
+    const bool fusedm = prm.hist != nullptr;
+    const bool want_eval = prm.acc != nullptr || fusedm;
     pdl_launch_dependents();
     pdl_wait();
     // this thread's token (vector path): in flight while the maps are staged
@@ -162,7 +168,16 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             if (prm.tok_rnode) prm.tok_rnode[(int64_t)layer * T + t] = (uint8_t)a_rnode;
         }
     }
-    if (prm.near_margin) {
+    if (fusedm) {
+        const unsigned b = __ballot_sync(0xffffffffu, near != 0);
+        if (lane == 0 && b) atomicAdd(&s_acc[ACC_NEAR], (unsigned long long)__popc(b));
+        // this warp's 32 tokens are sub-chunk `sub` of S5
+        __syncwarp();
+        const int64_t sub = (int64_t)blockIdx.x * PR_WARPS + warp;
+        int *h = prm.hist + (int64_t)layer * prm.hist_layer;
+        if (lane < D) h[(int64_t)lane * prm.hist_stride + sub] = (int)(s_cnt[warp][lane] & 0xffffu);
+        if (lane + 32 < D) h[(int64_t)(lane + 32) * prm.hist_stride + sub] = (int)(s_cnt[warp][lane + 32] & 0xffffu);
+    } else if (prm.near_margin) {
         const unsigned b = __ballot_sync(0xffffffffu, near != 0);
         if (lane == 0 && b) atomicAdd(&prm.near_margin[(size_t)layer * prm.near_stride], (unsigned long long)__popc(b));
     }
@@ -183,6 +198,17 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             atomicAdd(&s_acc[ACC_RNODE], (unsigned long long)a_rnode);
         }
         __syncthreads();
+        if (fusedm) {
+            uint32_t *pp = prm.part + ((size_t)layer * gridDim.x + blockIdx.x) * PD_PART;
+            if (threadIdx.x < ACC_N) pp[threadIdx.x] = (uint32_t)s_acc[threadIdx.x];
+            if (threadIdx.x < 64) {
+                unsigned rc = 0;
+#pragma unroll
+                for (int w2 = 0; w2 < PR_WARPS; ++w2) rc += s_cnt[w2][threadIdx.x] >> 16;
+                pp[ACC_N + threadIdx.x] = rc;
+            }
+            return;
+        }
         if (threadIdx.x < ACC_N && s_acc[threadIdx.x])
             atomicAdd(&prm.acc[(size_t)layer * ACC_N + threadIdx.x], s_acc[threadIdx.x]);
         if (threadIdx.x < 64) {
@@ -225,6 +251,9 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
     PruneParams prm;
     prm.acc = prm.recv = prm.ldirect = nullptr;
     prm.tok_rdev = prm.tok_rnode = nullptr;
+    prm.hist = nullptr;
+    prm.hist_stride = prm.hist_layer = 0;
+    prm.part = nullptr;
     if (after) {
         CAP_TRY(eval_zero_ws(L, E, topo.D, 1, true, ws, st));
         EvalWs ew = eval_ws_carve(ws, L, E, topo.D, 1);
@@ -281,6 +310,98 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
                                     ws, st, nullptr);
     }
     return CAP_OK;
+}
+
+// ---- cap_prune_dispatch: S4 + S5 in three launches ----------------------------------------------------------
+// ws: [evaluation sums of P = 1 (eval_ws_carve)] [hist | base | device totals per layer] [per-block partials]
+static int64_t pd_stride(int64_t T) { return dispatch_stride_subs((T + 31) / 32); }
+
+size_t prune_dispatch_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D)
+{
+    const int64_t stride = pd_stride(T);
+    const size_t ll = (size_t)(L < 1 ? 1 : L);
+    return eval_ws_bytes(L, 0, E, k, D, 1) + 256 + ll * (size_t)(2 * stride * D + 64) * sizeof(int) + 256 +
+           ll * (size_t)(stride / PR_WARPS) * PD_PART * sizeof(uint32_t) + 256 +
+           ll * (size_t)PD_MAXRB * PD_PART * sizeof(unsigned long long);
+}
+
+int launch_prune_dispatch(const int32_t *idx, const float *w, const int32_t *token_src, int32_t L, int64_t T,
+                          int32_t k, int32_t E, const int32_t *expert_dev, const cap_topology &topo, float p,
+                          uint8_t *kept, int64_t *near_margin, const cap_eval_out *after, int32_t *sorted_pairs,
+                          int32_t *pair_pos, int64_t *offsets, void *ws, cudaStream_t st)
+{
+    if (L == 0) return CAP_OK;
+    const int D = topo.D;
+    if (T == 0) {
+        // nothing to prune or to lay out: the stand-alone calls handle the empty outputs
+        CAP_TRY(launch_prune(idx, w, token_src, L, T, k, E, expert_dev, topo, p, kept, near_margin, after, ws, st));
+        return launch_dispatch_batched(idx, kept, L, T, k, E, expert_dev, D, sorted_pairs, pair_pos, offsets, ws, st);
+    }
+    const int64_t stride = pd_stride(T);
+    const int64_t nblk = stride / PR_WARPS;
+    EvalWs ew = eval_ws_carve(ws, L, E, D, 1);
+    uintptr_t a = reinterpret_cast<uintptr_t>(ws) + eval_ws_bytes(L, 0, E, k, D, 1);
+    a = (a + 255) & ~(uintptr_t)255;
+    int *hist = reinterpret_cast<int *>(a);
+    a += (size_t)L * (size_t)(2 * stride * D + 64) * sizeof(int);
+    a = (a + 255) & ~(uintptr_t)255;
+    uint32_t *part = reinterpret_cast<uint32_t *>(a);
+    a += (size_t)L * (size_t)nblk * PD_PART * sizeof(uint32_t);
+    a = (a + 255) & ~(uintptr_t)255;
+    unsigned long long *red = reinterpret_cast<unsigned long long *>(a);
+
+    PruneParams prm;
+    prm.acc = prm.recv = prm.ldirect = nullptr;
+    prm.tok_rdev = after ? after->tok_remote_dev : nullptr;
+    prm.tok_rnode = after ? after->tok_remote_node : nullptr;
+    prm.fin = FinalParams{};
+    prm.idx = idx;
+    prm.w = w;
+    prm.token_src = token_src;
+    prm.expert_dev = expert_dev;
+    prm.dev_node = topo.dev_node;
+    prm.kept = kept;
+    prm.near_margin = nullptr;
+    prm.near_stride = 0;
+    prm.T = T;
+    prm.k = k;
+    prm.E = E;
+    prm.D = D;
+    prm.N = topo.N;
+    prm.cost_local = topo.cost_local;
+    prm.cost_intra = topo.cost_intra;
+    prm.cost_inter = topo.cost_inter;
+    prm.p = p;
+    prm.small = (unsigned long long)T * (unsigned long long)D < (1ull << 32);
+    prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
+              (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
+    prm.hist = hist;
+    prm.hist_stride = stride;
+    prm.hist_layer = 2 * stride * D + 64;
+    prm.part = part;
+    const dim3 grid((unsigned)nblk, (unsigned)L);       // padding blocks (no tokens) zero their hist entries
+    const size_t smem = sizeof(int) * ((size_t)E + 64);
+    {
+        KernelTimerScope ts("prune", st);
+        if (k <= 4) launch_pdl(prune_kernel<4>, grid, dim3(PR_THREADS), smem, st, prm);
+        else if (k <= 8) launch_pdl(prune_kernel<8>, grid, dim3(PR_THREADS), smem, st, prm);
+        else if (k <= 12) launch_pdl(prune_kernel<12>, grid, dim3(PR_THREADS), smem, st, prm);
+        else launch_pdl(prune_kernel<16>, grid, dim3(PR_THREADS), smem, st, prm);
+    }
+    note_launch();
+    CAP_TRY(check_launch("prune_kernel"));
+    DsReduce rd;
+    rd.part = part;
+    rd.red = red;
+    rd.per_rb = (int32_t)((nblk + PD_MAXRB - 1) / PD_MAXRB < 64 ? 64 : (nblk + PD_MAXRB - 1) / PD_MAXRB);
+    rd.nrb = (int32_t)((nblk + rd.per_rb - 1) / rd.per_rb);
+    rd.acc = ew.acc;
+    rd.recv = ew.recv;
+    rd.nblk = nblk;
+    cap_eval_out none = {};
+    FinalParams fin = make_final_params(L, E, 1, expert_dev, topo, nullptr, after ? *after : none, ws, near_margin);
+    return launch_dispatch_tail(idx, kept, L, T * k, E, expert_dev, D, sorted_pairs, pair_pos, offsets, hist, stride, k,
+                                rd, &fin, st);
 }
 
 }  // namespace cap

@@ -204,6 +204,65 @@ def test_prune_edge_cases(k):
                 assert_eval_equal(aft, ref, False, f"after {costs} {p} ")
 
 
+@pytest.mark.parametrize("L,T,k,E,D,N", [(1, 1, 1, 4, 2, 1), (2, 33, 3, 8, 4, 2), (1, 4099, 8, 128, 16, 2),
+                                         (3, 1500, 8, 128, 8, 2), (1, 9000, 10, 512, 64, 8), (2, 700, 16, 64, 5, 5),
+                                         (1, 70000, 4, 64, 33, 3)])
+def test_prune_dispatch_equals_prune_then_dispatch(L, T, k, E, D, N):
+    """cap_prune_dispatch (S4 + S5 in three launches: the pruning kernel leaves the sort's histogram, the scan and
+    scatter launches finish the after-metrics) against the oracle's prune followed by its dispatch layout, per
+    layer: kept masks, near-margin counts, after-metrics, sorted pairs, inverse positions, offsets."""
+    rng = np.random.default_rng(L * 1000 + T + k)
+    idx = _trace(rng, L, T, E, k)
+    w = rng.random((L, T, k)).astype(np.float32) + np.float32(0.02)
+    w = -np.sort(-w, axis=-1)
+    w = (w / w.sum(-1, keepdims=True, dtype=np.float32)).astype(np.float32)
+    w[0, : min(T, 40)] = np.float32(1.0 / k)                 # exact ratio ties
+    pi = np.stack([rng.permutation(E) % D for _ in range(L)]).astype(np.int32)
+    dn = np.sort(rng.integers(0, N, D)).astype(np.int32)
+    dn[0], dn[-1] = 0, N - 1
+    src = rng.integers(0, D, (L, T)).astype(np.int32)
+    topo = cap.topology(dev(dn), 0, 1, 4, bytes_per_token=64, N=N)
+    for p, s, want_after in ((0.1, None, True), (0.4, src, True), (0.0, None, True), (0.25, src, False)):
+        kept_r, near_r = O.prune(idx, w, pi, dn, p, token_src=s, cost_local=0, cost_intra=1, cost_inter=4)
+        n0 = cap.launch_count()
+        kept_d, near_d, aft, sp_d, off_d, pos_d = cap.prune_dispatch(dev(idx), dev(w), dev(s), dev(pi), topo, p,
+                                                                     want_after=want_after)
+        torch.cuda.synchronize()
+        assert cap.launch_count() - n0 == 3
+        tag = f"p={p} src={s is not None} "
+        assert np.array_equal(host(kept_d), kept_r), tag + "kept"
+        assert np.array_equal(host(near_d), near_r), tag + "near"
+        if want_after:
+            ref = O.eval_placements(idx, pi[:, None], dn, kept=kept_r, token_src=s, cost_local=0, cost_intra=1,
+                                    cost_inter=4, bytes_per_token=64)
+            assert_eval_equal(aft, ref, False, tag + "after ")
+        for l in range(L):
+            sp_r, off_r, pos_r = O.dispatch_layout(idx[l], pi[l], D, kept=kept_r[l])
+            n = int(off_r[-1])
+            assert np.array_equal(host(off_d[l]), off_r), tag + f"offsets layer {l}"
+            assert np.array_equal(host(sp_d[l])[:n], sp_r), tag + f"sorted_pairs layer {l}"
+            assert np.array_equal(host(pos_d[l]), pos_r), tag + f"pair_pos layer {l}"
+
+
+def test_prune_dispatch_empty_and_workspace():
+    E, k, D = 64, 4, 8
+    dn = dev((np.arange(D) // 4).astype(np.int32))
+    topo = cap.topology(dn, 0, 1, 4, bytes_per_token=8, N=2)
+    pi = dev((np.arange(E) % D).astype(np.int32)[None])
+    idx = torch.zeros((1, 0, k), dtype=torch.int32, device="cuda")
+    w = torch.zeros((1, 0, k), dtype=torch.float32, device="cuda")
+    kept, near, aft, sp, off, pos = cap.prune_dispatch(idx, w, None, pi, topo, 0.2)
+    torch.cuda.synchronize()
+    assert host(off).tolist() == [[0] * (D + 1)] and host(near).tolist() == [0]
+    assert int(aft.dev_visits.sum()) == 0
+    idx = torch.zeros((1, 100, k), dtype=torch.int32, device="cuda")
+    w = torch.full((1, 100, k), 0.25, dtype=torch.float32, device="cuda")
+    with pytest.raises(cap.CapError, match="EWORKSPACE"):
+        cap.prune_dispatch(idx, w, None, pi, topo, 0.2, ws=torch.empty(64, dtype=torch.uint8, device="cuda"))
+    with pytest.raises(cap.CapError, match="EINVAL"):
+        cap.prune_dispatch(idx, w, None, pi, topo, 1.0)
+
+
 @pytest.mark.parametrize("T,k,E,D", [(1, 1, 4, 2), (5, 3, 8, 4), (2048, 1, 16, 3), (4097, 8, 128, 16), (30000, 10, 512, 64)])
 def test_dispatch_edge_cases(T, k, E, D):
     rng = np.random.default_rng(T + D)
