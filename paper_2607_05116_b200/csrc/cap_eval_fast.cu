@@ -19,7 +19,7 @@ static int ceil_log2(long long v)
 }
 
 bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P,
-                    int target_ctas, size_t smem_budget, EvalFastGeom *g, bool explicit_src)
+                    int target_ctas, size_t smem_budget, EvalFastGeom *g, bool explicit_src, int rs_limit)
 {
     if (L < 1 || T < 1 || P < 1 || D < 1 || D > 64 || N < 1 || N > 8 || k < 1 || k > 16) return false;
     g->WD = D <= 8 ? 8 : D <= 16 ? 16 : D <= 32 ? 32 : 64;
@@ -35,7 +35,7 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
         const int R = dcol + ncol;
         const int RS = R | 1;
         int S = 1;
-        while (S < 64 && R * (S * 2) <= 320) S *= 2;
+        while (S < 64 && R * (S * 2) <= rs_limit) S *= 2;
         const size_t tbl = (size_t)(E + 1) * RS * 16;
         const size_t offs = (size_t)2 * EF_PASSES * S * g->KP * 4;
         const size_t xch = (size_t)(S / 2) * R * EF_NPL * 16;
@@ -122,13 +122,13 @@ size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D,
     size_t best = 0;
     for (int N = 2; N <= 8; N *= 2) {
         EvalFastGeom g;
-        if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), ef_budget(), &g)) continue;
+        if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), ef_budget(), &g, false, EF_RS_ALONE)) continue;
         const size_t b = g.rec_slots * 4 + 256 + g.rec_words * 4 + 256 + g.table_words * 4 + 256;
         if (b > best) best = b;
     }
     for (int N = 2; N <= 8; N *= 2) {      // explicit token_src: more record slots, the permutation and the sort
         EvalFastGeom g;
-        if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), ef_budget(), &g, true)) continue;
+        if (!eval_fast_geom(L, T, k, E, D, N, P, sm_count(), ef_budget(), &g, true, EF_RS_ALONE)) continue;
         const size_t b = g.rec_slots * 4 + 256 + g.rec_words * 4 + 256 + g.table_words * 4 + 256 + (size_t)L * T * 4 + 256 +
                          (size_t)L * (D + 1) * 8 + 256 + (size_t)L * 64 * 4 + 256 + dispatch_ws_bytes_batched(L, T, 1, D) + 256;
         if (b > best) best = b;
@@ -826,7 +826,8 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
 {
     *used = false;
     EvalFastGeom g;
-    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g, token_src != nullptr)) return CAP_OK;
+    if (!eval_fast_geom(L, T, k, E, topo.D, topo.N, P, sm_count(), ef_budget(), &g, token_src != nullptr, EF_RS_ALONE))
+        return CAP_OK;
     EvalFastWs fw = eval_fast_ws_carve(ws, L, E, topo.D, P, g, T);
     if (token_src) {
         // explicit sources (reading R5): group the token ids by source device with the stable counting sort of S5

@@ -22,7 +22,9 @@ constexpr int EF_RECW = 16;     // record layout [word][EF_RECW planes]: a word'
 constexpr int EF_PASSES = 8;    // tokens per thread per block of the CSA tree
 constexpr int EF_MAXBLK = 31;   // blocks per run: 248 inputs per thread < 2^EF_BT
 constexpr int EF_PRE = 16;      // prefetched index entries per thread
-constexpr int EF_MAXTHREADS = 352;
+constexpr int EF_MAXTHREADS = 384;
+constexpr int EF_RS_FUSED = 320;        // (column, sub-slot) threads of the scoring warps inside the fused kernel
+constexpr int EF_RS_ALONE = 384;        // of the stand-alone scoring kernel: a whole SM's registers at 168 per thread
 
 struct EvalFastGeom {
     int WD, WN;          // field widths (bits) of the device / node codes
@@ -46,7 +48,8 @@ struct EvalFastGeom {
 // false when the fast path does not apply to these sizes (the generic kernel is used instead)
 // explicit_src: the tokens come grouped by an arbitrary token_src (any number of source boundaries per block)
 bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t N, int32_t P,
-                    int target_ctas, size_t smem_budget, EvalFastGeom *g, bool explicit_src = false);
+                    int target_ctas, size_t smem_budget, EvalFastGeom *g, bool explicit_src = false,
+                    int rs_limit = EF_RS_FUSED);
 size_t eval_fast_ws_bytes(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32_t P);
 
 struct EvalFastWs {
