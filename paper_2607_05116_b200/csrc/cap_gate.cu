@@ -239,6 +239,8 @@ int launch_gate_topk(const float *logits, const float *bias, int32_t L, int64_t 
     if (fast) return CAP_OK;
     CAP_TRY(launch_gate_sig(logits, bias, L, T, cfg, idx, w, st, &fast));
     if (fast) return CAP_OK;
+    CAP_TRY(launch_gate_wide(logits, bias, L, T, cfg, idx, w, st, &fast));
+    if (fast) return CAP_OK;
     GateParams prm;
     prm.logits = logits;
     prm.bias = bias;

@@ -122,6 +122,9 @@ int launch_gate_fast(const float *logits, const float *bias, int32_t L, int64_t 
 // S1 fast path for sigmoid (+ bias, + groups of 32) scoring (cap_gate_sig.cu): *used = false when it does not apply
 int launch_gate_sig(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
                     int32_t *idx, float *w, cudaStream_t st, bool *used);
+// S1 fast path for E = 512, k <= 10, softmax + renormalisation (cap_gate_wide.cu): *used = false when it does not apply
+int launch_gate_wide(const float *logits, const float *bias, int32_t L, int64_t T, const cap_gate_cfg &cfg,
+                     int32_t *idx, float *w, cudaStream_t st, bool *used);
 // S2 fast path (cap_coact_mma.cu): tcgen05 int8 A^T A; outputs must be zeroed by the caller
 int launch_coact_mma(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k, int32_t E,
                      int64_t *counts, int32_t *coact, cudaStream_t st, bool *used);
