@@ -297,7 +297,7 @@ int launch_dispatch_tail(const int32_t *idx, const uint8_t *kept, int32_t L, int
     const bool extra = rd.part != nullptr;
     {
     KernelTimerScope ts("dispatch_scan", st);
-    launch_pdl(dispatch_scan_kernel, dim3((unsigned)(D + (extra ? rd.nrb : 0)), (unsigned)L), dim3(stride >= 128 * 16 ? 512 : 128), 0, st,
+    launch_pdl_edge(dispatch_scan_kernel, dim3((unsigned)(D + (extra ? rd.nrb : 0)), (unsigned)L), dim3(stride >= 128 * 16 ? 512 : 128), 0, st,
                (const int *)hist, base, D, stride, lb, rd);
     }
     note_launch();

@@ -1,6 +1,7 @@
 // Internal declarations shared by the CUDA translation units of libcap_b200.so.
 // Nothing here is shared with oracle/ (the CPU oracle is an independent restatement).
 #pragma once
+#include <cstdlib>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
