@@ -34,7 +34,18 @@ coact_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, 
         const int i = idx[base + a];
         if ((unsigned)i >= (unsigned)E) continue;    // out-of-range ids: undefined result, memory-safe (cap.h)
         atomicAdd(&cnt[i], 1);
-        int *rowp = use_smem ? hist + (size_t)i * E : coact + (size_t)i * E;
+        if (!use_smem) {
+            // straight into global memory: only the pairs with a larger partner id, i.e. the upper triangle (half the
+            // reductions); coact_mirror_kernel copies it below the diagonal and writes the diagonal from the counts
+            // (a token's expert ids are distinct: include/cap.h)
+            for (int b = 0; b < k; ++b) {
+                if (b == a || (kept && !kept[base + b])) continue;
+                const int j = idx[base + b];
+                if ((unsigned)j < (unsigned)E && j > i) atomicAdd(&coact[(size_t)i * E + j], 1);
+            }
+            continue;
+        }
+        int *rowp = hist + (size_t)i * E;
         for (int b = 0; b < k; ++b) {
             if (b != a && kept && !kept[base + b]) continue;
             const int j = idx[base + b];
@@ -51,6 +62,34 @@ coact_kernel(const int32_t *__restrict__ idx, const uint8_t *__restrict__ kept, 
     for (int i = threadIdx.x; i < E; i += blockDim.x) {
         int v = cnt[i];
         if (v) atomicAdd(&counts[i], (unsigned long long)v);
+    }
+}
+
+// the lower triangle and the diagonal of every layer's matrix after the upper-triangle pass of coact_kernel
+__global__ void __launch_bounds__(256)
+coact_mirror_kernel(const unsigned long long *__restrict__ counts, int *__restrict__ coact, int E)
+{
+    coact += (size_t)blockIdx.y * E * E;
+    counts += (size_t)blockIdx.y * E;
+    __shared__ int tile[32][33];
+    // 32 x 32 tiles of the upper triangle (tile row <= tile column), transposed through shared memory
+    const int nt = (E + 31) / 32;
+    int tr = 0, rem = blockIdx.x;
+    while (rem >= nt - tr) {
+        rem -= nt - tr;
+        ++tr;
+    }
+    const int tc = tr + rem;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int r = ty; r < 32; r += 8) {
+        const int i = tr * 32 + r, j = tc * 32 + tx;
+        tile[r][tx] = (i < E && j < E && j > i) ? coact[(size_t)i * E + j] : 0;
+    }
+    __syncthreads();
+    for (int r = ty; r < 32; r += 8) {
+        const int i = tc * 32 + r, j = tr * 32 + tx;          // element (i, j) below the diagonal <- (j, i)
+        if (i < E && j < E && j < i) coact[(size_t)i * E + j] = tile[tx][r];
+        if (i < E && tr == tc && j == i) coact[(size_t)i * E + i] = (int)counts[i];
     }
 }
 
@@ -78,14 +117,19 @@ int launch_coactivation(const int32_t *idx, const uint8_t *kept, int32_t L, int6
     if (tpb < 256) tpb = 256;
     const int64_t nblk = (T + tpb - 1) / tpb;
     dim3 grid((unsigned)nblk, (unsigned)L);
-    {
-        KernelTimerScope ts("coact", st);
-        coact_kernel<<<grid, 256, smem, st>>>(idx, kept, T, k, E,
-                                              reinterpret_cast<unsigned long long *>(counts), coact, tpb,
-                                              use_smem);
-    }
+    KernelTimerScope ts("coact", st);
+    coact_kernel<<<grid, 256, smem, st>>>(idx, kept, T, k, E, reinterpret_cast<unsigned long long *>(counts), coact, tpb,
+                                          use_smem);
     note_launch();
-    return check_launch("coact_kernel");
+    CAP_TRY(check_launch("coact_kernel"));
+    if (!use_smem) {
+        const int nt = (E + 31) / 32;
+        coact_mirror_kernel<<<dim3((unsigned)(nt * (nt + 1) / 2), (unsigned)L), 256, 0, st>>>(
+            reinterpret_cast<const unsigned long long *>(counts), coact, E);
+        note_launch();
+        return check_launch("coact_mirror_kernel");
+    }
+    return CAP_OK;
 }
 
 }  // namespace cap
