@@ -485,23 +485,28 @@ struct DecodeParams {
     } while (0)
 
 constexpr int DEC_WARPS = 4;
-template <int NA>
+// WPW = warps per table word.  4: one word per block, the four warps split its records and exchange their sums
+// through shared memory (config 3: ~290 records per word).  1: every warp decodes a word of its own -- no block
+// barrier after the prologue, four words per block (configs 2, 4, 5: 40-90 records per word, where the fixed
+// part of a block, not the records, was the cost: 130 us on config 4, 60 us on config 5 with one word per block).
+template <int NA, int WPW>
 __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParams q)
 {
+    constexpr int NG = DEC_WARPS / WPW;                  // words per block
     __shared__ unsigned long long nodeset[8];
     __shared__ unsigned char s_dn[64];
-    __shared__ uint32_t s_part[DEC_WARPS - 1][3][NA];
-    __shared__ unsigned long long s_lp[4][64];          // load_pairs of the block's candidates (<= 4 per device word)
+    __shared__ uint32_t s_part[WPW > 1 ? WPW - 1 : 1][3][NA];
+    __shared__ unsigned long long s_lp[NG][4][64];      // load_pairs of a word's candidates (<= 4 per device word)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int w0 = blockIdx.x, pc = blockIdx.y, layer = blockIdx.z;
+    const int grp = warp / WPW, wl = warp % WPW, gt = wl * 32 + lane;
+    const int w0 = blockIdx.x * NG + grp, pc = blockIdx.y, layer = blockIdx.z;
     const bool devword = w0 < q.DW;
     const int fw = devword ? q.WD : q.WN;                 // field width of this word
     const int nwords = (devword && q.WD == 64) ? 2 : 1;   // both halves of a 64-bit device field
     pdl_launch_dependents();
     pdl_wait();
-    if (devword && q.WD == 64 && (w0 & 1)) return;        // done by the block of the even word
     if (threadIdx.x < 64) s_dn[threadIdx.x] = (int)threadIdx.x < q.D ? (unsigned char)q.dev_node[threadIdx.x] : 0;
-    for (int i = threadIdx.x; i < 4 * 64; i += blockDim.x) (&s_lp[0][0])[i] = 0ull;
+    for (int i = threadIdx.x; i < NG * 4 * 64; i += blockDim.x) (&s_lp[0][0][0])[i] = 0ull;
     __syncthreads();
     if (threadIdx.x < 8) {
         const int n = threadIdx.x;              // from the shared copy: one round of global loads, not D
@@ -510,23 +515,28 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
             if (s_dn[d] == n) m |= 1ull << d;
         nodeset[n] = m;
     }
-    // candidates of this block: device word -> 32 / WD of them (one for WD >= 32); their load_pairs
+    // words past the table, and the odd half of a 64-bit device field (done with the even word): nothing to do.
+    // WPW = 4: uniform over the block.  WPW = 1: per warp -- no block barrier may follow the next one.
+    const bool idle = w0 >= q.W || (devword && q.WD == 64 && (w0 & 1));
+    if (WPW > 1 && idle) return;
+    // candidates of this word: device word -> 32 / WD of them (one for WD >= 32); their load_pairs
     const int ncand = devword ? (q.WD >= 32 ? 1 : 32 / q.WD) : 0;
     const int pl0 = devword ? (q.WD == 64 ? (w0 >> 1) : w0 * 32 / q.WD) : 0;
-    if (devword && (q.out.load_pairs || q.out.imbalance)) {
+    if (!idle && devword && (q.out.load_pairs || q.out.imbalance)) {
         const long long *cnt = q.counts + (size_t)layer * q.E;
         for (int c = 0; c < ncand; ++c) {
             const int p = pc * q.Pc + pl0 + c;
             if (pl0 + c >= q.Pc || p >= q.P) continue;
             const int32_t *pi = q.expert_dev + ((size_t)layer * q.P + p) * q.E;
-            for (int e = threadIdx.x; e < q.E; e += blockDim.x) {
+            for (int e = gt; e < q.E; e += 32 * WPW) {
                 const int d = pi[e];
                 const long long v = __ldcg(cnt + e);
-                if ((unsigned)d < (unsigned)q.D && v) atomicAdd(&s_lp[c][d], (unsigned long long)v);
+                if ((unsigned)d < (unsigned)q.D && v) atomicAdd(&s_lp[grp][c][d], (unsigned long long)v);
             }
         }
     }
-    __syncthreads();
+    __syncthreads();                                      // the last block barrier of the WPW = 1 variant
+    if (idle) return;
     // running per-candidate results over the words of this block (meaningful on the field's leader lane)
     unsigned long long a_gt = 0ull, a_gl = 0ull, a_gs = 0ull;
     long long mx = 0, sm = 0, mxr = 0, smr = 0;
@@ -537,17 +547,17 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
 #pragma unroll
         for (int p = 0; p < NA; ++p) tot[p] = loc[p] = sam[p] = 0u;
         constexpr int DEC_SL = 2;     // record slots a thread has in flight
-        for (int s0 = threadIdx.x; s0 < q.nslots; s0 += 32 * DEC_WARPS * DEC_SL) {
+        for (int s0 = gt; s0 < q.nslots; s0 += 32 * WPW * DEC_SL) {
             int srcs[DEC_SL];
 #pragma unroll
             for (int j = 0; j < DEC_SL; ++j) {
-                const int s = s0 + j * 32 * DEC_WARPS;
+                const int s = s0 + j * 32 * WPW;
                 srcs[j] = s < q.nslots ? q.rec_src[sbase + s] : -1;
             }
             uint32_t av[DEC_SL][EF_NPL];
 #pragma unroll
             for (int j = 0; j < DEC_SL; ++j) {
-                const int s = s0 + j * 32 * DEC_WARPS;
+                const int s = s0 + j * 32 * WPW;
                 // one 64-byte run per (slot, word); not conditional on srcs[j]: the loads go out together with the
                 // header loads (unused slots hold stale planes, skipped below)
                 const uint4 *pp = reinterpret_cast<const uint4 *>(q.rec_planes + ((sbase + s) * (size_t)q.W + w) * EF_RECW);
@@ -588,18 +598,20 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
             CAP_DEC_BFLY(loc, off);
             CAP_DEC_BFLY(sam, off);
         }
-        // every lane of a warp now holds the warp's sums; warps 1.. hand theirs to warp 0
-        __syncthreads();                 // s_part of the previous word has been read
-        if (warp > 0 && lane < 3) {
+        // every lane of a warp now holds the warp's sums; with several warps per word, warps 1.. hand theirs to warp 0
+        if (WPW > 1) {
+            __syncthreads();                 // s_part of the previous word has been read
+            if (wl > 0 && lane < 3) {
 #pragma unroll
-            for (int p = 0; p < NA; ++p) {
-                const uint32_t v = lane == 0 ? tot[p] : lane == 1 ? loc[p] : sam[p];
-                s_part[warp - 1][lane][p] = v;
+                for (int p = 0; p < NA; ++p) {
+                    const uint32_t v = lane == 0 ? tot[p] : lane == 1 ? loc[p] : sam[p];
+                    s_part[wl - 1][lane][p] = v;
+                }
             }
+            __syncthreads();
         }
-        __syncthreads();
-        if (warp == 0) {
-            for (int o = 0; o < DEC_WARPS - 1; ++o) {
+        if (wl == 0) {
+            for (int o = 0; o < WPW - 1; ++o) {
                 uint32_t a[NA];
 #pragma unroll
                 for (int p = 0; p < NA; ++p) a[p] = s_part[o][0][p];
@@ -625,12 +637,12 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
             const bool pvalid = pl < q.Pc && p < q.P;
             const size_t o = (size_t)layer * q.P + p;
             const int gw = fw < 32 ? fw : 32;
-            unsigned long long gt = vt, gl = vl, gs = vs;
+            unsigned long long gt2 = vt, gl = vl, gs = vs;
             long long l = 0, r = 0;
             if (devword) {
                 const int c = pl - pl0;
                 if (pvalid && f < q.D) {
-                    l = (long long)s_lp[c & 3][f];
+                    l = (long long)s_lp[grp][c & 3][f];
                     r = (long long)vt;
                     if (q.out.load_pairs) q.out.load_pairs[o * q.D + f] = l;
                     if (q.out.recv_tokens) q.out.recv_tokens[o * q.D + f] = r;
@@ -638,7 +650,7 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
             }
             long long wmx = l, wsm = l, wmxr = r, wsmr = r;
             for (int off = 1; off < gw; off <<= 1) {
-                gt += __shfl_xor_sync(0xffffffffu, gt, off);
+                gt2 += __shfl_xor_sync(0xffffffffu, gt2, off);
                 gl += __shfl_xor_sync(0xffffffffu, gl, off);
                 gs += __shfl_xor_sync(0xffffffffu, gs, off);
                 wmx = max(wmx, __shfl_xor_sync(0xffffffffu, wmx, off));
@@ -646,7 +658,7 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
                 wsm += __shfl_xor_sync(0xffffffffu, wsm, off);
                 wsmr += __shfl_xor_sync(0xffffffffu, wsmr, off);
             }
-            a_gt += gt;
+            a_gt += gt2;
             a_gl += gl;
             a_gs += gs;
             mx = max(mx, wmx);
@@ -731,12 +743,23 @@ static int decode_launch(const DecodeParams &dq, dim3 dgrid, cudaStream_t st)
     const int na = dq.na;
     {
         KernelTimerScope ts("eval_decode", st);
-        if (na <= 12) launch_pdl(eval_decode_kernel<12>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 16) launch_pdl(eval_decode_kernel<16>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 20) launch_pdl(eval_decode_kernel<20>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 24) launch_pdl(eval_decode_kernel<24>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else if (na <= 28) launch_pdl(eval_decode_kernel<28>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
-        else launch_pdl(eval_decode_kernel<32>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        if (dq.nslots <= 128) {
+            // few records per word: a warp per word, four words per block
+            const dim3 g1((dgrid.x + DEC_WARPS - 1) / DEC_WARPS, dgrid.y, dgrid.z);
+            if (na <= 12) launch_pdl(eval_decode_kernel<12, 1>, g1, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 16) launch_pdl(eval_decode_kernel<16, 1>, g1, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 20) launch_pdl(eval_decode_kernel<20, 1>, g1, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 24) launch_pdl(eval_decode_kernel<24, 1>, g1, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 28) launch_pdl(eval_decode_kernel<28, 1>, g1, dim3(32 * DEC_WARPS), 0, st, dq);
+            else launch_pdl(eval_decode_kernel<32, 1>, g1, dim3(32 * DEC_WARPS), 0, st, dq);
+        } else {
+            if (na <= 12) launch_pdl(eval_decode_kernel<12, DEC_WARPS>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 16) launch_pdl(eval_decode_kernel<16, DEC_WARPS>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 20) launch_pdl(eval_decode_kernel<20, DEC_WARPS>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 24) launch_pdl(eval_decode_kernel<24, DEC_WARPS>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+            else if (na <= 28) launch_pdl(eval_decode_kernel<28, DEC_WARPS>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+            else launch_pdl(eval_decode_kernel<32, DEC_WARPS>, dgrid, dim3(32 * DEC_WARPS), 0, st, dq);
+        }
     }
     note_launch();
     return check_launch("eval_decode_kernel");
