@@ -2,7 +2,7 @@
 
 One "step" = one pass of every stage of SURVEY.md section 8(a) over one batch of synthetic
 router logits: cap_trace_fused (S1 gate top-k + S2 counts/co-activation + S3 scoring of P
-candidate placements) -> cap_prune under the chosen placement (S4) -> cap_dispatch_layout (S5).
+candidate placements) -> cap_prune_dispatch under the chosen placement (S4 + S5, all layers, three launches).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--config target] [--T tokens] [--impl cap|reference]
 
@@ -212,7 +212,8 @@ def config_dict(cfg, extra=None):
                      f"D={cfg.D} over N={cfg.N} nodes (cost 0/1/{cfg.cost_inter}) P={cfg.P} "
                      f"tau={cfg.taus[-1]} {'sigmoid+bias group-limited' if cfg.scoring else 'softmax'} renorm",
          "stages": "S1 gate top-k + S2 counts/co-activation + S3 P-candidate scoring (cap_trace_fused) "
-                   "-> S4 cap_prune -> S5 cap_dispatch_layout (all layers in one batched call)",
+                   "-> S4 + S5 cap_prune_dispatch (all layers, three launches); the last launch of S3 (decode) runs on a side "
+                   "stream beside S4 / S5 (cap_trace_fused_begin / _finish)",
          "tokens_per_step_per_gpu": cfg.L * cfg.T}
     if extra:
         d.update(extra)
