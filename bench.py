@@ -460,6 +460,14 @@ def run_cap(args, cfg, W):
     us_place = time_us(lambda: cap.coact_placement(pipe.fb.counts, pipe.fb.coact, D, cfg.N, ws=ws_pl))
     maps0 = d_sets[0][2]
     us_obj = time_us(lambda: cap.pairwise_objective(pipe.fb.counts, pipe.fb.coact, maps0, pipe.topo))
+    # the paper's order for re-placement: statistics of the PRUNED trace, then Algorithm 1
+    cnt_k = torch.empty_like(pipe.fb.counts)
+    co_k = torch.empty_like(pipe.fb.coact)
+
+    def pruned_stats_then_place():
+        cap.coactivation(pipe.fb.idx, pipe.kept, E, counts=cnt_k, coact=co_k)
+        cap.coact_placement(cnt_k, co_k, D, cfg.N, ws=ws_pl)
+    us_pruned_place = time_us(pruned_stats_then_place)
     ws_rows = cap.workspace(cap.CALL_DISPATCH_ROWS, 1, T, E, k, D, 0, device=dev)
     pi0 = maps0[0, 0].contiguous()
     us_rows = time_us(lambda: cap.dispatch_rows(pipe.fb.idx[0], pipe.kept[0], pi0, D, ws=ws_rows))
@@ -549,6 +557,10 @@ def run_cap(args, cfg, W):
             "us_per_call": us_place, "layers": L, "greedy_steps_per_layer": (E - D) + (D - cfg.N),
             "what": "cap_coact_placement (P:L106-144, L148, L162-164) on the step's counts / coact; latency-bound "
                     "sequential greedy, one CTA per layer; not part of `value`"},
+            "pruned_stats_then_placement": {
+                "us_per_call": us_pruned_place,
+                "what": "cap_coactivation with the step's kept mask (statistics of the pruned trace, P:L224) followed by "
+                        "cap_coact_placement on them: the paper's order for re-placement after pruning"},
             "pairwise_objective": {"us_per_call": us_obj, "candidates": P, "what": "cap_pairwise_objective (Eq. 2-3) "
                                    "on the step's counts / coact and its P candidate maps"},
             "dispatch_rows": {"us_per_call": us_rows, "what": "cap_dispatch_rows (P:L58, Fig. 2) for layer 0 under "

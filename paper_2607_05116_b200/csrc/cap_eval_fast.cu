@@ -250,17 +250,21 @@ __device__ __forceinline__ void ef_add_planes(uint4 (&a)[EF_NPL], const uint4 *b
     }
 }
 
-template <int KP>
+// KU <= KP: slots that can hold an expert (k rounded up to even); the offsets of slots KU.. point at the zero
+// row and are not loaded (k = 10 in a KP = 12 kernel: 10 row loads per token instead of 12)
+template <int KP, int KU>
 __device__ __forceinline__ uint4 ef_token_mask(const unsigned char *tblc, const uint32_t *op)
 {
     uint4 m = make_uint4(0u, 0u, 0u, 0u);
+    const uint4 z = make_uint4(0u, 0u, 0u, 0u);
 #pragma unroll
     for (int q = 0; q < KP / 4; ++q) {
+        if (4 * q >= KU) break;
         const uint4 o = *reinterpret_cast<const uint4 *>(op + 4 * q);
         const uint4 v0 = *reinterpret_cast<const uint4 *>(tblc + o.x);
-        const uint4 v1 = *reinterpret_cast<const uint4 *>(tblc + o.y);
-        const uint4 v2 = *reinterpret_cast<const uint4 *>(tblc + o.z);
-        const uint4 v3 = *reinterpret_cast<const uint4 *>(tblc + o.w);
+        const uint4 v1 = 4 * q + 1 < KU ? *reinterpret_cast<const uint4 *>(tblc + o.y) : z;
+        const uint4 v2 = 4 * q + 2 < KU ? *reinterpret_cast<const uint4 *>(tblc + o.z) : z;
+        const uint4 v3 = 4 * q + 3 < KU ? *reinterpret_cast<const uint4 *>(tblc + o.w) : z;
         m.x = lop_or3(lop_or3(m.x, v0.x, v1.x), v2.x, v3.x);
         m.y = lop_or3(lop_or3(m.y, v0.y, v1.y), v2.y, v3.y);
         m.z = lop_or3(lop_or3(m.z, v0.z, v1.z), v2.z, v3.z);
@@ -289,7 +293,7 @@ __device__ __forceinline__ uint4 ef_token_mask(const unsigned char *tblc, const 
         }                                                                                         \
     } while (0)
 
-template <int KP>
+template <int KP, int KU>
 __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams q)
 {
     extern __shared__ __align__(16) unsigned char ef_sm[];
@@ -384,7 +388,7 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
                 uint4 x[EF_PASSES];
                 const uint32_t *ob = offs + buf * nent + sub * KP;
 #pragma unroll
-                for (int ps = 0; ps < EF_PASSES; ++ps) x[ps] = ef_token_mask<KP>(tblc, ob + ps * S * KP);
+                for (int ps = 0; ps < EF_PASSES; ++ps) x[ps] = ef_token_mask<KP, KU>(tblc, ob + ps * S * KP);
                 CAP_EF_WORD(x);
                 CAP_EF_WORD(y);
                 CAP_EF_WORD(z);
@@ -690,17 +694,17 @@ __global__ void __launch_bounds__(32 * DEC_WARPS) eval_decode_kernel(DecodeParam
 }
 
 // ---- launcher ------------------------------------------------------------------------------------------
-template <int KP>
+template <int KP, int KU>
 static int launch_kp(const EvalFastParams &prm, const EvalFastGeom &g, int L, cudaStream_t st)
 {
     // per device and cheap: set on every launch, to what this launch needs (the kernel also has 520 B of static
     // shared memory, so the full 227 KB would not be a legal dynamic size)
-    if (cudaFuncSetAttribute(eval_fast_kernel<KP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem) != cudaSuccess)
+    if (cudaFuncSetAttribute(eval_fast_kernel<KP, KU>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem) != cudaSuccess)
         return check_launch("eval_fast_kernel attribute");
     dim3 grid((unsigned)g.ncta_t, (unsigned)g.PC, (unsigned)L);
     {
         KernelTimerScope ts("eval", st);
-        eval_fast_kernel<KP><<<grid, g.nthreads, g.smem, st>>>(prm);
+        eval_fast_kernel<KP, KU><<<grid, g.nthreads, g.smem, st>>>(prm);
     }
     note_launch();
     return check_launch("eval_fast_kernel");
@@ -894,10 +898,10 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     prm.NPR = g.NPR;
     int rc;
     switch (g.KP) {
-    case 4: rc = launch_kp<4>(prm, g, L, st); break;
-    case 8: rc = launch_kp<8>(prm, g, L, st); break;
-    case 12: rc = launch_kp<12>(prm, g, L, st); break;
-    default: rc = launch_kp<16>(prm, g, L, st); break;
+    case 4: rc = launch_kp<4, 4>(prm, g, L, st); break;
+    case 8: rc = launch_kp<8, 8>(prm, g, L, st); break;
+    case 12: rc = k <= 10 ? launch_kp<12, 10>(prm, g, L, st) : launch_kp<12, 12>(prm, g, L, st); break;
+    default: rc = launch_kp<16, 16>(prm, g, L, st); break;
     }
     CAP_TRY(rc);
     CAP_TRY(ef_launch_decode(g, fw, L, T, E, P, topo, expert_dev, counts, out, st));
