@@ -137,28 +137,40 @@ __device__ __forceinline__ uint32_t ef_table_word(const int32_t *__restrict__ ma
 {
     if (e >= E || w >= DW + NW) return 0u;
     const bool devw = w < DW;
-    const int fpw = devw ? (WD == 64 ? 1 : 32 / WD) : 32 / WN;          // candidates in this word (<= 16)
-    const int pb = p0 + (devw ? (WD == 64 ? (w >> 1) : w * fpw) : (w - DW) * fpw);
-    int dv[16];
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        const int p = pb + j;
-        dv[j] = (j < fpw && p < P) ? maps[(size_t)p * E + e] : -1;
-    }
     uint32_t word = 0u;
     if (devw) {
+        // 1 (WD = 64: half a field per word, or WD = 32), 2 or 4 candidates per word: at most four independent loads
+        const int fpw = WD >= 32 ? 1 : 32 / WD;
+        const int pb = p0 + (WD == 64 ? (w >> 1) : w * fpw);
+        int dv[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int p = pb + j;
+            dv[j] = (j < fpw && p < P) ? maps[(size_t)p * E + e] : -1;
+        }
         if (WD == 64) {
             const int d = dv[0];
             if ((unsigned)d < (unsigned)D && (d >> 5) == (w & 1)) word = 1u << (d & 31);
         } else {
 #pragma unroll
             for (int j = 0; j < 4; ++j)
-                if (j < fpw && (unsigned)dv[j] < (unsigned)D) word |= 1u << (j * WD + dv[j]);
+                if ((unsigned)dv[j] < (unsigned)D) word |= 1u << (j * WD + dv[j]);
         }
     } else {
+        // 4, 8 or 16 candidates per node word, four loads in flight
+        const int fpw = 32 / WN;
+        const int pb = p0 + (w - DW) * fpw;
+        for (int j0 = 0; j0 < fpw; j0 += 4) {
+            int dv[4];
 #pragma unroll
-        for (int j = 0; j < 16; ++j)
-            if (j < fpw && (unsigned)dv[j] < (unsigned)D) word |= 1u << (j * WN + (node_of[dv[j]] & (WN - 1)));
+            for (int j = 0; j < 4; ++j) {
+                const int p = pb + j0 + j;
+                dv[j] = p < P ? maps[(size_t)p * E + e] : -1;
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                if ((unsigned)dv[j] < (unsigned)D) word |= 1u << ((j0 + j) * WN + (node_of[dv[j]] & (WN - 1)));
+        }
     }
     return word;
 }
