@@ -1,16 +1,18 @@
 // S1 fast path for wide routers (Eq. 1; BASELINE.json config 5: E = 512, top-10): softmax scoring,
-// renormalised weights, no group limit, k <= 10, E = 512.  Same structure as cap_gate_fast.cu -- persistent
-// blocks, producer warps stream 16-token tiles of logits into a shared-memory ring with TMA bulk copies,
-// consumer warps give every token a PAIR of lanes -- but each lane now streams 256 logits: groups of 8 are
-// sorted by the 19-comparator network and merged into a running sorted top-16 (half-cleaner against the lower
-// half of the list + bitonic merge), in a rolled loop (32 groups; unrolled it would not fit the instruction
-// cache).  Keys are the logits' own bit patterns with the low byte replaced by the position in the half row
-// (fp32 min / max order them); for the merge of the two halves the low NINE bits become the expert index.
-// A payload can only decide a comparison between keys that agree in all upper bits: if two neighbours among
-// the 11 largest agree in their upper 23 bits, or one of them is a zero, the warp redoes the token with exact
-// comparisons (k rounds of warp-wide arg-max, ties to the lower index), so the result is always the exact
-// top-k.  The generic warp-per-token kernel it replaces here ran 1.8 k warp instructions per token (ncu,
-// profiles/r2d_step.md); this one ~0.25 k.
+// renormalised weights, no group limit, k <= 10, E = 512.  Same ring as cap_gate_fast.cu -- persistent blocks,
+// producer warps stream 16-token tiles of logits (32 KB) into shared memory with TMA bulk copies -- but a token
+// gets FOUR lanes and a tile two warps (8 tokens each): with two lanes per token and one warp per tile only as
+// many warps worked as the ring has stages (6), and ncu showed the kernel waiting, not issuing.  Each lane
+// streams a quarter row (128 logits): groups of 8 are sorted by the 19-comparator network and merged into a
+// running sorted top-16 (half-cleaner against the lower half of the list + bitonic merge), in a rolled loop
+// (unrolled it would not fit the instruction cache); the four lists are merged by two butterfly steps.
+// Keys are the logits' own bit patterns with the low byte replaced by the position in the quarter row (fp32
+// min / max order them); for the cross-lane merges the low NINE bits become the expert index.  A payload can
+// only decide a comparison between keys that agree in all upper bits: if two neighbours among the 11 largest
+// agree in their upper 23 bits, or one of them is a zero, the warp redoes the token with exact comparisons
+// (k rounds of warp-wide arg-max, ties to the lower index), so the result is always the exact top-k.  The
+// generic warp-per-token kernel it replaces here ran 1.8 k warp instructions per token (ncu,
+// profiles/r2d_step.md); this one ~0.4 k.
 #include "cap_async.cuh"
 #include "cap_gate_fast.cuh"
 
@@ -77,16 +79,17 @@ __device__ __noinline__ void gate_select_exact_warp16(uint32_t row_smem, int lan
     }
 }
 
-// Lanes l and l ^ 16 share token l & 15; half h streams experts [256 h, 256 h + 256) of the row (2 KB, 1 KB
-// aligned halves; lane t reads 16-byte chunk c of its half at chunk position c ^ (t & 7), as in cap_gate_fast.cuh).
-__device__ __forceinline__ void gate_select_pair512(const float *row, int h, int t7, int k, int (&sel)[16])
+// Lanes l, l ^ 8, l ^ 16, l ^ 24 share token l & 7 of the warp's eight; quarter qd = l >> 3 streams experts
+// [128 qd, 128 qd + 128) of the row (2 KB, 512-byte aligned quarters; lane t reads 16-byte chunk c of its quarter
+// at chunk position c ^ (t & 7), as in cap_gate_fast.cuh).  All four lanes end with the same list.
+__device__ __forceinline__ void gate_select_quad512(const float *row, int qd, int t7, int k, int (&sel)[16])
 {
-    const uint32_t hb = (smem_u32(row) + (uint32_t)h * 1024u) | ((uint32_t)t7 << 4);
+    const uint32_t hb = (smem_u32(row) + (uint32_t)qd * 512u) | ((uint32_t)t7 << 4);
     float r[16];
 #pragma unroll
     for (int i = 0; i < 16; ++i) r[i] = __uint_as_float(0xff800000u);          // -inf: below every finite key
 #pragma unroll 1
-    for (int gi = 0; gi < 32; ++gi) {
+    for (int gi = 0; gi < 16; ++gi) {
         float4 va, vb;
         asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];"
                      : "=f"(va.x), "=f"(va.y), "=f"(va.z), "=f"(va.w)
@@ -108,23 +111,27 @@ __device__ __forceinline__ void gate_select_pair512(const float *row, int h, int
         sort8_desc(g);
         merge8_into16(r, g);
     }
-    // low nine bits <- expert index: undo the chunk swizzle (XOR of position bits 2..4), add 256 h
-    const uint32_t swz = (uint32_t)t7 << 2, hbit = (uint32_t)h << 8;
-    float gp[16];
+    // low nine bits <- expert index: undo the chunk swizzle (XOR of position bits 2..4), add 128 qd
+    const uint32_t swz = (uint32_t)t7 << 2, qbits = (uint32_t)qd << 7;
 #pragma unroll
     for (int i = 0; i < 16; ++i) {
         const uint32_t u = __float_as_uint(r[i]);
-        r[i] = __uint_as_float((u & 0xfffffe00u) | hbit | ((u & 0xffu) ^ swz));
+        r[i] = __uint_as_float((u & 0xfffffe00u) | qbits | ((u & 0x7fu) ^ swz));
     }
+    // two butterfly steps over the four quarters: the partner's list reversed, element-wise max, bitonic merge
 #pragma unroll
-    for (int i = 0; i < 16; ++i) gp[i] = __shfl_xor_sync(0xffffffffu, r[15 - i], 16);
+    for (int off = 8; off <= 16; off <<= 1) {
+        float gp[16];
 #pragma unroll
-    for (int i = 0; i < 16; ++i) r[i] = kmax(r[i], gp[i]);
+        for (int i = 0; i < 16; ++i) gp[i] = __shfl_xor_sync(0xffffffffu, r[15 - i], off);
 #pragma unroll
-    for (int s = 8; s >= 1; s >>= 1) {
+        for (int i = 0; i < 16; ++i) r[i] = kmax(r[i], gp[i]);
 #pragma unroll
-        for (int i = 0; i < 16; ++i)
-            if ((i & s) == 0) CAP_CE(r[i], r[i + s]);
+        for (int s = 8; s >= 1; s >>= 1) {
+#pragma unroll
+            for (int i = 0; i < 16; ++i)
+                if ((i & s) == 0) CAP_CE(r[i], r[i + s]);
+        }
     }
     // ambiguous: neighbours among the 11 largest that agree in every bit above the payload, or a zero among them
     bool amb = false;
@@ -135,7 +142,7 @@ __device__ __forceinline__ void gate_select_pair512(const float *row, int h, int
 #pragma unroll
     for (int i = 0; i < 16; ++i) sel[i] = (int)(__float_as_uint(r[i]) & 0x1ffu);
     const int lane = (int)(threadIdx.x & 31u);
-    unsigned todo = __ballot_sync(0xffffffffu, amb) & 0xffffu;     // one lane of each pair
+    unsigned todo = __ballot_sync(0xffffffffu, amb) & 0xffu;       // one lane of each quad
     const uint32_t row_s = smem_u32(row);
     while (todo) {
         const int src = __ffs((int)todo) - 1;
@@ -143,7 +150,7 @@ __device__ __forceinline__ void gate_select_pair512(const float *row, int h, int
         const uint32_t rs = __shfl_sync(0xffffffffu, row_s, src);
         int ex[16];
         gate_select_exact_warp16(rs, lane, k, ex);
-        if ((lane & 15) == src) {
+        if ((lane & 7) == src) {
 #pragma unroll
             for (int i = 0; i < 16; ++i) sel[i] = ex[i];
         }
@@ -151,27 +158,29 @@ __device__ __forceinline__ void gate_select_pair512(const float *row, int h, int
 }
 
 // Renormalised softmax weights (DESIGN.md R-S1.3): r_s = expS(x_s - x_0), Z summed in slot order, w_s = r_s / Z
-// (* scale).  Lane half h evaluates slots 8h..8h+7; w[0..8) = their weights.
-__device__ __forceinline__ void gate_weights_softmax_pair16(const float *row, int h, int k, const int (&sel)[16],
-                                                            float scale, float (&w)[8])
+// (* scale).  Quarter lane qd evaluates slots 4 qd .. 4 qd + 3; w[0..4) = their weights.
+__device__ __forceinline__ void gate_weights_softmax_quad16(const float *row, int qd, int k, const int (&sel)[16],
+                                                            float scale, float (&w)[4])
 {
     const float x0 = row[sel[0]];
-    float mine[8], other[8];
+    const int lane = (int)(threadIdx.x & 31u);
+    float mine[4];
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-        const int s = 8 * h + j;
-        const int e = h ? sel[8 + j] : sel[j];
-        mine[j] = s < k ? exp_s(__fsub_rn(row[e], x0)) : 0.0f;
-        other[j] = __shfl_xor_sync(0xffffffffu, mine[j], 16);
+    for (int j = 0; j < 4; ++j) {
+        int e = 0;
+#pragma unroll
+        for (int s = 0; s < 16; ++s) e = (s == 4 * qd + j) ? sel[s] : e;
+        mine[j] = 4 * qd + j < k ? exp_s(__fsub_rn(row[e], x0)) : 0.0f;
     }
-    float Z = h ? other[0] : mine[0];
+    float Z = 0.0f;
 #pragma unroll
-    for (int s = 1; s < 16; ++s) {
-        const float rs = (s < 8) ? (h ? other[s & 7] : mine[s & 7]) : (h ? mine[s & 7] : other[s & 7]);
-        if (s < k) Z = __fadd_rn(Z, rs);
+    for (int s = 0; s < 16; ++s) {
+        const float rs = __shfl_sync(0xffffffffu, mine[s & 3], (lane & 7) | ((s >> 2) << 3));
+        if (s == 0) Z = rs;
+        else if (s < k) Z = __fadd_rn(Z, rs);
     }
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
+    for (int j = 0; j < 4; ++j) {
         float v = __fdiv_rn(mine[j], Z);
         if (scale != 1.0f) v = __fmul_rn(v, scale);
         w[j] = v;
@@ -191,7 +200,7 @@ __global__ void __launch_bounds__(GW_THREADS) gate_wide_kernel(GateWideParams q)
     if (threadIdx.x == 0) {
         for (int s = 0; s < GW_NST; ++s) {
             mbar_init(&full_bar[s], 1);
-            mbar_init(&empty_bar[s], 1);
+            mbar_init(&empty_bar[s], 2);            // the two warps of a tile
             stage_use[s] = 0xffffffffu;
         }
         mbar_fence_init();
@@ -216,28 +225,33 @@ __global__ void __launch_bounds__(GW_THREADS) gate_wide_kernel(GateWideParams q)
             }
         }
     } else {
+        // consumers: warps 2m and 2m + 1 share tiles m, m + NC / 2, ...; each takes eight of the tile's tokens
         const int c = warp - GW_NP;
         const int k = q.k;
-        const int h = lane >> 4, tl = lane & 15;
-        for (int64_t j = c; j < nt; j += GW_NC) {
+        const int sub = c & 1, qd = lane >> 3, tl = lane & 7;
+        for (int64_t j = c >> 1; j < nt; j += GW_NC / 2) {
             const int st = (int)(j % GW_NST);
             const uint32_t use = (uint32_t)(j / GW_NST);
             while (ld_acquire_shared(&stage_use[st]) != use) __nanosleep(32);
             mbar_wait(&full_bar[st], use & 1u);
-            const int64_t tok = (tile0 + j) * GW_TILE + tl;
+            const int64_t tok = (tile0 + j) * GW_TILE + 8 * sub + tl;
             const bool valid = tok < q.LT;
             // rows past the end of a ragged last tile were not written: those lanes redo row 0
-            const float *row = reinterpret_cast<const float *>(gw_sm + (size_t)st * STAGEB + (valid ? tl : 0) * ROWB);
+            const float *row =
+                reinterpret_cast<const float *>(gw_sm + (size_t)st * STAGEB + (valid ? 8 * sub + tl : 0) * ROWB);
             int sel[16];
-            float wv[8];
-            gate_select_pair512(row, h, tl & 7, k, sel);
-            gate_weights_softmax_pair16(row, h, k, sel, q.scale, wv);
+            float wv[4];
+            gate_select_quad512(row, qd, tl, k, sel);
+            gate_weights_softmax_quad16(row, qd, k, sel, q.scale, wv);
             if (valid) {
 #pragma unroll
-                for (int jj = 0; jj < 8; ++jj) {
-                    const int s = 8 * h + jj;
+                for (int jj = 0; jj < 4; ++jj) {
+                    const int s = 4 * qd + jj;
+                    int e = 0;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) e = (i == s) ? sel[i] : e;
                     if (s < k) {
-                        q.idx[tok * k + s] = h ? sel[8 + jj] : sel[jj];
+                        q.idx[tok * k + s] = e;
                         q.w[tok * k + s] = wv[jj];
                     }
                 }
