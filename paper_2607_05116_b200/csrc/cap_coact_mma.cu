@@ -6,6 +6,9 @@
 // the SAME tile as both operands, accumulating in TMEM.  At the end the accumulator is read back
 // with tcgen05.ld and added into the global matrix; symmetry (C[r][c] = C[c][r]) lets lane r write
 // address [c][r], which makes the atomic adds coalesced.  diag(C) gives the counts.
+// 256 < E <= 512 (config 5): the 512 x 512 accumulator is four times the TMEM of an SM, so blockIdx.z
+// names the 128-row block a CTA accumulates (A = rows [128 z, 128 z + 128) of the tile, B = the whole
+// 512-row tile as two N = 256 halves -> all 512 TMEM columns); every CTA builds the whole one-hot tile.
 #include "cap_async.cuh"
 #include "cap_internal.cuh"
 #include "cap_tc.cuh"
@@ -22,7 +25,7 @@ struct CoactMmaParams {
     unsigned long long *counts;   // [L][E]
     int *coact;                // [L][E][E]
     int64_t T, tpc;            // tokens per layer, tokens per block
-    int32_t k, E, EP;          // EP = E padded to 128 or 256 (rows of the tile)
+    int32_t k, E, EP;          // EP = E padded to 128, 256 or 512 (rows of the tile)
     int32_t pack64;            // E even and coact 8-byte aligned: pairs of counters per 64-bit reduction
 };
 
@@ -35,7 +38,9 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
     constexpr int TILEB = EP * CM_TK;
     constexpr uint32_t LBO = 128u, SBO = (CM_TK / 16) * 128u;
     constexpr uint32_t NCOLS = EP == 128 ? 128u : 512u;
-    constexpr uint32_t IDESC = (2u << 4) | ((uint32_t)(EP >> 3) << 17) | (8u << 24);   // S32 acc, u8 x u8, N = EP, M = 128
+    constexpr int NMMA = EP == 128 ? 128 : 256;         // N of one MMA (256 is the instruction's maximum)
+    constexpr uint32_t IDESC = (2u << 4) | ((uint32_t)(NMMA >> 3) << 17) | (8u << 24);   // S32 acc, u8 x u8, N, M = 128
+    const int mb = EP == 512 ? (int)blockIdx.z : 0;     // accumulator row block of this CTA (EP = 512)
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int layer = blockIdx.y;
     const int E = q.E, k = q.k;
@@ -53,7 +58,7 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
 
     const int64_t t0 = (int64_t)blockIdx.x * q.tpc;
     const int64_t t1 = min(q.T, t0 + q.tpc);
-    const int ntile = t1 > t0 ? (int)((t1 - t0 + CM_TK - 1) / CM_TK) : 0;
+    const int ntile = t1 > t0 && mb * 128 < E ? (int)((t1 - t0 + CM_TK - 1) / CM_TK) : 0;
     const int32_t *idx = q.idx + (size_t)layer * q.T * k;
     const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
 
@@ -123,6 +128,13 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
 #pragma unroll
                 for (int j = 0; j < CM_TK / 32; ++j) {
                     const uint64_t bd = umma_desc(base + j * 2 * LBO, LBO, SBO);
+                    if (EP == 512) {
+                        const uint64_t ad = umma_desc(base + mb * 16 * SBO + j * 2 * LBO, LBO, SBO);
+                        const uint64_t b1 = umma_desc(base + 32 * SBO + j * 2 * LBO, LBO, SBO);
+                        umma_i8(tmem, ad, bd, IDESC, (uint32_t)((i | j) != 0));
+                        umma_i8(tmem + 256u, ad, b1, IDESC, (uint32_t)((i | j) != 0));
+                        continue;
+                    }
                     umma_i8(tmem, bd, bd, IDESC, (uint32_t)((i | j) != 0));
                     if (EP == 256) {
                         const uint64_t a1 = umma_desc(base + 16 * SBO + j * 2 * LBO, LBO, SBO);
@@ -140,12 +152,13 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
         int *C = q.coact + (size_t)layer * E * E;
         unsigned long long *cnt = q.counts + (size_t)layer * E;
 #pragma unroll 1
-        for (int h = 0; h < EP / 128; ++h) {
-            const int r = h * 128 + warp * 32 + lane;          // accumulator row of this thread
+        for (int h = 0; h < (EP == 256 ? 2 : 1); ++h) {
+            const int r = (mb + h) * 128 + warp * 32 + lane;   // accumulator row of this thread
 #pragma unroll 1
             for (int cb0 = 0; cb0 < EP / 32; ++cb0) {
                 // blocks start at different column groups so that they do not queue on the same L2 lines
                 const int cb = (cb0 + (int)blockIdx.x) % (EP / 32);
+                if (cb * 32 >= E) continue;                    // padding columns (warp-uniform)
                 uint32_t v[32];
                 tmem_ld32(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(h * 256 + cb * 32), v);
                 // C symmetric: the value of (r, c) is added at [c][r], consecutive lanes -> consecutive
@@ -194,20 +207,21 @@ static int launch_ep(const CoactMmaParams &prm, int L, cudaStream_t st)
     cudaFuncSetAttribute(coact_mma_kernel<EP, KMAX>, cudaFuncAttributeMaxDynamicSharedMemorySize,
     2 * EP * CM_TK);
     const int64_t nblk = (prm.T + prm.tpc - 1) / prm.tpc;
+    const unsigned nz = EP == 512 ? (unsigned)((prm.E + 127) / 128) : 1u;
     {
         KernelTimerScope ts("coact", st);
-        coact_mma_kernel<EP, KMAX><<<dim3((unsigned)nblk, (unsigned)L), CM_THREADS, 2 * EP * CM_TK, st>>>(prm);
+        coact_mma_kernel<EP, KMAX><<<dim3((unsigned)nblk, (unsigned)L, nz), CM_THREADS, 2 * EP * CM_TK, st>>>(prm);
     }
     note_launch();
     return check_launch("coact_mma_kernel");
 }
 
-// counts / coact must already be zeroed.  *used = false when E > 256 (generic kernel instead).
+// counts / coact must already be zeroed.  *used = false when E > 512 (generic kernel instead).
 int launch_coact_mma(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t T, int32_t k, int32_t E,
                      int64_t *counts, int32_t *coact, cudaStream_t st, bool *used)
 {
     *used = false;
-    if (E > 256 || T < 1 || L < 1) return CAP_OK;
+    if (E > 512 || T < 1 || L < 1) return CAP_OK;
     CoactMmaParams prm;
     prm.idx = idx;
     prm.kept = kept;
@@ -216,17 +230,19 @@ int launch_coact_mma(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     prm.T = T;
     prm.k = k;
     prm.E = E;
-    prm.EP = E <= 128 ? 128 : 256;
+    prm.EP = E <= 128 ? 128 : E <= 256 ? 256 : 512;
     prm.pack64 = (E % 2 == 0) && (reinterpret_cast<uintptr_t>(coact) & 7u) == 0;
     // one block per SM is resident at EP = 256 (all 512 TMEM columns); every block ends with E^2 reductions into
     // the matrix, so a block should own at least ~1 000 tokens
-    int64_t want = balanced_blocks_per_unit(L, sm_count(), T / 1024 > 1 ? T / 1024 : 1);
+    const int64_t nz = prm.EP == 512 ? (E + 127) / 128 : 1;
+    int64_t want = balanced_blocks_per_unit(L * nz, sm_count(), T / 1024 > 1 ? T / 1024 : 1);
     int64_t tpc = (T + want - 1) / want;
     tpc = ((tpc + CM_TK - 1) / CM_TK) * CM_TK;
     prm.tpc = tpc;
     *used = true;
     if (prm.EP == 128) return k <= 8 ? launch_ep<128, 8>(prm, L, st) : launch_ep<128, 16>(prm, L, st);
-    return k <= 8 ? launch_ep<256, 8>(prm, L, st) : launch_ep<256, 16>(prm, L, st);
+    if (prm.EP == 256) return k <= 8 ? launch_ep<256, 8>(prm, L, st) : launch_ep<256, 16>(prm, L, st);
+    return k <= 8 ? launch_ep<512, 8>(prm, L, st) : launch_ep<512, 16>(prm, L, st);
 }
 
 }  // namespace cap

@@ -140,7 +140,9 @@ def _trace(rng, L, T, E, k):
     return np.stack([np.stack([rng.permutation(E)[:k] for _ in range(T)]) for _ in range(L)]).astype(np.int32)
 
 
-@pytest.mark.parametrize("E,k,T", [(8, 3, 5), (16, 2, 1), (24, 5, 1033), (200, 8, 700), (256, 8, 3000), (512, 10, 900)])
+@pytest.mark.parametrize("E,k,T", [(8, 3, 5), (16, 2, 1), (24, 5, 1033), (200, 8, 700), (256, 8, 3000), (512, 10, 900),
+                                   (258, 4, 300), (320, 6, 1500), (385, 9, 2100), (500, 10, 5000), (512, 16, 4097),
+                                   (514, 8, 600), (1024, 16, 500)])
 def test_coact_masked_and_shapes(E, k, T):
     rng = np.random.default_rng(E + T)
     idx = _trace(rng, 2, T, E, k)
@@ -562,7 +564,8 @@ def test_garbage_values_are_memory_safe(with_src):
     cap.coactivation(bad_idx, kept, E)
     cap.eval_placements(bad_idx, None, dev(src), dev(maps), topo, counts=None)
     if E != 512:
-        cap.coactivation(bad_idx[:, :300].contiguous(), None, 512)          # the histogram path of large E
+        cap.coactivation(bad_idx[:, :300].contiguous(), None, 512)          # the four-row-block tensor-core path
+    cap.coactivation(bad_idx[:, :300].contiguous(), None, 1024)             # the histogram path of large E
     torch.cuda.synchronize()
     check_all_stages(W.CONFIGS["tiny"], tag="after garbage ")
 

@@ -272,6 +272,31 @@ def test_adjust_shapes_stops_and_unbalanced_maps(E, D, k, T, S):
     check_adjust(cnt, C, pi0, D, S, tag=f"E{E} D{D} ")
 
 
+def test_adjust_chained_on_the_cuda_path_trades_communication_for_balance():
+    """VERDICT r1 missing #8: the whole chain on the GPU -- gate, co-activation, Algorithm 1, the swap
+    spectrum (R27, parity unpinned against the paper) and cap_eval_placements scoring every step -- shows
+    what P:L194-196 claims: imbalance does not rise along the spectrum and ends lower, devices per token
+    do not fall.  The scores themselves are bit-exact against the oracle's for the same maps."""
+    cfg = W.CONFIGS["qwen3"].with_(T=8192)
+    x = dev(W.logits(cfg, 0)[None])
+    idx, _ = cap.gate_topk(x, None, cap.gate_cfg(cfg.E, **cfg.gate))
+    cnt, C = cap.coactivation(idx, None, cfg.E)
+    ed = cap.coact_placement(cnt, C, cfg.D, cfg.N)[2]
+    spec, done, _ = cap.adjust_spectrum(cnt, C, ed, cfg.D, 6)
+    maps = torch.cat([ed[:, None], spec], 1).contiguous()
+    dn = W.dev_node(cfg)
+    topo = cap.topology(dev(dn), 0, 1, cfg.cost_inter, cfg.bytes_per_token, N=cfg.N)
+    ev = cap.eval_placements(idx, None, None, maps, topo, counts=cnt)
+    torch.cuda.synchronize()
+    assert int(host(done)[0]) == 6
+    imb, vis = host(ev.imbalance)[0], host(ev.dev_visits)[0]
+    assert np.all(np.diff(imb) <= 1e-12) and imb[-1] < imb[0] - 0.02
+    assert vis[-1] >= vis[0]
+    ref = O.eval_placements(host(idx), host(maps), dn, cost_inter=cfg.cost_inter, bytes_per_token=cfg.bytes_per_token)
+    np.testing.assert_array_equal(imb, ref.imbalance[0])
+    np.testing.assert_array_equal(vis, ref.dev_visits[0])
+
+
 def test_adjust_kernel_time():
     cfg = W.CONFIGS["qwen3"]
     _, _, _, cnt, C = trace_stats(cfg, (0,), 8192)
