@@ -17,7 +17,7 @@ namespace cap {
 
 constexpr int CM_TK = 128;          // tokens per tile (4 MMAs of K = 32)
 constexpr int CM_THREADS = 128;
-constexpr int CM_NB = 4;            // tiles whose indices are fetched together
+constexpr int CM_NB = 2;            // tiles whose indices are fetched together (even: buffer = tile & 1)
 
 struct CoactMmaParams {
     const int32_t *idx;        // [L][T][k]
@@ -63,62 +63,87 @@ __global__ void __launch_bounds__(CM_THREADS) coact_mma_kernel(CoactMmaParams q)
     const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
 
     // The thread's token of each tile: its k expert rows as byte offsets into the tile (-1 = not
-    // kept).  Indices are fetched for CM_NB tiles at a time, so the global-load latency is paid once
-    // per batch instead of once per tile.
-    for (int ib = 0; ib < ntile; ib += CM_NB) {
-        int rowoff[CM_NB][KMAX];
-        // issue every load of the batch first (raw expert ids; -1 = absent), then turn them into offsets
-        const bool vec8 = KMAX == 8 && k == 8 && !kept && (reinterpret_cast<uintptr_t>(idx) & 15u) == 0;
+    // kept).  A thread only ever writes the bytes of its own token column, so a tile buffer is not
+    // cleared between uses: both buffers are zeroed once, and when a buffer comes back (its MMAs
+    // have completed) the thread takes back the ones it set two tiles ago and sets the new ones --
+    // k byte stores each instead of a 32 / 64 KB clear and a block barrier.  Indices are fetched
+    // one batch of CM_NB tiles ahead, so their global-load latency overlaps the tiles in work.
+    {
+        uint4 *t4 = reinterpret_cast<uint4 *>(cm_sm);
+        for (int j = tid; j < 2 * TILEB / 16; j += CM_THREADS) t4[j] = make_uint4(0u, 0u, 0u, 0u);
+    }
+    const bool vec8 = KMAX == 8 && k == 8 && !kept && (reinterpret_cast<uintptr_t>(idx) & 15u) == 0;
+    const bool vec2 = !vec8 && (k & 1) == 0 && !kept && (reinterpret_cast<uintptr_t>(idx) & 7u) == 0;
+    int raw[CM_NB][KMAX];
+    auto fetch = [&](int ib) {
 #pragma unroll
         for (int u = 0; u < CM_NB; ++u) {
             const int64_t tok = t0 + (int64_t)(ib + u) * CM_TK + tid;
+            const bool ok = tok < t1 && ib + u < ntile;
             if (vec8) {
                 int4 lo = make_int4(-1, -1, -1, -1), hi = lo;
-                if (tok < t1) {
+                if (ok) {
                     lo = __ldg(reinterpret_cast<const int4 *>(idx + tok * 8));
                     hi = __ldg(reinterpret_cast<const int4 *>(idx + tok * 8) + 1);
                 }
-                rowoff[u][0] = lo.x; rowoff[u][1] = lo.y; rowoff[u][2] = lo.z; rowoff[u][3] = lo.w;
-                rowoff[u][4 % KMAX] = hi.x; rowoff[u][5 % KMAX] = hi.y; rowoff[u][6 % KMAX] = hi.z;
-                rowoff[u][7 % KMAX] = hi.w;
+                raw[u][0] = lo.x; raw[u][1] = lo.y; raw[u][2] = lo.z; raw[u][3] = lo.w;
+                raw[u][4 % KMAX] = hi.x; raw[u][5 % KMAX] = hi.y; raw[u][6 % KMAX] = hi.z;
+                raw[u][7 % KMAX] = hi.w;
+            } else if (vec2) {
+#pragma unroll
+                for (int s = 0; s < KMAX; s += 2) {
+                    int2 v = make_int2(-1, -1);
+                    if (s < k && ok) v = __ldg(reinterpret_cast<const int2 *>(idx + tok * k + s));
+                    raw[u][s] = v.x;
+                    raw[u][(s + 1) % KMAX] = v.y;
+                }
             } else {
 #pragma unroll
                 for (int s = 0; s < KMAX; ++s) {
                     int e = -1;
-                    if (s < k && tok < t1) {
+                    if (s < k && ok) {
                         const int64_t a = tok * k + s;
                         e = __ldg(idx + a);
                         if (kept && !__ldg(kept + a)) e = -1;
                     }
-                    rowoff[u][s] = e;
+                    raw[u][s] = e;
                 }
             }
         }
+    };
+    int prev[2][KMAX];          // what this thread set in each buffer (offsets, -1 = nothing)
+#pragma unroll
+    for (int s = 0; s < KMAX; ++s) prev[0][s] = prev[1][s] = -1;
+    if (ntile > 0) fetch(0);
+    __syncthreads();            // the buffers are zero
+    for (int ib = 0; ib < ntile; ib += CM_NB) {
+        int rowoff[CM_NB][KMAX];
 #pragma unroll
         for (int u = 0; u < CM_NB; ++u) {
 #pragma unroll
             for (int s = 0; s < KMAX; ++s) {
-                const int e = rowoff[u][s];
+                const int e = raw[u][s];
                 rowoff[u][s] = (unsigned)e < (unsigned)E ? (e >> 3) * (int)SBO + (e & 7) * 16 : -1;
             }
         }
+        if (ib + CM_NB < ntile) fetch(ib + CM_NB);
 #pragma unroll
         for (int u = 0; u < CM_NB; ++u) {
             const int i = ib + u;
             if (i >= ntile) break;
-            const int buf = i & 1;
+            const int buf = u & 1;                 // = i & 1 (CM_NB is even)
             unsigned char *tile = cm_sm + (size_t)buf * TILEB;
             if (i >= 2) mbar_wait(&done_bar[buf], (uint32_t)(((i >> 1) - 1) & 1));   // tile i-2 consumed
-            uint4 *t4 = reinterpret_cast<uint4 *>(tile);
-#pragma unroll
-            for (int j = 0; j < TILEB / 16 / CM_THREADS; ++j)
-                t4[j * CM_THREADS + tid] = make_uint4(0u, 0u, 0u, 0u);
-            __syncthreads();
             {
                 unsigned char *col = tile + (tid >> 4) * LBO + (tid & 15);
 #pragma unroll
                 for (int s = 0; s < KMAX; ++s)
+                    if (prev[buf][s] >= 0) col[prev[buf][s]] = 0;
+#pragma unroll
+                for (int s = 0; s < KMAX; ++s) {
                     if (rowoff[u][s] >= 0) col[rowoff[u][s]] = 1;
+                    prev[buf][s] = rowoff[u][s];
+                }
             }
             proxy_fence_async();   // generic-proxy writes -> visible to the tensor core's async proxy
             __syncthreads();
