@@ -34,8 +34,10 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
         const int ncol = (Pc * g->WN + 127) / 128;
         const int R = dcol + ncol;
         const int RS = R | 1;
+        // stand-alone kernel: a sub-slot takes whole groups of 8 lanes (see eval_fast_kernel)
+        const int Rt = rs_limit == EF_RS_ALONE ? ((R + 7) & ~7) : R;
         int S = 1;
-        while (S < 64 && R * (S * 2) <= rs_limit) S *= 2;
+        while (S < 64 && Rt * (S * 2) <= rs_limit) S *= 2;
         const size_t tbl = (size_t)(E + 1) * RS * 16;
         const size_t offs = (size_t)2 * EF_PASSES * S * g->KP * 4;
         const size_t xch = (size_t)(S / 2) * R * EF_NPL * 16;
@@ -73,7 +75,8 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
         g->logS -= 1;
     }
     const int need_pre = (EF_PASSES * g->S * g->KP + EF_PRE - 1) / EF_PRE;
-    const int need = g->R * g->S > need_pre ? g->R * g->S : need_pre;
+    const int Rt = rs_limit == EF_RS_ALONE ? ((g->R + 7) & ~7) : g->R;
+    const int need = Rt * g->S > need_pre ? Rt * g->S : need_pre;
     g->nthreads = ((need + 31) / 32) * 32;
     if (g->nthreads > EF_MAXTHREADS) return false;
     const int64_t blk = (int64_t)EF_PASSES * g->S;
@@ -308,9 +311,16 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
     ef_copy_table(tbl, q.table + ((size_t)layer * q.PC + pc) * (size_t)(E + 1) * q.RS * 4, (E + 1) * q.RS,
                   tid, nthr);
 
-    const bool active = tid < R * S;
-    const int sub = active ? tid / R : 0;
-    const int col = active ? tid - sub * R : 0;
+    // (sub-slot, column) of a thread: a sub-slot takes ceil(R / 8) whole groups of 8 lanes.  A 128-bit shared-memory
+    // load is served 8 lanes at a time; with R consecutive threads per sub-slot (R = 21 on config 5, 36 on config 4)
+    // nearly every group of 8 held the tail of one table row and the head of another, i.e. two 16-byte-aligned
+    // pieces whose banks overlap: ncu counted 4.95 wavefronts per row load against 3.82 ideal.  Whole groups read
+    // one contiguous piece of one row: never a conflict, at the price of (8 - R % 8) % 8 idle lanes per sub-slot.
+    const int Rq = (R + 7) & ~7;
+    const int sub_t = tid / Rq, col_t = tid - sub_t * Rq;
+    const bool active = sub_t < S && col_t < R;
+    const int sub = active ? sub_t : 0;
+    const int col = active ? col_t : 0;
     const unsigned char *tblc = tbl + col * 16;
     const int32_t *idx = q.idx + (size_t)layer * q.T * k;
     const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
