@@ -29,21 +29,36 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
     const int Pfull = ((P + unit - 1) / unit) * unit;
     // largest chunk whose table fits: (E + 1) rows of RS * 16 bytes; the chunk shrinks in single-column steps and
     // the chunks are then equalised
+    const bool alone = rs_limit == EF_RS_ALONE;
     auto fits = [&](int Pc, bool commit) {
         const int dcol = Pc * g->WD / 128;
         const int ncol = (Pc * g->WN + 127) / 128;
         const int R = dcol + ncol;
-        const int RS = R | 1;
-        // stand-alone kernel: a sub-slot takes whole groups of 8 lanes (see eval_fast_kernel)
-        const int Rt = rs_limit == EF_RS_ALONE ? ((R + 7) & ~7) : R;
+        // stand-alone kernel: a sub-slot takes whole groups of 8 lanes (see eval_fast_kernel), every group reads one
+        // contiguous piece of one row, so the row stride needs no odd padding there
+        const int RS = alone ? R : (R | 1);
+        const int Rt = alone ? ((R + 7) & ~7) : R;
         int S = 1;
         while (S < 64 && Rt * (S * 2) <= rs_limit) S *= 2;
         const size_t tbl = (size_t)(E + 1) * RS * 16;
         const size_t offs = (size_t)2 * EF_PASSES * S * g->KP * 4;
-        const size_t xch = (size_t)(S / 2) * R * EF_NPL * 16;
+        // exchange area of the flush tree: all planes in one round, or (stand-alone kernel) four planes per round
+        // when that is what lets a larger chunk fit
+        int xpl = EF_NPL;
+        size_t xch = (size_t)(S / 2) * R * xpl * 16;
+        if (alone && tbl + offs + xch + 128 > smem_budget) {
+            xpl = 4;
+            xch = (size_t)(S / 2) * R * xpl * 16;
+        }
         const size_t smem = tbl + offs + xch + 128;
         if (smem > smem_budget || R > 320) return false;
+        if (xpl < EF_NPL) {
+            // rounds of the flush use the (idle) offsets ring as well: planes per round
+            xpl = (int)((offs + xch) / ((size_t)(S / 2 > 0 ? S / 2 : 1) * R * 16));
+            if (xpl >= EF_NPL) xpl = EF_NPL - 1;
+        }
         if (commit) {
+            g->xpl = xpl;
             g->Pc = Pc;
             g->DW = dcol * 4;
             g->NW = ncol * 4;
@@ -66,6 +81,38 @@ bool eval_fast_geom(int32_t L, int64_t T, int32_t k, int32_t E, int32_t D, int32
         int eq = (((Pfull + chunks - 1) / chunks + unit - 1) / unit) * unit;
         if (eq > Pc || !fits(eq, false)) eq = Pc;
         fits(eq, true);
+    }
+    if (alone) {
+        // The kernel is bound by the shared-memory wavefronts of its row loads -- chunks x ceil(R / 8) per (token,
+        // expert) -- provided it has the warps to keep them in flight (measured on config 5: 37 chunks of R = 16 on
+        // 8 warps 531 us, 29 chunks of R = 21 on 12 warps 455 us).  Among the chunk sizes that fit, keep those with
+        // the most threads (at least 320 when some chunk size reaches that) and take the smallest product.
+        auto probe = [&](int pc, EvalFastGeom *t) {
+            *t = *g;
+            EvalFastGeom *keep = g;
+            g = t;
+            const bool ok = fits(pc, true);
+            g = keep;
+            return ok;
+        };
+        int max_threads = 0;
+        for (int pc = Pc; pc >= unit; pc -= unit) {
+            EvalFastGeom t;
+            if (probe(pc, &t) && ((t.R + 7) & ~7) * t.S > max_threads) max_threads = ((t.R + 7) & ~7) * t.S;
+        }
+        const int need_threads = max_threads < 320 ? max_threads : 320;
+        long best = -1;
+        int best_pc = g->Pc;
+        for (int pc = Pc; pc >= unit; pc -= unit) {
+            EvalFastGeom t;
+            if (!probe(pc, &t) || ((t.R + 7) & ~7) * t.S < need_threads) continue;
+            const long cost = (long)((Pfull + pc - 1) / pc) * ((t.R + 7) / 8);
+            if (best < 0 || cost < best) {
+                best = cost;
+                best_pc = pc;
+            }
+        }
+        fits(best_pc, true);
     }
     g->PC = (P + g->Pc - 1) / g->Pc;
     // enough threads to own every (sub-slot, column) pair and to prefetch a block's index entries
@@ -203,7 +250,7 @@ struct EvalFastParams {
     const long long *srcoff;     // [L][D + 1]
     int64_t T, tpc;
     int32_t k, E, P, D;
-    int32_t WD, WN, Pc, PC, DW, NW, R, RS, S, logS, ncta_t, maxrec, NPR;
+    int32_t WD, WN, Pc, PC, DW, NW, R, RS, S, logS, ncta_t, maxrec, NPR, XPL;
     // optional fills done by the table kernel (saves separate memset nodes): 32-bit words
     uint32_t *fill_ptr[4];
     unsigned long long fill_words[4];
@@ -234,23 +281,6 @@ __global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
     uint32_t *t = const_cast<uint32_t *>(q.table) + ((size_t)layer * q.PC + pc) * (size_t)(q.E + 1) * rowq;
     t[i] = ef_table_word(q.expert_dev + ((size_t)layer * q.P) * q.E, s_node, q.E, q.P, q.D, pc * q.Pc,
                          q.WD, q.WN, q.DW, q.NW, e, w);
-}
-
-// bit-sliced a += b over EF_NPL planes of 4 words
-__device__ __forceinline__ void ef_add_planes(uint4 (&a)[EF_NPL], const uint4 *b, int stride)
-{
-    uint4 carry = make_uint4(0u, 0u, 0u, 0u);
-#pragma unroll
-    for (int p = 0; p < EF_NPL; ++p) {
-        const uint4 x = b[(size_t)p * stride];
-        uint4 s, c;
-        CAP_CSA(s.x, c.x, a[p].x, x.x, carry.x);
-        CAP_CSA(s.y, c.y, a[p].y, x.y, carry.y);
-        CAP_CSA(s.z, c.z, a[p].z, x.z, carry.z);
-        CAP_CSA(s.w, c.w, a[p].w, x.w, carry.w);
-        a[p] = s;
-        carry = c;
-    }
 }
 
 // KU <= KP: slots that can hold an expert (k rounded up to even); the offsets of slots KU.. point at the zero
@@ -409,16 +439,77 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
             buf ^= 1;
         }
         // ---- flush: add the S sub-slots in the bit-sliced domain, write the record ----
-        for (int lvl = 0; lvl < q.logS; ++lvl) {
-            const int half = S >> (lvl + 1);
-            const int stride = half * R;
-            if (active && sub >= half && sub < 2 * half) {
+        if (q.XPL >= EF_NPL) {
+            // the exchange area holds every plane of half the sub-slots: one round per level
+            for (int lvl = 0; lvl < q.logS; ++lvl) {
+                const int half = S >> (lvl + 1);
+                const int stride = half * R;
+                if (active && sub >= half && sub < 2 * half) {
 #pragma unroll
-                for (int p = 0; p < EF_NPL; ++p) xch[(size_t)p * stride + (sub - half) * R + col] = pl[p];
+                    for (int p = 0; p < EF_NPL; ++p) xch[(size_t)p * stride + (sub - half) * R + col] = pl[p];
+                }
+                __syncthreads();
+                if (active && sub < half) {
+                    const uint4 *b = xch + sub * R + col;
+                    uint4 carry = make_uint4(0u, 0u, 0u, 0u);
+#pragma unroll
+                    for (int p = 0; p < EF_NPL; ++p) {
+                        const uint4 x = b[(size_t)p * stride];
+                        uint4 s_, c_;
+                        CAP_CSA(s_.x, c_.x, pl[p].x, x.x, carry.x);
+                        CAP_CSA(s_.y, c_.y, pl[p].y, x.y, carry.y);
+                        CAP_CSA(s_.z, c_.z, pl[p].z, x.z, carry.z);
+                        CAP_CSA(s_.w, c_.w, pl[p].w, x.w, carry.w);
+                        pl[p] = s_;
+                        carry = c_;
+                    }
+                }
+                __syncthreads();
             }
-            __syncthreads();
-            if (active && sub < half) ef_add_planes(pl, xch + sub * R + col, stride);
-            __syncthreads();
+        } else {
+            // A small exchange area (the price of a larger candidate chunk): q.XPL planes per round, and only the
+            // planes that can be non-zero (counts < 2^np before level lvl).  The offsets ring in front of the area is
+            // idle during a flush (every thread has passed the barrier that ends the run's last block) and is
+            // used as exchange space too.
+            uint4 *xf = reinterpret_cast<uint4 *>(offs);
+            for (int lvl = 0; lvl < q.logS; ++lvl) {
+                const int half = S >> (lvl + 1);
+                const int stride = half * R;
+                const int np = EF_BT + lvl;
+                const bool wr = active && sub >= half && sub < 2 * half, rd = active && sub < half;
+                uint4 carry = make_uint4(0u, 0u, 0u, 0u);
+                for (int p0 = 0; p0 < np; p0 += q.XPL) {
+                    if (wr) {
+#pragma unroll
+                        for (int p = 0; p < EF_NPL; ++p)
+                            if (p >= p0 && p < p0 + q.XPL && p < np)
+                                xf[(size_t)(p - p0) * stride + (sub - half) * R + col] = pl[p];
+                    }
+                    __syncthreads();
+                    if (rd) {
+                        const uint4 *b = xf + sub * R + col;
+#pragma unroll
+                        for (int p = 0; p < EF_NPL; ++p) {
+                            if (p >= p0 && p < p0 + q.XPL && p < np) {
+                                const uint4 x = b[(size_t)(p - p0) * stride];
+                                uint4 s_, c_;
+                                CAP_CSA(s_.x, c_.x, pl[p].x, x.x, carry.x);
+                                CAP_CSA(s_.y, c_.y, pl[p].y, x.y, carry.y);
+                                CAP_CSA(s_.z, c_.z, pl[p].z, x.z, carry.z);
+                                CAP_CSA(s_.w, c_.w, pl[p].w, x.w, carry.w);
+                                pl[p] = s_;
+                                carry = c_;
+                            }
+                        }
+                    }
+                    __syncthreads();
+                }
+                if (rd) {
+#pragma unroll
+                    for (int p = EF_BT; p < EF_NPL; ++p)
+                        if (p == np) pl[p] = carry;      // plane np was zero on both sides
+                }
+            }
         }
         if (active && sub == 0) {
             uint32_t *rp = q.rec_planes + ((slot0 + nrec) * (size_t)(R * 4) + (size_t)col * 4) * EF_RECW;
@@ -903,6 +994,7 @@ int launch_eval_fast(const int32_t *idx, const uint8_t *kept, int32_t L, int64_t
     prm.RS = g.RS;
     prm.S = g.S;
     prm.logS = g.logS;
+    prm.XPL = g.xpl;
     prm.ncta_t = g.ncta_t;
     prm.maxrec = g.maxrec;
     prm.NPR = g.NPR;

@@ -33,6 +33,7 @@ struct EvalFastGeom {
     int R, RS;           // 16-byte columns per row used / row stride in columns (odd)
     int W;               // words per record plane = 4 R
     int S, logS;         // token sub-slots processed concurrently (power of two)
+    int xpl;             // planes per exchange round of the flush tree (stand-alone kernel; EF_NPL = one round)
     int KP;              // k padded to a multiple of 4
     int nthreads;
     int ncta_t;          // blocks along the token axis (per layer and candidate chunk)
