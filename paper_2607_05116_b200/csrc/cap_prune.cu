@@ -80,7 +80,9 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
         s_dn[threadIdx.x] = (int)threadIdx.x < D ? prm.dev_node[threadIdx.x] : 0;
         s_nodemask[threadIdx.x] = 0ull;
     }
-    for (int i = threadIdx.x; i < PR_WARPS * 64; i += blockDim.x) (&s_cnt[0][0])[i] = 0u;
+    static_assert(PR_WARPS * 64 == 2 * PR_THREADS, "two counters per thread");
+    (&s_cnt[0][0])[threadIdx.x] = 0u;
+    (&s_cnt[0][0])[threadIdx.x + PR_THREADS] = 0u;
     if (threadIdx.x < ACC_N) s_acc[threadIdx.x] = 0ull;
     __syncthreads();
     // devices of every node: one shared-memory OR per device (from the staged copy)
@@ -149,21 +151,22 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
         // evaluation of the kept trace under this placement (P = 1)
         if (want_eval) {
             const int srcn = s_dn[src];
-            unsigned long long nodebits = 0ull;
+            // nodes the kept devices sit on: one mask test per node (N <= 8) instead of a map look-up and a 64-bit
+            // shift per slot
+            unsigned nodebits = 0u;
+            for (int n = 0; n < prm.N; ++n) nodebits |= (keepmask & s_nodemask[n]) ? (1u << n) : 0u;
 #pragma unroll
             for (int i = 0; i < KMAX; ++i) {
                 const uint32_t r = runs.run[i];
                 const int dd = (int)(r & 63u);
-                if (r != 0u && ((keepmask >> dd) & 1ull)) {
-                    nodebits |= 1ull << s_dn[dd];
+                if (r != 0u && ((keepmask >> dd) & 1ull))
                     atomicAdd(&s_cnt[warp][dd], 0x10000u | ((r >> 8) & 0xffu));   // one token, run-length pairs
-                }
             }
             a_dev = __popcll(keepmask);
             a_loc = (unsigned)((keepmask >> src) & 1ull);
             a_same = __popcll(keepmask & s_nodemask[srcn]);
-            a_node = __popcll(nodebits);
-            a_rnode = a_node - (unsigned)((nodebits >> srcn) & 1ull);
+            a_node = __popc(nodebits);
+            a_rnode = a_node - ((nodebits >> srcn) & 1u);
             if (prm.tok_rdev) prm.tok_rdev[(int64_t)layer * T + t] = (uint8_t)(a_dev - a_loc);
             if (prm.tok_rnode) prm.tok_rnode[(int64_t)layer * T + t] = (uint8_t)a_rnode;
         }
