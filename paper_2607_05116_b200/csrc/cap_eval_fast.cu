@@ -286,18 +286,36 @@ __global__ void __launch_bounds__(256) eval_table_kernel(EvalFastParams q)
 // KU <= KP: slots that can hold an expert (k rounded up to even); the offsets of slots KU.. point at the zero
 // row and are not loaded (k = 10 in a KP = 12 kernel: 10 row loads per token instead of 12)
 template <int KP, int KU>
-__device__ __forceinline__ uint4 ef_token_mask(const unsigned char *tblc, const uint32_t *op)
+__device__ __forceinline__ uint4 ef_token_mask(const unsigned char *tblc, const uint16_t *op)
 {
+    // the token's row offsets are 16-bit, in 16-byte units (a table has at most 14 336 of them): 8 / 16 / 24 / 32
+    // bytes per token instead of twice that -- the offset loads were 12 % of the kernel's shared-memory wavefronts
     uint4 m = make_uint4(0u, 0u, 0u, 0u);
     const uint4 z = make_uint4(0u, 0u, 0u, 0u);
+    uint32_t pk[KP / 2];
+    if (KP % 8 == 0) {
+#pragma unroll
+        for (int q = 0; q < KP / 8; ++q) {
+            const uint4 o = *reinterpret_cast<const uint4 *>(op + 8 * q);
+            pk[4 * q] = o.x; pk[4 * q + 1] = o.y; pk[4 * q + 2] = o.z; pk[4 * q + 3] = o.w;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < KP / 4; ++q) {
+            if (4 * q >= KU) { pk[2 * q] = pk[2 * q + 1] = 0u; continue; }
+            const uint2 o = *reinterpret_cast<const uint2 *>(op + 4 * q);
+            pk[2 * q] = o.x; pk[2 * q + 1] = o.y;
+        }
+    }
 #pragma unroll
     for (int q = 0; q < KP / 4; ++q) {
         if (4 * q >= KU) break;
-        const uint4 o = *reinterpret_cast<const uint4 *>(op + 4 * q);
-        const uint4 v0 = *reinterpret_cast<const uint4 *>(tblc + o.x);
-        const uint4 v1 = 4 * q + 1 < KU ? *reinterpret_cast<const uint4 *>(tblc + o.y) : z;
-        const uint4 v2 = 4 * q + 2 < KU ? *reinterpret_cast<const uint4 *>(tblc + o.z) : z;
-        const uint4 v3 = 4 * q + 3 < KU ? *reinterpret_cast<const uint4 *>(tblc + o.w) : z;
+        const uint32_t o0 = (pk[2 * q] & 0xffffu) << 4, o1 = (pk[2 * q] >> 16) << 4;
+        const uint32_t o2 = (pk[2 * q + 1] & 0xffffu) << 4, o3 = (pk[2 * q + 1] >> 16) << 4;
+        const uint4 v0 = *reinterpret_cast<const uint4 *>(tblc + o0);
+        const uint4 v1 = 4 * q + 1 < KU ? *reinterpret_cast<const uint4 *>(tblc + o1) : z;
+        const uint4 v2 = 4 * q + 2 < KU ? *reinterpret_cast<const uint4 *>(tblc + o2) : z;
+        const uint4 v3 = 4 * q + 3 < KU ? *reinterpret_cast<const uint4 *>(tblc + o3) : z;
         m.x = lop_or3(lop_or3(m.x, v0.x, v1.x), v2.x, v3.x);
         m.y = lop_or3(lop_or3(m.y, v0.y, v1.y), v2.y, v3.y);
         m.z = lop_or3(lop_or3(m.z, v0.z, v1.z), v2.z, v3.z);
@@ -335,8 +353,9 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
     const int E = q.E, D = q.D, k = q.k, S = q.S, R = q.R;
     const int rowb = q.RS * 16;
     unsigned char *tbl = ef_sm;
-    uint32_t *offs = reinterpret_cast<uint32_t *>(tbl + (size_t)(E + 1) * rowb);
-    uint4 *xch = reinterpret_cast<uint4 *>(offs + 2 * EF_PASSES * S * KP);
+    uint32_t *offs_region = reinterpret_cast<uint32_t *>(tbl + (size_t)(E + 1) * rowb);
+    uint16_t *offs = reinterpret_cast<uint16_t *>(offs_region);       // 16-bit row offsets in 16-byte units (half the region)
+    uint4 *xch = reinterpret_cast<uint4 *>(offs_region + 2 * EF_PASSES * S * KP);
 
     ef_copy_table(tbl, q.table + ((size_t)layer * q.PC + pc) * (size_t)(E + 1) * q.RS * 4, (E + 1) * q.RS,
                   tid, nthr);
@@ -354,7 +373,8 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
     const unsigned char *tblc = tbl + col * 16;
     const int32_t *idx = q.idx + (size_t)layer * q.T * k;
     const uint8_t *kept = q.kept ? q.kept + (size_t)layer * q.T * k : nullptr;
-    const uint32_t zero_row = (uint32_t)E * rowb;
+    const uint32_t rowu = (uint32_t)q.RS;            // row stride in 16-byte units
+    const uint32_t zero_row = (uint32_t)E * rowu;
     const int nent = EF_PASSES * S * KP;          // index entries per block of tokens
     const int64_t T = q.T;
     __shared__ long long s_srcoff[65];
@@ -403,7 +423,7 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
                     if (tok < rend && s < k) {
                         const int64_t a = (perm ? (int64_t)perm[tok] : tok) * k + s;
                         const int e = idx[a];
-                        if ((!kept || kept[a]) && (unsigned)e < (unsigned)E) o = (uint32_t)e * rowb;
+                        if ((!kept || kept[a]) && (unsigned)e < (unsigned)E) o = (uint32_t)e * rowu;
                     }
                 }
                 pre[j] = o;
@@ -413,7 +433,7 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
 #pragma unroll
             for (int j = 0; j < EF_PRE; ++j) {
                 const int i = tid + j * nthr;
-                if (i < nent) offs[buf * nent + i] = pre[j];
+                if (i < nent) offs[buf * nent + i] = (uint16_t)pre[j];
             }
         };
         __syncthreads();     // the previous run's readers of offs are done
@@ -426,7 +446,7 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
             if (more) fetch(b + blk_tokens);
             if (active) {
                 uint4 x[EF_PASSES];
-                const uint32_t *ob = offs + buf * nent + sub * KP;
+                const uint16_t *ob = offs + buf * nent + sub * KP;
 #pragma unroll
                 for (int ps = 0; ps < EF_PASSES; ++ps) x[ps] = ef_token_mask<KP, KU>(tblc, ob + ps * S * KP);
                 CAP_EF_WORD(x);
@@ -471,7 +491,7 @@ __global__ void __launch_bounds__(EF_MAXTHREADS) eval_fast_kernel(EvalFastParams
             // planes that can be non-zero (counts < 2^np before level lvl).  The offsets ring in front of the area is
             // idle during a flush (every thread has passed the barrier that ends the run's last block) and is
             // used as exchange space too.
-            uint4 *xf = reinterpret_cast<uint4 *>(offs);
+            uint4 *xf = reinterpret_cast<uint4 *>(offs_region);
             for (int lvl = 0; lvl < q.logS; ++lvl) {
                 const int half = S >> (lvl + 1);
                 const int stride = half * R;
