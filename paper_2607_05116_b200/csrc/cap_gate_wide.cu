@@ -4,7 +4,7 @@
 // gets FOUR lanes and a tile two warps (8 tokens each): with two lanes per token and one warp per tile only as
 // many warps worked as the ring has stages (6), and ncu showed the kernel waiting, not issuing.  Each lane
 // streams a quarter row (128 logits): groups of 8 are sorted by the 19-comparator network and merged into a
-// running sorted top-16 (half-cleaner against the lower half of the list + bitonic merge), in a rolled loop
+// running sorted top-12 (half-cleaner against the lower part of the list + pruned bitonic merge), in a rolled loop
 // (unrolled it would not fit the instruction cache); the four lists are merged by two butterfly steps.
 // Keys are the logits' own bit patterns with the low byte replaced by the position in the quarter row (fp32
 // min / max order them); for the cross-lane merges the low NINE bits become the expert index.  A payload can
@@ -35,17 +35,24 @@ struct GateWideParams {
     float scale;
 };
 
-// r (16 keys, sorted descending) <- the 16 largest of r and g (8 keys, sorted descending)
-__device__ __forceinline__ void merge8_into16(float (&r)[16], const float (&g)[8])
+// r[0..11] (sorted descending) <- the 12 largest of r[0..11] and g (8 keys, sorted descending).  It is the
+// merge of a sorted 16-list with a sorted 8-list (half-cleaner r[8 + i] = max(r[8 + i], g[7 - i]), then a bitonic
+// merge over distances 8, 4, 2, 1) with r[12..15] = -inf, written out with everything that only feeds positions
+// 12..15 left out: the half-cleaner moves g[3..0] into those four positions (t), the distance-4 stage keeps only
+// the maxima of (8..11, 12..15), the last two stages skip them: 56 min / max instead of 72.  k <= 10 needs the 11
+// largest keys.
+__device__ __forceinline__ void merge8_into12(float (&r)[16], const float (&g)[8])
 {
-#pragma unroll
-    for (int i = 0; i < 8; ++i) r[8 + i] = kmax(r[8 + i], g[7 - i]);
-#pragma unroll
-    for (int s = 8; s >= 1; s >>= 1) {
-#pragma unroll
-        for (int i = 0; i < 16; ++i)
-            if ((i & s) == 0) CAP_CE(r[i], r[i + s]);
-    }
+    float t0 = g[3], t1 = g[2], t2 = g[1], t3 = g[0];
+    r[8] = kmax(r[8], g[7]); r[9] = kmax(r[9], g[6]); r[10] = kmax(r[10], g[5]); r[11] = kmax(r[11], g[4]);
+    CAP_CE(r[0], r[8]); CAP_CE(r[1], r[9]); CAP_CE(r[2], r[10]); CAP_CE(r[3], r[11]);
+    CAP_CE(r[4], t0); CAP_CE(r[5], t1); CAP_CE(r[6], t2); CAP_CE(r[7], t3);
+    CAP_CE(r[0], r[4]); CAP_CE(r[1], r[5]); CAP_CE(r[2], r[6]); CAP_CE(r[3], r[7]);
+    r[8] = kmax(r[8], t0); r[9] = kmax(r[9], t1); r[10] = kmax(r[10], t2); r[11] = kmax(r[11], t3);
+    CAP_CE(r[0], r[2]); CAP_CE(r[1], r[3]); CAP_CE(r[4], r[6]); CAP_CE(r[5], r[7]);
+    CAP_CE(r[8], r[10]); CAP_CE(r[9], r[11]);
+    CAP_CE(r[0], r[1]); CAP_CE(r[2], r[3]); CAP_CE(r[4], r[5]); CAP_CE(r[6], r[7]);
+    CAP_CE(r[8], r[9]); CAP_CE(r[10], r[11]);
 }
 
 // exact top-k (k <= 16) of one row of 512 logits by the whole warp: lane l holds experts [16 l, 16 l + 16)
@@ -109,7 +116,7 @@ __device__ __forceinline__ void gate_select_quad512(const float *row, int qd, in
         g[6] = __uint_as_float(__byte_perm(__float_as_uint(vb.z), p1, 0x3216u));
         g[7] = __uint_as_float(__byte_perm(__float_as_uint(vb.w), p1, 0x3217u));
         sort8_desc(g);
-        merge8_into16(r, g);
+        merge8_into12(r, g);                  // r[12..15] stay -inf
     }
     // low nine bits <- expert index: undo the chunk swizzle (XOR of position bits 2..4), add 128 qd
     const uint32_t swz = (uint32_t)t7 << 2, qbits = (uint32_t)qd << 7;
