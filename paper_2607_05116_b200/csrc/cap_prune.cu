@@ -301,6 +301,7 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
             // the unrolled O(K^2) select chains are sized by the template: k = 10 (config 5) in <12>, not <16>
             if (k <= 4) launch_pdl(prune_kernel<4>, grid, dim3(PR_THREADS), smem, st, prm);
             else if (k <= 8) launch_pdl(prune_kernel<8>, grid, dim3(PR_THREADS), smem, st, prm);
+            else if (k <= 10) launch_pdl(prune_kernel<10>, grid, dim3(PR_THREADS), smem, st, prm);
             else if (k <= 12) launch_pdl(prune_kernel<12>, grid, dim3(PR_THREADS), smem, st, prm);
             else launch_pdl(prune_kernel<16>, grid, dim3(PR_THREADS), smem, st, prm);
         }
@@ -390,6 +391,7 @@ int launch_prune_dispatch(const int32_t *idx, const float *w, const int32_t *tok
         // staging of its maps overlap the tail of whatever precedes it in the stream; it waits before its first read
         if (k <= 4) launch_pdl_edge(prune_kernel<4>, grid, dim3(PR_THREADS), smem, st, prm);
         else if (k <= 8) launch_pdl_edge(prune_kernel<8>, grid, dim3(PR_THREADS), smem, st, prm);
+        else if (k <= 10) launch_pdl_edge(prune_kernel<10>, grid, dim3(PR_THREADS), smem, st, prm);   // config 5: 32 comparators per network instead of 42
         else if (k <= 12) launch_pdl_edge(prune_kernel<12>, grid, dim3(PR_THREADS), smem, st, prm);
         else launch_pdl_edge(prune_kernel<16>, grid, dim3(PR_THREADS), smem, st, prm);
     }
