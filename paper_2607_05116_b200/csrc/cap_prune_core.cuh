@@ -9,7 +9,7 @@
 //      are flagged (R-S4.7).
 // Round 1 ranked the devices by counting (k^2 / 2 comparisons) and picked the r-th by k selects per rank
 // (k^2 more): 5.3 k instructions per token at k = 10 (ncu, profiles/r2d_s4s5.md).  The networks are Batcher's
-// merge exchange, valid for every size: 5 / 19 / 42 / 63 comparators for 4 / 8 / 12 / 16 slots.
+// merge exchange, valid for every size: 5 / 19 / 32 / 42 / 63 comparators for 4 / 8 / 10 / 12 / 16 slots.
 #pragma once
 #include <math_constants.h>
 
