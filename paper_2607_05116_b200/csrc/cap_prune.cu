@@ -35,7 +35,7 @@ struct PruneParams {
     unsigned long long *ldirect;  // [L][64] kept pairs per device
     uint8_t *tok_rdev, *tok_rnode;   // [L][T] or NULL
     int64_t T;
-    int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec, small;
+    int32_t k, E, D, N, cost_local, cost_intra, cost_inter, vec, vec2, small;
     float p;
     // cap_prune_dispatch: kept pairs per device of every warp's 32 tokens -> histogram rows of S5, the block's sums
     // -> part (plain stores; no accumulator has to be zeroed, no ticket)
@@ -107,6 +107,19 @@ __global__ void __launch_bounds__(PR_THREADS) prune_kernel(PruneParams prm)
             e[4 % KMAX] = i1.x; e[5 % KMAX] = i1.y; e[6 % KMAX] = i1.z; e[7 % KMAX] = i1.w;
             wv[0] = w0.x; wv[1] = w0.y; wv[2] = w0.z; wv[3] = w0.w;
             wv[4 % KMAX] = w1.x; wv[5 % KMAX] = w1.y; wv[6 % KMAX] = w1.z; wv[7 % KMAX] = w1.w;
+        } else if (KMAX % 2 == 0 && prm.vec2) {
+            // even k, 8-byte aligned arrays: 64-bit loads (k = 10: 5 + 5 instead of 10 + 10)
+#pragma unroll
+            for (int s = 0; s < KMAX; s += 2) {
+                int2 v = make_int2(0, 0);
+                float2 u = make_float2(0.f, 0.f);
+                if (s < k) {
+                    v = __ldg(reinterpret_cast<const int2 *>(prm.idx + base + s));
+                    u = __ldg(reinterpret_cast<const float2 *>(prm.w + base + s));
+                }
+                e[s] = v.x; e[(s + 1) % KMAX] = v.y;
+                wv[s] = u.x; wv[(s + 1) % KMAX] = u.y;
+            }
         } else {
 #pragma unroll
             for (int s = 0; s < KMAX; ++s) {
@@ -294,6 +307,7 @@ int launch_prune(const int32_t *idx, const float *w, const int32_t *token_src, i
         prm.small = (unsigned long long)T * (unsigned long long)topo.D < (1ull << 32);
         prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
                   (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
+        prm.vec2 = (k & 1) == 0 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 7u) == 0;
         dim3 grid((unsigned)((T + PR_THREADS - 1) / PR_THREADS), (unsigned)L);
         const size_t smem = sizeof(int) * ((size_t)E + 64);
         {
@@ -379,6 +393,7 @@ int launch_prune_dispatch(const int32_t *idx, const float *w, const int32_t *tok
     prm.small = (unsigned long long)T * (unsigned long long)D < (1ull << 32);
     prm.vec = k == 8 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 15u) == 0 &&
               (reinterpret_cast<uintptr_t>(kept) & 7u) == 0;
+    prm.vec2 = (k & 1) == 0 && ((reinterpret_cast<uintptr_t>(idx) | reinterpret_cast<uintptr_t>(w)) & 7u) == 0;
     prm.hist = hist;
     prm.hist_stride = stride;
     prm.hist_layer = 2 * stride * D + 64;
